@@ -1,0 +1,152 @@
+/*
+ * oci.h — C ABI of the B200 (sm_100a) one-cell-inversion library.
+ *
+ * Method: transient, mono-energetic, isotropic-scattering slab S_N transport
+ * (eq. 1), multiple balance in time (eqs. 2,3) and
+ * simple corner balance in space (eqs. 4-11), iterated within each
+ * time step by one-cell inversion (OCI, eqs. 19-28: every cell
+ * solves its dense 4N x 4N system with incident fluxes lagged one iterate,
+ * parallel block Jacobi) or, for comparison, by source iteration (SI,
+ * eqs. 12-18).  "P:nnn" = line nnn of /root/reference/PAPER.md.
+ *
+ * All arithmetic is fp64 and runs in hand-written CUDA kernels; there is no
+ * CPU fallback.  No torch / C++ types cross this boundary: plain pointers
+ * (each documented as HOST or DEVICE) and sizes.
+ *
+ * Layout conventions (all arrays C-contiguous, double unless noted)
+ *   angle index m = 0..N-1 ascending in mu_m (Gauss-Legendre, sum w = 2);
+ *   the mirror image of direction m is N-1-m.
+ *   slot s: 0 = (k,L)  1 = (k,R)  2 = (k+1/2,L)  3 = (k+1/2,R)
+ *           k = time-average unknown, k+1/2 = time-edge unknown (eqs. 2,3),
+ *           L/R = left/right half-cell (corner) average (eqs. 4-7).
+ *   per-cell unknown vector Psi_j[4m+s]  (eqs. 23,24).
+ *
+ * Ownership: the caller owns every array passed in or out; inputs are copied
+ * during the call.  The context is library-owned (oci_destroy).  Device
+ * memory is supplied by the caller as one workspace (oci_workspace_bytes /
+ * oci_setup) that must outlive the context; the library never allocates
+ * device memory.  One context is not thread-safe; distinct contexts are.
+ *
+ * Return codes: 0 OK; 1 OCI_NOT_CONVERGED (max_iters reached; the state is
+ * still committed); negative = failure, no state change:
+ *   -1 invalid argument   -2 call order   -3 CUDA error
+ *   -4 singular block     -5 workspace too small
+ * No exception crosses the ABI.  oci_last_error() describes the last failure.
+ */
+#ifndef OCI_B200_H
+#define OCI_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct oci_ctx oci_ctx;
+
+enum { OCI_OK = 0, OCI_NOT_CONVERGED = 1, OCI_E_INVALID = -1, OCI_E_ORDER = -2, OCI_E_CUDA = -3,
+       OCI_E_SINGULAR = -4, OCI_E_WORKSPACE = -5 };
+
+/* Boundary conditions (vacuum and reflecting P:31).
+ * INCIDENT_ISOTROPIC: `value` is the incident ANGULAR flux psi_m for every
+ * incoming direction, constant in time, used for both the k and k+1/2
+ * balance equations.  REFLECTING: incident psi_m = outgoing psi_{N-1-m} of the
+ * previous iterate (lagged in both OCI and SI). */
+enum { OCI_BC_VACUUM = 0, OCI_BC_INCIDENT_ISOTROPIC = 1, OCI_BC_REFLECTING = 2 };
+typedef struct { int32_t kind; double value; } oci_bc;
+
+/* Which kernel family oci_setup selected for the OCI apply (eq. 19):
+ * SHARED   - all cells share one (dx, Sigma, Sigma_s): one inverse, applied
+ *            as a dense [4N x 4N].[4N x cells] contraction on the fp64 tensor pipe;
+ * PER_CELL - one inverse per distinct triple, applied as a batched GEMV that
+ *            streams the inverses from HBM. */
+enum { OCI_PATH_SHARED = 0, OCI_PATH_PER_CELL = 1 };
+
+typedef struct {
+    int64_t cells;        /* J */
+    int32_t n_angles;     /* N */
+    int32_t block_dim;    /* n = 4N */
+    int64_t n_blocks;     /* distinct (dx, Sigma, Sigma_s) triples */
+    int32_t path;         /* OCI_PATH_* */
+    int32_t reserved;
+} oci_info;
+
+/* Problem statement (per-cell dx_j, Sigma_j, Sigma_s,j P:74-82).
+ * dx, sigma_t, sigma_s: HOST [cells].  v = particle speed, dt = time step.
+ * n_angles = N (even, >= 2).  Computes the Gauss-Legendre set on the host.
+ * Errors: -1 if cells<1, N odd or <2, any dx<=0, Sigma<0, Sigma_s<0, v<=0,
+ * dt<=0, a NULL pointer or an unknown BC kind. */
+int oci_create(oci_ctx** out, int64_t cells, const double* dx, const double* sigma_t,
+               const double* sigma_s, double v, double dt, int32_t n_angles, oci_bc left,
+               oci_bc right);
+
+/* DEVICE bytes the caller must supply to oci_setup. */
+int64_t oci_workspace_bytes(const oci_ctx* ctx);
+
+/* Form B = A - S (eqs. 13,16,20-22) for every distinct
+ * (dx, Sigma, Sigma_s) triple (bitwise-equal classification), invert each
+ * with partial pivoting on the device (the paper's `gesv`, hoisted out
+ * of the loops), form the 4x4 inverses SI needs, zero the state.
+ * d_workspace: DEVICE, 256-byte aligned, `bytes` >= oci_workspace_bytes().
+ * cuda_stream: a cudaStream_t (as void*) used for every later call, or NULL.
+ * Errors: -3, -4 (a block is singular), -5. */
+int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream);
+
+/* Initial / restart condition psi_{m,0}(x): HOST [cells][N][2] = (L,R)
+ * corner values at the previous time edge t_{k-1/2}.  Also seeds the iterate
+ * (slots 0,2 <- L, slots 1,3 <- R).  A complete checkpoint together with
+ * oci_get_angular_flux()[..][2:4].  _dev: same layout, DEVICE pointer. */
+int oci_set_flux(oci_ctx* ctx, const double* psi_edge);
+int oci_set_flux_dev(oci_ctx* ctx, const double* d_psi_edge);
+
+/* Isotropic source Q: HOST [cells][4] in slot order; NULL = 0; sticky
+ * until the next call.  _dev: DEVICE pointer. */
+int oci_set_source(oci_ctx* ctx, const double* q);
+int oci_set_source_dev(oci_ctx* ctx, const double* d_q);
+
+/* Advance one time step by OCI (oci_step) or SI (si_step): iterate until
+ *     max_{j,s} |phi^(l+1) - phi^(l)| <= tol * max_{j,s} |phi^(l+1)|
+ * over all four scalar-flux slots ("ceases changing"), tested on
+ * the device after every iteration; then commit psi_{k+1/2} as the next
+ * step's psi_{k-1/2}.  tol < 0 never converges: exactly max_iters iterations.
+ * iters (HOST, may be NULL): iterations done.  resid (HOST, may be NULL):
+ * last d/r (d if r == 0).  One host read-back per call (per launch chunk).
+ * Returns 0, 1 (OCI_NOT_CONVERGED), -1, -2, -3. */
+int oci_step(oci_ctx* ctx, double tol, int32_t max_iters, int32_t* iters, double* resid);
+int si_step(oci_ctx* ctx, double tol, int32_t max_iters, int32_t* iters, double* resid);
+
+/* Results of the current state.  phi: [cells][4] (eq. 18);
+ * psi: [cells][N][4].  HOST pointers; _dev variants take DEVICE pointers and
+ * are asynchronous on the context's stream. */
+int oci_get_scalar_flux(const oci_ctx* ctx, double* phi);
+int oci_get_angular_flux(const oci_ctx* ctx, double* psi);
+int oci_get_scalar_flux_dev(const oci_ctx* ctx, double* d_phi);
+int oci_get_angular_flux_dev(const oci_ctx* ctx, double* d_psi);
+
+/* Quadrature in use: HOST mu[N], w[N], ascending mu. */
+int oci_get_quadrature(const oci_ctx* ctx, double* mu, double* w);
+
+/* Problem / path description (valid after oci_create; n_blocks and path after oci_setup). */
+int oci_get_info(const oci_ctx* ctx, oci_info* info);
+
+/* Inverse of block `blk` as computed by oci_setup: HOST [4N][4N] row major
+ * (B^{-1}[i][k]).  For verification of the setup kernel. */
+int oci_get_block_inverse(const oci_ctx* ctx, int64_t blk, double* binv);
+
+/* Kernel timing for roofline reports.  When enabled, every launch of the
+ * OCI apply kernel (eq. 19) is bracketed by CUDA events on the context's
+ * stream; oci_get_kernel_time returns the accumulated milliseconds and launch
+ * count since the last enable and resets them. */
+int oci_enable_kernel_timing(oci_ctx* ctx, int32_t on);
+int oci_get_kernel_time(oci_ctx* ctx, double* ms, int64_t* launches);
+
+/* Number of kernels this library launched on this context so far. */
+int64_t oci_launch_count(const oci_ctx* ctx);
+
+const char* oci_last_error(const oci_ctx* ctx);
+void oci_destroy(oci_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OCI_B200_H */

@@ -1,0 +1,7 @@
+"""B200-native one-cell-inversion (OCI) transient slab S_N transport: thin Python binding over the
+C-ABI library `liboci_b200.so` (include/oci.h).  Argument marshalling only: every step of the path
+runs in the CUDA kernels under csrc/.  PyTorch supplies device memory and the stream, nothing else.
+There is no CPU fallback: importing works without a GPU (so the symbol table can be checked), any
+compute call without the CUDA library or a device raises."""
+from .binding import (OCI, OCIError, BC_VACUUM, BC_INCIDENT_ISOTROPIC, BC_REFLECTING, PATH_SHARED,  # noqa: F401
+                      PATH_PER_CELL, load_library, library_path, EXPORTED_SYMBOLS)

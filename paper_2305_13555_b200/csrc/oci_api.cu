@@ -1,0 +1,513 @@
+// Host driver behind the C ABI of include/oci.h: argument checking, quadrature, block
+// classification, workspace layout, the time-step loop and error
+// reporting.  Every arithmetic step of the path runs in the kernels of this directory.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <unordered_map>
+#include <vector>
+
+#include "oci_internal.h"
+
+namespace oci {
+int launch_oci_generic(const DevView& V, int src, int prev_slot, double tol, cudaStream_t s);
+int launch_oci_percell(const DevView& V, int src, int slot, int prev_slot, double tol, cudaStream_t s);
+int launch_oci_shared_fast(const DevView& V, int src, int slot, int prev_slot, double tol, cudaStream_t s);
+bool oci_shared_fast_supported(const DevView& V);
+}  // namespace oci
+
+using namespace oci;
+
+struct oci_ctx {
+    // problem
+    int64_t J = 0;
+    int32_t N = 0, n = 0;
+    double v = 0, dt = 0;
+    oci_bc bcL{}, bcR{};
+    std::vector<double> dx, sig, sigs, mu, w;
+    // classification
+    std::vector<int32_t> blk;
+    std::vector<int64_t> rep;
+    int64_t nblk = 0;
+    int32_t path = OCI_PATH_SHARED;
+    // device
+    DevView V{};
+    cudaStream_t stream = nullptr;
+    void* ws = nullptr;
+    int64_t ws_bytes = 0;
+    bool ready = false, have_flux = false;
+    int cur = 0;                       // psi[cur] holds the current iterate
+    int32_t predicted[2] = {0, 0};     // last iteration count of oci / si, sizes the launch chunk
+    unsigned long long* h_norms = nullptr;   // pinned
+    // timing
+    bool timing = false;
+    std::vector<cudaEvent_t> ev;
+    double kernel_ms = 0.0;
+    int64_t kernel_launches = 0;
+    int64_t launches = 0;
+    std::string err;
+};
+
+namespace {
+
+int fail(const oci_ctx* c, int code, const std::string& msg)
+{
+    if (c) const_cast<oci_ctx*>(c)->err = msg;
+    return code;
+}
+
+int cuda_fail(const oci_ctx* c, cudaError_t e, const char* where)
+{
+    return fail(c, OCI_E_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+
+#define CK(call)                                                      \
+    do {                                                              \
+        cudaError_t e_ = (call);                                      \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);      \
+    } while (0)
+
+// N-point Gauss-Legendre nodes and weights on [-1,1], ascending (weights sum to 2, the 1/2 of
+// eq. (1)).  Newton on P_N evaluated by the Bonnet recurrence, from the Tricomi initial guess;
+// the negative half is the mirror image of the positive half.
+void gauss_legendre(int N, std::vector<double>& mu, std::vector<double>& w)
+{
+    mu.assign(N, 0.0);
+    w.assign(N, 0.0);
+    const double pi = 3.141592653589793238462643383279502884;
+    for (int i = 0; i < N / 2; ++i) {
+        // i-th positive root counted from the largest
+        double x = (1.0 - (N - 1.0) / (8.0 * N * N * N)) * std::cos(pi * (4.0 * i + 3.0) / (4.0 * N + 2.0));
+        double deriv = 0.0;
+        for (int it = 0; it < 64; ++it) {
+            double pm1 = 1.0, p = x;
+            for (int k = 1; k < N; ++k) {
+                const double pn = ((2 * k + 1) * x * p - k * pm1) / (k + 1);
+                pm1 = p;
+                p = pn;
+            }
+            deriv = N * (pm1 - x * p) / (1.0 - x * x);
+            const double step = p / deriv;
+            x -= step;
+            if (std::fabs(step) <= 1e-16 * std::fabs(x)) {
+                pm1 = 1.0; p = x;
+                for (int k = 1; k < N; ++k) {
+                    const double pn = ((2 * k + 1) * x * p - k * pm1) / (k + 1);
+                    pm1 = p;
+                    p = pn;
+                }
+                deriv = N * (pm1 - x * p) / (1.0 - x * x);
+                break;
+            }
+        }
+        const double wt = 2.0 / ((1.0 - x * x) * deriv * deriv);
+        mu[N - 1 - i] = x;
+        mu[i] = -x;
+        w[N - 1 - i] = wt;
+        w[i] = wt;
+    }
+}
+
+struct Layout {
+    int64_t binv, psi0, psi1, cfix, phi, Q, qs, dx, sig, sigs, blk, rep, mu, w, coef, ainv4, norms, flags, total;
+};
+
+int64_t align_up(int64_t x) { return (x + 255) & ~int64_t(255); }
+
+Layout make_layout(int64_t J, int32_t N, int64_t nblk)
+{
+    const int64_t n = 4 * (int64_t)N;
+    Layout L{};
+    int64_t o = 0;
+    auto take = [&](int64_t bytes) { int64_t at = o; o = align_up(o + bytes); return at; };
+    L.binv = take(nblk * n * n * 8);
+    L.psi0 = take((J + 2) * n * 8);
+    L.psi1 = take((J + 2) * n * 8);
+    L.cfix = take(J * n * 8);
+    L.phi = take(J * 4 * 8);
+    L.Q = take(J * 4 * 8);
+    L.qs = take(J * 4 * 8);
+    L.dx = take(J * 8);
+    L.sig = take(J * 8);
+    L.sigs = take(J * 8);
+    L.blk = take(J * 4);
+    L.rep = take(nblk * 8);
+    L.mu = take(N * 8);
+    L.w = take(N * 8);
+    L.coef = take(n * 8);
+    L.ainv4 = take(nblk * N * 16 * 8);
+    L.norms = take(kNormSlots * 2 * 8);
+    L.flags = take(256);
+    L.total = o;
+    return L;
+}
+
+void classify(oci_ctx* c)
+{
+    struct Key {
+        uint64_t a, b, d;
+        bool operator==(const Key& o) const { return a == o.a && b == o.b && d == o.d; }
+    };
+    struct Hash {
+        size_t operator()(const Key& k) const
+        {
+            uint64_t h = k.a * 0x9E3779B97F4A7C15ull;
+            h ^= (k.b + 0x9E3779B97F4A7C15ull + (h << 6) + (h >> 2));
+            h ^= (k.d + 0x9E3779B97F4A7C15ull + (h << 6) + (h >> 2));
+            return (size_t)h;
+        }
+    };
+    auto bits = [](double x) { uint64_t u; std::memcpy(&u, &x, 8); return u; };
+    std::unordered_map<Key, int32_t, Hash> seen;
+    c->blk.resize(c->J);
+    c->rep.clear();
+    for (int64_t j = 0; j < c->J; ++j) {
+        Key k{bits(c->dx[j]), bits(c->sig[j]), bits(c->sigs[j])};
+        auto it = seen.find(k);
+        if (it == seen.end()) {
+            it = seen.emplace(k, (int32_t)c->rep.size()).first;
+            c->rep.push_back(j);
+        }
+        c->blk[j] = it->second;
+    }
+    c->nblk = (int64_t)c->rep.size();
+    c->path = (c->nblk == 1) ? OCI_PATH_SHARED : OCI_PATH_PER_CELL;
+}
+
+bool bc_ok(const oci_bc& b)
+{
+    return b.kind == OCI_BC_VACUUM || b.kind == OCI_BC_INCIDENT_ISOTROPIC || b.kind == OCI_BC_REFLECTING;
+}
+
+int launch_oci_iteration_any(oci_ctx* ctx, int src, int slot, int prev_slot, double tol)
+{
+    const DevView& V = ctx->V;
+    if (ctx->path == OCI_PATH_PER_CELL) return launch_oci_percell(V, src, slot, prev_slot, tol, ctx->stream);
+    if (oci_shared_fast_supported(V)) return launch_oci_shared_fast(V, src, slot, prev_slot, tol, ctx->stream);
+    int k = launch_oci_generic(V, src, prev_slot, tol, ctx->stream);
+    k += launch_phi_norm(V, src ^ 1, slot, prev_slot, tol, true, ctx->stream);
+    return k;
+}
+
+int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iters, double* resid)
+{
+    if (!ctx) return OCI_E_INVALID;
+    if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "step before oci_setup");
+    if (!ctx->have_flux) return fail(ctx, OCI_E_ORDER, "step before oci_set_flux");
+    if (max_iters < 1 || tol != tol) return fail(ctx, OCI_E_INVALID, "max_iters < 1 or tol is NaN");
+    DevView& V = ctx->V;
+    cudaStream_t s = ctx->stream;
+
+    ctx->launches += launch_cfix(V, ctx->cur, s);                         // a2 (+ a8 of the previous step)
+    int32_t done_iters = 0;
+    bool conv = false;
+    double d = 0.0, r = 0.0;
+    int32_t guess = ctx->predicted[si ? 1 : 0] > 0 ? ctx->predicted[si ? 1 : 0] + 1 : 8;
+    while (done_iters < max_iters && !conv) {
+        int32_t cnt = guess - done_iters;
+        if (cnt < 4) cnt = 4;
+        if (cnt > kNormSlots) cnt = kNormSlots;
+        if (cnt > max_iters - done_iters) cnt = max_iters - done_iters;
+        CK(cudaMemsetAsync(V.norms, 0, sizeof(unsigned long long) * 2 * cnt, s));
+        for (int32_t i = 0; i < cnt; ++i) {
+            if (ctx->timing && !si) CK(cudaEventRecord(ctx->ev[2 * i], s));
+            if (si) ctx->launches += launch_si_iteration(V, ctx->cur, i, i - 1, tol, s);
+            else ctx->launches += launch_oci_iteration_any(ctx, (ctx->cur + done_iters + i) & 1, i, i - 1, tol);
+            if (ctx->timing && !si) CK(cudaEventRecord(ctx->ev[2 * i + 1], s));
+        }
+        CK(cudaMemcpyAsync(ctx->h_norms, V.norms, sizeof(unsigned long long) * 2 * cnt, cudaMemcpyDeviceToHost, s));
+        CK(cudaStreamSynchronize(s));                                       // the one read-back (a7)
+        CK(cudaGetLastError());
+        int32_t executed = cnt;
+        for (int32_t i = 0; i < cnt; ++i) {
+            std::memcpy(&d, &ctx->h_norms[2 * i], 8);
+            std::memcpy(&r, &ctx->h_norms[2 * i + 1], 8);
+            if (converged(tol, d, r)) { conv = true; executed = i + 1; break; }
+        }
+        if (ctx->timing && !si) {
+            for (int32_t i = 0; i < executed; ++i) {
+                float ms = 0.f;
+                CK(cudaEventElapsedTime(&ms, ctx->ev[2 * i], ctx->ev[2 * i + 1]));
+                ctx->kernel_ms += ms;
+                ctx->kernel_launches += 1;
+            }
+        }
+        done_iters += executed;
+    }
+    if (!si) ctx->cur = (ctx->cur + done_iters) & 1;                       // a8: pointer convention
+    ctx->predicted[si ? 1 : 0] = done_iters;
+    if (iters) *iters = done_iters;
+    if (resid) *resid = (r > 0.0) ? d / r : d;
+    return conv ? OCI_OK : OCI_NOT_CONVERGED;
+}
+
+}  // namespace
+
+extern "C" {
+
+int oci_create(oci_ctx** out, int64_t cells, const double* dx, const double* sigma_t, const double* sigma_s,
+               double v, double dt, int32_t n_angles, oci_bc left, oci_bc right)
+{
+    if (!out) return OCI_E_INVALID;
+    *out = nullptr;
+    if (cells < 1 || !dx || !sigma_t || !sigma_s) return OCI_E_INVALID;
+    if (n_angles < 2 || (n_angles & 1) || n_angles > 4096) return OCI_E_INVALID;
+    if (!(v > 0.0) || !(dt > 0.0) || !std::isfinite(v) || !std::isfinite(dt)) return OCI_E_INVALID;
+    if (!bc_ok(left) || !bc_ok(right) || !std::isfinite(left.value) || !std::isfinite(right.value))
+        return OCI_E_INVALID;
+    for (int64_t j = 0; j < cells; ++j)
+        if (!(dx[j] > 0.0) || !(sigma_t[j] >= 0.0) || !(sigma_s[j] >= 0.0) || !std::isfinite(dx[j]) ||
+            !std::isfinite(sigma_t[j]) || !std::isfinite(sigma_s[j]))
+            return OCI_E_INVALID;
+    oci_ctx* c = new (std::nothrow) oci_ctx();
+    if (!c) return OCI_E_INVALID;
+    c->J = cells;
+    c->N = n_angles;
+    c->n = 4 * n_angles;
+    c->v = v;
+    c->dt = dt;
+    c->bcL = left;
+    c->bcR = right;
+    c->dx.assign(dx, dx + cells);
+    c->sig.assign(sigma_t, sigma_t + cells);
+    c->sigs.assign(sigma_s, sigma_s + cells);
+    gauss_legendre(n_angles, c->mu, c->w);
+    classify(c);
+    *out = c;
+    return OCI_OK;
+}
+
+int64_t oci_workspace_bytes(const oci_ctx* ctx)
+{
+    if (!ctx) return 0;
+    return make_layout(ctx->J, ctx->N, ctx->nblk).total;
+}
+
+int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
+{
+    if (!ctx || !d_workspace) return fail(ctx, OCI_E_INVALID, "NULL context or workspace");
+    if (((uintptr_t)d_workspace & 255) != 0) return fail(ctx, OCI_E_INVALID, "workspace not 256-byte aligned");
+    const Layout L = make_layout(ctx->J, ctx->N, ctx->nblk);
+    if (bytes < L.total) return fail(ctx, OCI_E_WORKSPACE, "workspace too small");
+    ctx->ready = false;
+    ctx->have_flux = false;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->ws = d_workspace;
+    ctx->ws_bytes = bytes;
+    char* base = (char*)d_workspace;
+    DevView& V = ctx->V;
+    const int64_t n = ctx->n;
+    V.J = ctx->J; V.N = ctx->N; V.n = ctx->n; V.nblk = ctx->nblk;
+    V.binv = (double*)(base + L.binv);
+    V.psi[0] = (double*)(base + L.psi0) + n;      // skip the left ghost row
+    V.psi[1] = (double*)(base + L.psi1) + n;
+    V.cfix = (double*)(base + L.cfix);
+    V.phi = (double*)(base + L.phi);
+    V.Q = (double*)(base + L.Q);
+    V.qs = (double*)(base + L.qs);
+    V.dx = (double*)(base + L.dx);
+    V.sig = (double*)(base + L.sig);
+    V.sigs = (double*)(base + L.sigs);
+    V.blk = (int32_t*)(base + L.blk);
+    V.rep = (int64_t*)(base + L.rep);
+    V.mu = (double*)(base + L.mu);
+    V.w = (double*)(base + L.w);
+    V.coef = (double*)(base + L.coef);
+    V.ainv4 = (double*)(base + L.ainv4);
+    V.norms = (unsigned long long*)(base + L.norms);
+    V.flags = (int32_t*)(base + L.flags);
+    V.v = ctx->v; V.dt = ctx->dt;
+    V.bcL = ctx->bcL.kind; V.bcR = ctx->bcR.kind;
+    V.bcLv = ctx->bcL.value; V.bcRv = ctx->bcR.value;
+
+    cudaStream_t s = ctx->stream;
+    // coef[4m+s] = |mu_m| on the rows that take an incident flux (eqs. 27,28), else 0
+    std::vector<double> coef(n, 0.0);
+    for (int m = 0; m < ctx->N; ++m) {
+        if (ctx->mu[m] > 0.0) { coef[4 * m + 0] = ctx->mu[m]; coef[4 * m + 2] = ctx->mu[m]; }
+        else { coef[4 * m + 1] = -ctx->mu[m]; coef[4 * m + 3] = -ctx->mu[m]; }
+    }
+    // everything the kernels may read before a set_* call must be finite: zero the state
+    CK(cudaMemsetAsync(base + L.psi0, 0, (size_t)(L.cfix - L.psi0), s));
+    CK(cudaMemsetAsync(base + L.cfix, 0, (size_t)(L.dx - L.cfix), s));
+    CK(cudaMemsetAsync(base + L.norms, 0, (size_t)(L.total - L.norms), s));
+    CK(cudaMemcpyAsync(V.dx, ctx->dx.data(), ctx->J * 8, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(V.sig, ctx->sig.data(), ctx->J * 8, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(V.sigs, ctx->sigs.data(), ctx->J * 8, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(V.blk, ctx->blk.data(), ctx->J * 4, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(V.rep, ctx->rep.data(), ctx->nblk * 8, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(V.mu, ctx->mu.data(), ctx->N * 8, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(V.w, ctx->w.data(), ctx->N * 8, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(V.coef, coef.data(), n * 8, cudaMemcpyHostToDevice, s));
+    CK(cudaStreamSynchronize(s));   // host vectors above are read by the async copies
+
+    ctx->launches += launch_form_and_invert(V, s);                       // a0, a1
+    int32_t flag = 0;
+    CK(cudaMemcpyAsync(&flag, V.flags, 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    CK(cudaGetLastError());
+    if (flag != 0) {
+        char buf[96];
+        std::snprintf(buf, sizeof buf, "block %d is singular", flag - 1);
+        return fail(ctx, OCI_E_SINGULAR, buf);
+    }
+    if (!ctx->h_norms) CK(cudaHostAlloc((void**)&ctx->h_norms, sizeof(unsigned long long) * 2 * kNormSlots, cudaHostAllocDefault));
+    if (ctx->ev.empty()) {
+        ctx->ev.resize(2 * kNormSlots);
+        for (auto& e : ctx->ev) CK(cudaEventCreate(&e));
+    }
+    ctx->cur = 0;
+    ctx->predicted[0] = ctx->predicted[1] = 0;
+    ctx->ready = true;
+    return OCI_OK;
+}
+
+static int set_flux_common(oci_ctx* ctx, const double* d_edge)
+{
+    ctx->launches += launch_set_flux(ctx->V, d_edge, 0, ctx->stream);
+    ctx->cur = 0;
+    ctx->launches += launch_phi_norm(ctx->V, 0, 0, -1, -1.0, false, ctx->stream);   // phi^(0), ghost rows
+    CK(cudaStreamSynchronize(ctx->stream));
+    CK(cudaGetLastError());
+    ctx->have_flux = true;
+    return OCI_OK;
+}
+
+int oci_set_flux(oci_ctx* ctx, const double* psi_edge)
+{
+    if (!ctx || !psi_edge) return fail(ctx, OCI_E_INVALID, "NULL argument");
+    if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_set_flux before oci_setup");
+    // stage through c_fix (recomputed at the start of every step, and at least as large)
+    CK(cudaMemcpyAsync(ctx->V.cfix, psi_edge, (size_t)ctx->J * ctx->N * 2 * 8, cudaMemcpyHostToDevice, ctx->stream));
+    return set_flux_common(ctx, ctx->V.cfix);
+}
+
+int oci_set_flux_dev(oci_ctx* ctx, const double* d_psi_edge)
+{
+    if (!ctx || !d_psi_edge) return fail(ctx, OCI_E_INVALID, "NULL argument");
+    if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_set_flux_dev before oci_setup");
+    return set_flux_common(ctx, d_psi_edge);
+}
+
+int oci_set_source(oci_ctx* ctx, const double* q)
+{
+    if (!ctx) return OCI_E_INVALID;
+    if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_set_source before oci_setup");
+    if (q) CK(cudaMemcpyAsync(ctx->V.Q, q, (size_t)ctx->J * 4 * 8, cudaMemcpyHostToDevice, ctx->stream));
+    else CK(cudaMemsetAsync(ctx->V.Q, 0, (size_t)ctx->J * 4 * 8, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return OCI_OK;
+}
+
+int oci_set_source_dev(oci_ctx* ctx, const double* d_q)
+{
+    if (!ctx) return OCI_E_INVALID;
+    if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_set_source_dev before oci_setup");
+    if (d_q) CK(cudaMemcpyAsync(ctx->V.Q, d_q, (size_t)ctx->J * 4 * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+    else CK(cudaMemsetAsync(ctx->V.Q, 0, (size_t)ctx->J * 4 * 8, ctx->stream));
+    return OCI_OK;
+}
+
+int oci_step(oci_ctx* ctx, double tol, int32_t max_iters, int32_t* iters, double* resid)
+{
+    return run_step(ctx, false, tol, max_iters, iters, resid);
+}
+
+int si_step(oci_ctx* ctx, double tol, int32_t max_iters, int32_t* iters, double* resid)
+{
+    return run_step(ctx, true, tol, max_iters, iters, resid);
+}
+
+static int get_common(const oci_ctx* ctx, double* dst, const double* src, size_t bytes, cudaMemcpyKind kind, bool sync)
+{
+    if (!ctx || !dst) return fail(ctx, OCI_E_INVALID, "NULL argument");
+    if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "get before oci_setup");
+    CK(cudaMemcpyAsync(dst, src, bytes, kind, ctx->stream));
+    if (sync) CK(cudaStreamSynchronize(ctx->stream));
+    return OCI_OK;
+}
+
+int oci_get_scalar_flux(const oci_ctx* ctx, double* phi)
+{
+    return get_common(ctx, phi, ctx ? ctx->V.phi : nullptr, ctx ? (size_t)ctx->J * 32 : 0, cudaMemcpyDeviceToHost, true);
+}
+int oci_get_angular_flux(const oci_ctx* ctx, double* psi)
+{
+    return get_common(ctx, psi, ctx ? ctx->V.psi[ctx->cur] : nullptr, ctx ? (size_t)ctx->J * ctx->n * 8 : 0,
+                      cudaMemcpyDeviceToHost, true);
+}
+int oci_get_scalar_flux_dev(const oci_ctx* ctx, double* d_phi)
+{
+    return get_common(ctx, d_phi, ctx ? ctx->V.phi : nullptr, ctx ? (size_t)ctx->J * 32 : 0, cudaMemcpyDeviceToDevice, false);
+}
+int oci_get_angular_flux_dev(const oci_ctx* ctx, double* d_psi)
+{
+    return get_common(ctx, d_psi, ctx ? ctx->V.psi[ctx->cur] : nullptr, ctx ? (size_t)ctx->J * ctx->n * 8 : 0,
+                      cudaMemcpyDeviceToDevice, false);
+}
+
+int oci_get_quadrature(const oci_ctx* ctx, double* mu, double* w)
+{
+    if (!ctx || !mu || !w) return fail(ctx, OCI_E_INVALID, "NULL argument");
+    std::memcpy(mu, ctx->mu.data(), ctx->N * 8);
+    std::memcpy(w, ctx->w.data(), ctx->N * 8);
+    return OCI_OK;
+}
+
+int oci_get_info(const oci_ctx* ctx, oci_info* info)
+{
+    if (!ctx || !info) return fail(ctx, OCI_E_INVALID, "NULL argument");
+    info->cells = ctx->J;
+    info->n_angles = ctx->N;
+    info->block_dim = ctx->n;
+    info->n_blocks = ctx->nblk;
+    info->path = ctx->path;
+    info->reserved = 0;
+    return OCI_OK;
+}
+
+int oci_get_block_inverse(const oci_ctx* ctx, int64_t blk, double* binv)
+{
+    if (!ctx || !binv) return fail(ctx, OCI_E_INVALID, "NULL argument");
+    if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_get_block_inverse before oci_setup");
+    if (blk < 0 || blk >= ctx->nblk) return fail(ctx, OCI_E_INVALID, "block index out of range");
+    const size_t nn = (size_t)ctx->n * ctx->n;
+    CK(cudaMemcpyAsync(binv, ctx->V.binv + (size_t)blk * nn, nn * 8, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return OCI_OK;
+}
+
+int oci_enable_kernel_timing(oci_ctx* ctx, int32_t on)
+{
+    if (!ctx) return OCI_E_INVALID;
+    ctx->timing = on != 0;
+    ctx->kernel_ms = 0.0;
+    ctx->kernel_launches = 0;
+    return OCI_OK;
+}
+
+int oci_get_kernel_time(oci_ctx* ctx, double* ms, int64_t* launches)
+{
+    if (!ctx) return OCI_E_INVALID;
+    if (ms) *ms = ctx->kernel_ms;
+    if (launches) *launches = ctx->kernel_launches;
+    ctx->kernel_ms = 0.0;
+    ctx->kernel_launches = 0;
+    return OCI_OK;
+}
+
+int64_t oci_launch_count(const oci_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+const char* oci_last_error(const oci_ctx* ctx) { return ctx ? ctx->err.c_str() : "NULL context"; }
+
+void oci_destroy(oci_ctx* ctx)
+{
+    if (!ctx) return;
+    if (ctx->h_norms) cudaFreeHost(ctx->h_norms);
+    for (auto& e : ctx->ev) cudaEventDestroy(e);
+    delete ctx;
+}
+
+}  // extern "C"

@@ -1,0 +1,58 @@
+// Internal declarations shared by the host driver (oci_api.cu) and the kernels.
+// Not part of the C ABI (include/oci.h is).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "oci.h"
+
+namespace oci {
+
+constexpr int kNormSlots = 64;  // iterations launched between two host read-backs, at most
+
+// Device-side view of one problem.  Passed to kernels by value.
+// Psi buffers have one ghost row before row 0 and one after row J-1: psi[b]
+// points at row 0, rows -1 and J hold the boundary data in the slots a
+// neighbour cell would occupy, so the iteration kernels need no boundary
+// branches.
+struct DevView {
+    int64_t J;
+    int32_t N;
+    int32_t n;                  // 4N
+    int64_t nblk;
+    double* binv;               // [nblk][n][n]  B^{-1}, row major
+    double* psi[2];             // ping-pong iterates, [(J+2)][n] each
+    double* cfix;               // [J][n]   iteration-invariant part of the RHS (a2)
+    double* phi;                // [J][4]
+    double* Q;                  // [J][4]
+    double* qs;                 // [J][4]   SI scattering source (d1)
+    double* dx;                 // [J]
+    double* sig;                // [J]
+    double* sigs;               // [J]
+    int32_t* blk;               // [J] -> block id
+    int64_t* rep;               // [nblk] -> a representative cell
+    double* mu;                 // [N]
+    double* w;                  // [N]
+    double* coef;               // [n]  |mu_m| on the rows that take an incident flux, else 0
+    double* ainv4;              // [nblk][N][16]  (A_m)^{-1} for SI
+    unsigned long long* norms;  // [kNormSlots][2]  bit patterns of (d, r), atomicMax targets
+    int32_t* flags;             // [0] = 1 + index of a singular block, 0 if none
+    double v, dt;
+    int32_t bcL, bcR;
+    double bcLv, bcRv;
+};
+
+// The stopping rule (reading S2), evaluated identically on host and device.
+__host__ __device__ inline bool converged(double tol, double d, double r) { return tol >= 0.0 && d <= tol * r; }
+
+// ---- launchers (each returns the number of kernels it launched) ----
+int launch_form_and_invert(const DevView& V, cudaStream_t s);
+int launch_set_flux(const DevView& V, const double* d_psi_edge, int buf, cudaStream_t s);
+int launch_cfix(const DevView& V, int buf, cudaStream_t s);
+int launch_phi_norm(const DevView& V, int buf, int slot, int prev_slot, double tol, bool with_norms,
+                    cudaStream_t s);
+int launch_oci_iteration(const DevView& V, int path, int src, int slot, int prev_slot, double tol,
+                         cudaStream_t s);
+int launch_si_iteration(const DevView& V, int buf, int slot, int prev_slot, double tol, cudaStream_t s);
+
+}  // namespace oci
