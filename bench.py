@@ -1,0 +1,374 @@
+#!/usr/bin/env python
+"""bench.py — OCI unknown-updates/s and time-to-converge per time step on one B200 (BASELINE.json).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: one `oci_step`
+(c_fix, all OCI iterations to tol 1e-10 on the scalar flux with the device-side stop, commit) of
+the headline workload, config 3 of BASELINE.json (S32, 131,072 cells: the largest in unknowns, the
+shared-block tensor path).  The other configs are parity-test cases; a compact per-config table
+(OCI and the GPU SI comparator, S4..S128) rides along in `per_config` because the metric is quoted
+"S4-S128", but the headline `value` is config 3 (or --config).
+
+Timing: W untimed warm-up steps, state reset to the initial condition (untimed), then exactly K
+steps between CUDA events on the library's stream, barrier + synchronize on both sides, max over
+ranks.  The working set (three 128 MiB arrays) is larger than the 126 MB L2.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded
+sample of the same workload; see DESIGN.md "Measurement".
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from workloads import make_problem  # noqa: E402
+
+METRIC = "oci_unknown_updates_per_s"
+UNIT = "unknown-updates/s"
+
+# DRAM traffic per launch of the dominant kernel from the committed `ncu --set full` capture
+# (profiles/), bytes; None until a capture exists for that kernel.
+NCU_TRAFFIC_BYTES = {}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+# ------------------------------------------------------------------------------------------ oracle arm
+def oracle_sample_problem(cfg):
+    """A bounded sample of config `cfg` for the CPU oracle (about 10-30 s of CPU work per run)."""
+    sample = {1: None, 2: None, 3: 32768, 4: 2048, 5: 512}[cfg]
+    p = make_problem(cfg, cells=sample)
+    desc = (f"config {cfg} at full size" if sample is None else
+            f"config {cfg} with the first {sample} of {FULL_CELLS[cfg]} cells (same materials, angles, dt, BCs)")
+    return p, desc
+
+
+FULL_CELLS = {1: 20, 2: 1000, 3: 131072, 4: 16384, 5: 4096}
+
+
+def time_oracle(cfg, steps, warmup, threads):
+    from oracle import Oracle
+    p, desc = oracle_sample_problem(cfg)
+    o = Oracle.from_problem(p, threads=threads)
+    for k in range(warmup):
+        o.set_source(p.source(k))
+        o.oci_step(p.tol, p.max_iters)
+    o.set_flux(p.psi0)
+    updates, iters = 0, []
+    t0 = time.perf_counter()
+    for k in range(steps):
+        o.set_source(p.source(k))
+        st, it, _ = o.oci_step(p.tol, p.max_iters)
+        updates += p.unknowns * it
+        iters.append(it)
+    dt = time.perf_counter() - t0
+    return dict(value=updates / dt, seconds=dt, iters=iters, sample=f"{desc}, {steps} time steps, OCI to tol {p.tol:g}",
+                ms_per_step=dt / steps * 1e3, cells=p.cells)
+
+
+def run_reference(args):
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return 0
+    from oracle import threads_available
+    threads = threads_available()
+    steps = max(1, min(args.steps, 2)) if args.config in (3, 4, 5) else args.steps
+    r = time_oracle(args.config, steps, min(args.warmup, 1), threads)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": make_problem(args.config, cells=1).name, "note": "CPU oracle on a bounded sample"},
+        "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": threads, "kind": "oracle", "sample": r["sample"]},
+        "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "iters_per_step": r["iters"],
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------ GPU arm
+def time_gpu_steps(torch, g, p, steps, scheme, sampler=None, barrier=None):
+    """Reset to the IC (untimed), then time exactly `steps` steps with CUDA events on the library's
+    (= torch's current) stream.  Returns (ms, iters list)."""
+    g.set_flux(p.psi0)
+    qdev = {}
+    for k in range(steps):                      # inputs resident in HBM before the timed region
+        q = p.source(k)
+        if q is not None and id(q) not in qdev:
+            qdev[id(q)] = torch.from_numpy(np.ascontiguousarray(q)).cuda()
+    step = g.oci_step if scheme == "oci" else g.si_step
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if barrier:
+        barrier()
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.start()
+    iters = []
+    e0.record()
+    for k in range(steps):
+        q = p.source(k)
+        g.set_source_dev(qdev[id(q)] if q is not None else None)
+        st, it, _ = step(p.tol, p.max_iters)
+        iters.append(it)
+    e1.record()
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    return e0.elapsed_time(e1), iters
+
+
+def time_gpu_e2e(torch, g, p, steps):
+    """Same K steps through the C ABI with HOST buffers: the initial condition and every step's
+    source are copied host->device from pinned memory and every step's scalar flux is read back,
+    all inside the timed region."""
+    psi0 = torch.from_numpy(np.ascontiguousarray(p.psi0)).pin_memory()
+    qpin = {}
+    for k in range(steps):
+        q = p.source(k)
+        if q is not None and id(q) not in qpin:
+            qpin[id(q)] = torch.from_numpy(np.ascontiguousarray(q)).pin_memory()
+    phi = torch.empty((p.cells, 4), dtype=torch.float64).pin_memory()
+    h2d = psi0.numel() * 8
+    d2h = 0
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    g.set_flux(psi0.numpy())
+    updates = 0
+    for k in range(steps):
+        q = p.source(k)
+        g.set_source(qpin[id(q)].numpy() if q is not None else None)
+        h2d += p.cells * 32 if q is not None else 0
+        st, it, _ = g.oci_step(p.tol, p.max_iters)
+        updates += p.unknowns * it
+        g.get_scalar_flux(out=phi.numpy())
+        d2h += p.cells * 32
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    return updates / (ms * 1e-3), h2d / steps, d2h / steps
+
+
+def per_config_table(torch, P, skip=None):
+    """OCI vs the GPU SI comparator for every BASELINE config (each for its own number of steps)."""
+    out = {}
+    for cfg in (1, 2, 3, 4, 5):
+        p = make_problem(cfg)
+        g = P.OCI.from_problem(p)
+        row = {"S_N": p.n_angles, "cells": p.cells, "path": "shared" if g.get_info()["path"] == 0 else "per_cell"}
+        for scheme in ("oci", "si"):
+            for k in range(2):                   # warm-up
+                g.set_source(p.source(k))
+                (g.oci_step if scheme == "oci" else g.si_step)(p.tol, p.max_iters)
+            ms, iters = time_gpu_steps(torch, g, p, p.n_steps, scheme)
+            row[f"{scheme}_ms_per_step"] = ms / p.n_steps
+            row[f"{scheme}_iters"] = iters
+            row[f"{scheme}_updates_per_s"] = p.unknowns * sum(iters) / (ms * 1e-3)
+        row["si_over_oci_time"] = row["si_ms_per_step"] / row["oci_ms_per_step"]
+        out[f"cfg{cfg}"] = row
+        g.close()
+        del g
+        torch.cuda.empty_cache()
+    return out
+
+
+def run_ours(args):
+    import torch
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        print(json.dumps({"error": "no CUDA device; this benchmark has no CPU fallback"}))
+        return 1
+    torch.cuda.set_device(local)
+    import paper_2305_13555_b200 as P
+    barrier = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+        barrier = dist.barrier
+
+    peaks, peak_src = load_peaks()
+    p = make_problem(args.config)
+    g = P.OCI.from_problem(p, device=f"cuda:{local}")
+    info = g.get_info()
+    shared = info["path"] == P.PATH_SHARED
+    n = info["block_dim"]
+
+    # warm-up steps (untimed)
+    for k in range(args.warmup):
+        g.set_source(p.source(k))
+        g.oci_step(p.tol, p.max_iters)
+
+    # ---- headline: K steps, inputs resident in HBM
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = g.launch_count()
+    ms, iters = time_gpu_steps(torch, g, p, args.steps, "oci", sampler, barrier)
+    launches = g.launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    updates = p.unknowns * sum(iters)
+    if world > 1:
+        import torch.distributed as dist
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        u = torch.tensor([float(updates)], dtype=torch.float64, device="cuda")
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+        updates = float(u.item())
+    value = updates / (ms * 1e-3)
+
+    # ---- the dominant kernel alone (events around every OCI apply launch, same steps again)
+    g.enable_kernel_timing(True)
+    _, iters2 = time_gpu_steps(torch, g, p, args.steps, "oci")
+    kms, klaunch = g.get_kernel_time()
+    g.enable_kernel_timing(False)
+    k_avg_ms = kms / max(klaunch, 1)
+    if shared:
+        flops = 2.0 * n * n * p.cells
+        peak_live = P.probe_fp64_tensor_tflops(f"cuda:{local}")
+        nominal_ratio = 45.0 / 2250.0        # guide: B200 fp64 tensor 45 TF vs bf16 2250 TF nominal
+        peak_scaled = peaks["bf16_tflops"] * nominal_ratio
+        peak = max(peak_live, peak_scaled)
+        achieved = flops / (k_avg_ms * 1e-3) * 1e-12
+        roofline = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                    "traffic": NCU_TRAFFIC_BYTES.get(args.config),
+                    "kernel": "oci apply (eq. 19), fp64 DMMA", "algorithmic_flops_per_launch": flops,
+                    "avg_launch_ms": k_avg_ms, "launches_timed": klaunch,
+                    "peak_source": f"max(live DMMA issue-rate probe {peak_live:.2f}, MEASURED_PEAKS bf16 {peak_src} x 45/2250 = {peak_scaled:.2f})"}
+    else:
+        bytes_ = p.cells * (n * n * 8.0 + 4.0 * n * 8.0 + 64.0)   # inverse + c_fix, 2 half rows, Psi out; phi
+        achieved = bytes_ / (k_avg_ms * 1e-3) * 1e-9
+        roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "frac": achieved / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get(args.config),
+                    "kernel": "oci apply (eq. 19), batched GEMV", "algorithmic_bytes_per_launch": bytes_,
+                    "avg_launch_ms": k_avg_ms, "launches_timed": klaunch, "peak_source": f"MEASURED_PEAKS hbm_gbs ({peak_src})"}
+
+    # ---- end to end through the C ABI with host buffers
+    e2e_val, h2d, d2h = time_gpu_e2e(torch, g, p, args.steps)
+    if world > 1:
+        import torch.distributed as dist
+        t = torch.tensor([e2e_val], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        e2e_val = float(t.item())
+    g.close()
+    del g
+    torch.cuda.empty_cache()
+
+    line = None
+    if rank == 0:
+        per_cfg = per_config_table(torch, P) if (world == 1 and not args.no_table) else None
+        cpu = None
+        if world == 1 and not args.no_cpu:
+            from oracle import threads_available
+            th = threads_available()
+            r = time_oracle(args.config, 1 if args.config in (3, 4, 5) else 5, 0, th)
+            cpu = {"value": r["value"], "unit": UNIT, "cores": th, "kind": "oracle", "sample": r["sample"],
+                   "ms_per_step_on_sample": r["ms_per_step"], "sample_cells": r["cells"]}
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": p.name, "S_N": p.n_angles, "cells": p.cells, "unknowns": p.unknowns, "tol": p.tol,
+                       "path": "shared" if shared else "per_cell", "parallelism": f"replicas x{world}" if world > 1 else "1 gpu",
+                       "l2": "working set larger than L2 (3 x %.0f MiB)" % (p.unknowns * 8 / 2**20) if p.unknowns * 24 > 126e6 else "flushed by per-step c_fix rewrite; working set fits L2"},
+            "iters_per_step": iters, "time_to_converge_ms_per_step": ms / args.steps,
+            "roofline": roofline, "cpu_baseline": cpu,
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "gpu_launches": int(launches), "clocks": clocks, "per_config": per_cfg,
+        }
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-table", action="store_true", help="skip the per-config OCI/SI table")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -140,6 +140,11 @@ int oci_get_block_inverse(const oci_ctx* ctx, int64_t blk, double* binv);
 int oci_enable_kernel_timing(oci_ctx* ctx, int32_t on);
 int oci_get_kernel_time(oci_ctx* ctx, double* ms, int64_t* launches);
 
+/* Roofline denominator for the SHARED path: sustained fp64 tensor-pipe (DMMA) issue rate of the
+ * current device in TFLOP/s, measured by a registers-only probe kernel (about 0.1 s).
+ * d_scratch: DEVICE, >= 8 bytes.  cuda_stream: cudaStream_t or NULL.  No context needed. */
+int oci_probe_fp64_tensor_tflops(void* d_scratch, void* cuda_stream, double* tflops);
+
 /* Number of kernels this library launched on this context so far. */
 int64_t oci_launch_count(const oci_ctx* ctx);
 

@@ -16,7 +16,7 @@ EXPORTED_SYMBOLS = [
     "oci_set_source_dev", "oci_step", "si_step", "oci_get_scalar_flux", "oci_get_angular_flux",
     "oci_get_scalar_flux_dev", "oci_get_angular_flux_dev", "oci_get_quadrature", "oci_get_info",
     "oci_get_block_inverse", "oci_enable_kernel_timing", "oci_get_kernel_time", "oci_launch_count",
-    "oci_last_error", "oci_destroy",
+    "oci_probe_fp64_tensor_tflops", "oci_last_error", "oci_destroy",
 ]
 
 
@@ -81,6 +81,8 @@ def load_library():
     L.oci_enable_kernel_timing.argtypes = [vp, i32]
     L.oci_get_kernel_time.restype = C.c_int
     L.oci_get_kernel_time.argtypes = [vp, _dp, C.POINTER(i64)]
+    L.oci_probe_fp64_tensor_tflops.restype = C.c_int
+    L.oci_probe_fp64_tensor_tflops.argtypes = [vp, vp, _dp]
     L.oci_launch_count.restype = i64
     L.oci_launch_count.argtypes = [vp]
     L.oci_last_error.restype = C.c_char_p
@@ -93,6 +95,21 @@ def load_library():
 
 def _hp(a):
     return a.ctypes.data_as(_dp)
+
+
+def probe_fp64_tensor_tflops(device="cuda:0") -> float:
+    """oci_probe_fp64_tensor_tflops on torch's current stream."""
+    import torch
+    L = load_library()
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        scratch = torch.zeros(8, dtype=torch.float64, device=dev)
+        out = C.c_double(0.0)
+        rc = L.oci_probe_fp64_tensor_tflops(C.c_void_p(scratch.data_ptr()),
+                                            C.c_void_p(torch.cuda.current_stream(dev).cuda_stream), C.byref(out))
+        if rc != 0:
+            raise OCIError(rc, "oci_probe_fp64_tensor_tflops failed")
+    return out.value
 
 
 class OCI:
@@ -193,8 +210,9 @@ class OCI:
     def si_step(self, tol=1e-10, max_iters=10_000):
         return self._step(self._L.si_step, tol, max_iters)
 
-    def get_scalar_flux(self):
-        a = np.empty((self.cells, 4))
+    def get_scalar_flux(self, out=None):
+        a = np.empty((self.cells, 4)) if out is None else out
+        assert a.dtype == np.float64 and a.flags.c_contiguous and a.shape == (self.cells, 4)
         self._check(self._L.oci_get_scalar_flux(self._h, _hp(a)))
         return a
 

@@ -1,0 +1,55 @@
+// fp64 tensor-pipe (DMMA.8x8x4) issue-rate probe: the roofline denominator for the shared-block
+// path, measured live on the device bench.py runs on (MEASURED_PEAKS.json carries no fp64 figure).
+// 16 warps x 2 CTAs per SM, 8 independent accumulator chains per warp, registers only.
+#include <cstdio>
+
+#include "device_utils.cuh"
+
+namespace oci {
+
+__global__ void __launch_bounds__(512) dmma_issue_kernel(double* out, int iters, double a0, double b0)
+{
+    double acc[8][2];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { acc[i][0] = threadIdx.x * 1e-9; acc[i][1] = i * 1e-9; }
+    const double a = a0 + threadIdx.x * 1e-12, b = b0;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) dmma(acc[i][0], acc[i][1], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += acc[i][0] + acc[i][1];
+    if (s == 123.456) out[0] = s;   // keep the chains alive without a store in the common case
+}
+
+}  // namespace oci
+
+extern "C" int oci_probe_fp64_tensor_tflops(void* d_scratch, void* cuda_stream, double* tflops)
+{
+    if (!tflops || !d_scratch) return OCI_E_INVALID;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return OCI_E_CUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return OCI_E_CUDA;
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return OCI_E_CUDA;
+    const int iters = 40000, grid = sms * 2;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0, s);
+        oci::dmma_issue_kernel<<<grid, 512, 0, s>>>((double*)d_scratch, iters, 1.0000001, 0.9999999);
+        cudaEventRecord(e1, s);
+        if (cudaEventSynchronize(e1) != cudaSuccess) return OCI_E_CUDA;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double fl = 2.0 * 256.0 * 8.0 * (double)iters * 16.0 * grid;
+        const double tf = fl / (ms * 1e-3) * 1e-12;
+        if (rep > 0 && tf > best) best = tf;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (cudaGetLastError() != cudaSuccess) return OCI_E_CUDA;
+    *tflops = best;
+    return OCI_OK;
+}
