@@ -40,6 +40,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [nvcc] + NVCC_FLAGS + ["-I", os.path.join(ROOT, "include"), "-I", CSRC]
     if verbose:
         cmd += ["-Xptxas", "-v"]
+    cmd += os.environ.get("OCI_NVCC_EXTRA", "").split()
     cmd += ["-o", LIB] + sources()
     subprocess.check_call(cmd)
     return LIB
