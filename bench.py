@@ -49,53 +49,102 @@ def load_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    """SM clock and throttle reasons DURING the timed region (B200_PROFILING.md recipe).  The timed
+    region is only milliseconds long, so NVML is polled in-process from a thread (every ~2 ms);
+    `nvidia-smi -lms` is the fallback when the NVML binding is missing."""
+
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
 
     def __init__(self, index):
-        self.index, self.proc, self.lines = index, None, []
-
-    def start(self):
-        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-             "clocks_event_reasons.sw_power_cap")
+        self.index, self.sm, self.bits, self.power = index, [], 0, []
+        self.stop_flag, self.thread, self.proc, self.lines, self.h, self.nv = False, None, None, [], None, None
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.t = threading.Thread(target=self._read, daemon=True)
-            self.t.start()
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = index
+            if vis:
+                ent = vis.split(",")[index].strip()
+                phys = int(ent) if ent.isdigit() else index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.nv = pynvml
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
         except Exception:
-            self.proc = None
+            self.h = None
+
+    def _poll(self):
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                self.sm.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                self.bits |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            time.sleep(0.002)
 
     def _read(self):
         for line in self.proc.stdout:
             self.lines.append(line.strip())
 
-    def stop(self):
-        if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
+    def start(self):
+        self.stop_flag = False
+        if self.h is not None:
+            self.thread = threading.Thread(target=self._poll, daemon=True)
+            self.thread.start()
+            return
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
         try:
-            self.proc.wait(timeout=2)
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}",
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
         except Exception:
-            self.proc.kill()
-        sm, mx, reasons = [], [], set()
+            self.proc = None
+
+    def pause(self):
+        """Stop sampling (end of a timed region); start() resumes and keeps accumulating."""
+        self.stop_flag = True
+        if self.h is not None and self.thread:
+            self.thread.join(timeout=1)
+            self.thread = None
+        elif self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+            self._parse_smi()
+            self.proc = None
+
+    def _parse_smi(self):
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        inv = {v: k for k, v in self.REASONS.items()}
         for ln in self.lines:
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 7:
                 continue
             try:
-                sm.append(float(f[0]))
-                mx.append(float(f[1]))
+                self.sm.append(float(f[0]))
+                self.max_mhz = float(f[1])
+                self.power.append(float(f[2]))
             except ValueError:
                 continue
             for nm, val in zip(names, f[3:7]):
                 if val.lower().startswith("active"):
-                    reasons.add(nm)
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+                    self.bits |= inv[nm]
+        self.lines = []
+
+    def result(self, note=""):
+        if self.h is None and not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "samples": 0, "reasons": ["clock sampling unavailable"]}
+        reasons = sorted(nm for bit, nm in self.REASONS.items() if self.bits & bit)
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": getattr(self, "max_mhz", None),
+                "samples": len(self.sm), "power_w_max": max(self.power) if self.power else None,
+                "reasons": reasons, "how": ("NVML polled in-process" if self.h is not None else "nvidia-smi -lms 20") + note}
 
 
 def dist_env():
@@ -185,6 +234,8 @@ def time_gpu_steps(torch, g, p, steps, scheme, sampler=None, barrier=None):
         iters.append(it)
     e1.record()
     torch.cuda.synchronize()
+    if sampler:
+        sampler.pause()
     if barrier:
         barrier()
     return e0.elapsed_time(e1), iters
@@ -276,7 +327,6 @@ def run_ours(args):
     l0 = g.launch_count()
     ms, iters = time_gpu_steps(torch, g, p, args.steps, "oci", sampler, barrier)
     launches = g.launch_count() - l0
-    clocks = sampler.stop() if sampler else None
     updates = p.unknowns * sum(iters)
     if world > 1:
         import torch.distributed as dist
@@ -290,7 +340,8 @@ def run_ours(args):
 
     # ---- the dominant kernel alone (events around every OCI apply launch, same steps again)
     g.enable_kernel_timing(True)
-    _, iters2 = time_gpu_steps(torch, g, p, args.steps, "oci")
+    _, iters2 = time_gpu_steps(torch, g, p, args.steps, "oci", sampler)
+    clocks = sampler.result(" during the headline and the per-kernel timed regions") if sampler else None
     kms, klaunch = g.get_kernel_time()
     g.enable_kernel_timing(False)
     k_avg_ms = kms / max(klaunch, 1)
