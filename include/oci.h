@@ -62,13 +62,21 @@ typedef struct { int32_t kind; double value; } oci_bc;
  *            streams the inverses from HBM. */
 enum { OCI_PATH_SHARED = 0, OCI_PATH_PER_CELL = 1 };
 
+/* Which apply kernel serves that path for this block size (informational; valid after oci_setup):
+ * GENERIC  - any n, shared block, simple shared-memory tiles;
+ * RESIDENT - shared block, n in {64,128}: B^{-1} resident in registers, cells streamed by TMA;
+ * KTILED   - shared block, n a multiple of 32 up to 1024: both operands streamed in K chunks by
+ *            tensor-map TMA from L2 (config 4, n = 512);
+ * PER_CELL - batched GEMV streaming one inverse per cell from HBM. */
+enum { OCI_KERNEL_GENERIC = 0, OCI_KERNEL_RESIDENT = 1, OCI_KERNEL_KTILED = 2, OCI_KERNEL_PER_CELL = 3 };
+
 typedef struct {
     int64_t cells;        /* J */
     int32_t n_angles;     /* N */
     int32_t block_dim;    /* n = 4N */
     int64_t n_blocks;     /* distinct (dx, Sigma, Sigma_s) triples */
     int32_t path;         /* OCI_PATH_* */
-    int32_t reserved;
+    int32_t apply_kernel; /* OCI_KERNEL_* */
 } oci_info;
 
 /* Problem statement (per-cell dx_j, Sigma_j, Sigma_s,j P:74-82).

@@ -10,6 +10,7 @@ from . import build as _build
 
 BC_VACUUM, BC_INCIDENT_ISOTROPIC, BC_REFLECTING = 0, 1, 2
 PATH_SHARED, PATH_PER_CELL = 0, 1
+KERNEL_GENERIC, KERNEL_RESIDENT, KERNEL_KTILED, KERNEL_PER_CELL = 0, 1, 2, 3
 
 EXPORTED_SYMBOLS = [
     "oci_create", "oci_workspace_bytes", "oci_setup", "oci_set_flux", "oci_set_flux_dev", "oci_set_source",
@@ -32,7 +33,7 @@ class _bc(C.Structure):
 
 class _info(C.Structure):
     _fields_ = [("cells", C.c_int64), ("n_angles", C.c_int32), ("block_dim", C.c_int32),
-                ("n_blocks", C.c_int64), ("path", C.c_int32), ("reserved", C.c_int32)]
+                ("n_blocks", C.c_int64), ("path", C.c_int32), ("apply_kernel", C.c_int32)]
 
 
 _dp = C.POINTER(C.c_double)
@@ -235,7 +236,8 @@ class OCI:
     def get_info(self):
         i = _info()
         self._check(self._L.oci_get_info(self._h, C.byref(i)))
-        return dict(cells=i.cells, n_angles=i.n_angles, block_dim=i.block_dim, n_blocks=i.n_blocks, path=i.path)
+        return dict(cells=i.cells, n_angles=i.n_angles, block_dim=i.block_dim, n_blocks=i.n_blocks, path=i.path,
+                    apply_kernel=i.apply_kernel)
 
     def get_block_inverse(self, blk=0):
         n = 4 * self.n_angles

@@ -16,6 +16,9 @@ int launch_oci_generic(const DevView& V, int src, int prev_slot, double tol, cud
 int launch_oci_percell(const DevView& V, int src, int slot, int prev_slot, double tol, cudaStream_t s);
 int launch_oci_shared_fast(const DevView& V, int src, int slot, int prev_slot, double tol, cudaStream_t s);
 bool oci_shared_fast_supported(const DevView& V);
+bool oci_ktiled_supported(const DevView& V);
+bool oci_ktiled_prepare(const DevView& V, KtiledMaps* M);
+int launch_oci_ktiled(const DevView& V, const KtiledMaps& M, int src, int slot, int prev_slot, double tol, cudaStream_t s);
 }  // namespace oci
 
 using namespace oci;
@@ -34,6 +37,8 @@ struct oci_ctx {
     int32_t path = OCI_PATH_SHARED;
     // device
     DevView V{};
+    alignas(64) KtiledMaps maps{};
+    bool use_ktiled = false;
     cudaStream_t stream = nullptr;
     void* ws = nullptr;
     int64_t ws_bytes = 0;
@@ -111,7 +116,7 @@ void gauss_legendre(int N, std::vector<double>& mu, std::vector<double>& w)
 }
 
 struct Layout {
-    int64_t binv, psi0, psi1, cfix, phi, Q, qs, dx, sig, sigs, blk, rep, mu, w, coef, ainv4, norms, flags, total;
+    int64_t binv, psi0, psi1, cfix, phi, Q, qs, dx, sig, sigs, blk, rep, mu, w, coef, ainv4, phi_part, norms, tickets, flags, total;
 };
 
 int64_t align_up(int64_t x) { return (x + 255) & ~int64_t(255); }
@@ -138,7 +143,9 @@ Layout make_layout(int64_t J, int32_t N, int64_t nblk)
     L.w = take(N * 8);
     L.coef = take(n * 8);
     L.ainv4 = take(nblk * N * 16 * 8);
+    L.phi_part = take(nblk == 1 ? ((n + 127) / 128) * J * 4 * 8 : 0);
     L.norms = take(kNormSlots * 2 * 8);
+    L.tickets = take(nblk == 1 ? ((J + 63) / 64) * 4 : 0);
     L.flags = take(256);
     L.total = o;
     return L;
@@ -186,6 +193,7 @@ int launch_oci_iteration_any(oci_ctx* ctx, int src, int slot, int prev_slot, dou
     const DevView& V = ctx->V;
     if (ctx->path == OCI_PATH_PER_CELL) return launch_oci_percell(V, src, slot, prev_slot, tol, ctx->stream);
     if (oci_shared_fast_supported(V)) return launch_oci_shared_fast(V, src, slot, prev_slot, tol, ctx->stream);
+    if (ctx->use_ktiled) return launch_oci_ktiled(V, ctx->maps, src, slot, prev_slot, tol, ctx->stream);
     int k = launch_oci_generic(V, src, prev_slot, tol, ctx->stream);
     k += launch_phi_norm(V, src ^ 1, slot, prev_slot, tol, true, ctx->stream);
     return k;
@@ -316,6 +324,8 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     V.w = (double*)(base + L.w);
     V.coef = (double*)(base + L.coef);
     V.ainv4 = (double*)(base + L.ainv4);
+    V.phi_part = (double*)(base + L.phi_part);
+    V.tickets = (int32_t*)(base + L.tickets);
     V.norms = (unsigned long long*)(base + L.norms);
     V.flags = (int32_t*)(base + L.flags);
     V.v = ctx->v; V.dt = ctx->dt;
@@ -332,7 +342,7 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     // everything the kernels may read before a set_* call must be finite: zero the state
     CK(cudaMemsetAsync(base + L.psi0, 0, (size_t)(L.cfix - L.psi0), s));
     CK(cudaMemsetAsync(base + L.cfix, 0, (size_t)(L.dx - L.cfix), s));
-    CK(cudaMemsetAsync(base + L.norms, 0, (size_t)(L.total - L.norms), s));
+    CK(cudaMemsetAsync(base + L.phi_part, 0, (size_t)(L.total - L.phi_part), s));
     CK(cudaMemcpyAsync(V.dx, ctx->dx.data(), ctx->J * 8, cudaMemcpyHostToDevice, s));
     CK(cudaMemcpyAsync(V.sig, ctx->sig.data(), ctx->J * 8, cudaMemcpyHostToDevice, s));
     CK(cudaMemcpyAsync(V.sigs, ctx->sigs.data(), ctx->J * 8, cudaMemcpyHostToDevice, s));
@@ -358,6 +368,8 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
         ctx->ev.resize(2 * kNormSlots);
         for (auto& e : ctx->ev) CK(cudaEventCreate(&e));
     }
+    ctx->use_ktiled = ctx->path == OCI_PATH_SHARED && !oci_shared_fast_supported(V) && oci_ktiled_supported(V) &&
+                      oci_ktiled_prepare(V, &ctx->maps);
     ctx->cur = 0;
     ctx->predicted[0] = ctx->predicted[1] = 0;
     ctx->ready = true;
@@ -464,7 +476,9 @@ int oci_get_info(const oci_ctx* ctx, oci_info* info)
     info->block_dim = ctx->n;
     info->n_blocks = ctx->nblk;
     info->path = ctx->path;
-    info->reserved = 0;
+    info->apply_kernel = ctx->path == OCI_PATH_PER_CELL ? OCI_KERNEL_PER_CELL
+                         : (ctx->ready && oci_shared_fast_supported(ctx->V)) ? OCI_KERNEL_RESIDENT
+                         : ctx->use_ktiled ? OCI_KERNEL_KTILED : OCI_KERNEL_GENERIC;
     return OCI_OK;
 }
 

@@ -1,6 +1,7 @@
 // Internal declarations shared by the host driver (oci_api.cu) and the kernels.
 // Not part of the C ABI (include/oci.h is).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -35,11 +36,18 @@ struct DevView {
     double* w;                  // [N]
     double* coef;               // [n]  |mu_m| on the rows that take an incident flux, else 0
     double* ainv4;              // [nblk][N][16]  (A_m)^{-1} for SI
+    double* phi_part;           // [ceil(n/128)][J][4]  per-item scalar-flux partials (K-tiled kernel)
+    int32_t* tickets;           // [ceil(J/64)]  arrival counters of the K-tiled kernel's cell tiles (0 between launches)
     unsigned long long* norms;  // [kNormSlots][2]  bit patterns of (d, r), atomicMax targets
     int32_t* flags;             // [0] = 1 + index of a singular block, 0 if none
     double v, dt;
     int32_t bcL, bcR;
     double bcLv, bcRv;
+};
+
+// Tensor maps of the K-tiled shared-block kernel (oci_iter_shared_ktiled.cu), encoded once in oci_setup.
+struct KtiledMaps {
+    CUtensorMap cfix, psi[2], binv;
 };
 
 // The stopping rule (reading S2), evaluated identically on host and device.

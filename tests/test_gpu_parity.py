@@ -138,6 +138,40 @@ def test_edge_cases(J, N, bcL, bcR, hetero, scheme):
     assert rel(r["g_psi"], r["o_psi"]) < 1e-9
 
 
+@pytest.mark.parametrize("scheme", ["oci"])
+@pytest.mark.parametrize("J,N,bcL,bcR", [
+    (1, 8, (REF, 0.0), (REF, 0.0)),          # n = 32: one K-tiled item, mostly empty
+    (63, 24, (INC, 1.0), (REF, 0.0)),        # n = 96
+    (64, 40, (REF, 0.0), (VAC, 0.0)),        # n = 160: two output tiles, the second ragged; exactly one cell tile
+    (65, 64, (REF, 0.0), (REF, 0.0)),        # n = 256: cell tile + 1
+    (200, 128, (VAC, 0.0), (INC, 0.7)),      # n = 512 (config-4 block size), 4 output tiles, ragged cells
+    (130, 256, (REF, 0.0), (REF, 0.0)),      # n = 1024: the largest block the kernel takes
+])
+def test_ktiled_kernel_shapes(J, N, bcL, bcR, scheme):
+    """Shared-block sizes served by the K-tiled TMA/DMMA kernel: ragged cell and output tiles, both
+    mirrors, the cross-CTA scalar-flux ticket (n > 128)."""
+    import paper_2305_13555_b200 as P
+    p = _custom(J, N, bcL, bcR, seed=J * 1000 + N, hetero=False)
+    g = P.OCI.from_problem(p)
+    assert g.get_info()["apply_kernel"] == P.KERNEL_KTILED
+    g.close()
+    r = run_pair(p, scheme, steps=2, tol=-1.0, max_iters=4, threads=16)
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-12
+    assert rel(r["g_phi"], r["o_phi"]) < 1e-12
+    r = run_pair(p, scheme, steps=2, tol=1e-10, max_iters=10_000, threads=16)
+    assert r["g_iters"] == r["o_iters"]
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-9
+
+
+def test_apply_kernel_selection():
+    import paper_2305_13555_b200 as P
+    for cfg, cells, want in ((1, 20, P.KERNEL_GENERIC), (2, 50, P.KERNEL_RESIDENT), (3, 50, P.KERNEL_RESIDENT),
+                             (4, 50, P.KERNEL_KTILED), (5, 20, P.KERNEL_PER_CELL)):
+        g = P.OCI.from_problem(make_problem(cfg, cells=cells))
+        assert g.get_info()["apply_kernel"] == want, cfg
+        g.close()
+
+
 def test_not_converged_status_and_restart():
     """max_iters reached -> status 1 with the state committed; set_flux restarts; many chunks."""
     import paper_2305_13555_b200 as P
