@@ -36,8 +36,10 @@ METRIC = "oci_unknown_updates_per_s"
 UNIT = "unknown-updates/s"
 
 # DRAM traffic per launch of the dominant kernel from the committed `ncu --set full` capture
-# (profiles/), bytes; None until a capture exists for that kernel.
-NCU_TRAFFIC_BYTES = {}
+# (profiles/), bytes per launch; None where no capture exists for that config's kernel.
+NCU_TRAFFIC_BYTES = {3: 374.17e6,    # profiles/r1_resident_cfg3_full.txt: 272.80 MB read + 101.37 MB written
+                     4: 178.67e6,    # profiles/r1_ktiled_cfg4_full.txt:   136.89 MB read +  41.78 MB written
+                     5: 2168.2e6}    # profiles/r1_percell_cfg5_full.txt:  2164.5 MB read +   3.8 MB written
 
 
 def load_peaks():
@@ -296,6 +298,19 @@ def per_config_table(torch, P, skip=None):
     return out
 
 
+def aggregate_over_ranks(torch, ms, amount, device):
+    """Whole-job figures for N independent replicas: time = MAX over ranks, amount
+    (updates, or a per-rank rate) = SUM over ranks.  `device` None = single process."""
+    if device is None:
+        return float(ms), float(amount)
+    import torch.distributed as dist
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    u = torch.tensor([float(amount)], dtype=torch.float64, device=device)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
 def run_ours(args):
     import torch
     rank, world, local = dist_env()
@@ -328,14 +343,7 @@ def run_ours(args):
     ms, iters = time_gpu_steps(torch, g, p, args.steps, "oci", sampler, barrier)
     launches = g.launch_count() - l0
     updates = p.unknowns * sum(iters)
-    if world > 1:
-        import torch.distributed as dist
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-        u = torch.tensor([float(updates)], dtype=torch.float64, device="cuda")
-        dist.all_reduce(u, op=dist.ReduceOp.SUM)
-        updates = float(u.item())
+    ms, updates = aggregate_over_ranks(torch, ms, updates, "cuda" if world > 1 else None)
     value = updates / (ms * 1e-3)
 
     # ---- the dominant kernel alone (events around every OCI apply launch, same steps again)
@@ -367,11 +375,7 @@ def run_ours(args):
 
     # ---- end to end through the C ABI with host buffers
     e2e_val, h2d, d2h = time_gpu_e2e(torch, g, p, args.steps)
-    if world > 1:
-        import torch.distributed as dist
-        t = torch.tensor([e2e_val], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        e2e_val = float(t.item())
+    _, e2e_val = aggregate_over_ranks(torch, 0.0, e2e_val, "cuda" if world > 1 else None)
     g.close()
     del g
     torch.cuda.empty_cache()
