@@ -19,7 +19,10 @@ __device__ __forceinline__ bool step_done(const unsigned long long* __restrict__
 // independent of the reduction order, so host and device agree on the iteration count.
 __device__ __forceinline__ void atomic_max_nonneg(unsigned long long* addr, double v)
 {
-    atomicMax(addr, (unsigned long long)__double_as_longlong(v));
+    // same-address atomics serialise in L2 (about 25 ns each with thousands of CTAs): skip the ones
+    // that cannot raise the maximum (the plain read may be stale low, never high: max only grows)
+    const unsigned long long bits = (unsigned long long)__double_as_longlong(v);
+    if (bits > __ldcg(addr)) atomicMax(addr, bits);
 }
 
 __device__ __forceinline__ double warp_max(double v)

@@ -116,7 +116,7 @@ void gauss_legendre(int N, std::vector<double>& mu, std::vector<double>& w)
 }
 
 struct Layout {
-    int64_t binv, psi0, psi1, cfix, phi, Q, qs, dx, sig, sigs, blk, rep, mu, w, coef, ainv4, phi_part, norms, tickets, flags, total;
+    int64_t binv, psi0, psi1, cfix, phi, Q, qs, dx, sig, sigs, blk, rep, mu, w, coef, ainv4, si_scan, phi_part, norms, tickets, flags, total;
 };
 
 int64_t align_up(int64_t x) { return (x + 255) & ~int64_t(255); }
@@ -143,6 +143,10 @@ Layout make_layout(int64_t J, int32_t N, int64_t nblk)
     L.w = take(N * 8);
     L.coef = take(n * 8);
     L.ainv4 = take(nblk * N * 16 * 8);
+    {
+        const int S = si_chunk_cells(J, N);
+        L.si_scan = take(((J + S - 1) / S) * N * 8 * 8);
+    }
     L.phi_part = take(nblk == 1 ? ((n + 127) / 128) * J * 4 * 8 : 0);
     L.norms = take(kNormSlots * 2 * 8);
     L.tickets = take(nblk == 1 ? ((J + 63) / 64) * 4 : 0);
@@ -324,6 +328,7 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     V.w = (double*)(base + L.w);
     V.coef = (double*)(base + L.coef);
     V.ainv4 = (double*)(base + L.ainv4);
+    V.si_scan = (double*)(base + L.si_scan);
     V.phi_part = (double*)(base + L.phi_part);
     V.tickets = (int32_t*)(base + L.tickets);
     V.norms = (unsigned long long*)(base + L.norms);

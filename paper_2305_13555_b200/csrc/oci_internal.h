@@ -36,6 +36,7 @@ struct DevView {
     double* w;                  // [N]
     double* coef;               // [n]  |mu_m| on the rows that take an incident flux, else 0
     double* ainv4;              // [nblk][N][16]  (A_m)^{-1} for SI
+    double* si_scan;            // [chunks][N][8]  SI scan: chunk maps (P, z) and chunk inflows (si_sweep.cu)
     double* phi_part;           // [ceil(n/128)][J][4]  per-item scalar-flux partials (K-tiled kernel)
     int32_t* tickets;           // [ceil(J/64)]  arrival counters of the K-tiled kernel's cell tiles (0 between launches)
     unsigned long long* norms;  // [kNormSlots][2]  bit patterns of (d, r), atomicMax targets
@@ -52,6 +53,17 @@ struct KtiledMaps {
 
 // The stopping rule (reading S2), evaluated identically on host and device.
 __host__ __device__ inline bool converged(double tol, double d, double r) { return tol >= 0.0 && d <= tol * r; }
+
+// Cells per chunk of the SI scan (si_sweep.cu): one chunk for tiny slabs (launch-latency bound), else
+// the largest of 64, 32, 16, 8 that still gives every SM about 8 warps of (chunk, angle) threads.
+inline int si_chunk_cells(int64_t J, int32_t N)
+{
+    if (J <= 32) return (int)J;
+    const int64_t lanes = N >= 32 ? (N + 31) / 32 * 32 : N;
+    for (int S = 64; S > 8; S >>= 1)
+        if (((J + S - 1) / S) * lanes >= (int64_t)148 * 8 * 32) return S;
+    return 8;
+}
 
 // ---- launchers (each returns the number of kernels it launched) ----
 int launch_form_and_invert(const DevView& V, cudaStream_t s);

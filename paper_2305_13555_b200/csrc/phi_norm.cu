@@ -29,27 +29,59 @@ __device__ __forceinline__ void refresh_ghost_rows(const DevView& V, double* P, 
 }
 
 template <bool NORMS>
-__global__ void __launch_bounds__(256) phi_norm_kernel(DevView V, int buf, int slot, int prev_slot, double tol)
+__global__ void __launch_bounds__(256, 2) phi_norm_kernel(DevView V, int buf, int slot, int prev_slot, double tol)
 {
     if (NORMS && step_done(V.norms, prev_slot, tol)) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int n = V.n;
+    constexpr int CP = 8;
     double* P = V.psi[buf];
+    const double* __restrict__ Pr = P;
     double dmax = 0.0, rmax = 0.0;
-    for (int64_t j = (int64_t)blockIdx.x * 8 + warp; j < V.J; j += (int64_t)gridDim.x * 8) {
-        const double* row = P + j * n;
-        double acc = 0.0;
-        for (int idx = lane; idx < n; idx += 32) acc = fma(V.w[idx >> 2], row[idx], acc);
-        acc += __shfl_xor_sync(0xffffffffu, acc, 4);
-        acc += __shfl_xor_sync(0xffffffffu, acc, 8);
-        acc += __shfl_xor_sync(0xffffffffu, acc, 16);
-        if (lane < 4) {
-            const double old = V.phi[j * 4 + lane];
-            V.phi[j * 4 + lane] = acc;
-            dmax = fmax(dmax, fabs(acc - old));
-            rmax = fmax(rmax, fabs(acc));
+    // CP cells per warp pass; a lane owns the 16-byte units idx = 2*lane (+64 i) of each row, i.e. slots
+    // (0,1) of an angle on even lanes and (2,3) on odd lanes.  Every load of a pass (rows and the old
+    // phi) is unconditional (cell index clamped) so that all of them are in flight together: the
+    // kernel is bound by memory latency x bytes in flight, not by arithmetic.
+    for (int64_t j0 = ((int64_t)blockIdx.x * 8 + warp) * CP; j0 < V.J; j0 += (int64_t)gridDim.x * 8 * CP) {
+        double a0[CP], a1[CP];
+        double2 oldv[CP];
+#pragma unroll
+        for (int c = 0; c < CP; ++c) {
+            a0[c] = a1[c] = 0.0;
+            const int64_t j = (j0 + c < V.J) ? j0 + c : V.J - 1;
+            oldv[c] = (NORMS && lane < 2) ? *reinterpret_cast<const double2*>(V.phi + j * 4 + 2 * lane) : make_double2(0.0, 0.0);
         }
-        if (j == 0 || j == V.J - 1) refresh_ghost_rows(V, P, j, lane);
+#pragma unroll 2
+        for (int idx = 2 * lane; idx < n; idx += 64) {
+            const double wq = V.w[idx >> 2];
+#pragma unroll
+            for (int c = 0; c < CP; ++c) {
+                const int64_t j = (j0 + c < V.J) ? j0 + c : V.J - 1;
+                const double2 v = *reinterpret_cast<const double2*>(Pr + j * n + idx);
+                a0[c] = fma(wq, v.x, a0[c]);
+                a1[c] = fma(wq, v.y, a1[c]);
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < CP; ++c) {
+#pragma unroll
+            for (int o = 2; o < 32; o <<= 1) {
+                a0[c] += __shfl_xor_sync(0xffffffffu, a0[c], o);
+                a1[c] += __shfl_xor_sync(0xffffffffu, a1[c], o);
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < CP; ++c) {
+            const int64_t j = j0 + c;
+            if (j < V.J) {
+                if (lane < 2) {
+                    *reinterpret_cast<double2*>(V.phi + j * 4 + 2 * lane) = make_double2(a0[c], a1[c]);
+                    dmax = fmax(dmax, fmax(fabs(a0[c] - oldv[c].x), fabs(a1[c] - oldv[c].y)));
+                    rmax = fmax(rmax, fmax(fabs(a0[c]), fabs(a1[c])));
+                }
+                if (j == 0 || j == V.J - 1) refresh_ghost_rows(V, P, j, lane);
+            }
+        }
     }
     if (NORMS) {
         __shared__ double sd[8], sr[8];
@@ -68,7 +100,7 @@ __global__ void __launch_bounds__(256) phi_norm_kernel(DevView V, int buf, int s
 int launch_phi_norm(const DevView& V, int buf, int slot, int prev_slot, double tol, bool with_norms,
                     cudaStream_t s)
 {
-    int64_t blocks = (V.J + 7) / 8;
+    int64_t blocks = (V.J + 63) / 64;
     if (blocks > 148 * 16) blocks = 148 * 16;
     if (with_norms) phi_norm_kernel<true><<<(unsigned)blocks, 256, 0, s>>>(V, buf, slot, prev_slot, tol);
     else phi_norm_kernel<false><<<(unsigned)blocks, 256, 0, s>>>(V, buf, slot, prev_slot, tol);

@@ -227,23 +227,26 @@ int launch_set_flux(const DevView& V, const double* d_psi_edge, int buf, cudaStr
 
 // a2: c_fix[j][4m+s] = (h/4) Q[j][s] + (s<2 ? alpha * psi_{k-1/2}[j][m][s] : 0), where psi_{k-1/2} is the
 // time-edge half (slots 2,3) of the iterate the previous step ended on: this read IS the commit (a8).
-__global__ void cfix_kernel(DevView V, int buf)
+__global__ void __launch_bounds__(256) cfix_kernel(DevView V, int buf)
 {
+    // thread = (cell j, angle m): one 16-byte load of the time-edge pair, two 16-byte stores
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const int n = V.n;
-    if (t >= V.J * n) return;
-    const int64_t j = t / n;
-    const int idx = (int)(t - j * n);
-    const int s = idx & 3;
+    const int N = V.N;
+    if (t >= V.J * N) return;
+    const int64_t j = t / N;
     const double h = V.dx[j];
-    double val = h * 0.25 * V.Q[j * 4 + s];
-    if (s < 2) val += h / (2.0 * V.v * V.dt) * V.psi[buf][t + 2];
-    V.cfix[t] = val;
+    const double q4 = h * 0.25, al = h / (2.0 * V.v * V.dt);
+    const double2 q01 = *reinterpret_cast<const double2*>(V.Q + j * 4);
+    const double2 q23 = *reinterpret_cast<const double2*>(V.Q + j * 4 + 2);
+    const double2 e = *reinterpret_cast<const double2*>(V.psi[buf] + t * 4 + 2);
+    // same operation order as one thread per element: val = h/4 Q; val += alpha psi (s < 2)
+    *reinterpret_cast<double2*>(V.cfix + t * 4) = make_double2(q4 * q01.x + al * e.x, q4 * q01.y + al * e.y);
+    *reinterpret_cast<double2*>(V.cfix + t * 4 + 2) = make_double2(q4 * q23.x, q4 * q23.y);
 }
 
 int launch_cfix(const DevView& V, int buf, cudaStream_t s)
 {
-    int64_t tot = V.J * V.n;
+    int64_t tot = V.J * V.N;
     cfix_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, s>>>(V, buf);
     return 1;
 }
