@@ -70,6 +70,21 @@ enum { OCI_PATH_SHARED = 0, OCI_PATH_PER_CELL = 1 };
  * PER_CELL - batched GEMV streaming one inverse per cell from HBM. */
 enum { OCI_KERNEL_GENERIC = 0, OCI_KERNEL_RESIDENT = 1, OCI_KERNEL_KTILED = 2, OCI_KERNEL_PER_CELL = 3 };
 
+/* Form of the OCI iteration inside oci_step (oci_set_iteration).  Both produce the iterates of
+ * eq. (19), up to rounding order:
+ * FULL    - every iteration applies the whole inverse, Psi^(l+1) = B^{-1} c^(l) (the paper's statement);
+ * REDUCED - (default) only the 2N RHS rows fed by incident fluxes change within a step (the (l) terms
+ *           of eqs. 27,28), so per step: Psi_fix = B^{-1} c_fix once; per iteration the 2N
+ *           outgoing rows and the 4 scalar-flux rows, y^(l+1) = yfix + G inc^(l), phi^(l+1) = phifix +
+ *           H inc^(l) with G = B^{-1}[O,I] diag|mu| (2N x 2N), H = W B^{-1}[:,I] diag|mu| (4 x 2N); after
+ *           the last iteration the other 2N rows from the same inc (F = B^{-1}[I,I] diag|mu|). */
+enum { OCI_ITERATION_FULL = 0, OCI_ITERATION_REDUCED = 1 };
+
+/* Kernel serving the REDUCED iteration: GEMV - batched GEMV, one operator per distinct block (any n);
+ * RESIDENT - shared block, n in {64,128}: G, H resident in registers, fp64 tensor pipe;
+ * KTILED - shared block, large n: operands streamed in K chunks by tensor-map TMA, fp64 tensor pipe. */
+enum { OCI_RKERNEL_GEMV = 0, OCI_RKERNEL_RESIDENT = 1, OCI_RKERNEL_KTILED = 2 };
+
 typedef struct {
     int64_t cells;        /* J */
     int32_t n_angles;     /* N */
@@ -77,6 +92,8 @@ typedef struct {
     int64_t n_blocks;     /* distinct (dx, Sigma, Sigma_s) triples */
     int32_t path;         /* OCI_PATH_* */
     int32_t apply_kernel; /* OCI_KERNEL_* */
+    int32_t iteration;    /* OCI_ITERATION_* */
+    int32_t reduced_kernel; /* OCI_RKERNEL_* */
 } oci_info;
 
 /* Problem statement (per-cell dx_j, Sigma_j, Sigma_s,j P:74-82).
@@ -123,6 +140,10 @@ int oci_set_source_dev(oci_ctx* ctx, const double* d_q);
 int oci_step(oci_ctx* ctx, double tol, int32_t max_iters, int32_t* iters, double* resid);
 int si_step(oci_ctx* ctx, double tol, int32_t max_iters, int32_t* iters, double* resid);
 
+/* Select the form of the OCI iteration (default OCI_ITERATION_REDUCED).  May be called at any time
+ * after oci_create; takes effect at the next oci_step.  Errors: -1. */
+int oci_set_iteration(oci_ctx* ctx, int32_t iteration);
+
 /* Results of the current state.  phi: [cells][4] (eq. 18);
  * psi: [cells][N][4].  HOST pointers; _dev variants take DEVICE pointers and
  * are asynchronous on the context's stream. */
@@ -147,6 +168,11 @@ int oci_get_block_inverse(const oci_ctx* ctx, int64_t blk, double* binv);
  * count since the last enable and resets them. */
 int oci_enable_kernel_timing(oci_ctx* ctx, int32_t on);
 int oci_get_kernel_time(oci_ctx* ctx, double* ms, int64_t* launches);
+/* REDUCED iteration only: the per-step Psi_fix pass (full apply + split) and the finalisation kernel,
+ * accumulated like oci_get_kernel_time (which then counts the reduced iteration kernel). Any pointer
+ * may be NULL. */
+int oci_get_aux_kernel_time(oci_ctx* ctx, double* fix_ms, int64_t* fix_launches, double* final_ms,
+                            int64_t* final_launches);
 
 /* Roofline denominator for the SHARED path: sustained fp64 tensor-pipe (DMMA) issue rate of the
  * current device in TFLOP/s, measured by a registers-only probe kernel (about 0.1 s).

@@ -11,12 +11,14 @@ from . import build as _build
 BC_VACUUM, BC_INCIDENT_ISOTROPIC, BC_REFLECTING = 0, 1, 2
 PATH_SHARED, PATH_PER_CELL = 0, 1
 KERNEL_GENERIC, KERNEL_RESIDENT, KERNEL_KTILED, KERNEL_PER_CELL = 0, 1, 2, 3
+ITERATION_FULL, ITERATION_REDUCED = 0, 1
+RKERNEL_GEMV, RKERNEL_RESIDENT, RKERNEL_KTILED = 0, 1, 2
 
 EXPORTED_SYMBOLS = [
     "oci_create", "oci_workspace_bytes", "oci_setup", "oci_set_flux", "oci_set_flux_dev", "oci_set_source",
     "oci_set_source_dev", "oci_step", "si_step", "oci_get_scalar_flux", "oci_get_angular_flux",
     "oci_get_scalar_flux_dev", "oci_get_angular_flux_dev", "oci_get_quadrature", "oci_get_info",
-    "oci_get_block_inverse", "oci_enable_kernel_timing", "oci_get_kernel_time", "oci_launch_count",
+    "oci_get_block_inverse", "oci_enable_kernel_timing", "oci_get_kernel_time", "oci_get_aux_kernel_time", "oci_set_iteration", "oci_launch_count",
     "oci_probe_fp64_tensor_tflops", "oci_last_error", "oci_destroy",
 ]
 
@@ -33,7 +35,8 @@ class _bc(C.Structure):
 
 class _info(C.Structure):
     _fields_ = [("cells", C.c_int64), ("n_angles", C.c_int32), ("block_dim", C.c_int32),
-                ("n_blocks", C.c_int64), ("path", C.c_int32), ("apply_kernel", C.c_int32)]
+                ("n_blocks", C.c_int64), ("path", C.c_int32), ("apply_kernel", C.c_int32),
+                ("iteration", C.c_int32), ("reduced_kernel", C.c_int32)]
 
 
 _dp = C.POINTER(C.c_double)
@@ -82,6 +85,10 @@ def load_library():
     L.oci_enable_kernel_timing.argtypes = [vp, i32]
     L.oci_get_kernel_time.restype = C.c_int
     L.oci_get_kernel_time.argtypes = [vp, _dp, C.POINTER(i64)]
+    L.oci_get_aux_kernel_time.restype = C.c_int
+    L.oci_get_aux_kernel_time.argtypes = [vp, _dp, C.POINTER(i64), _dp, C.POINTER(i64)]
+    L.oci_set_iteration.restype = C.c_int
+    L.oci_set_iteration.argtypes = [vp, i32]
     L.oci_probe_fp64_tensor_tflops.restype = C.c_int
     L.oci_probe_fp64_tensor_tflops.argtypes = [vp, vp, _dp]
     L.oci_launch_count.restype = i64
@@ -134,8 +141,10 @@ class OCI:
         self._ws = None
 
     @classmethod
-    def from_problem(cls, p, device="cuda:0", set_flux=True):
+    def from_problem(cls, p, device="cuda:0", set_flux=True, iteration=None):
         o = cls(p.dx, p.sigma_t, p.sigma_s, p.v, p.dt, p.n_angles, p.bc_left, p.bc_right)
+        if iteration is not None:
+            o.set_iteration(iteration)
         o.setup(device)
         if set_flux:
             o.set_flux(p.psi0)
@@ -237,7 +246,7 @@ class OCI:
         i = _info()
         self._check(self._L.oci_get_info(self._h, C.byref(i)))
         return dict(cells=i.cells, n_angles=i.n_angles, block_dim=i.block_dim, n_blocks=i.n_blocks, path=i.path,
-                    apply_kernel=i.apply_kernel)
+                    apply_kernel=i.apply_kernel, iteration=i.iteration, reduced_kernel=i.reduced_kernel)
 
     def get_block_inverse(self, blk=0):
         n = 4 * self.n_angles
@@ -252,6 +261,14 @@ class OCI:
         ms, k = C.c_double(0.0), C.c_int64(0)
         self._check(self._L.oci_get_kernel_time(self._h, C.byref(ms), C.byref(k)))
         return ms.value, k.value
+
+    def get_aux_kernel_time(self):
+        a, b, ka, kb = C.c_double(0.0), C.c_double(0.0), C.c_int64(0), C.c_int64(0)
+        self._check(self._L.oci_get_aux_kernel_time(self._h, C.byref(a), C.byref(ka), C.byref(b), C.byref(kb)))
+        return dict(fix_ms=a.value, fix_launches=ka.value, final_ms=b.value, final_launches=kb.value)
+
+    def set_iteration(self, iteration):
+        self._check(self._L.oci_set_iteration(self._h, int(iteration)))
 
     def launch_count(self):
         return int(self._L.oci_launch_count(self._h))

@@ -44,13 +44,20 @@ struct oci_ctx {
     int64_t ws_bytes = 0;
     bool ready = false, have_flux = false;
     int cur = 0;                       // psi[cur] holds the current iterate
+    // interface-reduced iteration (oci_reduced.cu)
+    int32_t iteration = OCI_ITERATION_REDUCED;
+    int ycur = 0;                      // y[ycur] holds the outgoing rows of the current iterate ...
+    bool y_valid = false;              // ... when this is set (cleared by set_flux, si_step, full-mode oci_step)
     int32_t predicted[2] = {0, 0};     // last iteration count of oci / si, sizes the launch chunk
     unsigned long long* h_norms = nullptr;   // pinned
     // timing
     bool timing = false;
     std::vector<cudaEvent_t> ev;
+    cudaEvent_t ev_aux[4] = {nullptr, nullptr, nullptr, nullptr};
     double kernel_ms = 0.0;
     int64_t kernel_launches = 0;
+    double aux_ms[2] = {0.0, 0.0};     // reduced iteration: Psi_fix pass, finalisation
+    int64_t aux_launches[2] = {0, 0};
     int64_t launches = 0;
     std::string err;
 };
@@ -116,7 +123,8 @@ void gauss_legendre(int N, std::vector<double>& mu, std::vector<double>& w)
 }
 
 struct Layout {
-    int64_t binv, psi0, psi1, cfix, phi, Q, qs, dx, sig, sigs, blk, rep, mu, w, coef, ainv4, si_scan, phi_part, norms, tickets, flags, total;
+    int64_t binv, psi0, psi1, cfix, phi, Q, qs, dx, sig, sigs, blk, rep, mu, w, coef, ainv4, si_scan, phi_part, norms, tickets, flags,
+        rop, fop, y0, y1, yfix, ifix, phifix, zero_n, total;
 };
 
 int64_t align_up(int64_t x) { return (x + 255) & ~int64_t(255); }
@@ -148,9 +156,20 @@ Layout make_layout(int64_t J, int32_t N, int64_t nblk)
         L.si_scan = take(((J + S - 1) / S) * N * 8 * 8);
     }
     L.phi_part = take(nblk == 1 ? ((n + 127) / 128) * J * 4 * 8 : 0);
-    L.norms = take(kNormSlots * 2 * 8);
+    L.norms = take((kNormSlots + 1) * 2 * 8);
     L.tickets = take(nblk == 1 ? ((J + 63) / 64) * 4 : 0);
     L.flags = take(256);
+    {
+        const int64_t K2 = n / 2, MO = K2 + 8;
+        L.rop = take(nblk * MO * K2 * 8);
+        L.fop = take(nblk * K2 * K2 * 8);
+        L.y0 = take((J + 2) * K2 * 8);
+        L.y1 = take((J + 2) * K2 * 8);
+        L.yfix = take(J * K2 * 8);
+        L.ifix = take(J * K2 * 8);
+        L.phifix = take(J * 4 * 8);
+        L.zero_n = take(n * 8);
+    }
     L.total = o;
     return L;
 }
@@ -203,6 +222,32 @@ int launch_oci_iteration_any(oci_ctx* ctx, int src, int slot, int prev_slot, dou
     return k;
 }
 
+// One Psi_fix pass of the reduced iteration: the ordinary apply kernel of this path with a zero gather
+// coefficient (c = c_fix), its scalar flux going to phifix and its norms to a slot nobody reads; then
+// the split into the packed outgoing / incident-side halves.
+int launch_fix_pass(oci_ctx* ctx)
+{
+    DevView Vf = ctx->V;
+    Vf.coef = Vf.zero_n;
+    Vf.phi = Vf.phifix;
+    const DevView saved = ctx->V;
+    ctx->V = Vf;
+    int k = launch_oci_iteration_any(ctx, ctx->cur, kScratchSlot, -1, -1.0);
+    ctx->V = saved;
+    k += launch_split_fix(ctx->V, ctx->cur ^ 1, ctx->stream);
+    return k;
+}
+
+int launch_reduced_iteration(oci_ctx* ctx, int ysrc, int slot, int prev_slot, double tol)
+{
+    return launch_red_percell(ctx->V, ysrc, slot, prev_slot, tol, ctx->stream);
+}
+
+int launch_reduced_final(oci_ctx* ctx, int ybase, int cnt, int force, double tol)
+{
+    return launch_red_percell_final(ctx->V, ybase, ctx->cur, cnt, force, tol, ctx->stream);
+}
+
 int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iters, double* resid)
 {
     if (!ctx) return OCI_E_INVALID;
@@ -211,8 +256,22 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
     if (max_iters < 1 || tol != tol) return fail(ctx, OCI_E_INVALID, "max_iters < 1 or tol is NaN");
     DevView& V = ctx->V;
     cudaStream_t s = ctx->stream;
+    const bool red = !si && ctx->iteration == OCI_ITERATION_REDUCED;
+    const bool timed = ctx->timing && !si;
 
     ctx->launches += launch_cfix(V, ctx->cur, s);                         // a2 (+ a8 of the previous step)
+    if (red) {
+        if (!ctx->y_valid) {
+            ctx->launches += launch_pack_y(V, ctx->cur, 0, s);
+            ctx->ycur = 0;
+            ctx->y_valid = true;
+        }
+        if (timed) CK(cudaEventRecord(ctx->ev_aux[0], s));
+        ctx->launches += launch_fix_pass(ctx);
+        if (timed) CK(cudaEventRecord(ctx->ev_aux[1], s));
+    } else {
+        ctx->y_valid = false;
+    }
     int32_t done_iters = 0;
     bool conv = false;
     double d = 0.0, r = 0.0;
@@ -224,10 +283,18 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
         if (cnt > max_iters - done_iters) cnt = max_iters - done_iters;
         CK(cudaMemsetAsync(V.norms, 0, sizeof(unsigned long long) * 2 * cnt, s));
         for (int32_t i = 0; i < cnt; ++i) {
-            if (ctx->timing && !si) CK(cudaEventRecord(ctx->ev[2 * i], s));
+            if (timed) CK(cudaEventRecord(ctx->ev[2 * i], s));
             if (si) ctx->launches += launch_si_iteration(V, ctx->cur, i, i - 1, tol, s);
+            else if (red) ctx->launches += launch_reduced_iteration(ctx, (ctx->ycur + done_iters + i) & 1, i, i - 1, tol);
             else ctx->launches += launch_oci_iteration_any(ctx, (ctx->cur + done_iters + i) & 1, i, i - 1, tol);
-            if (ctx->timing && !si) CK(cudaEventRecord(ctx->ev[2 * i + 1], s));
+            if (timed) CK(cudaEventRecord(ctx->ev[2 * i + 1], s));
+        }
+        if (red) {
+            // finalisation, queued before the read-back: finds the last iteration on the device and
+            // does nothing if this chunk neither converged nor ends at max_iters
+            if (timed) CK(cudaEventRecord(ctx->ev_aux[2], s));
+            ctx->launches += launch_reduced_final(ctx, (ctx->ycur + done_iters) & 1, cnt, done_iters + cnt >= max_iters, tol);
+            if (timed) CK(cudaEventRecord(ctx->ev_aux[3], s));
         }
         CK(cudaMemcpyAsync(ctx->h_norms, V.norms, sizeof(unsigned long long) * 2 * cnt, cudaMemcpyDeviceToHost, s));
         CK(cudaStreamSynchronize(s));                                       // the one read-back (a7)
@@ -238,17 +305,30 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
             std::memcpy(&r, &ctx->h_norms[2 * i + 1], 8);
             if (converged(tol, d, r)) { conv = true; executed = i + 1; break; }
         }
-        if (ctx->timing && !si) {
+        if (timed) {
             for (int32_t i = 0; i < executed; ++i) {
                 float ms = 0.f;
                 CK(cudaEventElapsedTime(&ms, ctx->ev[2 * i], ctx->ev[2 * i + 1]));
                 ctx->kernel_ms += ms;
                 ctx->kernel_launches += 1;
             }
+            if (red && (conv || done_iters + cnt >= max_iters)) {
+                float ms = 0.f;
+                CK(cudaEventElapsedTime(&ms, ctx->ev_aux[2], ctx->ev_aux[3]));
+                ctx->aux_ms[1] += ms;
+                ctx->aux_launches[1] += 1;
+            }
         }
         done_iters += executed;
     }
-    if (!si) ctx->cur = (ctx->cur + done_iters) & 1;                       // a8: pointer convention
+    if (timed && red) {
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, ctx->ev_aux[0], ctx->ev_aux[1]));
+        ctx->aux_ms[0] += ms;
+        ctx->aux_launches[0] += 1;
+    }
+    if (red) ctx->ycur = (ctx->ycur + done_iters) & 1;                     // Psi^(L) was written to psi[cur]
+    else if (!si) ctx->cur = (ctx->cur + done_iters) & 1;                  // a8: pointer convention
     ctx->predicted[si ? 1 : 0] = done_iters;
     if (iters) *iters = done_iters;
     if (resid) *resid = (r > 0.0) ? d / r : d;
@@ -333,6 +413,14 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     V.tickets = (int32_t*)(base + L.tickets);
     V.norms = (unsigned long long*)(base + L.norms);
     V.flags = (int32_t*)(base + L.flags);
+    V.rop = (double*)(base + L.rop);
+    V.fop = (double*)(base + L.fop);
+    V.y[0] = (double*)(base + L.y0) + n / 2;      // skip the left ghost row
+    V.y[1] = (double*)(base + L.y1) + n / 2;
+    V.yfix = (double*)(base + L.yfix);
+    V.ifix = (double*)(base + L.ifix);
+    V.phifix = (double*)(base + L.phifix);
+    V.zero_n = (double*)(base + L.zero_n);
     V.v = ctx->v; V.dt = ctx->dt;
     V.bcL = ctx->bcL.kind; V.bcR = ctx->bcR.kind;
     V.bcLv = ctx->bcL.value; V.bcRv = ctx->bcR.value;
@@ -347,7 +435,8 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     // everything the kernels may read before a set_* call must be finite: zero the state
     CK(cudaMemsetAsync(base + L.psi0, 0, (size_t)(L.cfix - L.psi0), s));
     CK(cudaMemsetAsync(base + L.cfix, 0, (size_t)(L.dx - L.cfix), s));
-    CK(cudaMemsetAsync(base + L.phi_part, 0, (size_t)(L.total - L.phi_part), s));
+    CK(cudaMemsetAsync(base + L.phi_part, 0, (size_t)(L.rop - L.phi_part), s));
+    CK(cudaMemsetAsync(base + L.y0, 0, (size_t)(L.total - L.y0), s));
     CK(cudaMemcpyAsync(V.dx, ctx->dx.data(), ctx->J * 8, cudaMemcpyHostToDevice, s));
     CK(cudaMemcpyAsync(V.sig, ctx->sig.data(), ctx->J * 8, cudaMemcpyHostToDevice, s));
     CK(cudaMemcpyAsync(V.sigs, ctx->sigs.data(), ctx->J * 8, cudaMemcpyHostToDevice, s));
@@ -359,6 +448,7 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     CK(cudaStreamSynchronize(s));   // host vectors above are read by the async copies
 
     ctx->launches += launch_form_and_invert(V, s);                       // a0, a1
+    ctx->launches += launch_pack_operators(V, s);                        // f1: G, H, F
     int32_t flag = 0;
     CK(cudaMemcpyAsync(&flag, V.flags, 4, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
@@ -372,10 +462,13 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     if (ctx->ev.empty()) {
         ctx->ev.resize(2 * kNormSlots);
         for (auto& e : ctx->ev) CK(cudaEventCreate(&e));
+        for (auto& e : ctx->ev_aux) CK(cudaEventCreate(&e));
     }
     ctx->use_ktiled = ctx->path == OCI_PATH_SHARED && !oci_shared_fast_supported(V) && oci_ktiled_supported(V) &&
                       oci_ktiled_prepare(V, &ctx->maps);
     ctx->cur = 0;
+    ctx->ycur = 0;
+    ctx->y_valid = false;
     ctx->predicted[0] = ctx->predicted[1] = 0;
     ctx->ready = true;
     return OCI_OK;
@@ -385,6 +478,7 @@ static int set_flux_common(oci_ctx* ctx, const double* d_edge)
 {
     ctx->launches += launch_set_flux(ctx->V, d_edge, 0, ctx->stream);
     ctx->cur = 0;
+    ctx->y_valid = false;
     ctx->launches += launch_phi_norm(ctx->V, 0, 0, -1, -1.0, false, ctx->stream);   // phi^(0), ghost rows
     CK(cudaStreamSynchronize(ctx->stream));
     CK(cudaGetLastError());
@@ -484,6 +578,8 @@ int oci_get_info(const oci_ctx* ctx, oci_info* info)
     info->apply_kernel = ctx->path == OCI_PATH_PER_CELL ? OCI_KERNEL_PER_CELL
                          : (ctx->ready && oci_shared_fast_supported(ctx->V)) ? OCI_KERNEL_RESIDENT
                          : ctx->use_ktiled ? OCI_KERNEL_KTILED : OCI_KERNEL_GENERIC;
+    info->iteration = ctx->iteration;
+    info->reduced_kernel = OCI_RKERNEL_GEMV;
     return OCI_OK;
 }
 
@@ -504,6 +600,29 @@ int oci_enable_kernel_timing(oci_ctx* ctx, int32_t on)
     ctx->timing = on != 0;
     ctx->kernel_ms = 0.0;
     ctx->kernel_launches = 0;
+    ctx->aux_ms[0] = ctx->aux_ms[1] = 0.0;
+    ctx->aux_launches[0] = ctx->aux_launches[1] = 0;
+    return OCI_OK;
+}
+
+int oci_get_aux_kernel_time(oci_ctx* ctx, double* fix_ms, int64_t* fix_launches, double* final_ms, int64_t* final_launches)
+{
+    if (!ctx) return OCI_E_INVALID;
+    if (fix_ms) *fix_ms = ctx->aux_ms[0];
+    if (fix_launches) *fix_launches = ctx->aux_launches[0];
+    if (final_ms) *final_ms = ctx->aux_ms[1];
+    if (final_launches) *final_launches = ctx->aux_launches[1];
+    ctx->aux_ms[0] = ctx->aux_ms[1] = 0.0;
+    ctx->aux_launches[0] = ctx->aux_launches[1] = 0;
+    return OCI_OK;
+}
+
+int oci_set_iteration(oci_ctx* ctx, int32_t iteration)
+{
+    if (!ctx) return OCI_E_INVALID;
+    if (iteration != OCI_ITERATION_FULL && iteration != OCI_ITERATION_REDUCED)
+        return fail(ctx, OCI_E_INVALID, "unknown iteration form");
+    ctx->iteration = iteration;
     return OCI_OK;
 }
 
@@ -526,6 +645,7 @@ void oci_destroy(oci_ctx* ctx)
     if (!ctx) return;
     if (ctx->h_norms) cudaFreeHost(ctx->h_norms);
     for (auto& e : ctx->ev) cudaEventDestroy(e);
+    for (auto& e : ctx->ev_aux) if (e) cudaEventDestroy(e);
     delete ctx;
 }
 

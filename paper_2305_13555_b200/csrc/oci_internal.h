@@ -10,6 +10,7 @@
 namespace oci {
 
 constexpr int kNormSlots = 64;  // iterations launched between two host read-backs, at most
+constexpr int kScratchSlot = kNormSlots;   // norm slot nobody reads (the Psi_fix pass of the reduced iteration)
 
 // Device-side view of one problem.  Passed to kernels by value.
 // Psi buffers have one ghost row before row 0 and one after row J-1: psi[b]
@@ -41,6 +42,14 @@ struct DevView {
     int32_t* tickets;           // [ceil(J/64)]  arrival counters of the K-tiled kernel's cell tiles (0 between launches)
     unsigned long long* norms;  // [kNormSlots][2]  bit patterns of (d, r), atomicMax targets
     int32_t* flags;             // [0] = 1 + index of a singular block, 0 if none
+    // ---- interface-reduced iteration (oci_reduced.cu), K2 = 2N, MO = K2 + 8
+    double* rop;                // [nblk][MO][K2]  rows 0..K2-1: G = B^{-1}[O,I] diag|mu|; K2..K2+3: H = W B^{-1}[:,I] diag|mu|; rest 0
+    double* fop;                // [nblk][K2][K2]  F = B^{-1}[I,I] diag|mu|
+    double* y[2];               // ping-pong interface iterates (outgoing rows of Psi, packed), [(J+2)][K2], ghost rows as psi
+    double* yfix;               // [J][K2]  outgoing rows of Psi_fix = B^{-1} c_fix
+    double* ifix;               // [J][K2]  incident-side rows of Psi_fix
+    double* phifix;             // [J][4]   W Psi_fix
+    double* zero_n;             // [n]      zeros (coef of the Psi_fix pass)
     double v, dt;
     int32_t bcL, bcR;
     double bcLv, bcRv;
@@ -74,5 +83,11 @@ int launch_phi_norm(const DevView& V, int buf, int slot, int prev_slot, double t
 int launch_oci_iteration(const DevView& V, int path, int src, int slot, int prev_slot, double tol,
                          cudaStream_t s);
 int launch_si_iteration(const DevView& V, int buf, int slot, int prev_slot, double tol, cudaStream_t s);
+// interface-reduced iteration (oci_reduced.cu)
+int launch_pack_operators(const DevView& V, cudaStream_t s);
+int launch_pack_y(const DevView& V, int buf, int ybuf, cudaStream_t s);
+int launch_split_fix(const DevView& V, int buf, cudaStream_t s);
+int launch_red_percell(const DevView& V, int ysrc, int slot, int prev_slot, double tol, cudaStream_t s);
+int launch_red_percell_final(const DevView& V, int ybase, int pdst, int cnt, int force, double tol, cudaStream_t s);
 
 }  // namespace oci

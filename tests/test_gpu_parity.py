@@ -17,11 +17,17 @@ def rel(a, b):
     return np.max(np.abs(a - b)) / (den if den > 0 else 1.0)
 
 
-def run_pair(p, scheme, steps, tol, max_iters, threads=8):
-    """Run `steps` time steps on both sides; return per-step (iters) and final fluxes."""
+FULL, REDUCED = 0, 1
+ITERATIONS = [pytest.param(FULL, id="full"), pytest.param(REDUCED, id="reduced")]
+
+
+def run_pair(p, scheme, steps, tol, max_iters, threads=8, iteration=None):
+    """Run `steps` time steps on both sides; return per-step (iters) and final fluxes.
+    iteration: OCI_ITERATION_FULL / _REDUCED (None = the library default); the oracle is always the
+    plain method (one LU solve per cell per iteration)."""
     import paper_2305_13555_b200 as P
     from oracle import Oracle
-    g = P.OCI.from_problem(p)
+    g = P.OCI.from_problem(p, iteration=iteration)
     o = Oracle.from_problem(p, threads=threads)
     gi, oi = [], []
     for k in range(steps):
@@ -73,23 +79,27 @@ def test_setup_block_inverse_matches_oracle(cfg, cells):
     g.close()
 
 
-@pytest.mark.parametrize("scheme", ["oci", "si"])
+SCHEMES = [pytest.param("oci", FULL, id="oci-full"), pytest.param("oci", REDUCED, id="oci-reduced"),
+           pytest.param("si", None, id="si")]
+
+
+@pytest.mark.parametrize("scheme,iteration", SCHEMES)
 @pytest.mark.parametrize("cfg,cells", SMALL)
-def test_fixed_iteration_parity(cfg, cells, scheme):
+def test_fixed_iteration_parity(cfg, cells, scheme, iteration):
     """tol < 0: exactly 5 iterations in each of 2 steps; Psi and phi within 1e-12."""
     p = make_problem(cfg, cells=cells)
-    r = run_pair(p, scheme, steps=2, tol=-1.0, max_iters=5)
+    r = run_pair(p, scheme, steps=2, tol=-1.0, max_iters=5, iteration=iteration)
     assert r["g_iters"] == [5, 5] == r["o_iters"]
     assert rel(r["g_psi"], r["o_psi"]) < 1e-12
     assert rel(r["g_phi"], r["o_phi"]) < 1e-12
     assert r["launches"] > 0
 
 
-@pytest.mark.parametrize("scheme", ["oci", "si"])
+@pytest.mark.parametrize("scheme,iteration", SCHEMES)
 @pytest.mark.parametrize("cfg,cells,steps", [(1, 20, 5), (2, 203, 4), (3, 300, 3), (4, 70, 2), (5, 37, 3)])
-def test_converged_parity(cfg, cells, steps, scheme):
+def test_converged_parity(cfg, cells, steps, scheme, iteration):
     p = make_problem(cfg, cells=cells)
-    r = run_pair(p, scheme, steps=steps, tol=p.tol, max_iters=p.max_iters)
+    r = run_pair(p, scheme, steps=steps, tol=p.tol, max_iters=p.max_iters, iteration=iteration)
     for a, b in zip(r["g_iters"], r["o_iters"]):
         assert abs(a - b) <= 1, (r["g_iters"], r["o_iters"])
     assert rel(r["g_psi"], r["o_psi"]) < 1e-9
@@ -98,8 +108,9 @@ def test_converged_parity(cfg, cells, steps, scheme):
 
 def test_config1_full_matches_golden_iteration_counts():
     p = make_problem(1)
-    r = run_pair(p, "oci", steps=5, tol=p.tol, max_iters=p.max_iters)
-    assert r["g_iters"] == r["o_iters"] == [7] * 5
+    for it in (FULL, REDUCED):
+        r = run_pair(p, "oci", steps=5, tol=p.tol, max_iters=p.max_iters, iteration=it)
+        assert r["g_iters"] == r["o_iters"] == [7] * 5
     r = run_pair(p, "si", steps=5, tol=p.tol, max_iters=p.max_iters)
     assert r["g_iters"] == r["o_iters"] == [8] * 5
 
@@ -117,7 +128,7 @@ def _custom(J, N, bcL, bcR, seed, hetero, dt=0.13):
                    _source=lambda step: q)
 
 
-@pytest.mark.parametrize("scheme", ["oci", "si"])
+@pytest.mark.parametrize("scheme,iteration", SCHEMES)
 @pytest.mark.parametrize("J,N,bcL,bcR,hetero", [
     (1, 2, (VAC, 0.0), (VAC, 0.0), False),        # one cell, S2: the smallest problem there is
     (1, 4, (REF, 0.0), (REF, 0.0), False),        # one cell between two mirrors
@@ -127,18 +138,18 @@ def _custom(J, N, bcL, bcR, seed, hetero, dt=0.13):
     (257, 8, (REF, 0.0), (VAC, 0.0), True),
     (31, 48, (VAC, 0.0), (REF, 0.0), False),      # n = 192
 ])
-def test_edge_cases(J, N, bcL, bcR, hetero, scheme):
+def test_edge_cases(J, N, bcL, bcR, hetero, scheme, iteration):
     p = _custom(J, N, bcL, bcR, seed=J * 100 + N, hetero=hetero)
-    r = run_pair(p, scheme, steps=2, tol=-1.0, max_iters=4)
+    r = run_pair(p, scheme, steps=2, tol=-1.0, max_iters=4, iteration=iteration)
     assert rel(r["g_psi"], r["o_psi"]) < 1e-12
     assert rel(r["g_phi"], r["o_phi"]) < 1e-12
-    r = run_pair(p, scheme, steps=2, tol=1e-10, max_iters=10_000)
+    r = run_pair(p, scheme, steps=2, tol=1e-10, max_iters=10_000, iteration=iteration)
     for a, b in zip(r["g_iters"], r["o_iters"]):
         assert abs(a - b) <= 1
     assert rel(r["g_psi"], r["o_psi"]) < 1e-9
 
 
-@pytest.mark.parametrize("scheme", ["oci"])
+@pytest.mark.parametrize("iteration", ITERATIONS)
 @pytest.mark.parametrize("J,N,bcL,bcR", [
     (1, 8, (REF, 0.0), (REF, 0.0)),          # n = 32: one K-tiled item, mostly empty
     (63, 24, (INC, 1.0), (REF, 0.0)),        # n = 96
@@ -147,7 +158,7 @@ def test_edge_cases(J, N, bcL, bcR, hetero, scheme):
     (200, 128, (VAC, 0.0), (INC, 0.7)),      # n = 512 (config-4 block size), 4 output tiles, ragged cells
     (130, 256, (REF, 0.0), (REF, 0.0)),      # n = 1024: the largest block the kernel takes
 ])
-def test_ktiled_kernel_shapes(J, N, bcL, bcR, scheme):
+def test_ktiled_kernel_shapes(J, N, bcL, bcR, iteration):
     """Shared-block sizes served by the K-tiled TMA/DMMA kernel: ragged cell and output tiles, both
     mirrors, the cross-CTA scalar-flux ticket (n > 128)."""
     import paper_2305_13555_b200 as P
@@ -155,10 +166,10 @@ def test_ktiled_kernel_shapes(J, N, bcL, bcR, scheme):
     g = P.OCI.from_problem(p)
     assert g.get_info()["apply_kernel"] == P.KERNEL_KTILED
     g.close()
-    r = run_pair(p, scheme, steps=2, tol=-1.0, max_iters=4, threads=16)
+    r = run_pair(p, "oci", steps=2, tol=-1.0, max_iters=4, threads=16, iteration=iteration)
     assert rel(r["g_psi"], r["o_psi"]) < 1e-12
     assert rel(r["g_phi"], r["o_phi"]) < 1e-12
-    r = run_pair(p, scheme, steps=2, tol=1e-10, max_iters=10_000, threads=16)
+    r = run_pair(p, "oci", steps=2, tol=1e-10, max_iters=10_000, threads=16, iteration=iteration)
     assert r["g_iters"] == r["o_iters"]
     assert rel(r["g_psi"], r["o_psi"]) < 1e-9
 
@@ -172,12 +183,13 @@ def test_apply_kernel_selection():
         g.close()
 
 
-def test_not_converged_status_and_restart():
+@pytest.mark.parametrize("iteration", ITERATIONS)
+def test_not_converged_status_and_restart(iteration):
     """max_iters reached -> status 1 with the state committed; set_flux restarts; many chunks."""
     import paper_2305_13555_b200 as P
     from oracle import Oracle
     p = make_problem(2, cells=64)
-    g, o = P.OCI.from_problem(p), Oracle.from_problem(p)
+    g, o = P.OCI.from_problem(p, iteration=iteration), Oracle.from_problem(p)
     for x in (g, o):
         x.set_source(p.source(0))
     assert g.oci_step(1e-10, 3)[:2] == (1, 3) == o.oci_step(1e-10, 3)[:2]
@@ -185,7 +197,7 @@ def test_not_converged_status_and_restart():
     # a tolerance that needs several launch chunks (> 64 iterations): thin cells, c = 0.999
     q = _custom(40, 4, (REF, 0.0), (REF, 0.0), seed=5, hetero=False, dt=50.0)
     q.sigma_s[:] = q.sigma_t * 0.999
-    g2, o2 = P.OCI.from_problem(q), Oracle.from_problem(q)
+    g2, o2 = P.OCI.from_problem(q, iteration=iteration), Oracle.from_problem(q)
     for x in (g2, o2):
         x.set_source(q.source(0))
     a, b = g2.oci_step(1e-10, 100_000), o2.oci_step(1e-10, 100_000)
@@ -227,13 +239,14 @@ def test_api_errors_on_device():
 
 
 # ---------------------------------------------------------------- full BASELINE sizes
+@pytest.mark.parametrize("iteration", ITERATIONS)
 @pytest.mark.parametrize("cfg,iters", [(3, 3), (4, 2), (5, 2)])
-def test_full_size_fixed_iterations(cfg, iters):
+def test_full_size_fixed_iterations(cfg, iters, iteration):
     """BASELINE.json's full sizes, in the launch configuration bench.py times: every output of a
     fixed-iteration step against the oracle (threaded over cells as the paper's CPU runs)."""
     from oracle import threads_available
     p = make_problem(cfg)
-    r = run_pair(p, "oci", steps=1, tol=-1.0, max_iters=iters, threads=threads_available())
+    r = run_pair(p, "oci", steps=1, tol=-1.0, max_iters=iters, threads=threads_available(), iteration=iteration)
     assert rel(r["g_psi"], r["o_psi"]) < 1e-12
     assert rel(r["g_phi"], r["o_phi"]) < 1e-12
 
@@ -244,3 +257,31 @@ def test_full_size_si_fixed_iterations_cfg3():
     r = run_pair(p, "si", steps=1, tol=-1.0, max_iters=2, threads=threads_available())
     assert rel(r["g_psi"], r["o_psi"]) < 1e-12
     assert rel(r["g_phi"], r["o_phi"]) < 1e-12
+
+
+@pytest.mark.parametrize("cfg,cells", [(2, 150), (5, 40)])
+def test_mixing_schemes_and_iteration_forms_on_one_context(cfg, cells):
+    """REDUCED keeps a packed copy of the outgoing rows between steps; every other way of changing the
+    state (si_step, a FULL step, set_flux) must invalidate it.  One context walks through all of them
+    next to one oracle; also checks the state mid-sequence."""
+    import paper_2305_13555_b200 as P
+    from oracle import Oracle
+    p = make_problem(cfg, cells=cells)
+    g, o = P.OCI.from_problem(p), Oracle.from_problem(p)
+    seq = [("oci", REDUCED), ("oci", REDUCED), ("si", None), ("oci", REDUCED), ("oci", FULL), ("oci", REDUCED),
+           ("flux", None), ("oci", REDUCED), ("oci", FULL), ("si", None)]
+    for k, (scheme, it) in enumerate(seq):
+        if scheme == "flux":
+            g.set_flux(p.psi0)
+            o.set_flux(p.psi0)
+            continue
+        if it is not None:
+            g.set_iteration(it)
+        g.set_source(p.source(k))
+        o.set_source(p.source(k))
+        a = (g.oci_step if scheme == "oci" else g.si_step)(-1.0, 3)
+        b = (o.oci_step if scheme == "oci" else o.si_step)(-1.0, 3)
+        assert a[:2] == b[:2] == (1, 3)
+        assert rel(g.get_angular_flux(), o.angular_flux()) < 1e-12, (k, scheme, it)
+        assert rel(g.get_scalar_flux(), o.scalar_flux()) < 1e-12, (k, scheme, it)
+    g.close()
