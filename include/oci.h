@@ -73,12 +73,16 @@ enum { OCI_KERNEL_GENERIC = 0, OCI_KERNEL_RESIDENT = 1, OCI_KERNEL_KTILED = 2, O
 /* Form of the OCI iteration inside oci_step (oci_set_iteration).  Both produce the iterates of
  * eq. (19), up to rounding order:
  * FULL    - every iteration applies the whole inverse, Psi^(l+1) = B^{-1} c^(l) (the paper's statement);
- * REDUCED - (default) only the 2N RHS rows fed by incident fluxes change within a step (the (l) terms
+ * REDUCED - only the 2N RHS rows fed by incident fluxes change within a step (the (l) terms
  *           of eqs. 27,28), so per step: Psi_fix = B^{-1} c_fix once; per iteration the 2N
  *           outgoing rows and the 4 scalar-flux rows, y^(l+1) = yfix + G inc^(l), phi^(l+1) = phifix +
  *           H inc^(l) with G = B^{-1}[O,I] diag|mu| (2N x 2N), H = W B^{-1}[:,I] diag|mu| (4 x 2N); after
  *           the last iteration the other 2N rows from the same inc (F = B^{-1}[I,I] diag|mu|). */
-enum { OCI_ITERATION_FULL = 0, OCI_ITERATION_REDUCED = 1 };
+enum { OCI_ITERATION_FULL = 0, OCI_ITERATION_REDUCED = 1, OCI_ITERATION_AUTO = 2 };
+/* AUTO (the default) = REDUCED wherever a kernel of the reduced form is the faster one for this
+ * problem: always on the PER_CELL path, on the SHARED path when a tensor-core kernel of the reduced
+ * form serves the block size (or the block is small); FULL otherwise.  oci_get_info reports the
+ * resolved form after oci_setup. */
 
 /* Kernel serving the REDUCED iteration: GEMV - batched GEMV, one operator per distinct block (any n);
  * RESIDENT - shared block, n in {64,128}: G, H resident in registers, fp64 tensor pipe;
@@ -140,7 +144,7 @@ int oci_set_source_dev(oci_ctx* ctx, const double* d_q);
 int oci_step(oci_ctx* ctx, double tol, int32_t max_iters, int32_t* iters, double* resid);
 int si_step(oci_ctx* ctx, double tol, int32_t max_iters, int32_t* iters, double* resid);
 
-/* Select the form of the OCI iteration (default OCI_ITERATION_REDUCED).  May be called at any time
+/* Select the form of the OCI iteration (default OCI_ITERATION_AUTO).  May be called at any time
  * after oci_create; takes effect at the next oci_step.  Errors: -1. */
 int oci_set_iteration(oci_ctx* ctx, int32_t iteration);
 

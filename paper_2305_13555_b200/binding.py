@@ -11,7 +11,7 @@ from . import build as _build
 BC_VACUUM, BC_INCIDENT_ISOTROPIC, BC_REFLECTING = 0, 1, 2
 PATH_SHARED, PATH_PER_CELL = 0, 1
 KERNEL_GENERIC, KERNEL_RESIDENT, KERNEL_KTILED, KERNEL_PER_CELL = 0, 1, 2, 3
-ITERATION_FULL, ITERATION_REDUCED = 0, 1
+ITERATION_FULL, ITERATION_REDUCED, ITERATION_AUTO = 0, 1, 2
 RKERNEL_GEMV, RKERNEL_RESIDENT, RKERNEL_KTILED = 0, 1, 2
 
 EXPORTED_SYMBOLS = [

@@ -45,7 +45,7 @@ struct oci_ctx {
     bool ready = false, have_flux = false;
     int cur = 0;                       // psi[cur] holds the current iterate
     // interface-reduced iteration (oci_reduced.cu)
-    int32_t iteration = OCI_ITERATION_REDUCED;
+    int32_t iteration = OCI_ITERATION_AUTO;
     int ycur = 0;                      // y[ycur] holds the outgoing rows of the current iterate ...
     bool y_valid = false;              // ... when this is set (cleared by set_flux, si_step, full-mode oci_step)
     int32_t predicted[2] = {0, 0};     // last iteration count of oci / si, sizes the launch chunk
@@ -238,13 +238,24 @@ int launch_fix_pass(oci_ctx* ctx)
     return k;
 }
 
+// AUTO: the reduced form wherever its kernel is the faster one (oci.h)
+int32_t resolved_iteration(const oci_ctx* ctx)
+{
+    if (ctx->iteration != OCI_ITERATION_AUTO) return ctx->iteration;
+    if (ctx->path == OCI_PATH_PER_CELL) return OCI_ITERATION_REDUCED;
+    if (ctx->ready && oci_red_resident_supported(ctx->V)) return OCI_ITERATION_REDUCED;
+    return ctx->n <= 32 ? OCI_ITERATION_REDUCED : OCI_ITERATION_FULL;
+}
+
 int launch_reduced_iteration(oci_ctx* ctx, int ysrc, int slot, int prev_slot, double tol)
 {
+    if (oci_red_resident_supported(ctx->V)) return launch_red_resident(ctx->V, ysrc, slot, prev_slot, tol, ctx->stream);
     return launch_red_percell(ctx->V, ysrc, slot, prev_slot, tol, ctx->stream);
 }
 
 int launch_reduced_final(oci_ctx* ctx, int ybase, int cnt, int force, double tol)
 {
+    if (oci_red_resident_supported(ctx->V)) return launch_red_resident_final(ctx->V, ybase, ctx->cur, cnt, force, tol, ctx->stream);
     return launch_red_percell_final(ctx->V, ybase, ctx->cur, cnt, force, tol, ctx->stream);
 }
 
@@ -256,7 +267,7 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
     if (max_iters < 1 || tol != tol) return fail(ctx, OCI_E_INVALID, "max_iters < 1 or tol is NaN");
     DevView& V = ctx->V;
     cudaStream_t s = ctx->stream;
-    const bool red = !si && ctx->iteration == OCI_ITERATION_REDUCED;
+    const bool red = !si && resolved_iteration(ctx) == OCI_ITERATION_REDUCED;
     const bool timed = ctx->timing && !si;
 
     ctx->launches += launch_cfix(V, ctx->cur, s);                         // a2 (+ a8 of the previous step)
@@ -578,8 +589,8 @@ int oci_get_info(const oci_ctx* ctx, oci_info* info)
     info->apply_kernel = ctx->path == OCI_PATH_PER_CELL ? OCI_KERNEL_PER_CELL
                          : (ctx->ready && oci_shared_fast_supported(ctx->V)) ? OCI_KERNEL_RESIDENT
                          : ctx->use_ktiled ? OCI_KERNEL_KTILED : OCI_KERNEL_GENERIC;
-    info->iteration = ctx->iteration;
-    info->reduced_kernel = OCI_RKERNEL_GEMV;
+    info->iteration = resolved_iteration(ctx);
+    info->reduced_kernel = (ctx->ready && oci_red_resident_supported(ctx->V)) ? OCI_RKERNEL_RESIDENT : OCI_RKERNEL_GEMV;
     return OCI_OK;
 }
 
@@ -620,7 +631,7 @@ int oci_get_aux_kernel_time(oci_ctx* ctx, double* fix_ms, int64_t* fix_launches,
 int oci_set_iteration(oci_ctx* ctx, int32_t iteration)
 {
     if (!ctx) return OCI_E_INVALID;
-    if (iteration != OCI_ITERATION_FULL && iteration != OCI_ITERATION_REDUCED)
+    if (iteration != OCI_ITERATION_FULL && iteration != OCI_ITERATION_REDUCED && iteration != OCI_ITERATION_AUTO)
         return fail(ctx, OCI_E_INVALID, "unknown iteration form");
     ctx->iteration = iteration;
     return OCI_OK;

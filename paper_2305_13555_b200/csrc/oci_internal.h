@@ -89,5 +89,8 @@ int launch_pack_y(const DevView& V, int buf, int ybuf, cudaStream_t s);
 int launch_split_fix(const DevView& V, int buf, cudaStream_t s);
 int launch_red_percell(const DevView& V, int ysrc, int slot, int prev_slot, double tol, cudaStream_t s);
 int launch_red_percell_final(const DevView& V, int ybase, int pdst, int cnt, int force, double tol, cudaStream_t s);
+bool oci_red_resident_supported(const DevView& V);
+int launch_red_resident(const DevView& V, int ysrc, int slot, int prev_slot, double tol, cudaStream_t s);
+int launch_red_resident_final(const DevView& V, int ybase, int pdst, int cnt, int force, double tol, cudaStream_t s);
 
 }  // namespace oci
