@@ -37,9 +37,10 @@ UNIT = "unknown-updates/s"
 
 # DRAM traffic per launch of the dominant kernel from the committed `ncu --set full` capture
 # (profiles/), bytes per launch; None where no capture exists for that config's kernel.
-NCU_TRAFFIC_BYTES = {3: 374.17e6,    # profiles/r1_resident_cfg3_full.txt: 272.80 MB read + 101.37 MB written
-                     4: 178.67e6,    # profiles/r1_ktiled_cfg4_full.txt:   136.89 MB read +  41.78 MB written
-                     5: 2168.2e6}    # profiles/r1_percell_cfg5_full.txt:  2164.5 MB read +   3.8 MB written
+# Keyed by (config, reduced iteration form?).
+NCU_TRAFFIC_BYTES = {(3, False): 374.17e6,    # profiles/r1_resident_cfg3_full.txt: 272.80 MB read + 101.37 MB written
+                     (4, False): 178.67e6,    # profiles/r1_ktiled_cfg4_full.txt:   136.89 MB read +  41.78 MB written
+                     (5, False): 2168.2e6}    # profiles/r1_percell_cfg5_full.txt:  2164.5 MB read +   3.8 MB written
 
 
 def load_peaks():
@@ -353,25 +354,40 @@ def run_ours(args):
     kms, klaunch = g.get_kernel_time()
     g.enable_kernel_timing(False)
     k_avg_ms = kms / max(klaunch, 1)
+    # work the timed kernel EXECUTES per launch: the full apply is [n x n] per cell; the reduced
+    # iteration is [(2N+4) x 2N] per cell (G and the four scalar-flux rows H)
+    reduced = info["iteration"] == P.ITERATION_REDUCED
+    K2 = n // 2
+    M_op, K_op = (K2 + 4, K2) if reduced else (n, n)
+    aux = g.get_aux_kernel_time()
+    fix_ms, fix_n, fin_ms, fin_n = aux["fix_ms"], aux["fix_launches"], aux["final_ms"], aux["final_launches"]
+    breakdown = {"iteration_kernel_ms": k_avg_ms, "iterations_per_step": klaunch / args.steps,
+                 "fix_pass_ms_per_step": fix_ms / max(fix_n, 1) if reduced else None,
+                 "final_pass_ms_per_step": fin_ms / max(fin_n, 1) if reduced else None,
+                 "operator_rows_x_cols": [M_op, K_op], "form": "reduced" if reduced else "full"}
     if shared:
-        flops = 2.0 * n * n * p.cells
+        flops = 2.0 * M_op * K_op * p.cells
         peak_live = P.probe_fp64_tensor_tflops(f"cuda:{local}")
         nominal_ratio = 45.0 / 2250.0        # guide: B200 fp64 tensor 45 TF vs bf16 2250 TF nominal
         peak_scaled = peaks["bf16_tflops"] * nominal_ratio
         peak = max(peak_live, peak_scaled)
         achieved = flops / (k_avg_ms * 1e-3) * 1e-12
         roofline = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                    "traffic": NCU_TRAFFIC_BYTES.get(args.config),
-                    "kernel": "oci apply (eq. 19), fp64 DMMA", "algorithmic_flops_per_launch": flops,
+                    "traffic": NCU_TRAFFIC_BYTES.get((args.config, reduced)),
+                    "kernel": "oci %s iteration (eq. 19), fp64 DMMA" % breakdown["form"], "algorithmic_flops_per_launch": flops,
                     "avg_launch_ms": k_avg_ms, "launches_timed": klaunch,
                     "peak_source": f"max(live DMMA issue-rate probe {peak_live:.2f}, MEASURED_PEAKS bf16 {peak_src} x 45/2250 = {peak_scaled:.2f})"}
     else:
-        bytes_ = p.cells * (n * n * 8.0 + 4.0 * n * 8.0 + 64.0)   # inverse + c_fix, 2 half rows, Psi out; phi
+        if reduced:   # operator + gathered half rows, yfix in, y out; phifix and old phi in, phi out
+            bytes_ = p.cells * (M_op * K_op * 8.0 + 3.0 * K2 * 8.0 + 96.0)
+        else:         # inverse + c_fix, 2 half rows, Psi out; phi
+            bytes_ = p.cells * (n * n * 8.0 + 4.0 * n * 8.0 + 64.0)
         achieved = bytes_ / (k_avg_ms * 1e-3) * 1e-9
         roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                    "frac": achieved / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get(args.config),
-                    "kernel": "oci apply (eq. 19), batched GEMV", "algorithmic_bytes_per_launch": bytes_,
+                    "frac": achieved / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get((args.config, reduced)),
+                    "kernel": "oci %s iteration (eq. 19), batched GEMV" % breakdown["form"], "algorithmic_bytes_per_launch": bytes_,
                     "avg_launch_ms": k_avg_ms, "launches_timed": klaunch, "peak_source": f"MEASURED_PEAKS hbm_gbs ({peak_src})"}
+    roofline["step_breakdown"] = breakdown
 
     # ---- end to end through the C ABI with host buffers
     e2e_val, h2d, d2h = time_gpu_e2e(torch, g, p, args.steps)
