@@ -41,4 +41,35 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
                  : "d"(a), "d"(b));
 }
 
+// ---- packed interface layout of the reduced step (oci_reduced.cu has the definition)
+__device__ __forceinline__ int o_row(int q, int N)   // full index of packed outgoing row q
+{
+    const int N2 = N >> 1;
+    const int half = q >= N, r = q - half * N;
+    const int h = r >= N2, mm = r - h * N2;
+    return 4 * (half * N2 + mm) + (half ? 2 * h + 1 : 2 * h);
+}
+
+// packed index of the mirror image (m -> N-1-m) of packed row q, same time slot
+__device__ __forceinline__ int mirror_q(int q, int N)
+{
+    const int N2 = N >> 1;
+    const int half = q >= N, r = q - half * N;
+    const int h = r >= N2, mm = r - h * N2;
+    return (1 - half) * N + h * N2 + (N2 - 1 - mm);
+}
+
+// First iteration index (1-based) whose norms satisfy the stopping rule, 0 if none of the `cnt` queued
+// iterations did.  Slots past the last executed iteration are still zero from the memset, and
+// converged(tol, 0, 0) holds for tol >= 0, so the scan must stop at the first hit.
+__device__ __forceinline__ int first_converged(const unsigned long long* __restrict__ norms, int cnt, double tol)
+{
+    for (int i = 0; i < cnt; ++i) {
+        const double d = __longlong_as_double((long long)__ldcg(norms + 2 * i + 0));
+        const double r = __longlong_as_double((long long)__ldcg(norms + 2 * i + 1));
+        if (converged(tol, d, r)) return i + 1;
+    }
+    return 0;
+}
+
 }  // namespace oci

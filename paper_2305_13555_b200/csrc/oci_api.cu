@@ -46,8 +46,10 @@ struct oci_ctx {
     int cur = 0;                       // psi[cur] holds the current iterate
     // interface-reduced iteration (oci_reduced.cu)
     int32_t iteration = OCI_ITERATION_AUTO;
-    int ycur = 0;                      // y[ycur] holds the outgoing rows of the current iterate ...
-    bool y_valid = false;              // ... when this is set (cleared by set_flux, si_step, full-mode oci_step)
+    int ycur = 0;                      // (y[ycur], z) hold the current iterate in packed form ...
+    bool yz_valid = false;             // ... when this is set (cleared by set_flux, si_step, a FULL-form oci_step)
+    bool psi_valid = false;            // psi[cur] holds the current iterate in the full layout (cleared by a REDUCED step)
+    int32_t red_kernel = OCI_RKERNEL_GEMV;
     int32_t predicted[2] = {0, 0};     // last iteration count of oci / si, sizes the launch chunk
     unsigned long long* h_norms = nullptr;   // pinned
     // timing
@@ -124,7 +126,7 @@ void gauss_legendre(int N, std::vector<double>& mu, std::vector<double>& w)
 
 struct Layout {
     int64_t binv, psi0, psi1, cfix, phi, Q, qs, dx, sig, sigs, blk, rep, mu, w, coef, ainv4, si_scan, phi_part, norms, tickets, flags,
-        rop, fop, y0, y1, yfix, ifix, phifix, zero_n, total;
+        xop, rop, fop, y0, y1, z, yfix, ifix, phifix, q16, total;
 };
 
 int64_t align_up(int64_t x) { return (x + 255) & ~int64_t(255); }
@@ -160,15 +162,17 @@ Layout make_layout(int64_t J, int32_t N, int64_t nblk)
     L.tickets = take(nblk == 1 ? ((J + 63) / 64) * 4 : 0);
     L.flags = take(256);
     {
-        const int64_t K2 = n / 2, MO = K2 + 8;
-        L.rop = take(nblk * MO * K2 * 8);
+        const int64_t K2 = n / 2;
+        L.xop = take(nblk * (2 * K2 + 8) * (K2 + 16) * 8);
+        L.rop = take(nblk * (K2 + 8) * K2 * 8);
         L.fop = take(nblk * K2 * K2 * 8);
         L.y0 = take((J + 2) * K2 * 8);
         L.y1 = take((J + 2) * K2 * 8);
+        L.z = take(J * K2 * 8);
         L.yfix = take(J * K2 * 8);
         L.ifix = take(J * K2 * 8);
         L.phifix = take(J * 4 * 8);
-        L.zero_n = take(n * 8);
+        L.q16 = take(nblk == 1 && N % 64 == 0 ? J * 16 * 8 : 0);
     }
     L.total = o;
     return L;
@@ -222,41 +226,28 @@ int launch_oci_iteration_any(oci_ctx* ctx, int src, int slot, int prev_slot, dou
     return k;
 }
 
-// One Psi_fix pass of the reduced iteration: the ordinary apply kernel of this path with a zero gather
-// coefficient (c = c_fix), its scalar flux going to phifix and its norms to a slot nobody reads; then
-// the split into the packed outgoing / incident-side halves.
-int launch_fix_pass(oci_ctx* ctx)
-{
-    DevView Vf = ctx->V;
-    Vf.coef = Vf.zero_n;
-    Vf.phi = Vf.phifix;
-    const DevView saved = ctx->V;
-    ctx->V = Vf;
-    int k = launch_oci_iteration_any(ctx, ctx->cur, kScratchSlot, -1, -1.0);
-    ctx->V = saved;
-    k += launch_split_fix(ctx->V, ctx->cur ^ 1, ctx->stream);
-    return k;
-}
-
-// AUTO: the reduced form wherever its kernel is the faster one (oci.h)
+// AUTO: the reduced form wherever a kernel of that form is the faster one (oci.h)
 int32_t resolved_iteration(const oci_ctx* ctx)
 {
     if (ctx->iteration != OCI_ITERATION_AUTO) return ctx->iteration;
     if (ctx->path == OCI_PATH_PER_CELL) return OCI_ITERATION_REDUCED;
-    if (ctx->ready && oci_red_resident_supported(ctx->V)) return OCI_ITERATION_REDUCED;
+    if (ctx->ready && ctx->red_kernel != OCI_RKERNEL_GEMV) return OCI_ITERATION_REDUCED;
     return ctx->n <= 32 ? OCI_ITERATION_REDUCED : OCI_ITERATION_FULL;
 }
 
-int launch_reduced_iteration(oci_ctx* ctx, int ysrc, int slot, int prev_slot, double tol)
+int launch_reduced_pass(oci_ctx* ctx, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force)
 {
-    if (oci_red_resident_supported(ctx->V)) return launch_red_resident(ctx->V, ysrc, slot, prev_slot, tol, ctx->stream);
-    return launch_red_percell(ctx->V, ysrc, slot, prev_slot, tol, ctx->stream);
+    if (ctx->red_kernel == OCI_RKERNEL_RESIDENT)
+        return launch_red_resident(ctx->V, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
+    return launch_red_gemv(ctx->V, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
 }
 
-int launch_reduced_final(oci_ctx* ctx, int ybase, int cnt, int force, double tol)
+// the full-layout Psi on demand (a change of layout, no arithmetic)
+int ensure_psi(oci_ctx* ctx)
 {
-    if (oci_red_resident_supported(ctx->V)) return launch_red_resident_final(ctx->V, ybase, ctx->cur, cnt, force, tol, ctx->stream);
-    return launch_red_percell_final(ctx->V, ybase, ctx->cur, cnt, force, tol, ctx->stream);
+    if (ctx->psi_valid) return 0;
+    ctx->psi_valid = true;
+    return launch_unpack_yz(ctx->V, ctx->cur, ctx->ycur, ctx->stream);
 }
 
 int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iters, double* resid)
@@ -270,18 +261,20 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
     const bool red = !si && resolved_iteration(ctx) == OCI_ITERATION_REDUCED;
     const bool timed = ctx->timing && !si;
 
-    ctx->launches += launch_cfix(V, ctx->cur, s);                         // a2 (+ a8 of the previous step)
     if (red) {
-        if (!ctx->y_valid) {
-            ctx->launches += launch_pack_y(V, ctx->cur, 0, s);
+        if (!ctx->yz_valid) {
+            ctx->launches += launch_pack_yz(V, ctx->cur, 0, s);
             ctx->ycur = 0;
-            ctx->y_valid = true;
+            ctx->yz_valid = true;
         }
+        ctx->psi_valid = false;
         if (timed) CK(cudaEventRecord(ctx->ev_aux[0], s));
-        ctx->launches += launch_fix_pass(ctx);
+        ctx->launches += launch_reduced_pass(ctx, PASS_FIX, ctx->ycur, 0, -1, tol, 0, 0);   // a2 (+ a8 of the previous step)
         if (timed) CK(cudaEventRecord(ctx->ev_aux[1], s));
     } else {
-        ctx->y_valid = false;
+        ctx->launches += ensure_psi(ctx);
+        ctx->yz_valid = false;
+        ctx->launches += launch_cfix(V, ctx->cur, s);                      // a2 (+ a8 of the previous step)
     }
     int32_t done_iters = 0;
     bool conv = false;
@@ -296,7 +289,7 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
         for (int32_t i = 0; i < cnt; ++i) {
             if (timed) CK(cudaEventRecord(ctx->ev[2 * i], s));
             if (si) ctx->launches += launch_si_iteration(V, ctx->cur, i, i - 1, tol, s);
-            else if (red) ctx->launches += launch_reduced_iteration(ctx, (ctx->ycur + done_iters + i) & 1, i, i - 1, tol);
+            else if (red) ctx->launches += launch_reduced_pass(ctx, PASS_ITER, (ctx->ycur + done_iters + i) & 1, i, i - 1, tol, 0, 0);
             else ctx->launches += launch_oci_iteration_any(ctx, (ctx->cur + done_iters + i) & 1, i, i - 1, tol);
             if (timed) CK(cudaEventRecord(ctx->ev[2 * i + 1], s));
         }
@@ -304,7 +297,7 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
             // finalisation, queued before the read-back: finds the last iteration on the device and
             // does nothing if this chunk neither converged nor ends at max_iters
             if (timed) CK(cudaEventRecord(ctx->ev_aux[2], s));
-            ctx->launches += launch_reduced_final(ctx, (ctx->ycur + done_iters) & 1, cnt, done_iters + cnt >= max_iters, tol);
+            ctx->launches += launch_reduced_pass(ctx, PASS_FINAL, (ctx->ycur + done_iters) & 1, 0, -1, tol, cnt, done_iters + cnt >= max_iters);
             if (timed) CK(cudaEventRecord(ctx->ev_aux[3], s));
         }
         CK(cudaMemcpyAsync(ctx->h_norms, V.norms, sizeof(unsigned long long) * 2 * cnt, cudaMemcpyDeviceToHost, s));
@@ -338,7 +331,7 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
         ctx->aux_ms[0] += ms;
         ctx->aux_launches[0] += 1;
     }
-    if (red) ctx->ycur = (ctx->ycur + done_iters) & 1;                     // Psi^(L) was written to psi[cur]
+    if (red) ctx->ycur = (ctx->ycur + done_iters) & 1;                     // a8: (y[ycur], z) is the committed state
     else if (!si) ctx->cur = (ctx->cur + done_iters) & 1;                  // a8: pointer convention
     ctx->predicted[si ? 1 : 0] = done_iters;
     if (iters) *iters = done_iters;
@@ -424,14 +417,16 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     V.tickets = (int32_t*)(base + L.tickets);
     V.norms = (unsigned long long*)(base + L.norms);
     V.flags = (int32_t*)(base + L.flags);
+    V.xop = (double*)(base + L.xop);
     V.rop = (double*)(base + L.rop);
     V.fop = (double*)(base + L.fop);
     V.y[0] = (double*)(base + L.y0) + n / 2;      // skip the left ghost row
     V.y[1] = (double*)(base + L.y1) + n / 2;
+    V.z = (double*)(base + L.z);
     V.yfix = (double*)(base + L.yfix);
     V.ifix = (double*)(base + L.ifix);
     V.phifix = (double*)(base + L.phifix);
-    V.zero_n = (double*)(base + L.zero_n);
+    V.q16 = (double*)(base + L.q16);
     V.v = ctx->v; V.dt = ctx->dt;
     V.bcL = ctx->bcL.kind; V.bcR = ctx->bcR.kind;
     V.bcLv = ctx->bcL.value; V.bcRv = ctx->bcR.value;
@@ -446,7 +441,7 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     // everything the kernels may read before a set_* call must be finite: zero the state
     CK(cudaMemsetAsync(base + L.psi0, 0, (size_t)(L.cfix - L.psi0), s));
     CK(cudaMemsetAsync(base + L.cfix, 0, (size_t)(L.dx - L.cfix), s));
-    CK(cudaMemsetAsync(base + L.phi_part, 0, (size_t)(L.rop - L.phi_part), s));
+    CK(cudaMemsetAsync(base + L.phi_part, 0, (size_t)(L.xop - L.phi_part), s));
     CK(cudaMemsetAsync(base + L.y0, 0, (size_t)(L.total - L.y0), s));
     CK(cudaMemcpyAsync(V.dx, ctx->dx.data(), ctx->J * 8, cudaMemcpyHostToDevice, s));
     CK(cudaMemcpyAsync(V.sig, ctx->sig.data(), ctx->J * 8, cudaMemcpyHostToDevice, s));
@@ -477,9 +472,11 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     }
     ctx->use_ktiled = ctx->path == OCI_PATH_SHARED && !oci_shared_fast_supported(V) && oci_ktiled_supported(V) &&
                       oci_ktiled_prepare(V, &ctx->maps);
+    ctx->red_kernel = oci_red_resident_supported(V) ? OCI_RKERNEL_RESIDENT : OCI_RKERNEL_GEMV;
     ctx->cur = 0;
     ctx->ycur = 0;
-    ctx->y_valid = false;
+    ctx->yz_valid = false;
+    ctx->psi_valid = true;
     ctx->predicted[0] = ctx->predicted[1] = 0;
     ctx->ready = true;
     return OCI_OK;
@@ -489,7 +486,8 @@ static int set_flux_common(oci_ctx* ctx, const double* d_edge)
 {
     ctx->launches += launch_set_flux(ctx->V, d_edge, 0, ctx->stream);
     ctx->cur = 0;
-    ctx->y_valid = false;
+    ctx->yz_valid = false;
+    ctx->psi_valid = true;
     ctx->launches += launch_phi_norm(ctx->V, 0, 0, -1, -1.0, false, ctx->stream);   // phi^(0), ghost rows
     CK(cudaStreamSynchronize(ctx->stream));
     CK(cudaGetLastError());
@@ -557,6 +555,7 @@ int oci_get_scalar_flux(const oci_ctx* ctx, double* phi)
 }
 int oci_get_angular_flux(const oci_ctx* ctx, double* psi)
 {
+    if (ctx && ctx->ready) const_cast<oci_ctx*>(ctx)->launches += ensure_psi(const_cast<oci_ctx*>(ctx));
     return get_common(ctx, psi, ctx ? ctx->V.psi[ctx->cur] : nullptr, ctx ? (size_t)ctx->J * ctx->n * 8 : 0,
                       cudaMemcpyDeviceToHost, true);
 }
@@ -566,6 +565,7 @@ int oci_get_scalar_flux_dev(const oci_ctx* ctx, double* d_phi)
 }
 int oci_get_angular_flux_dev(const oci_ctx* ctx, double* d_psi)
 {
+    if (ctx && ctx->ready) const_cast<oci_ctx*>(ctx)->launches += ensure_psi(const_cast<oci_ctx*>(ctx));
     return get_common(ctx, d_psi, ctx ? ctx->V.psi[ctx->cur] : nullptr, ctx ? (size_t)ctx->J * ctx->n * 8 : 0,
                       cudaMemcpyDeviceToDevice, false);
 }
@@ -590,7 +590,7 @@ int oci_get_info(const oci_ctx* ctx, oci_info* info)
                          : (ctx->ready && oci_shared_fast_supported(ctx->V)) ? OCI_KERNEL_RESIDENT
                          : ctx->use_ktiled ? OCI_KERNEL_KTILED : OCI_KERNEL_GENERIC;
     info->iteration = resolved_iteration(ctx);
-    info->reduced_kernel = (ctx->ready && oci_red_resident_supported(ctx->V)) ? OCI_RKERNEL_RESIDENT : OCI_RKERNEL_GEMV;
+    info->reduced_kernel = ctx->red_kernel;
     return OCI_OK;
 }
 

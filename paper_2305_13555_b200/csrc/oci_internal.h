@@ -42,14 +42,16 @@ struct DevView {
     int32_t* tickets;           // [ceil(J/64)]  arrival counters of the K-tiled kernel's cell tiles (0 between launches)
     unsigned long long* norms;  // [kNormSlots][2]  bit patterns of (d, r), atomicMax targets
     int32_t* flags;             // [0] = 1 + index of a singular block, 0 if none
-    // ---- interface-reduced iteration (oci_reduced.cu), K2 = 2N, MO = K2 + 8
-    double* rop;                // [nblk][MO][K2]  rows 0..K2-1: G = B^{-1}[O,I] diag|mu|; K2..K2+3: H = W B^{-1}[:,I] diag|mu|; rest 0
+    // ---- interface-reduced step (oci_reduced.cu), K2 = 2N
+    double* xop;                // [nblk][2*K2+8][K2+16]  FIX operator X (rows: O, I, scalar flux; zero padded)
+    double* rop;                // [nblk][K2+8][K2]  rows 0..K2-1: G = B^{-1}[O,I] diag|mu|; K2..K2+3: H = W B^{-1}[:,I] diag|mu|; rest 0
     double* fop;                // [nblk][K2][K2]  F = B^{-1}[I,I] diag|mu|
-    double* y[2];               // ping-pong interface iterates (outgoing rows of Psi, packed), [(J+2)][K2], ghost rows as psi
-    double* yfix;               // [J][K2]  outgoing rows of Psi_fix = B^{-1} c_fix
-    double* ifix;               // [J][K2]  incident-side rows of Psi_fix
+    double* y[2];               // ping-pong interface iterates (O rows of Psi, packed), [(J+2)][K2], ghost rows as psi
+    double* z;                  // [J][K2]  I rows of Psi, packed (written by the FINAL pass)
+    double* yfix;               // [J][K2]  O rows of Psi_fix = B^{-1} c_fix
+    double* ifix;               // [J][K2]  I rows of Psi_fix
     double* phifix;             // [J][4]   W Psi_fix
-    double* zero_n;             // [n]      zeros (coef of the Psi_fix pass)
+    double* q16;                // [J][16]  Q padded to one 128-byte row (K-tiled FIX pass only; else unused)
     double v, dt;
     int32_t bcL, bcR;
     double bcLv, bcRv;
@@ -83,14 +85,17 @@ int launch_phi_norm(const DevView& V, int buf, int slot, int prev_slot, double t
 int launch_oci_iteration(const DevView& V, int path, int src, int slot, int prev_slot, double tol,
                          cudaStream_t s);
 int launch_si_iteration(const DevView& V, int buf, int slot, int prev_slot, double tol, cudaStream_t s);
-// interface-reduced iteration (oci_reduced.cu)
+// interface-reduced step (oci_reduced.cu, oci_reduced_resident.cu, oci_reduced_ktiled.cu)
+enum { PASS_FIX = 0, PASS_ITER = 1, PASS_FINAL = 2 };
 int launch_pack_operators(const DevView& V, cudaStream_t s);
-int launch_pack_y(const DevView& V, int buf, int ybuf, cudaStream_t s);
-int launch_split_fix(const DevView& V, int buf, cudaStream_t s);
-int launch_red_percell(const DevView& V, int ysrc, int slot, int prev_slot, double tol, cudaStream_t s);
-int launch_red_percell_final(const DevView& V, int ybase, int pdst, int cnt, int force, double tol, cudaStream_t s);
+int launch_pack_yz(const DevView& V, int buf, int ybuf, cudaStream_t s);
+int launch_unpack_yz(const DevView& V, int buf, int ybuf, cudaStream_t s);
+// ybase: FIX - the y buffer of the current iterate; ITER - the source buffer; FINAL - the source buffer
+// of the first of the `cnt` queued iterations
+int launch_red_gemv(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
+                    cudaStream_t s);
 bool oci_red_resident_supported(const DevView& V);
-int launch_red_resident(const DevView& V, int ysrc, int slot, int prev_slot, double tol, cudaStream_t s);
-int launch_red_resident_final(const DevView& V, int ybase, int pdst, int cnt, int force, double tol, cudaStream_t s);
+int launch_red_resident(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
+                        cudaStream_t s);
 
 }  // namespace oci

@@ -1,24 +1,26 @@
-// Interface-reduced OCI iteration (oci_reduced.cu has the derivation), shared block, K2 = 2N in {32, 64}
-// (n = 64, 128: configs 2 and 3): the fp64 tensor-core form.
+// Interface-reduced OCI step (oci_reduced.cu has the derivation), shared block, K2 = 2N in {32, 64}
+// (n = 64, 128: configs 2 and 3): the fp64 tensor-core form of the three passes.
 //
-//   iteration:     [y^(l+1) | phi^(l+1)][j] = [yfix | phifix][j] + [G; H] inc^(l)[j]     ((K2+8) x K2, rows padded)
-//   finalisation:  Psi^(L)[j][I] = ifix[j] + F inc^(L-1)[j],  Psi^(L)[j][O] = y^(L)[j]      (K2 x K2)
+//   FIX  :  [yfix | phifix][j], ifix[j] = X [psi_{k-1/2}[j]; Q[j]]                      two row groups of X, K = K2+4
+//   ITER :  [y^(l+1) | phi^(l+1)][j] = [yfix | phifix][j] + [G; H] inc^(l)[j]           (K2+8) x K2, rows padded
+//   FINAL:  z[j] = ifix[j] + F inc^(L-1)[j]                                            K2 x K2
 //
-// At config 3 one iteration is 1.1 GFLOP against 0.2 GB of HBM traffic: the fp64 tensor pipe and HBM are
+// At config 3 one iteration is 1.2 GFLOP against 0.2 GB of HBM traffic: the fp64 tensor pipe and HBM are
 // equally loaded (arithmetic intensity 5.7 flop/B = the machine balance), so the design keeps both busy
 // with the least synchronisation possible:
 //
 //   * one persistent CTA per SM, 8 warps, and EVERY WARP IS AN INDEPENDENT WORKER on tiles of 16 cells:
 //     it owns all output rows of its cells, so there is no cross-warp reduction and no CTA barrier after
-//     start-up (the scalar-flux rows H are just one more n8 block of the same warp);
-//   * the operator (39 KB at K2 = 64) lives in shared memory, rows padded to K2+4 doubles so that the
-//     DMMA fragment loads are bank-conflict free; per k-step a warp loads 2 A fragments (cells) and
-//     NB B fragments (operator) for 2*NB DMMA.8x8x4: shared-memory bandwidth is ~30 % used;
-//   * the RHS needs NO assembly: inc[j] = [y[j+1][0:N] | y[j-1][N:2N]] (|mu| is folded into the operator),
-//     so each lane issues one 1-D bulk TMA copy (cp.async.bulk, half a row of a neighbour) straight into
-//     the warp's private two-stage ring; the next tile is requested before the current one is computed;
-//   * yfix / phifix / old phi are read straight from global memory in accumulator layout at the start
-//     of the tile and only consumed in the epilogue (added to the accumulators, 16-byte stores).
+//     start-up (the scalar-flux rows are just one more n8 block of the same warp);
+//   * the operator (39 KB for ITER, 74 KB for FIX at K2 = 64) lives in shared memory, rows padded to K2+4
+//     doubles so that the DMMA fragment loads are bank-conflict free; per k-step a warp loads 2 A fragments
+//     (cells) and NB B fragments (operator) for 2*NB DMMA.8x8x4;
+//   * the input vectors need NO assembly: inc[j] = [y[j+1][0:N] | y[j-1][N:2N]] (|mu| is folded into the
+//     operator) and psi_{k-1/2}[j] = four runs of N/2 doubles of y[j], z[j] (alpha folded into X), so each
+//     lane issues 1-D bulk TMA copies (cp.async.bulk) straight into the warp's private two-stage ring; the
+//     next tile is requested before the current one is computed;
+//   * yfix / ifix / phifix / old phi are read straight from global memory in accumulator layout at the
+//     start of the tile and only consumed in the epilogue (added to the accumulators, 16-byte stores).
 #include "device_utils.cuh"
 
 namespace oci {
@@ -58,39 +60,50 @@ __device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t
                  : "memory");
 }
 
-__device__ __forceinline__ int first_converged_rr(const unsigned long long* __restrict__ norms, int cnt, double tol)
-{
-    for (int i = 0; i < cnt; ++i) {
-        const double d = __longlong_as_double((long long)__ldcg(norms + 2 * i + 0));
-        const double r = __longlong_as_double((long long)__ldcg(norms + 2 * i + 1));
-        if (converged(tol, d, r)) return i + 1;
-    }
-    return 0;
-}
 
-template <int K2, bool FINAL>
+template <int K2, int PASS>
 struct RCfg {
-    static constexpr int LD = K2 + 4;                         // padded row (doubles): LD = 4 (mod 16)
-    static constexpr int NB = FINAL ? K2 / 8 : K2 / 8 + 1;    // n8 output blocks (the last one = phi rows)
-    static constexpr int KS = K2 / 4;
-    static constexpr int OP_DOUBLES = NB * 8 * LD;
+    static constexpr int KIN = PASS == PASS_FIX ? K2 + 4 : K2;          // operator columns (k extent)
+    static constexpr int LD = K2 + 4;                                    // padded row (doubles): LD = 4 (mod 16)
+    static constexpr int NB0 = PASS == PASS_FINAL ? K2 / 8 : K2 / 8 + 1; // n8 blocks of row group 0 (last = scalar flux)
+    static constexpr int NB1 = PASS == PASS_FIX ? K2 / 8 : 0;            // row group 1 (FIX only: the I rows)
+    static constexpr int KS = KIN / 4;
+    static constexpr int OP_DOUBLES = (NB0 + NB1) * 8 * LD;
     static constexpr int STAGE_DOUBLES = RT_M * LD;
     static constexpr size_t SMEM = sizeof(double) * (OP_DOUBLES + RT_WARPS * RT_STAGES * STAGE_DOUBLES) +
                                    RT_WARPS * RT_STAGES * 8 + 16;
 };
 
+// acc[g][t] += A(cells 8g..8g+7) . Op(rows 8t..8t+7)^T over KS k-steps
+template <int NB, int KS, int LD>
+__device__ __forceinline__ void tile_dmma(double (&acc)[2][NB][2], const double* __restrict__ arow, const double* __restrict__ brow)
+{
+#pragma unroll 4
+    for (int ks = 0; ks < KS; ++ks) {
+        double a[2], b[NB];
+#pragma unroll
+        for (int g = 0; g < 2; ++g) a[g] = arow[(8 * g) * LD + 4 * ks];
+#pragma unroll
+        for (int t = 0; t < NB; ++t) b[t] = brow[(8 * t) * LD + 4 * ks];
+#pragma unroll
+        for (int g = 0; g < 2; ++g)
+#pragma unroll
+            for (int t = 0; t < NB; ++t) dmma(acc[g][t][0], acc[g][t][1], a[g], b[t]);
+    }
+}
+
 }  // namespace
 
-template <int K2, bool FINAL>
+template <int K2, int PASS>
 __global__ void __launch_bounds__(RT_WARPS * 32, 1)
-oci_red_resident_kernel(DevView V, int ybase, int slot, int prev_slot, double tol, int pdst, int cnt, int force)
+oci_red_resident_kernel(DevView V, int ybase, int slot, int prev_slot, double tol, int cnt, int force)
 {
-    using C = RCfg<K2, FINAL>;
+    using C = RCfg<K2, PASS>;
     int ysrc = ybase;
-    if (!FINAL) {
+    if (PASS == PASS_ITER) {
         if (step_done(V.norms, prev_slot, tol)) return;
-    } else {
-        int L = first_converged_rr(V.norms, cnt, tol);
+    } else if (PASS == PASS_FINAL) {
+        int L = first_converged(V.norms, cnt, tol);
         if (L == 0) {
             if (!force) return;
             L = cnt;
@@ -98,23 +111,27 @@ oci_red_resident_kernel(DevView V, int ybase, int slot, int prev_slot, double to
         ysrc = (ybase + L - 1) & 1;
     }
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double* op_s = reinterpret_cast<double*>(smem_raw);                         // [NB*8][LD]
+    double* op_s = reinterpret_cast<double*>(smem_raw);                         // [(NB0+NB1)*8][LD]
     double* ring = op_s + C::OP_DOUBLES;                                        // [warps][stages][RT_M][LD]
     uint64_t* full = reinterpret_cast<uint64_t*>(ring + RT_WARPS * RT_STAGES * C::STAGE_DOUBLES);
 
-    constexpr int N = K2 / 2, n = 2 * K2;
+    constexpr int N = K2 / 2, N2 = K2 / 4;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g4 = lane >> 2, t4 = lane & 3;
     const int64_t J = V.J;
     const double* __restrict__ Ys = V.y[ysrc];
     double* __restrict__ Yd = V.y[ysrc ^ 1];
 
-    // operator -> shared memory (rows K2.. of the iteration operator: H, then zero padding)
+    // operator -> shared memory.  FIX: X rows [O | I | phi] are regrouped as [O | phi | I]
     {
-        const double* __restrict__ src = FINAL ? V.fop : V.rop;
-        for (int e = tid; e < C::NB * 8 * (K2 / 2); e += RT_WARPS * 32) {
-            const int r = e / (K2 / 2), c2 = e - r * (K2 / 2);
-            *reinterpret_cast<double2*>(op_s + r * C::LD + 2 * c2) = *reinterpret_cast<const double2*>(src + (size_t)r * K2 + 2 * c2);
+        const double* __restrict__ src = PASS == PASS_FIX ? V.xop : PASS == PASS_ITER ? V.rop : V.fop;
+        constexpr int GLD = PASS == PASS_FIX ? K2 + 16 : K2;
+        constexpr int C2 = C::KIN / 2;
+        for (int e = tid; e < (C::NB0 + C::NB1) * 8 * C2; e += RT_WARPS * 32) {
+            const int r = e / C2, c2 = e - r * C2;
+            int gr = r;
+            if (PASS == PASS_FIX) gr = r < K2 ? r : (r < K2 + 8 ? r + K2 : r - 8);
+            *reinterpret_cast<double2*>(op_s + r * C::LD + 2 * c2) = *reinterpret_cast<const double2*>(src + (size_t)gr * GLD + 2 * c2);
         }
     }
     if (lane == 0) {
@@ -129,25 +146,41 @@ oci_red_resident_kernel(DevView V, int ybase, int slot, int prev_slot, double to
     double* my_ring = ring + warp * RT_STAGES * C::STAGE_DOUBLES;
     uint64_t* my_full = full + warp * RT_STAGES;
 
-    // one bulk copy per lane: lanes 0..15 the first half of y[j+1] (mu<0 leaves cell j+1 through its left
-    // face), lanes 16..31 the second half of y[j-1]
+    // bulk copies, one per lane and round.  ITER / FINAL: lanes 0..15 the first half of y[j+1] (mu<0 leaves
+    // cell j+1 through its left face), lanes 16..31 the second half of y[j-1].  FIX: the four h = 1 runs of
+    // y[j], z[j] and Q[j]
     auto prefetch = [&](int it) {
         const int s = it & 1;
         const int64_t j0 = (wid + (int64_t)it * nw) * RT_M;
         const int rows = (int)((J - j0 < RT_M) ? (J - j0) : RT_M);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        if (lane == 0) mbar_expect_tx(&my_full[s], (uint32_t)rows * K2 * 8);
+        if (lane == 0) mbar_expect_tx(&my_full[s], (uint32_t)rows * C::KIN * 8);
         __syncwarp();
-        const int row = lane & 15, half = lane >> 4;
-        if (row < rows) {
-            const int64_t j = j0 + row;
-            const double* src = half ? Ys + (j - 1) * K2 + N : Ys + (j + 1) * K2;
-            tma_load_1d(my_ring + s * C::STAGE_DOUBLES + row * C::LD + half * N, src, N * 8, &my_full[s]);
+        double* st = my_ring + s * C::STAGE_DOUBLES;
+        if (PASS == PASS_FIX) {
+            for (int idx = lane; idx < 5 * RT_M; idx += 32) {
+                const int row = idx & (RT_M - 1), seg = idx / RT_M;
+                if (row < rows) {
+                    const int64_t j = j0 + row;
+                    const double* src = seg == 0   ? Ys + j * K2 + N2
+                                        : seg == 1 ? Ys + j * K2 + N + N2
+                                        : seg == 2 ? V.z + j * K2 + N2
+                                        : seg == 3 ? V.z + j * K2 + N + N2
+                                                   : V.Q + j * 4;
+                    tma_load_1d(st + row * C::LD + seg * N2, src, seg == 4 ? 32 : N2 * 8, &my_full[s]);
+                }
+            }
+        } else {
+            const int row = lane & 15, half = lane >> 4;
+            if (row < rows) {
+                const int64_t j = j0 + row;
+                const double* src = half ? Ys + (j - 1) * K2 + N : Ys + (j + 1) * K2;
+                tma_load_1d(st + row * C::LD + half * N, src, N * 8, &my_full[s]);
+            }
         }
     };
 
     double dmax = 0.0, rmax = 0.0;
-    const double* __restrict__ fixp = FINAL ? V.ifix : V.yfix;
     if (my_tiles > 0) prefetch(0);
 
     for (int it = 0; it < my_tiles; ++it) {
@@ -157,97 +190,102 @@ oci_red_resident_kernel(DevView V, int ybase, int slot, int prev_slot, double to
         if (it + 1 < my_tiles) prefetch(it + 1);
 
         // ---- global operands of the epilogue, requested now, consumed after the DMMAs
-        double2 fx[2][K2 / 8], yl[2][FINAL ? K2 / 8 : 1];
+        double2 fx[2][PASS == PASS_FIX ? 1 : K2 / 8];
         double2 pf[2], po[2];
+        if (PASS != PASS_FIX) {
+            const double* __restrict__ fixp = PASS == PASS_FINAL ? V.ifix : V.yfix;
 #pragma unroll
-        for (int g = 0; g < 2; ++g) {
-            const int r = 8 * g + g4;
-            const int64_t j = (r < rows) ? j0 + r : j0;             // clamped: unconditional loads
+            for (int g = 0; g < 2; ++g) {
+                const int r = 8 * g + g4;
+                const int64_t j = (r < rows) ? j0 + r : j0;             // clamped: unconditional loads
 #pragma unroll
-            for (int t = 0; t < K2 / 8; ++t) {
-                fx[g][t] = *reinterpret_cast<const double2*>(fixp + j * K2 + 8 * t + 2 * t4);
-                if (FINAL) yl[g][t] = *reinterpret_cast<const double2*>(Yd + j * K2 + 8 * t + 2 * t4);
-            }
-            if (!FINAL) {
-                pf[g] = *reinterpret_cast<const double2*>(V.phifix + j * 4 + 2 * (t4 & 1));
-                po[g] = *reinterpret_cast<const double2*>(V.phi + j * 4 + 2 * (t4 & 1));
+                for (int t = 0; t < K2 / 8; ++t) fx[g][t] = *reinterpret_cast<const double2*>(fixp + j * K2 + 8 * t + 2 * t4);
+                if (PASS == PASS_ITER) {
+                    pf[g] = *reinterpret_cast<const double2*>(V.phifix + j * 4 + 2 * (t4 & 1));
+                    po[g] = *reinterpret_cast<const double2*>(V.phi + j * 4 + 2 * (t4 & 1));
+                }
             }
         }
 
-        double acc[2][C::NB][2];
+        double acc[2][C::NB0][2];
 #pragma unroll
         for (int g = 0; g < 2; ++g)
 #pragma unroll
-            for (int t = 0; t < C::NB; ++t) acc[g][t][0] = acc[g][t][1] = 0.0;
+            for (int t = 0; t < C::NB0; ++t) acc[g][t][0] = acc[g][t][1] = 0.0;
 
         mbar_wait(&my_full[s], (it >> 1) & 1);
         const double* arow = my_ring + s * C::STAGE_DOUBLES + g4 * C::LD + t4;
         const double* brow = op_s + g4 * C::LD + t4;
-#pragma unroll 4
-        for (int ks = 0; ks < C::KS; ++ks) {
-            double a[2], b[C::NB];
-#pragma unroll
-            for (int g = 0; g < 2; ++g) a[g] = arow[(8 * g) * C::LD + 4 * ks];
-#pragma unroll
-            for (int t = 0; t < C::NB; ++t) b[t] = brow[(8 * t) * C::LD + 4 * ks];
-#pragma unroll
-            for (int g = 0; g < 2; ++g)
-#pragma unroll
-                for (int t = 0; t < C::NB; ++t) dmma(acc[g][t][0], acc[g][t][1], a[g], b[t]);
-        }
+        tile_dmma<C::NB0, C::KS, C::LD>(acc, arow, brow);
 
-        // ---- epilogue
+        // ---- epilogue of row group 0
 #pragma unroll
         for (int g = 0; g < 2; ++g) {
             const int r = 8 * g + g4;
             const int64_t j = j0 + r;
             if (r < rows) {
-                if (!FINAL) {
+                if (PASS == PASS_ITER) {
 #pragma unroll
                     for (int t = 0; t < K2 / 8; ++t)
                         *reinterpret_cast<double2*>(Yd + j * K2 + 8 * t + 2 * t4) =
                             make_double2(fx[g][t].x + acc[g][t][0], fx[g][t].y + acc[g][t][1]);
                     if (t4 < 2) {                                   // phi rows: columns 0..3 of the last block
-                        const double p0 = pf[g].x + acc[g][C::NB - 1][0], p1 = pf[g].y + acc[g][C::NB - 1][1];
+                        const double p0 = pf[g].x + acc[g][C::NB0 - 1][0], p1 = pf[g].y + acc[g][C::NB0 - 1][1];
                         *reinterpret_cast<double2*>(V.phi + j * 4 + 2 * t4) = make_double2(p0, p1);
                         dmax = fmax(dmax, fmax(fabs(p0 - po[g].x), fabs(p1 - po[g].y)));
                         rmax = fmax(rmax, fmax(fabs(p0), fabs(p1)));
                     }
-                } else {
-                    double* __restrict__ P = V.psi[pdst];
+                } else if (PASS == PASS_FINAL) {
 #pragma unroll
-                    for (int t = 0; t < K2 / 8; ++t) {
-                        const int m = 4 * t + t4;                   // packed columns 2m, 2m+1 = slots k, k+1/2
-                        const double i0 = fx[g][t].x + acc[g][t][0], i1 = fx[g][t].y + acc[g][t][1];
-                        const bool neg = m < N / 2;                 // mu<0: O = slots 0,2; I = slots 1,3
-                        *reinterpret_cast<double2*>(P + j * n + 4 * m) = neg ? make_double2(yl[g][t].x, i0) : make_double2(i0, yl[g][t].x);
-                        *reinterpret_cast<double2*>(P + j * n + 4 * m + 2) = neg ? make_double2(yl[g][t].y, i1) : make_double2(i1, yl[g][t].y);
-                    }
+                    for (int t = 0; t < K2 / 8; ++t)
+                        *reinterpret_cast<double2*>(V.z + j * K2 + 8 * t + 2 * t4) =
+                            make_double2(fx[g][t].x + acc[g][t][0], fx[g][t].y + acc[g][t][1]);
+                } else {
+#pragma unroll
+                    for (int t = 0; t < K2 / 8; ++t)
+                        *reinterpret_cast<double2*>(V.yfix + j * K2 + 8 * t + 2 * t4) = make_double2(acc[g][t][0], acc[g][t][1]);
+                    if (t4 < 2)
+                        *reinterpret_cast<double2*>(V.phifix + j * 4 + 2 * t4) =
+                            make_double2(acc[g][C::NB0 - 1][0], acc[g][C::NB0 - 1][1]);
+                }
+            }
+        }
+        if (PASS == PASS_FIX) {
+            // ---- row group 1: the I rows of Psi_fix from the same input tile
+            double acc1[2][C::NB1 > 0 ? C::NB1 : 1][2];
+#pragma unroll
+            for (int g = 0; g < 2; ++g)
+#pragma unroll
+                for (int t = 0; t < C::NB1; ++t) acc1[g][t][0] = acc1[g][t][1] = 0.0;
+            tile_dmma<(C::NB1 > 0 ? C::NB1 : 1), C::KS, C::LD>(acc1, arow, brow + C::NB0 * 8 * C::LD);
+#pragma unroll
+            for (int g = 0; g < 2; ++g) {
+                const int r = 8 * g + g4;
+                const int64_t j = j0 + r;
+                if (r < rows) {
+#pragma unroll
+                    for (int t = 0; t < C::NB1; ++t)
+                        *reinterpret_cast<double2*>(V.ifix + j * K2 + 8 * t + 2 * t4) = make_double2(acc1[g][t][0], acc1[g][t][1]);
                 }
             }
         }
         __syncwarp();
-        // ---- reflecting ghost rows (reading S4) by the warp that owns the edge cell
-        const bool gl = j0 == 0 && V.bcL == OCI_BC_REFLECTING;
-        const bool gr = j0 + rows == J && V.bcR == OCI_BC_REFLECTING;
-        if (gl || gr) {
-            __threadfence_block();
-            for (int p = lane; p < K2; p += 32) {
-                const int mir = 2 * (N - 1 - (p >> 1)) + (p & 1);
-                const int m = p >> 1, h = p & 1;
-                if (!FINAL) {
-                    if (gl && p >= N) Yd[-(int64_t)K2 + p] = __ldcg(Yd + mir);
-                    if (gr && p < N) Yd[J * K2 + p] = __ldcg(Yd + (J - 1) * K2 + mir);
-                } else {
-                    double* __restrict__ P = V.psi[pdst];
-                    if (gl && p >= N) P[-(int64_t)n + 4 * m + 2 * h + 1] = __ldcg(Yd + mir);
-                    if (gr && p < N) P[J * n + 4 * m + 2 * h] = __ldcg(Yd + (J - 1) * K2 + mir);
+        // ---- reflecting ghost rows of y (reading S4) by the warp that owns the edge cell
+        if (PASS == PASS_ITER) {
+            const bool gl = j0 == 0 && V.bcL == OCI_BC_REFLECTING;
+            const bool gr = j0 + rows == J && V.bcR == OCI_BC_REFLECTING;
+            if (gl || gr) {
+                __threadfence_block();
+                for (int q = lane; q < K2; q += 32) {
+                    const int mir = mirror_q(q, N);
+                    if (gl && q >= N) Yd[-(int64_t)K2 + q] = __ldcg(Yd + mir);
+                    if (gr && q < N) Yd[J * K2 + q] = __ldcg(Yd + (J - 1) * K2 + mir);
                 }
+                __syncwarp();
             }
-            __syncwarp();
         }
     }
-    if (!FINAL) {
+    if (PASS == PASS_ITER) {
         dmax = warp_max(dmax);
         rmax = warp_max(rmax);
         if (lane == 0 && my_tiles > 0) {
@@ -260,8 +298,8 @@ oci_red_resident_kernel(DevView V, int ybase, int slot, int prev_slot, double to
 bool oci_red_resident_supported(const DevView& V) { return V.nblk == 1 && (V.n == 128 || V.n == 64); }
 
 namespace {
-template <int K2, bool FINAL>
-void launch_rr(const DevView& V, int ybase, int slot, int prev_slot, double tol, int pdst, int cnt, int force, cudaStream_t s)
+template <int K2, int PASS>
+void launch_rr(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
 {
     static int sm_count = 0;
     static bool attr = false;
@@ -271,28 +309,30 @@ void launch_rr(const DevView& V, int ybase, int slot, int prev_slot, double tol,
         cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
     }
     if (!attr) {
-        cudaFuncSetAttribute(oci_red_resident_kernel<K2, FINAL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)RCfg<K2, FINAL>::SMEM);
+        cudaFuncSetAttribute(oci_red_resident_kernel<K2, PASS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)RCfg<K2, PASS>::SMEM);
         attr = true;
     }
     const int64_t ntiles = (V.J + RT_M - 1) / RT_M;
     const int64_t ctas = (ntiles + RT_WARPS - 1) / RT_WARPS;
     const unsigned grid = (unsigned)(ctas < sm_count ? ctas : sm_count);
-    oci_red_resident_kernel<K2, FINAL><<<grid, RT_WARPS * 32, RCfg<K2, FINAL>::SMEM, s>>>(V, ybase, slot, prev_slot, tol, pdst, cnt, force);
+    oci_red_resident_kernel<K2, PASS><<<grid, RT_WARPS * 32, RCfg<K2, PASS>::SMEM, s>>>(V, ybase, slot, prev_slot, tol, cnt, force);
+}
+
+template <int K2>
+void launch_rr_pass(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
+{
+    if (pass == PASS_FIX) launch_rr<K2, PASS_FIX>(V, ybase, 0, -1, tol, 0, 0, s);
+    else if (pass == PASS_ITER) launch_rr<K2, PASS_ITER>(V, ybase, slot, prev_slot, tol, 0, 0, s);
+    else launch_rr<K2, PASS_FINAL>(V, ybase, 0, -1, tol, cnt, force, s);
 }
 }  // namespace
 
-int launch_red_resident(const DevView& V, int ysrc, int slot, int prev_slot, double tol, cudaStream_t s)
+int launch_red_resident(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
+                        cudaStream_t s)
 {
-    if (V.n == 128) launch_rr<64, false>(V, ysrc, slot, prev_slot, tol, 0, 0, 0, s);
-    else launch_rr<32, false>(V, ysrc, slot, prev_slot, tol, 0, 0, 0, s);
-    return 1;
-}
-
-int launch_red_resident_final(const DevView& V, int ybase, int pdst, int cnt, int force, double tol, cudaStream_t s)
-{
-    if (V.n == 128) launch_rr<64, true>(V, ybase, 0, -1, tol, pdst, cnt, force, s);
-    else launch_rr<32, true>(V, ybase, 0, -1, tol, pdst, cnt, force, s);
+    if (V.n == 128) launch_rr_pass<64>(V, pass, ybase, slot, prev_slot, tol, cnt, force, s);
+    else launch_rr_pass<32>(V, pass, ybase, slot, prev_slot, tol, cnt, force, s);
     return 1;
 }
 
