@@ -38,6 +38,7 @@ struct oci_ctx {
     // device
     DevView V{};
     alignas(64) KtiledMaps maps{};
+    alignas(64) RedKtiledMaps rmaps{};
     bool use_ktiled = false;
     cudaStream_t stream = nullptr;
     void* ws = nullptr;
@@ -237,6 +238,8 @@ int32_t resolved_iteration(const oci_ctx* ctx)
 
 int launch_reduced_pass(oci_ctx* ctx, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force)
 {
+    if (ctx->red_kernel == OCI_RKERNEL_KTILED)
+        return launch_red_ktiled(ctx->V, ctx->rmaps, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
     if (ctx->red_kernel == OCI_RKERNEL_RESIDENT)
         return launch_red_resident(ctx->V, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
     return launch_red_gemv(ctx->V, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
@@ -472,7 +475,9 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     }
     ctx->use_ktiled = ctx->path == OCI_PATH_SHARED && !oci_shared_fast_supported(V) && oci_ktiled_supported(V) &&
                       oci_ktiled_prepare(V, &ctx->maps);
-    ctx->red_kernel = oci_red_resident_supported(V) ? OCI_RKERNEL_RESIDENT : OCI_RKERNEL_GEMV;
+    ctx->red_kernel = oci_red_resident_supported(V) ? OCI_RKERNEL_RESIDENT
+                      : (oci_red_ktiled_supported(V) && oci_red_ktiled_prepare(V, &ctx->rmaps)) ? OCI_RKERNEL_KTILED
+                                                                                                 : OCI_RKERNEL_GEMV;
     ctx->cur = 0;
     ctx->ycur = 0;
     ctx->yz_valid = false;
@@ -511,12 +516,21 @@ int oci_set_flux_dev(oci_ctx* ctx, const double* d_psi_edge)
     return set_flux_common(ctx, d_psi_edge);
 }
 
+// Q padded to one 128-byte row per cell for the K-tiled FIX pass (a strided copy, the pad stays zero)
+static int refresh_q16(oci_ctx* ctx)
+{
+    if (ctx->red_kernel != OCI_RKERNEL_KTILED) return OCI_OK;
+    CK(cudaMemcpy2DAsync(ctx->V.q16, 128, ctx->V.Q, 32, 32, (size_t)ctx->J, cudaMemcpyDeviceToDevice, ctx->stream));
+    return OCI_OK;
+}
+
 int oci_set_source(oci_ctx* ctx, const double* q)
 {
     if (!ctx) return OCI_E_INVALID;
     if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_set_source before oci_setup");
     if (q) CK(cudaMemcpyAsync(ctx->V.Q, q, (size_t)ctx->J * 4 * 8, cudaMemcpyHostToDevice, ctx->stream));
     else CK(cudaMemsetAsync(ctx->V.Q, 0, (size_t)ctx->J * 4 * 8, ctx->stream));
+    if (int rc = refresh_q16(ctx)) return rc;
     CK(cudaStreamSynchronize(ctx->stream));
     return OCI_OK;
 }
@@ -527,7 +541,7 @@ int oci_set_source_dev(oci_ctx* ctx, const double* d_q)
     if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_set_source_dev before oci_setup");
     if (d_q) CK(cudaMemcpyAsync(ctx->V.Q, d_q, (size_t)ctx->J * 4 * 8, cudaMemcpyDeviceToDevice, ctx->stream));
     else CK(cudaMemsetAsync(ctx->V.Q, 0, (size_t)ctx->J * 4 * 8, ctx->stream));
-    return OCI_OK;
+    return refresh_q16(ctx);
 }
 
 int oci_step(oci_ctx* ctx, double tol, int32_t max_iters, int32_t* iters, double* resid)

@@ -62,6 +62,11 @@ struct KtiledMaps {
     CUtensorMap cfix, psi[2], binv;
 };
 
+// Tensor maps of the K-tiled kernels of the reduced step (oci_reduced_ktiled.cu), encoded once in oci_setup.
+struct RedKtiledMaps {
+    CUtensorMap y[2], z, q16, xop, xop8, rop, rop8, fop;
+};
+
 // The stopping rule (reading S2), evaluated identically on host and device.
 __host__ __device__ inline bool converged(double tol, double d, double r) { return tol >= 0.0 && d <= tol * r; }
 
@@ -94,6 +99,12 @@ int launch_unpack_yz(const DevView& V, int buf, int ybuf, cudaStream_t s);
 // of the first of the `cnt` queued iterations
 int launch_red_gemv(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
                     cudaStream_t s);
+// row-major fp64 matrix [rows][cols] -> 2-D tensor map, box = box_rows x 16 columns, 128-byte swizzle, zero fill
+bool oci_encode_2d(CUtensorMap* m, const double* base, uint64_t rows, uint64_t cols, uint32_t box_rows);
+bool oci_red_ktiled_supported(const DevView& V);
+bool oci_red_ktiled_prepare(const DevView& V, RedKtiledMaps* M);
+int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int ybase, int slot, int prev_slot, double tol,
+                      int cnt, int force, cudaStream_t s);
 bool oci_red_resident_supported(const DevView& V);
 int launch_red_resident(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
                         cudaStream_t s);

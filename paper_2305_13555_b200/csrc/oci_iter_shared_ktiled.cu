@@ -311,8 +311,10 @@ EncodeTiledFn encode_fn()
     return fn;
 }
 
+}  // namespace
+
 // row-major fp64 matrix [rows][cols]; box = box_rows x 16 columns, 128-byte swizzle, zero fill outside
-bool encode_2d(CUtensorMap* m, const double* base, uint64_t rows, uint64_t cols, uint32_t box_rows)
+bool oci_encode_2d(CUtensorMap* m, const double* base, uint64_t rows, uint64_t cols, uint32_t box_rows)
 {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
@@ -324,7 +326,6 @@ bool encode_2d(CUtensorMap* m, const double* base, uint64_t rows, uint64_t cols,
               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
-}  // namespace
 
 bool oci_ktiled_supported(const DevView& V)
 {
@@ -334,10 +335,10 @@ bool oci_ktiled_supported(const DevView& V)
 bool oci_ktiled_prepare(const DevView& V, KtiledMaps* M)
 {
     const uint64_t n = (uint64_t)V.n;
-    return encode_2d(&M->cfix, V.cfix, (uint64_t)V.J, n, KT_M) &&
-           encode_2d(&M->psi[0], V.psi[0] - n, (uint64_t)V.J + 2, n, KT_M) &&
-           encode_2d(&M->psi[1], V.psi[1] - n, (uint64_t)V.J + 2, n, KT_M) &&
-           encode_2d(&M->binv, V.binv, n, n, KT_N);
+    return oci_encode_2d(&M->cfix, V.cfix, (uint64_t)V.J, n, KT_M) &&
+           oci_encode_2d(&M->psi[0], V.psi[0] - n, (uint64_t)V.J + 2, n, KT_M) &&
+           oci_encode_2d(&M->psi[1], V.psi[1] - n, (uint64_t)V.J + 2, n, KT_M) &&
+           oci_encode_2d(&M->binv, V.binv, n, n, KT_N);
 }
 
 int launch_oci_ktiled(const DevView& V, const KtiledMaps& M, int src, int slot, int prev_slot, double tol, cudaStream_t s)

@@ -1,0 +1,359 @@
+// Interface-reduced OCI step (oci_reduced.cu has the derivation), shared block, large blocks
+// (N a multiple of 64, i.e. K2 = 2N a multiple of 128; config 4: K2 = 256): the K-tiled fp64 tensor-core
+// form of the three passes.  Each pass is a "gathered GEMM"
+//     out[j][i] = add[j][i] + sum_k Op[i][k] in_j[k]
+// whose input vector is a concatenation of row segments of arrays that already sit in HBM in the packed
+// layout (no assembly, |mu| / alpha / h/4 folded into the operator):
+//     ITER, FINAL:  in_j = [ y[j+1][0:N] | y[j-1][N:2N] ]
+//     FIX        :  in_j = [ y[j][N/2:N] | y[j][3N/2:2N] | z[j][N/2:N] | z[j][3N/2:2N] | Q16[j] ]
+// so every K chunk of the A operand is ONE 2-D tensor-map TMA box (64 cells x 16 k) from some (array,
+// column, row shift), and every chunk of the B operand one box (128 operator rows x 16 k).  The operator
+// (0.5 - 1.1 MB) stays in L2.
+//
+//   * persistent CTAs, one per SM; work item = 64 cells x 128 operator rows, full K; the items of one
+//     cell tile run on neighbouring SMs at the same time (the input tile is read from HBM once);
+//   * 8 MMA warps (2 x 4, each 32 cells x 32 rows, 16 DMMA.8x8x4 accumulators; 224 registers after
+//     setmaxnreg) + an auxiliary warpgroup (56 registers) one thread of which issues the TMA,
+//     8-stage ring of 26 KB stages, full / empty mbarriers;
+//   * shared memory is dense under the hardware 128-byte swizzle; one DMMA consumes the k-set
+//     {2s, 2s+1, 2s+8, 2s+9} of the chunk, which makes every fragment load bank-conflict free;
+//   * the four scalar-flux rows (H of ITER, W B^{-1} rows of FIX) ride along with item 0 of each cell tile
+//     as one more 8-row operator box; MMA warp (wm, wn) takes their k-step ks = wn of every chunk (one
+//     extra DMMA per four), the four partial sums meet in shared memory in the epilogue;
+//   * epilogue from registers: + yfix / ifix (requested at the start of the item), 16-byte stores, the
+//     reflecting ghost rows of y, phi and the two max-norms.
+#include <cuda.h>
+
+#include "device_utils.cuh"
+
+namespace oci {
+
+namespace {
+
+constexpr int RK_M = 64;      // cells per work item
+constexpr int RK_N = 128;     // operator rows per work item
+constexpr int RK_K = 16;      // k per chunk = one 128-byte swizzle row
+constexpr int RK_STAGES = 8;
+constexpr int RK_A_BYTES = RK_M * RK_K * 8;   // 8 KB
+constexpr int RK_B_BYTES = RK_N * RK_K * 8;   // 16 KB
+constexpr int RK_P_BYTES = 8 * RK_K * 8;      // 1 KB: the scalar-flux rows (4 used)
+constexpr int RK_STAGE_BYTES = RK_A_BYTES + RK_B_BYTES + RK_P_BYTES + 1024;   // keeps every stage 2 KB-aligned
+constexpr size_t RK_SMEM = 1024 /*alignment slack*/ + (size_t)RK_STAGES * RK_STAGE_BYTES + 4 * RK_M * 4 * 8 /*phi_s*/ +
+                           2 * RK_STAGES * 8 + 64;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+            smem_u32(dst)),
+        "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ void named_bar_sync(int id, int threads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+
+}  // namespace
+
+template <int PASS>
+__global__ void __launch_bounds__(384, 1)
+oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_y_alt,
+                      const __grid_constant__ CUtensorMap map_z, const __grid_constant__ CUtensorMap map_q,
+                      const __grid_constant__ CUtensorMap map_op, const __grid_constant__ CUtensorMap map_op8, int ybase, int slot,
+                      int prev_slot, double tol, int cnt, int force)
+{
+    // map_y = tensor map of y[ybase], map_y_alt = of y[ybase ^ 1]
+    int ysrc = ybase;
+    if (PASS == PASS_ITER) {
+        if (step_done(V.norms, prev_slot, tol)) return;
+    } else if (PASS == PASS_FINAL) {
+        int L = first_converged(V.norms, cnt, tol);
+        if (L == 0) {
+            if (!force) return;
+            L = cnt;
+        }
+        ysrc = (ybase + L - 1) & 1;
+    }
+    const CUtensorMap* my = (ysrc == ybase) ? &map_y : &map_y_alt;
+
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char* base = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    unsigned char* stages = base;                                                    // [S][A 8K | B 16K | P 1K | pad]
+    double* phi_s = reinterpret_cast<double*>(base + (size_t)RK_STAGES * RK_STAGE_BYTES);   // [4 wn][64][4]
+    uint64_t* full = reinterpret_cast<uint64_t*>(phi_s + 4 * RK_M * 4);
+    uint64_t* empty = full + RK_STAGES;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int N = V.N, K2 = V.n >> 1, N2 = N >> 1;
+    const int64_t J = V.J;
+    const int K = PASS == PASS_FIX ? K2 + RK_K : K2;
+    const int kch = K / RK_K;                                         // chunks per item
+    const int ntn = (PASS == PASS_FIX ? 2 * K2 : K2) / RK_N;          // items per cell tile
+    const int prow = PASS == PASS_FIX ? 2 * K2 : K2;                  // operator row of the scalar-flux block
+    const int64_t nct = (J + RK_M - 1) / RK_M;
+    const int64_t nitems = nct * ntn;
+    const int my_items = (int)((nitems - blockIdx.x + gridDim.x - 1) / gridDim.x);
+
+    if (tid == 0) {
+        for (int s = 0; s < RK_STAGES; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], 8);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp >= 8) {
+        // =========================== TMA producer (one thread of the auxiliary warpgroup) ===========================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        if (warp == 8 && lane == 0) {
+            asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(my)) : "memory");
+            asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&map_op)) : "memory");
+            if (PASS != PASS_FINAL) asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&map_op8)) : "memory");
+            if (PASS == PASS_FIX) {
+                asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&map_z)) : "memory");
+                asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&map_q)) : "memory");
+            }
+            int q = 0;
+            for (int it = 0; it < my_items; ++it) {
+                const int64_t item = (int64_t)blockIdx.x + (int64_t)it * gridDim.x;
+                const int j0 = (int)(item / ntn) * RK_M;
+                const int nt = (int)(item % ntn);
+                const int i0 = nt * RK_N;
+                const bool with_phi = PASS != PASS_FINAL && nt == 0;
+                for (int kc = 0; kc < kch; ++kc, ++q) {
+                    const int s = q % RK_STAGES;
+                    if (q >= RK_STAGES) mbar_wait(&empty[s], ((q / RK_STAGES) - 1) & 1);
+                    unsigned char* st = stages + (size_t)s * RK_STAGE_BYTES;
+                    const int k0 = kc * RK_K;
+                    mbar_expect_tx(&full[s], RK_A_BYTES + RK_B_BYTES + (with_phi ? RK_P_BYTES : 0));
+                    if (PASS == PASS_FIX) {
+                        // y / z map rows: y carries the ghost row first (row = cell + 1), z and Q16 do not
+                        if (k0 < N2) tma_load_2d(st, my, N2 + k0, j0 + 1, &full[s]);
+                        else if (k0 < N) tma_load_2d(st, my, N + k0, j0 + 1, &full[s]);
+                        else if (k0 < N + N2) tma_load_2d(st, &map_z, k0 - N2, j0, &full[s]);
+                        else if (k0 < K2) tma_load_2d(st, &map_z, k0, j0, &full[s]);
+                        else tma_load_2d(st, &map_q, 0, j0, &full[s]);
+                    } else {
+                        // k < N (mu<0) comes from the right neighbour, else from the left one (row a3)
+                        tma_load_2d(st, my, k0, j0 + 1 + (k0 < N ? 1 : -1), &full[s]);
+                    }
+                    tma_load_2d(st + RK_A_BYTES, &map_op, k0, i0, &full[s]);
+                    if (with_phi) tma_load_2d(st + RK_A_BYTES + RK_B_BYTES, &map_op8, k0, prow, &full[s]);
+                }
+            }
+        }
+        return;
+    }
+
+    // =========================== MMA warps ===========================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
+    const int g4 = lane >> 2, t4 = lane & 3;
+    const int wm = warp >> 2, wn = warp & 3;
+    // byte offset of this lane's fragment element inside a 128-byte swizzled row, per k-step:
+    // logical 16-byte unit ks + 4*(t4>>1), XOR row&7 (= g4), element t4&1
+    int foff[4];
+#pragma unroll
+    for (int ks = 0; ks < 4; ++ks) foff[ks] = (((ks + 4 * (t4 >> 1)) ^ g4) << 4) + ((t4 & 1) << 3);
+    const int a_row = (wm * 32 + g4) * 128;              // + g*1024
+    const int b_row = (wn * 32 + g4) * 128;              // + t*1024
+    const int p_off = g4 * 128 + foff[wn];               // scalar-flux block: this warp's k-step is ks = wn
+
+    double* __restrict__ Yd = V.y[ysrc ^ 1];
+    double dmax = 0.0, rmax = 0.0;
+    const bool refl_l = V.bcL == OCI_BC_REFLECTING, refl_r = V.bcR == OCI_BC_REFLECTING;
+
+    int q = 0;
+    for (int it = 0; it < my_items; ++it) {
+        const int64_t item = (int64_t)blockIdx.x + (int64_t)it * gridDim.x;
+        const int64_t ct = item / ntn;
+        const int nt = (int)(item % ntn);
+        const int64_t j0 = ct * RK_M;
+        const int i0 = nt * RK_N;
+        const bool with_phi = PASS != PASS_FINAL && nt == 0;
+
+        // ---- additive operand of the epilogue, requested now
+        double2 fx[4][4];
+        if (PASS != PASS_FIX) {
+            const double* __restrict__ fixp = PASS == PASS_FINAL ? V.ifix : V.yfix;
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+                int64_t j = j0 + wm * 32 + 8 * g + g4;
+                if (j >= J) j = J - 1;
+#pragma unroll
+                for (int t = 0; t < 4; ++t) fx[g][t] = *reinterpret_cast<const double2*>(fixp + j * K2 + i0 + wn * 32 + 8 * t + 2 * t4);
+            }
+        }
+
+        double acc[4][4][2], accp[4][2];
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+            accp[g][0] = accp[g][1] = 0.0;
+#pragma unroll
+            for (int t = 0; t < 4; ++t) acc[g][t][0] = acc[g][t][1] = 0.0;
+        }
+
+        for (int kc = 0; kc < kch; ++kc, ++q) {
+            const int s = q % RK_STAGES;
+            mbar_wait(&full[s], (q / RK_STAGES) & 1);
+            const unsigned char* st = stages + (size_t)s * RK_STAGE_BYTES;
+            const unsigned char* As = st + a_row;
+            const unsigned char* Bs = st + RK_A_BYTES + b_row;
+#pragma unroll
+            for (int ks = 0; ks < 4; ++ks) {
+                double a[4], b[4];
+#pragma unroll
+                for (int g = 0; g < 4; ++g) a[g] = *reinterpret_cast<const double*>(As + g * 1024 + foff[ks]);
+#pragma unroll
+                for (int t = 0; t < 4; ++t) b[t] = *reinterpret_cast<const double*>(Bs + t * 1024 + foff[ks]);
+#pragma unroll
+                for (int g = 0; g < 4; ++g)
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) dmma(acc[g][t][0], acc[g][t][1], a[g], b[t]);
+                if (with_phi && ks == wn) {
+                    const double bp = *reinterpret_cast<const double*>(st + RK_A_BYTES + RK_B_BYTES + p_off);
+#pragma unroll
+                    for (int g = 0; g < 4; ++g) dmma(accp[g][0], accp[g][1], a[g], bp);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);
+        }
+
+        // ---- epilogue
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+            const int r = wm * 32 + 8 * g + g4;
+            const int64_t j = j0 + r;
+            if (j < J) {
+#pragma unroll
+                for (int t = 0; t < 4; ++t) {
+                    const int i = i0 + wn * 32 + 8 * t + 2 * t4;
+                    if (PASS == PASS_ITER) {
+                        const double v0 = fx[g][t].x + acc[g][t][0], v1 = fx[g][t].y + acc[g][t][1];
+                        *reinterpret_cast<double2*>(Yd + j * K2 + i) = make_double2(v0, v1);
+                        // reading S4: the mirror image of the edge cell's outgoing flux becomes the ghost row
+                        if (j == 0 && refl_l && i < N) {
+                            Yd[-(int64_t)K2 + mirror_q(i, N)] = v0;
+                            Yd[-(int64_t)K2 + mirror_q(i + 1, N)] = v1;
+                        }
+                        if (j == J - 1 && refl_r && i >= N) {
+                            Yd[J * K2 + mirror_q(i, N)] = v0;
+                            Yd[J * K2 + mirror_q(i + 1, N)] = v1;
+                        }
+                    } else if (PASS == PASS_FINAL) {
+                        *reinterpret_cast<double2*>(V.z + j * K2 + i) = make_double2(fx[g][t].x + acc[g][t][0], fx[g][t].y + acc[g][t][1]);
+                    } else {
+                        double* dst = i < K2 ? V.yfix + j * K2 + i : V.ifix + j * K2 + (i - K2);
+                        *reinterpret_cast<double2*>(dst) = make_double2(acc[g][t][0], acc[g][t][1]);
+                    }
+                }
+            }
+            if (with_phi && t4 < 2) {     // columns 0..3 of the scalar-flux block: this warp's k-partial
+                phi_s[(wn * RK_M + r) * 4 + 2 * t4 + 0] = accp[g][0];
+                phi_s[(wn * RK_M + r) * 4 + 2 * t4 + 1] = accp[g][1];
+            }
+        }
+        if (PASS != PASS_FINAL) {
+            named_bar_sync(1, 256);
+            if (with_phi) {
+                // thread tid owns (cell tid/4, slot tid%4) of the item
+                const int64_t j = j0 + (tid >> 2);
+                const double ssum = phi_s[0 * RK_M * 4 + tid] + phi_s[1 * RK_M * 4 + tid] + phi_s[2 * RK_M * 4 + tid] + phi_s[3 * RK_M * 4 + tid];
+                if (j < J) {
+                    if (PASS == PASS_FIX) {
+                        V.phifix[j * 4 + (tid & 3)] = ssum;
+                    } else {
+                        const double a = V.phifix[j * 4 + (tid & 3)] + ssum;
+                        const double old = V.phi[j * 4 + (tid & 3)];
+                        V.phi[j * 4 + (tid & 3)] = a;
+                        dmax = fmax(dmax, fabs(a - old));
+                        rmax = fmax(rmax, fabs(a));
+                    }
+                }
+            }
+            named_bar_sync(1, 256);                                  // phi_s reusable
+        }
+    }
+    if (PASS == PASS_ITER) {
+        dmax = warp_max(dmax);
+        rmax = warp_max(rmax);
+        if (lane == 0) {
+            atomic_max_nonneg(&V.norms[2 * slot + 0], dmax);
+            atomic_max_nonneg(&V.norms[2 * slot + 1], rmax);
+        }
+    }
+}
+
+bool oci_red_ktiled_supported(const DevView& V)
+{
+    return V.nblk == 1 && V.N % 64 == 0 && V.n <= 2048 && V.J + 2 < (int64_t)1 << 31;
+}
+
+bool oci_red_ktiled_prepare(const DevView& V, RedKtiledMaps* M)
+{
+    const uint64_t K2 = (uint64_t)V.n / 2, J = (uint64_t)V.J;
+    return oci_encode_2d(&M->y[0], V.y[0] - K2, J + 2, K2, RK_M) && oci_encode_2d(&M->y[1], V.y[1] - K2, J + 2, K2, RK_M) &&
+           oci_encode_2d(&M->z, V.z, J, K2, RK_M) && oci_encode_2d(&M->q16, V.q16, J, 16, RK_M) &&
+           oci_encode_2d(&M->xop, V.xop, 2 * K2 + 8, K2 + 16, RK_N) && oci_encode_2d(&M->xop8, V.xop, 2 * K2 + 8, K2 + 16, 8) &&
+           oci_encode_2d(&M->rop, V.rop, K2 + 8, K2, RK_N) && oci_encode_2d(&M->rop8, V.rop, K2 + 8, K2, 8) &&
+           oci_encode_2d(&M->fop, V.fop, K2, K2, RK_N);
+}
+
+int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int ybase, int slot, int prev_slot, double tol, int cnt,
+                      int force, cudaStream_t s)
+{
+    static int sm_count = 0;
+    static bool attr = false;
+    if (sm_count == 0) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
+    }
+    if (!attr) {
+        cudaFuncSetAttribute(oci_red_ktiled_kernel<PASS_FIX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RK_SMEM);
+        cudaFuncSetAttribute(oci_red_ktiled_kernel<PASS_ITER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RK_SMEM);
+        cudaFuncSetAttribute(oci_red_ktiled_kernel<PASS_FINAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RK_SMEM);
+        attr = true;
+    }
+    const int K2 = V.n / 2;
+    const int64_t nitems = ((V.J + RK_M - 1) / RK_M) * ((pass == PASS_FIX ? 2 * K2 : K2) / RK_N);
+    const unsigned grid = (unsigned)(nitems < sm_count ? nitems : sm_count);
+    const CUtensorMap& ya = M.y[ybase & 1];
+    const CUtensorMap& yb = M.y[(ybase & 1) ^ 1];
+    if (pass == PASS_FIX)
+        oci_red_ktiled_kernel<PASS_FIX><<<grid, 384, RK_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.xop, M.xop8, ybase, 0, -1, tol, 0, 0);
+    else if (pass == PASS_ITER)
+        oci_red_ktiled_kernel<PASS_ITER><<<grid, 384, RK_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.rop, M.rop8, ybase, slot, prev_slot, tol, 0, 0);
+    else
+        oci_red_ktiled_kernel<PASS_FINAL><<<grid, 384, RK_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.fop, M.fop, ybase, 0, -1, tol, cnt, force);
+    return 1;
+}
+
+}  // namespace oci

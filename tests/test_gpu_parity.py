@@ -165,6 +165,8 @@ def test_ktiled_kernel_shapes(J, N, bcL, bcR, iteration):
     p = _custom(J, N, bcL, bcR, seed=J * 1000 + N, hetero=False)
     g = P.OCI.from_problem(p)
     assert g.get_info()["apply_kernel"] == P.KERNEL_KTILED
+    # the reduced form has a K-tiled tensor-core kernel of its own when N is a multiple of 64
+    assert g.get_info()["reduced_kernel"] == (P.RKERNEL_KTILED if N % 64 == 0 else P.RKERNEL_GEMV)
     g.close()
     r = run_pair(p, "oci", steps=2, tol=-1.0, max_iters=4, threads=16, iteration=iteration)
     assert rel(r["g_psi"], r["o_psi"]) < 1e-12
@@ -180,6 +182,9 @@ def test_apply_kernel_selection():
                              (4, 50, P.KERNEL_KTILED), (5, 20, P.KERNEL_PER_CELL)):
         g = P.OCI.from_problem(make_problem(cfg, cells=cells))
         assert g.get_info()["apply_kernel"] == want, cfg
+        assert g.get_info()["reduced_kernel"] == {1: P.RKERNEL_GEMV, 2: P.RKERNEL_RESIDENT, 3: P.RKERNEL_RESIDENT,
+                                                  4: P.RKERNEL_KTILED, 5: P.RKERNEL_GEMV}[cfg], cfg
+        assert g.get_info()["iteration"] == P.ITERATION_REDUCED, cfg      # AUTO resolves to the reduced form on all five
         g.close()
 
 
