@@ -42,21 +42,38 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
 }
 
 // ---- packed interface layout of the reduced step (oci_reduced.cu has the definition)
-__device__ __forceinline__ int o_row(int q, int N)   // full index of packed outgoing row q
+// q < N  (mu < 0, leaves through the left face):  q = h*(N/2) + mm          (k run, then k+1/2 run)
+// q >= N (mu > 0, leaves through the right face): q = N + (1-h)*(N/2) + mm  (k+1/2 run, then k run)
+// so that the k+1/2 entries of a row are the single run [N/2, 3N/2).
+__device__ __forceinline__ void unpack_q(int q, int N, int& half, int& h, int& mm)
 {
     const int N2 = N >> 1;
-    const int half = q >= N, r = q - half * N;
-    const int h = r >= N2, mm = r - h * N2;
-    return 4 * (half * N2 + mm) + (half ? 2 * h + 1 : 2 * h);
+    half = q >= N;
+    const int r = q - half * N;
+    const int second = r >= N2;
+    mm = r - second * N2;
+    h = half ? 1 - second : second;
+}
+
+__device__ __forceinline__ int pack_q(int half, int h, int mm, int N)
+{
+    const int N2 = N >> 1;
+    return half * N + (half ? 1 - h : h) * N2 + mm;
+}
+
+__device__ __forceinline__ int o_row(int q, int N)   // full index 4m+s of packed outgoing row q
+{
+    int half, h, mm;
+    unpack_q(q, N, half, h, mm);
+    return 4 * (half * (N >> 1) + mm) + (half ? 2 * h + 1 : 2 * h);
 }
 
 // packed index of the mirror image (m -> N-1-m) of packed row q, same time slot
 __device__ __forceinline__ int mirror_q(int q, int N)
 {
-    const int N2 = N >> 1;
-    const int half = q >= N, r = q - half * N;
-    const int h = r >= N2, mm = r - h * N2;
-    return (1 - half) * N + h * N2 + (N2 - 1 - mm);
+    int half, h, mm;
+    unpack_q(q, N, half, h, mm);
+    return pack_q(1 - half, h, (N >> 1) - 1 - mm, N);
 }
 
 // First iteration index (1-based) whose norms satisfy the stopping rule, 0 if none of the `cnt` queued

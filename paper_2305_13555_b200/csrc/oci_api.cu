@@ -39,6 +39,7 @@ struct oci_ctx {
     DevView V{};
     alignas(64) KtiledMaps maps{};
     alignas(64) RedKtiledMaps rmaps{};
+    alignas(64) RedResidentMaps rrmaps{};
     bool use_ktiled = false;
     cudaStream_t stream = nullptr;
     void* ws = nullptr;
@@ -241,7 +242,7 @@ int launch_reduced_pass(oci_ctx* ctx, int pass, int ybase, int slot, int prev_sl
     if (ctx->red_kernel == OCI_RKERNEL_KTILED)
         return launch_red_ktiled(ctx->V, ctx->rmaps, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
     if (ctx->red_kernel == OCI_RKERNEL_RESIDENT)
-        return launch_red_resident(ctx->V, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
+        return launch_red_resident(ctx->V, ctx->rrmaps, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
     return launch_red_gemv(ctx->V, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
 }
 
@@ -475,7 +476,7 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     }
     ctx->use_ktiled = ctx->path == OCI_PATH_SHARED && !oci_shared_fast_supported(V) && oci_ktiled_supported(V) &&
                       oci_ktiled_prepare(V, &ctx->maps);
-    ctx->red_kernel = oci_red_resident_supported(V) ? OCI_RKERNEL_RESIDENT
+    ctx->red_kernel = (oci_red_resident_supported(V) && oci_red_resident_prepare(V, &ctx->rrmaps)) ? OCI_RKERNEL_RESIDENT
                       : (oci_red_ktiled_supported(V) && oci_red_ktiled_prepare(V, &ctx->rmaps)) ? OCI_RKERNEL_KTILED
                                                                                                  : OCI_RKERNEL_GEMV;
     ctx->cur = 0;

@@ -67,6 +67,14 @@ struct RedKtiledMaps {
     CUtensorMap y[2], z, q16, xop, xop8, rop, rop8, fop;
 };
 
+// Tensor maps of the resident kernels of the reduced step (oci_reduced_resident.cu)
+struct RedResidentMaps {
+    CUtensorMap y_rows[2];   // box (K2+4) x 18: whole rows j0-1 .. j0+16 of y, padded pitch (ITER, FINAL)
+    CUtensorMap y_half[2];   // box (N+4) x 16 at column N/2: the k+1/2 run of y (FIX)
+    CUtensorMap z_half;      // same of z
+    CUtensorMap q;           // box 4 x 16 of Q
+};
+
 // The stopping rule (reading S2), evaluated identically on host and device.
 __host__ __device__ inline bool converged(double tol, double d, double r) { return tol >= 0.0 && d <= tol * r; }
 
@@ -99,14 +107,17 @@ int launch_unpack_yz(const DevView& V, int buf, int ybuf, cudaStream_t s);
 // of the first of the `cnt` queued iterations
 int launch_red_gemv(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
                     cudaStream_t s);
-// row-major fp64 matrix [rows][cols] -> 2-D tensor map, box = box_rows x 16 columns, 128-byte swizzle, zero fill
-bool oci_encode_2d(CUtensorMap* m, const double* base, uint64_t rows, uint64_t cols, uint32_t box_rows);
+// row-major fp64 matrix [rows][cols] -> 2-D tensor map, box = box_rows x box_cols, zero fill outside; swizzle128
+// needs box_cols = 16
+bool oci_encode_2d(CUtensorMap* m, const double* base, uint64_t rows, uint64_t cols, uint32_t box_rows, uint32_t box_cols,
+                   bool swizzle128);
 bool oci_red_ktiled_supported(const DevView& V);
 bool oci_red_ktiled_prepare(const DevView& V, RedKtiledMaps* M);
 int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int ybase, int slot, int prev_slot, double tol,
                       int cnt, int force, cudaStream_t s);
 bool oci_red_resident_supported(const DevView& V);
-int launch_red_resident(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
+bool oci_red_resident_prepare(const DevView& V, RedResidentMaps* M);
+int launch_red_resident(const DevView& V, const RedResidentMaps& M, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
                         cudaStream_t s);
 
 }  // namespace oci

@@ -313,18 +313,20 @@ EncodeTiledFn encode_fn()
 
 }  // namespace
 
-// row-major fp64 matrix [rows][cols]; box = box_rows x 16 columns, 128-byte swizzle, zero fill outside
-bool oci_encode_2d(CUtensorMap* m, const double* base, uint64_t rows, uint64_t cols, uint32_t box_rows)
+// row-major fp64 matrix [rows][cols] -> 2-D tensor map with a box of box_rows x box_cols, zero fill outside;
+// swizzle128: box_cols must be 16 (one 128-byte row per box row), else the box lands dense in shared memory
+bool oci_encode_2d(CUtensorMap* m, const double* base, uint64_t rows, uint64_t cols, uint32_t box_rows, uint32_t box_cols,
+                   bool swizzle128)
 {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     cuuint64_t dims[2] = {cols, rows};
     cuuint64_t strides[1] = {cols * 8};
-    cuuint32_t box[2] = {KT_K, box_rows};
+    cuuint32_t box[2] = {box_cols, box_rows};
     cuuint32_t estr[2] = {1, 1};
     return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(base), dims, strides, box, estr,
-              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+              CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+              CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 bool oci_ktiled_supported(const DevView& V)
@@ -335,10 +337,10 @@ bool oci_ktiled_supported(const DevView& V)
 bool oci_ktiled_prepare(const DevView& V, KtiledMaps* M)
 {
     const uint64_t n = (uint64_t)V.n;
-    return oci_encode_2d(&M->cfix, V.cfix, (uint64_t)V.J, n, KT_M) &&
-           oci_encode_2d(&M->psi[0], V.psi[0] - n, (uint64_t)V.J + 2, n, KT_M) &&
-           oci_encode_2d(&M->psi[1], V.psi[1] - n, (uint64_t)V.J + 2, n, KT_M) &&
-           oci_encode_2d(&M->binv, V.binv, n, n, KT_N);
+    return oci_encode_2d(&M->cfix, V.cfix, (uint64_t)V.J, n, KT_M, KT_K, true) &&
+           oci_encode_2d(&M->psi[0], V.psi[0] - n, (uint64_t)V.J + 2, n, KT_M, KT_K, true) &&
+           oci_encode_2d(&M->psi[1], V.psi[1] - n, (uint64_t)V.J + 2, n, KT_M, KT_K, true) &&
+           oci_encode_2d(&M->binv, V.binv, n, n, KT_N, KT_K, true);
 }
 
 int launch_oci_ktiled(const DevView& V, const KtiledMaps& M, int src, int slot, int prev_slot, double tol, cudaStream_t s)

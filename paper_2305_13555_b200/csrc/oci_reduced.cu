@@ -24,13 +24,14 @@
 // rounding order the iterates are those of the plain method, so iteration counts and fluxes are held to
 // the same parity tolerances as the full form.
 //
-// Packed state.  q = half*N + h*(N/2) + mm with angle m = half*(N/2) + mm, h = 0 for the k slot and 1 for
-// the k+1/2 slot: O(q) = 4m + (half ? 2h+1 : 2h).  y[j][q] = Psi[j][O(q)], z[j][q] = Psi[j][O(q)^1].  With
-// ascending mu the first N entries of y[j] leave through the left face and feed cell j-1, the last N feed
-// cell j+1: inc[j][q] = y[j+1][q] (q < N), y[j-1][q] (q >= N); |mu| is folded into G, H, F.  The y buffers
-// carry ghost rows -1 and J like the Psi buffers do.  psi_{k-1/2}[j] (the commit, row a8) is the h = 1
-// quarter-rows of y[j] and z[j]: four contiguous runs of N/2 doubles, which is what lets a TMA unit
-// fetch them.  The full-layout Psi is produced from (y, z) only when somebody asks for it
+// Packed state.  Angle m = half*(N/2) + mm, h = 0 for the k slot and 1 for the k+1/2 slot:
+//     q = h*(N/2) + mm            (half = 0, mu<0)        q = N + (1-h)*(N/2) + mm     (half = 1, mu>0)
+// O(q) = 4m + (half ? 2h+1 : 2h);  y[j][q] = Psi[j][O(q)],  z[j][q] = Psi[j][O(q)^1].  With ascending mu the
+// first N entries of y[j] leave through the left face and feed cell j-1, the last N feed cell j+1:
+// inc[j][q] = y[j+1][q] (q < N), y[j-1][q] (q >= N); |mu| is folded into G, H, F.  The y buffers carry ghost
+// rows -1 and J like the Psi buffers do.  psi_{k-1/2}[j] (the commit, row a8) is the h = 1 entries of y[j]
+// and z[j]: with this order ONE contiguous run [N/2, 3N/2) of each row, which is what lets a TMA unit
+// fetch it as a box.  The full-layout Psi is produced from (y, z) only when somebody asks for it
 // (oci_get_angular_flux, si_step, a FULL-form step): a change of layout, no arithmetic.
 //
 // This file: the operator packing (setup), the Psi <-> (y, z) layout kernels, and the generic kernels
@@ -42,7 +43,8 @@ namespace oci {
 
 namespace {
 
-// RHS row (full index) that column u < 2N of the FIX operator feeds: u walks the h = 1 runs of y then z
+// RHS row (full index) that column u < 2N of the FIX operator feeds: u < N walks y[j][N/2 + u], u >= N walks
+// z[j][N/2 + (u - N)] (the k+1/2 runs)
 __device__ __forceinline__ int fix_col_row(int u, int N)
 {
     const int N2 = N >> 1;
@@ -213,10 +215,8 @@ __global__ void __launch_bounds__(256) oci_red_gemv_kernel(DevView V, int ybase,
     if (PASS == PASS_FIX) {
         for (int u = tid; u < K; u += 256) {
             double v;
-            if (u < N2) v = Ys[j * K2 + N2 + u];
-            else if (u < N) v = Ys[j * K2 + N + u];
-            else if (u < N + N2) v = V.z[j * K2 + N2 + (u - N)];
-            else if (u < K2) v = V.z[j * K2 + u];
+            if (u < N) v = Ys[j * K2 + N2 + u];
+            else if (u < K2) v = V.z[j * K2 + N2 + (u - N)];
             else v = V.Q[j * 4 + (u - K2)];
             in[u] = v;
         }

@@ -5,7 +5,7 @@
 // whose input vector is a concatenation of row segments of arrays that already sit in HBM in the packed
 // layout (no assembly, |mu| / alpha / h/4 folded into the operator):
 //     ITER, FINAL:  in_j = [ y[j+1][0:N] | y[j-1][N:2N] ]
-//     FIX        :  in_j = [ y[j][N/2:N] | y[j][3N/2:2N] | z[j][N/2:N] | z[j][3N/2:2N] | Q16[j] ]
+//     FIX        :  in_j = [ y[j][N/2:3N/2] | z[j][N/2:3N/2] | Q16[j] ]
 // so every K chunk of the A operand is ONE 2-D tensor-map TMA box (64 cells x 16 k) from some (array,
 // column, row shift), and every chunk of the B operand one box (128 operator rows x 16 k).  The operator
 // (0.5 - 1.1 MB) stays in L2.
@@ -155,10 +155,8 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
                     mbar_expect_tx(&full[s], RK_A_BYTES + RK_B_BYTES + (with_phi ? RK_P_BYTES : 0));
                     if (PASS == PASS_FIX) {
                         // y / z map rows: y carries the ghost row first (row = cell + 1), z and Q16 do not
-                        if (k0 < N2) tma_load_2d(st, my, N2 + k0, j0 + 1, &full[s]);
-                        else if (k0 < N) tma_load_2d(st, my, N + k0, j0 + 1, &full[s]);
-                        else if (k0 < N + N2) tma_load_2d(st, &map_z, k0 - N2, j0, &full[s]);
-                        else if (k0 < K2) tma_load_2d(st, &map_z, k0, j0, &full[s]);
+                        if (k0 < N) tma_load_2d(st, my, N2 + k0, j0 + 1, &full[s]);
+                        else if (k0 < K2) tma_load_2d(st, &map_z, N2 + k0 - N, j0, &full[s]);
                         else tma_load_2d(st, &map_q, 0, j0, &full[s]);
                     } else {
                         // k < N (mu<0) comes from the right neighbour, else from the left one (row a3)
@@ -319,11 +317,11 @@ bool oci_red_ktiled_supported(const DevView& V)
 bool oci_red_ktiled_prepare(const DevView& V, RedKtiledMaps* M)
 {
     const uint64_t K2 = (uint64_t)V.n / 2, J = (uint64_t)V.J;
-    return oci_encode_2d(&M->y[0], V.y[0] - K2, J + 2, K2, RK_M) && oci_encode_2d(&M->y[1], V.y[1] - K2, J + 2, K2, RK_M) &&
-           oci_encode_2d(&M->z, V.z, J, K2, RK_M) && oci_encode_2d(&M->q16, V.q16, J, 16, RK_M) &&
-           oci_encode_2d(&M->xop, V.xop, 2 * K2 + 8, K2 + 16, RK_N) && oci_encode_2d(&M->xop8, V.xop, 2 * K2 + 8, K2 + 16, 8) &&
-           oci_encode_2d(&M->rop, V.rop, K2 + 8, K2, RK_N) && oci_encode_2d(&M->rop8, V.rop, K2 + 8, K2, 8) &&
-           oci_encode_2d(&M->fop, V.fop, K2, K2, RK_N);
+    return oci_encode_2d(&M->y[0], V.y[0] - K2, J + 2, K2, RK_M, RK_K, true) && oci_encode_2d(&M->y[1], V.y[1] - K2, J + 2, K2, RK_M, RK_K, true) &&
+           oci_encode_2d(&M->z, V.z, J, K2, RK_M, RK_K, true) && oci_encode_2d(&M->q16, V.q16, J, 16, RK_M, RK_K, true) &&
+           oci_encode_2d(&M->xop, V.xop, 2 * K2 + 8, K2 + 16, RK_N, RK_K, true) && oci_encode_2d(&M->xop8, V.xop, 2 * K2 + 8, K2 + 16, 8, RK_K, true) &&
+           oci_encode_2d(&M->rop, V.rop, K2 + 8, K2, RK_N, RK_K, true) && oci_encode_2d(&M->rop8, V.rop, K2 + 8, K2, 8, RK_K, true) &&
+           oci_encode_2d(&M->fop, V.fop, K2, K2, RK_N, RK_K, true);
 }
 
 int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int ybase, int slot, int prev_slot, double tol, int cnt,

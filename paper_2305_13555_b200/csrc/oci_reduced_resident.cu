@@ -15,12 +15,16 @@
 //   * the operator (39 KB for ITER, 74 KB for FIX at K2 = 64) lives in shared memory, rows padded to K2+4
 //     doubles so that the DMMA fragment loads are bank-conflict free; per k-step a warp loads 2 A fragments
 //     (cells) and NB B fragments (operator) for 2*NB DMMA.8x8x4;
-//   * the input vectors need NO assembly: inc[j] = [y[j+1][0:N] | y[j-1][N:2N]] (|mu| is folded into the
-//     operator) and psi_{k-1/2}[j] = four runs of N/2 doubles of y[j], z[j] (alpha folded into X), so each
-//     lane issues 1-D bulk TMA copies (cp.async.bulk) straight into the warp's private two-stage ring; the
-//     next tile is requested before the current one is computed;
+//   * the input vectors need NO assembly (|mu|, alpha, h/4 are folded into the operators) and arrive as
+//     tensor-map TMA boxes issued by one lane into the warp's private two-stage ring, the next tile
+//     requested before the current one is computed.  ITER / FINAL: inc[j] = [y[j+1][0:N] | y[j-1][N:2N]], so
+//     a tile of 16 cells is ONE box of the 18 whole rows j0-1 .. j0+16 of y; the box is 4 columns wider than
+//     the array (zero filled), which gives the padded, bank-conflict-free row pitch for free.  FIX:
+//     psi_{k-1/2}[j] = the k+1/2 runs y[j][N/2:3N/2], z[j][N/2:3N/2]: two boxes of N+4 columns, plus Q;
 //   * yfix / ifix / phifix / old phi are read straight from global memory in accumulator layout at the
 //     start of the tile and only consumed in the epilogue (added to the accumulators, 16-byte stores).
+#include <cuda.h>
+
 #include "device_utils.cuh"
 
 namespace oci {
@@ -52,39 +56,46 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
         "DONE_%=:\n"
         "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar)
 {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+            smem_u32(dst)),
+        "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(smem_u32(bar))
+        : "memory");
 }
 
 
 template <int K2, int PASS>
 struct RCfg {
-    static constexpr int KIN = PASS == PASS_FIX ? K2 + 4 : K2;          // operator columns (k extent)
-    static constexpr int LD = K2 + 4;                                    // padded row (doubles): LD = 4 (mod 16)
+    static constexpr int N = K2 / 2;
+    static constexpr int LD = K2 + 4;                                    // operator row pitch (doubles): LD = 4 (mod 16)
+    static constexpr int LDH = N + 4;                                    // FIX: pitch of the y / z half-row boxes
     static constexpr int NB0 = PASS == PASS_FINAL ? K2 / 8 : K2 / 8 + 1; // n8 blocks of row group 0 (last = scalar flux)
     static constexpr int NB1 = PASS == PASS_FIX ? K2 / 8 : 0;            // row group 1 (FIX only: the I rows)
-    static constexpr int KS = KIN / 4;
+    static constexpr int KIN = PASS == PASS_FIX ? K2 + 4 : K2;           // operator columns
     static constexpr int OP_DOUBLES = (NB0 + NB1) * 8 * LD;
-    static constexpr int STAGE_DOUBLES = RT_M * LD;
-    static constexpr size_t SMEM = sizeof(double) * (OP_DOUBLES + RT_WARPS * RT_STAGES * STAGE_DOUBLES) +
+    // stage: ITER / FINAL [18][LD] (rows j0-1 .. j0+16 of y); FIX [16][LDH] y | [16][LDH] z | [16][4] Q
+    static constexpr int STAGE_BYTES_RAW = PASS == PASS_FIX ? (2 * RT_M * LDH + RT_M * 4) * 8 : (RT_M + 2) * LD * 8;
+    static constexpr int STAGE_BYTES = (STAGE_BYTES_RAW + 127) / 128 * 128;
+    static constexpr int TX_BYTES = STAGE_BYTES_RAW;                     // a box always delivers all its bytes (zero fill)
+    static constexpr size_t SMEM = 128 + sizeof(double) * OP_DOUBLES + (size_t)RT_WARPS * RT_STAGES * STAGE_BYTES +
                                    RT_WARPS * RT_STAGES * 8 + 16;
+    static_assert((OP_DOUBLES * 8) % 128 == 0, "ring must stay 128-byte aligned");
 };
 
-// acc[g][t] += A(cells 8g..8g+7) . Op(rows 8t..8t+7)^T over KS k-steps
-template <int NB, int KS, int LD>
-__device__ __forceinline__ void tile_dmma(double (&acc)[2][NB][2], const double* __restrict__ arow, const double* __restrict__ brow)
+// acc[g][t] += A(cells 8g..8g+7) . Op(rows 8t..8t+7)^T over KS k-steps; a: this lane's element of cell row
+// g4 (pitch LDA), b: of operator row g4 (pitch LDB)
+template <int NB, int KS, int LDA, int LDB>
+__device__ __forceinline__ void tile_dmma(double (&acc)[2][NB][2], const double* __restrict__ a0, const double* __restrict__ b0)
 {
 #pragma unroll 4
     for (int ks = 0; ks < KS; ++ks) {
         double a[2], b[NB];
 #pragma unroll
-        for (int g = 0; g < 2; ++g) a[g] = arow[(8 * g) * LD + 4 * ks];
+        for (int g = 0; g < 2; ++g) a[g] = a0[(8 * g) * LDA + 4 * ks];
 #pragma unroll
-        for (int t = 0; t < NB; ++t) b[t] = brow[(8 * t) * LD + 4 * ks];
+        for (int t = 0; t < NB; ++t) b[t] = b0[(8 * t) * LDB + 4 * ks];
 #pragma unroll
         for (int g = 0; g < 2; ++g)
 #pragma unroll
@@ -92,12 +103,38 @@ __device__ __forceinline__ void tile_dmma(double (&acc)[2][NB][2], const double*
     }
 }
 
+// all k-steps of one row group of a tile
+template <int K2, int PASS, int NB>
+__device__ __forceinline__ void tile_group(double (&acc)[2][NB][2], const unsigned char* st, const double* __restrict__ brow, int g4,
+                                           int t4)
+{
+    using C = RCfg<K2, PASS>;
+    constexpr int N = K2 / 2;
+    if (PASS == PASS_FIX) {
+        const double* yp = reinterpret_cast<const double*>(st) + g4 * C::LDH + t4;
+        const double* zp = yp + RT_M * C::LDH;
+        const double* qp = reinterpret_cast<const double*>(st) + 2 * RT_M * C::LDH + g4 * 4 + t4;
+        tile_dmma<NB, N / 4, C::LDH, C::LD>(acc, yp, brow);
+        tile_dmma<NB, N / 4, C::LDH, C::LD>(acc, zp, brow + N);
+        tile_dmma<NB, 1, 4, C::LD>(acc, qp, brow + K2);
+    } else {
+        // cell r of the tile: k < N from y row r+2 (cell j+1), k >= N from y row r (cell j-1)
+        const double* lo = reinterpret_cast<const double*>(st) + (g4 + 2) * C::LD + t4;
+        const double* hi = reinterpret_cast<const double*>(st) + g4 * C::LD + t4 + N;
+        tile_dmma<NB, N / 4, C::LD, C::LD>(acc, lo, brow);
+        tile_dmma<NB, N / 4, C::LD, C::LD>(acc, hi, brow + N);
+    }
+}
+
 }  // namespace
 
 template <int K2, int PASS>
 __global__ void __launch_bounds__(RT_WARPS * 32, 1)
-oci_red_resident_kernel(DevView V, int ybase, int slot, int prev_slot, double tol, int cnt, int force)
+oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_a_alt,
+                        const __grid_constant__ CUtensorMap map_z, const __grid_constant__ CUtensorMap map_q, int ybase, int slot,
+                        int prev_slot, double tol, int cnt, int force)
 {
+    // map_a: tensor map of y[ybase] (whole-row boxes for ITER / FINAL, half-row boxes for FIX), map_a_alt: of y[ybase ^ 1]
     using C = RCfg<K2, PASS>;
     int ysrc = ybase;
     if (PASS == PASS_ITER) {
@@ -110,17 +147,51 @@ oci_red_resident_kernel(DevView V, int ybase, int slot, int prev_slot, double to
         }
         ysrc = (ybase + L - 1) & 1;
     }
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    double* op_s = reinterpret_cast<double*>(smem_raw);                         // [(NB0+NB1)*8][LD]
-    double* ring = op_s + C::OP_DOUBLES;                                        // [warps][stages][RT_M][LD]
-    uint64_t* full = reinterpret_cast<uint64_t*>(ring + RT_WARPS * RT_STAGES * C::STAGE_DOUBLES);
+    const CUtensorMap* my = (ysrc == ybase) ? &map_a : &map_a_alt;
+
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char* sbase = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+    double* op_s = reinterpret_cast<double*>(sbase);                            // [(NB0+NB1)*8][LD]
+    unsigned char* ring = sbase + sizeof(double) * C::OP_DOUBLES;               // [warps][stages][STAGE_BYTES]
+    uint64_t* full = reinterpret_cast<uint64_t*>(ring + (size_t)RT_WARPS * RT_STAGES * C::STAGE_BYTES);
 
     constexpr int N = K2 / 2, N2 = K2 / 4;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g4 = lane >> 2, t4 = lane & 3;
     const int64_t J = V.J;
-    const double* __restrict__ Ys = V.y[ysrc];
     double* __restrict__ Yd = V.y[ysrc ^ 1];
+
+    const int64_t ntiles = (J + RT_M - 1) / RT_M;
+    const int64_t wid = (int64_t)blockIdx.x * RT_WARPS + warp, nw = (int64_t)gridDim.x * RT_WARPS;
+    const int my_tiles = wid < ntiles ? (int)((ntiles - wid + nw - 1) / nw) : 0;
+    unsigned char* my_ring = ring + (size_t)warp * RT_STAGES * C::STAGE_BYTES;
+    uint64_t* my_full = full + warp * RT_STAGES;
+
+    if (lane == 0) {
+        for (int s = 0; s < RT_STAGES; ++s) mbar_init(&my_full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+
+    // one lane requests a tile: tensor-map boxes straight into the warp's private ring
+    auto prefetch = [&](int it) {
+        if (lane == 0) {
+            const int s = it & 1;
+            const int j0 = (int)((wid + (int64_t)it * nw) * RT_M);
+            unsigned char* st = my_ring + (size_t)s * C::STAGE_BYTES;
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            mbar_expect_tx(&my_full[s], C::TX_BYTES);
+            if (PASS == PASS_FIX) {
+                tma_load_2d(st, my, N2, j0 + 1, &my_full[s]);                                     // y map row = cell + 1
+                tma_load_2d(st + RT_M * C::LDH * 8, &map_z, N2, j0, &my_full[s]);
+                tma_load_2d(st + 2 * RT_M * C::LDH * 8, &map_q, 0, j0, &my_full[s]);
+            } else {
+                tma_load_2d(st, my, 0, j0, &my_full[s]);                                          // rows j0-1 .. j0+16
+            }
+        }
+        __syncwarp();
+    };
+    if (my_tiles > 0) prefetch(0);           // in flight while the operator is staged below
 
     // operator -> shared memory.  FIX: X rows [O | I | phi] are regrouped as [O | phi | I]
     {
@@ -134,54 +205,10 @@ oci_red_resident_kernel(DevView V, int ybase, int slot, int prev_slot, double to
             *reinterpret_cast<double2*>(op_s + r * C::LD + 2 * c2) = *reinterpret_cast<const double2*>(src + (size_t)gr * GLD + 2 * c2);
         }
     }
-    if (lane == 0) {
-        for (int s = 0; s < RT_STAGES; ++s) mbar_init(&full[warp * RT_STAGES + s], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
     __syncthreads();
 
-    const int64_t ntiles = (J + RT_M - 1) / RT_M;
-    const int64_t wid = (int64_t)blockIdx.x * RT_WARPS + warp, nw = (int64_t)gridDim.x * RT_WARPS;
-    const int my_tiles = wid < ntiles ? (int)((ntiles - wid + nw - 1) / nw) : 0;
-    double* my_ring = ring + warp * RT_STAGES * C::STAGE_DOUBLES;
-    uint64_t* my_full = full + warp * RT_STAGES;
-
-    // bulk copies, one per lane and round.  ITER / FINAL: lanes 0..15 the first half of y[j+1] (mu<0 leaves
-    // cell j+1 through its left face), lanes 16..31 the second half of y[j-1].  FIX: the four h = 1 runs of
-    // y[j], z[j] and Q[j]
-    auto prefetch = [&](int it) {
-        const int s = it & 1;
-        const int64_t j0 = (wid + (int64_t)it * nw) * RT_M;
-        const int rows = (int)((J - j0 < RT_M) ? (J - j0) : RT_M);
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        if (lane == 0) mbar_expect_tx(&my_full[s], (uint32_t)rows * C::KIN * 8);
-        __syncwarp();
-        double* st = my_ring + s * C::STAGE_DOUBLES;
-        if (PASS == PASS_FIX) {
-            for (int idx = lane; idx < 5 * RT_M; idx += 32) {
-                const int row = idx & (RT_M - 1), seg = idx / RT_M;
-                if (row < rows) {
-                    const int64_t j = j0 + row;
-                    const double* src = seg == 0   ? Ys + j * K2 + N2
-                                        : seg == 1 ? Ys + j * K2 + N + N2
-                                        : seg == 2 ? V.z + j * K2 + N2
-                                        : seg == 3 ? V.z + j * K2 + N + N2
-                                                   : V.Q + j * 4;
-                    tma_load_1d(st + row * C::LD + seg * N2, src, seg == 4 ? 32 : N2 * 8, &my_full[s]);
-                }
-            }
-        } else {
-            const int row = lane & 15, half = lane >> 4;
-            if (row < rows) {
-                const int64_t j = j0 + row;
-                const double* src = half ? Ys + (j - 1) * K2 + N : Ys + (j + 1) * K2;
-                tma_load_1d(st + row * C::LD + half * N, src, N * 8, &my_full[s]);
-            }
-        }
-    };
-
     double dmax = 0.0, rmax = 0.0;
-    if (my_tiles > 0) prefetch(0);
+    const double* brow = op_s + g4 * C::LD + t4;
 
     for (int it = 0; it < my_tiles; ++it) {
         const int s = it & 1;
@@ -214,9 +241,8 @@ oci_red_resident_kernel(DevView V, int ybase, int slot, int prev_slot, double to
             for (int t = 0; t < C::NB0; ++t) acc[g][t][0] = acc[g][t][1] = 0.0;
 
         mbar_wait(&my_full[s], (it >> 1) & 1);
-        const double* arow = my_ring + s * C::STAGE_DOUBLES + g4 * C::LD + t4;
-        const double* brow = op_s + g4 * C::LD + t4;
-        tile_dmma<C::NB0, C::KS, C::LD>(acc, arow, brow);
+        const unsigned char* st = my_ring + (size_t)s * C::STAGE_BYTES;
+        tile_group<K2, PASS, C::NB0>(acc, st, brow, g4, t4);
 
         // ---- epilogue of row group 0
 #pragma unroll
@@ -252,19 +278,20 @@ oci_red_resident_kernel(DevView V, int ybase, int slot, int prev_slot, double to
         }
         if (PASS == PASS_FIX) {
             // ---- row group 1: the I rows of Psi_fix from the same input tile
-            double acc1[2][C::NB1 > 0 ? C::NB1 : 1][2];
+            constexpr int NB1 = C::NB1 > 0 ? C::NB1 : 1;
+            double acc1[2][NB1][2];
 #pragma unroll
             for (int g = 0; g < 2; ++g)
 #pragma unroll
-                for (int t = 0; t < C::NB1; ++t) acc1[g][t][0] = acc1[g][t][1] = 0.0;
-            tile_dmma<(C::NB1 > 0 ? C::NB1 : 1), C::KS, C::LD>(acc1, arow, brow + C::NB0 * 8 * C::LD);
+                for (int t = 0; t < NB1; ++t) acc1[g][t][0] = acc1[g][t][1] = 0.0;
+            tile_group<K2, PASS, NB1>(acc1, st, brow + C::NB0 * 8 * C::LD, g4, t4);
 #pragma unroll
             for (int g = 0; g < 2; ++g) {
                 const int r = 8 * g + g4;
                 const int64_t j = j0 + r;
                 if (r < rows) {
 #pragma unroll
-                    for (int t = 0; t < C::NB1; ++t)
+                    for (int t = 0; t < NB1; ++t)
                         *reinterpret_cast<double2*>(V.ifix + j * K2 + 8 * t + 2 * t4) = make_double2(acc1[g][t][0], acc1[g][t][1]);
                 }
             }
@@ -295,11 +322,22 @@ oci_red_resident_kernel(DevView V, int ybase, int slot, int prev_slot, double to
     }
 }
 
-bool oci_red_resident_supported(const DevView& V) { return V.nblk == 1 && (V.n == 128 || V.n == 64); }
+bool oci_red_resident_supported(const DevView& V) { return V.nblk == 1 && (V.n == 128 || V.n == 64) && V.J + 18 < (int64_t)1 << 31; }
+
+bool oci_red_resident_prepare(const DevView& V, RedResidentMaps* M)
+{
+    const uint64_t K2 = (uint64_t)V.n / 2, N = (uint64_t)V.N, J = (uint64_t)V.J;
+    for (int b = 0; b < 2; ++b)
+        if (!oci_encode_2d(&M->y_rows[b], V.y[b] - K2, J + 2, K2, RT_M + 2, (uint32_t)K2 + 4, false) ||
+            !oci_encode_2d(&M->y_half[b], V.y[b] - K2, J + 2, K2, RT_M, (uint32_t)N + 4, false))
+            return false;
+    return oci_encode_2d(&M->z_half, V.z, J, K2, RT_M, (uint32_t)N + 4, false) && oci_encode_2d(&M->q, V.Q, J, 4, RT_M, 4, false);
+}
 
 namespace {
 template <int K2, int PASS>
-void launch_rr(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
+void launch_rr(const DevView& V, const RedResidentMaps& M, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
+               cudaStream_t s)
 {
     static int sm_count = 0;
     static bool attr = false;
@@ -316,23 +354,28 @@ void launch_rr(const DevView& V, int ybase, int slot, int prev_slot, double tol,
     const int64_t ntiles = (V.J + RT_M - 1) / RT_M;
     const int64_t ctas = (ntiles + RT_WARPS - 1) / RT_WARPS;
     const unsigned grid = (unsigned)(ctas < sm_count ? ctas : sm_count);
-    oci_red_resident_kernel<K2, PASS><<<grid, RT_WARPS * 32, RCfg<K2, PASS>::SMEM, s>>>(V, ybase, slot, prev_slot, tol, cnt, force);
+    const int b = ybase & 1;
+    const CUtensorMap& ya = PASS == PASS_FIX ? M.y_half[b] : M.y_rows[b];
+    const CUtensorMap& yb = PASS == PASS_FIX ? M.y_half[b ^ 1] : M.y_rows[b ^ 1];
+    oci_red_resident_kernel<K2, PASS><<<grid, RT_WARPS * 32, RCfg<K2, PASS>::SMEM, s>>>(V, ya, yb, M.z_half, M.q, ybase, slot, prev_slot,
+                                                                                        tol, cnt, force);
 }
 
 template <int K2>
-void launch_rr_pass(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
+void launch_rr_pass(const DevView& V, const RedResidentMaps& M, int pass, int ybase, int slot, int prev_slot, double tol, int cnt,
+                    int force, cudaStream_t s)
 {
-    if (pass == PASS_FIX) launch_rr<K2, PASS_FIX>(V, ybase, 0, -1, tol, 0, 0, s);
-    else if (pass == PASS_ITER) launch_rr<K2, PASS_ITER>(V, ybase, slot, prev_slot, tol, 0, 0, s);
-    else launch_rr<K2, PASS_FINAL>(V, ybase, 0, -1, tol, cnt, force, s);
+    if (pass == PASS_FIX) launch_rr<K2, PASS_FIX>(V, M, ybase, 0, -1, tol, 0, 0, s);
+    else if (pass == PASS_ITER) launch_rr<K2, PASS_ITER>(V, M, ybase, slot, prev_slot, tol, 0, 0, s);
+    else launch_rr<K2, PASS_FINAL>(V, M, ybase, 0, -1, tol, cnt, force, s);
 }
 }  // namespace
 
-int launch_red_resident(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
-                        cudaStream_t s)
+int launch_red_resident(const DevView& V, const RedResidentMaps& M, int pass, int ybase, int slot, int prev_slot, double tol, int cnt,
+                        int force, cudaStream_t s)
 {
-    if (V.n == 128) launch_rr_pass<64>(V, pass, ybase, slot, prev_slot, tol, cnt, force, s);
-    else launch_rr_pass<32>(V, pass, ybase, slot, prev_slot, tol, cnt, force, s);
+    if (V.n == 128) launch_rr_pass<64>(V, M, pass, ybase, slot, prev_slot, tol, cnt, force, s);
+    else launch_rr_pass<32>(V, M, pass, ybase, slot, prev_slot, tol, cnt, force, s);
     return 1;
 }
 
