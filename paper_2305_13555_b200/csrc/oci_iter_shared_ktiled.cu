@@ -86,7 +86,8 @@ oci_iter_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_cfix, 
 {
     if (step_done(V.norms, prev_slot, tol)) return;
     extern __shared__ unsigned char smem_raw[];
-    unsigned char* base = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    // aligned up inside the shared window (pointer arithmetic on the array keeps the LDS/STS address space)
+    unsigned char* base = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     unsigned char* stages = base;                                                    // [S][cfix 8K | nbr 8K | binv 16K]
     double* phi_s = reinterpret_cast<double*>(base + (size_t)KT_STAGES * KT_STAGE_BYTES);   // [4 wn][64][4]
     double* coef_s = phi_s + 4 * KT_M * 4;                                            // [n]

@@ -103,7 +103,8 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
     const CUtensorMap* my = (ysrc == ybase) ? &map_y : &map_y_alt;
 
     extern __shared__ unsigned char smem_raw[];
-    unsigned char* base = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    // aligned up inside the shared window (pointer arithmetic on the array keeps the LDS/STS address space)
+    unsigned char* base = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     unsigned char* stages = base;                                                    // [S][A 8K | B 16K | P 1K | pad]
     double* phi_s = reinterpret_cast<double*>(base + (size_t)RK_STAGES * RK_STAGE_BYTES);   // [4 wn][64][4]
     uint64_t* full = reinterpret_cast<uint64_t*>(phi_s + 4 * RK_M * 4);
@@ -152,6 +153,9 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
                     if (q >= RK_STAGES) mbar_wait(&empty[s], ((q / RK_STAGES) - 1) & 1);
                     unsigned char* st = stages + (size_t)s * RK_STAGE_BYTES;
                     const int k0 = kc * RK_K;
+                    // the MMA warps read this stage through the generic proxy (LDS); order those reads, made
+                    // visible by the empty barrier, before the async-proxy write of the TMA unit
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                     mbar_expect_tx(&full[s], RK_A_BYTES + RK_B_BYTES + (with_phi ? RK_P_BYTES : 0));
                     if (PASS == PASS_FIX) {
                         // y / z map rows: y carries the ghost row first (row = cell + 1), z and Q16 do not

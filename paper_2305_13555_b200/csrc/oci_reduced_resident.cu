@@ -150,7 +150,8 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
     const CUtensorMap* my = (ysrc == ybase) ? &map_a : &map_a_alt;
 
     extern __shared__ unsigned char smem_raw[];
-    unsigned char* sbase = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+    // aligned up inside the shared window (pointer arithmetic on the array keeps the LDS/STS address space)
+    unsigned char* sbase = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
     double* op_s = reinterpret_cast<double*>(sbase);                            // [(NB0+NB1)*8][LD]
     unsigned char* ring = sbase + sizeof(double) * C::OP_DOUBLES;               // [warps][stages][STAGE_BYTES]
     uint64_t* full = reinterpret_cast<uint64_t*>(ring + (size_t)RT_WARPS * RT_STAGES * C::STAGE_BYTES);
