@@ -73,6 +73,9 @@ struct RedResidentMaps {
     CUtensorMap y_half[2];   // box (N+4) x 16 at column N/2: the k+1/2 run of y (FIX)
     CUtensorMap z_half;      // same of z
     CUtensorMap q;           // box 4 x 16 of Q
+    CUtensorMap rop, fop;    // the ITER / FINAL operator as one box of rows padded to K2+4
+    CUtensorMap xop_rows;    // K2 rows of X (the O rows, the I rows), columns 0 .. K2+3
+    CUtensorMap xop_phi;     // the 8-row scalar-flux block of X
 };
 
 // The stopping rule (reading S2), evaluated identically on host and device.

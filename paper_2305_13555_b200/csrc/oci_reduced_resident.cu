@@ -71,58 +71,122 @@ struct RCfg {
     static constexpr int N = K2 / 2;
     static constexpr int LD = K2 + 4;                                    // operator row pitch (doubles): LD = 4 (mod 16)
     static constexpr int LDH = N + 4;                                    // FIX: pitch of the y / z half-row boxes
-    static constexpr int NB0 = PASS == PASS_FINAL ? K2 / 8 : K2 / 8 + 1; // n8 blocks of row group 0 (last = scalar flux)
-    static constexpr int NB1 = PASS == PASS_FIX ? K2 / 8 : 0;            // row group 1 (FIX only: the I rows)
+    static constexpr int NSL = K2 / 8;                                   // n8 output blocks ("slices") of y / z / yfix / ifix
+    static constexpr int NB0 = PASS == PASS_FINAL ? NSL : NSL + 1;       // blocks of row group 0 (last = scalar flux)
+    static constexpr int NB1 = PASS == PASS_FIX ? NSL : 0;               // row group 1 (FIX only: the I rows)
     static constexpr int KIN = PASS == PASS_FIX ? K2 + 4 : K2;           // operator columns
+    static constexpr int KS = KIN / 4;                                   // k-steps of one phase
+    static constexpr int DIST = K2 / 16;                                 // pipelined epilogue: load-to-use distance (k-steps)
     static constexpr int OP_DOUBLES = (NB0 + NB1) * 8 * LD;
     // stage: ITER / FINAL [18][LD] (rows j0-1 .. j0+16 of y); FIX [16][LDH] y | [16][LDH] z | [16][4] Q
     static constexpr int STAGE_BYTES_RAW = PASS == PASS_FIX ? (2 * RT_M * LDH + RT_M * 4) * 8 : (RT_M + 2) * LD * 8;
     static constexpr int STAGE_BYTES = (STAGE_BYTES_RAW + 127) / 128 * 128;
     static constexpr int TX_BYTES = STAGE_BYTES_RAW;                     // a box always delivers all its bytes (zero fill)
     static constexpr size_t SMEM = 128 + sizeof(double) * OP_DOUBLES + (size_t)RT_WARPS * RT_STAGES * STAGE_BYTES +
-                                   RT_WARPS * RT_STAGES * 8 + 16;
+                                   (RT_WARPS * RT_STAGES + 1) * 8 + 16;
     static_assert((OP_DOUBLES * 8) % 128 == 0, "ring must stay 128-byte aligned");
 };
 
-// acc[g][t] += A(cells 8g..8g+7) . Op(rows 8t..8t+7)^T over KS k-steps; a: this lane's element of cell row
-// g4 (pitch LDA), b: of operator row g4 (pitch LDB)
-template <int NB, int KS, int LDA, int LDB>
-__device__ __forceinline__ void tile_dmma(double (&acc)[2][NB][2], const double* __restrict__ a0, const double* __restrict__ b0)
-{
-#pragma unroll 4
-    for (int ks = 0; ks < KS; ++ks) {
-        double a[2], b[NB];
-#pragma unroll
-        for (int g = 0; g < 2; ++g) a[g] = a0[(8 * g) * LDA + 4 * ks];
-#pragma unroll
-        for (int t = 0; t < NB; ++t) b[t] = b0[(8 * t) * LDB + 4 * ks];
-#pragma unroll
-        for (int g = 0; g < 2; ++g)
-#pragma unroll
-            for (int t = 0; t < NB; ++t) dmma(acc[g][t][0], acc[g][t][1], a[g], b[t]);
-    }
-}
+// what a finished accumulator tile still owes: its epilogue, drained during the NEXT phase's DMMA stream
+enum { PK_ITER = 0, PK_FINAL = 1, PK_FIX0 = 2, PK_FIX1 = 3 };
 
-// all k-steps of one row group of a tile
-template <int K2, int PASS, int NB>
-__device__ __forceinline__ void tile_group(double (&acc)[2][NB][2], const unsigned char* st, const double* __restrict__ brow, int g4,
-                                           int t4)
+// A-fragment element of k-step ks, cell block g, for this lane (pa = stage + lane offset; see the kernel)
+template <int K2, int PASS>
+__device__ __forceinline__ double a_frag(const double* __restrict__ pa, const double* __restrict__ pq, int ks, int g)
 {
     using C = RCfg<K2, PASS>;
     constexpr int N = K2 / 2;
     if (PASS == PASS_FIX) {
-        const double* yp = reinterpret_cast<const double*>(st) + g4 * C::LDH + t4;
-        const double* zp = yp + RT_M * C::LDH;
-        const double* qp = reinterpret_cast<const double*>(st) + 2 * RT_M * C::LDH + g4 * 4 + t4;
-        tile_dmma<NB, N / 4, C::LDH, C::LD>(acc, yp, brow);
-        tile_dmma<NB, N / 4, C::LDH, C::LD>(acc, zp, brow + N);
-        tile_dmma<NB, 1, 4, C::LD>(acc, qp, brow + K2);
-    } else {
-        // cell r of the tile: k < N from y row r+2 (cell j+1), k >= N from y row r (cell j-1)
-        const double* lo = reinterpret_cast<const double*>(st) + (g4 + 2) * C::LD + t4;
-        const double* hi = reinterpret_cast<const double*>(st) + g4 * C::LD + t4 + N;
-        tile_dmma<NB, N / 4, C::LD, C::LD>(acc, lo, brow);
-        tile_dmma<NB, N / 4, C::LD, C::LD>(acc, hi, brow + N);
+        if (ks < N / 4) return pa[(8 * g) * C::LDH + 4 * ks];                            // y half rows
+        if (ks < N / 2) return pa[(RT_M + 8 * g) * C::LDH + 4 * (ks - N / 4)];           // z half rows
+        return pq[(8 * g) * 4];                                                          // Q
+    }
+    // cell r of the tile: k < N from y row r+2 (cell j+1), k >= N from y row r (cell j-1)
+    return pa[(8 * g + (ks < N / 4 ? 2 : 0)) * C::LD + 4 * ks];
+}
+
+// Where a pending epilogue reads and writes (per kernel launch).
+struct EpiCtx {
+    const double* __restrict__ fixp;   // additive operand (yfix for ITER, ifix for FINAL)
+    double* __restrict__ out;          // y[dst] (ITER), z (FINAL), yfix (FIX0), ifix (FIX1)
+    const double* __restrict__ phifix;
+    double* __restrict__ phi;
+    double* __restrict__ phifix_out;
+};
+
+// One phase = all k-steps of one row group of one tile (NBC n8 blocks, accumulators acc) with the epilogue of
+// the PREVIOUS phase (pend, NBP blocks, cells pj0 .. pj0+prows-1) drained between the DMMAs one slice per
+// k-step: its loads are issued DIST k-steps before they are needed and its 16-byte stores are spread out, so
+// the warp never leaves the DMMA stream for a burst of memory instructions.  MMA = false: drain only.
+template <int K2, int PASS, int NBC, int NBP, int PK, bool MMA>
+__device__ __forceinline__ void phase(double (&acc)[2][NBC][2], const double* __restrict__ pa, const double* __restrict__ pq,
+                                      const double* __restrict__ brow, const double (&pend)[2][NBP][2], int64_t pj0, int prows,
+                                      const EpiCtx& E, int g4, int t4, double& dmax, double& rmax)
+{
+    using C = RCfg<K2, PASS>;
+    constexpr int NSL = C::NSL, KS = C::KS;
+    constexpr bool LOADS = PK == PK_ITER || PK == PK_FINAL;
+    constexpr int DIST = LOADS ? C::DIST : 0;
+    double2 fxw[NSL][2];
+    double2 pf[2], po[2];
+    int64_t pj[2];
+    bool ok[2];
+#pragma unroll
+    for (int g = 0; g < 2; ++g) {
+        const int r = 8 * g + g4;
+        ok[g] = r < prows;
+        pj[g] = pj0 + (ok[g] ? r : 0);                     // clamped: unconditional loads
+    }
+#pragma unroll
+    for (int ks = 0; ks < KS; ++ks) {
+        if (MMA) {
+            double a[2], b[NBC];
+#pragma unroll
+            for (int g = 0; g < 2; ++g) a[g] = a_frag<K2, PASS>(pa, pq, ks, g);
+#pragma unroll
+            for (int t = 0; t < NBC; ++t) b[t] = brow[(8 * t) * C::LD + 4 * ks];
+#pragma unroll
+            for (int g = 0; g < 2; ++g)
+#pragma unroll
+                for (int t = 0; t < NBC; ++t) dmma(acc[g][t][0], acc[g][t][1], a[g], b[t]);
+        }
+        // ---- pending epilogue: loads of slice ks
+        if (LOADS && ks < NSL) {
+#pragma unroll
+            for (int g = 0; g < 2; ++g) fxw[ks][g] = *reinterpret_cast<const double2*>(E.fixp + pj[g] * K2 + 8 * ks + 2 * t4);
+        }
+        if (PK == PK_ITER && ks == NSL) {
+#pragma unroll
+            for (int g = 0; g < 2; ++g) {
+                pf[g] = *reinterpret_cast<const double2*>(E.phifix + pj[g] * 4 + 2 * (t4 & 1));
+                po[g] = *reinterpret_cast<const double2*>(E.phi + pj[g] * 4 + 2 * (t4 & 1));
+            }
+        }
+        // ---- pending epilogue: slice ks - DIST is added and stored
+        const int t = ks - DIST;
+        if (t >= 0 && t < NSL) {
+#pragma unroll
+            for (int g = 0; g < 2; ++g) {
+                double2 v = make_double2(pend[g][t][0], pend[g][t][1]);
+                if (LOADS) { v.x += fxw[t][g].x; v.y += fxw[t][g].y; }
+                if (ok[g]) *reinterpret_cast<double2*>(E.out + pj[g] * K2 + 8 * t + 2 * t4) = v;
+            }
+        }
+        if ((PK == PK_ITER || PK == PK_FIX0) && ks == NSL + DIST) {     // scalar-flux block: columns 0..3 of block NSL
+#pragma unroll
+            for (int g = 0; g < 2; ++g) {
+                if (ok[g] && t4 < 2) {
+                    if (PK == PK_ITER) {
+                        const double p0 = pf[g].x + pend[g][NBP - 1][0], p1 = pf[g].y + pend[g][NBP - 1][1];
+                        *reinterpret_cast<double2*>(E.phi + pj[g] * 4 + 2 * t4) = make_double2(p0, p1);
+                        dmax = fmax(dmax, fmax(fabs(p0 - po[g].x), fabs(p1 - po[g].y)));
+                        rmax = fmax(rmax, fmax(fabs(p0), fabs(p1)));
+                    } else {
+                        *reinterpret_cast<double2*>(E.phifix_out + pj[g] * 4 + 2 * t4) = make_double2(pend[g][NBP - 1][0], pend[g][NBP - 1][1]);
+                    }
+                }
+            }
+        }
     }
 }
 
@@ -131,10 +195,12 @@ __device__ __forceinline__ void tile_group(double (&acc)[2][NB][2], const unsign
 template <int K2, int PASS>
 __global__ void __launch_bounds__(RT_WARPS * 32, 1)
 oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_a_alt,
-                        const __grid_constant__ CUtensorMap map_z, const __grid_constant__ CUtensorMap map_q, int ybase, int slot,
+                        const __grid_constant__ CUtensorMap map_z, const __grid_constant__ CUtensorMap map_q,
+                        const __grid_constant__ CUtensorMap map_op, const __grid_constant__ CUtensorMap map_op2, int ybase, int slot,
                         int prev_slot, double tol, int cnt, int force)
 {
-    // map_a: tensor map of y[ybase] (whole-row boxes for ITER / FINAL, half-row boxes for FIX), map_a_alt: of y[ybase ^ 1]
+    // map_a: tensor map of y[ybase] (whole-row boxes for ITER / FINAL, half-row boxes for FIX), map_a_alt: of
+    // y[ybase ^ 1]; map_op (+ map_op2 for the scalar-flux rows of X): the operator as boxes of padded rows
     using C = RCfg<K2, PASS>;
     int ysrc = ybase;
     if (PASS == PASS_ITER) {
@@ -155,6 +221,7 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
     double* op_s = reinterpret_cast<double*>(sbase);                            // [(NB0+NB1)*8][LD]
     unsigned char* ring = sbase + sizeof(double) * C::OP_DOUBLES;               // [warps][stages][STAGE_BYTES]
     uint64_t* full = reinterpret_cast<uint64_t*>(ring + (size_t)RT_WARPS * RT_STAGES * C::STAGE_BYTES);
+    uint64_t* op_bar = full + RT_WARPS * RT_STAGES;
 
     constexpr int N = K2 / 2, N2 = K2 / 4;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -168,11 +235,24 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
     unsigned char* my_ring = ring + (size_t)warp * RT_STAGES * C::STAGE_BYTES;
     uint64_t* my_full = full + warp * RT_STAGES;
 
-    if (lane == 0) {
-        for (int s = 0; s < RT_STAGES; ++s) mbar_init(&my_full[s], 1);
+    if (tid == 0) {
+        for (int s = 0; s < RT_WARPS * RT_STAGES; ++s) mbar_init(&full[s], 1);
+        mbar_init(op_bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    __syncwarp();
+    __syncthreads();
+
+    // the operator: one to three boxes of padded rows.  FIX: X rows [O | I | phi] land regrouped as [O | phi | I]
+    if (tid == 0) {
+        mbar_expect_tx(op_bar, C::OP_DOUBLES * 8);
+        if (PASS == PASS_FIX) {
+            tma_load_2d(op_s, &map_op, 0, 0, op_bar);
+            tma_load_2d(op_s + K2 * C::LD, &map_op2, 0, 2 * K2, op_bar);
+            tma_load_2d(op_s + (K2 + 8) * C::LD, &map_op, 0, K2, op_bar);
+        } else {
+            tma_load_2d(op_s, &map_op, 0, 0, op_bar);
+        }
+    }
 
     // one lane requests a tile: tensor-map boxes straight into the warp's private ring
     auto prefetch = [&](int it) {
@@ -192,48 +272,52 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
         }
         __syncwarp();
     };
-    if (my_tiles > 0) prefetch(0);           // in flight while the operator is staged below
+    if (my_tiles > 0) prefetch(0);
 
-    // operator -> shared memory.  FIX: X rows [O | I | phi] are regrouped as [O | phi | I]
-    {
-        const double* __restrict__ src = PASS == PASS_FIX ? V.xop : PASS == PASS_ITER ? V.rop : V.fop;
-        constexpr int GLD = PASS == PASS_FIX ? K2 + 16 : K2;
-        constexpr int C2 = C::KIN / 2;
-        for (int e = tid; e < (C::NB0 + C::NB1) * 8 * C2; e += RT_WARPS * 32) {
-            const int r = e / C2, c2 = e - r * C2;
-            int gr = r;
-            if (PASS == PASS_FIX) gr = r < K2 ? r : (r < K2 + 8 ? r + K2 : r - 8);
-            *reinterpret_cast<double2*>(op_s + r * C::LD + 2 * c2) = *reinterpret_cast<const double2*>(src + (size_t)gr * GLD + 2 * c2);
-        }
-    }
-    __syncthreads();
+    EpiCtx E;
+    E.fixp = PASS == PASS_FINAL ? V.ifix : V.yfix;
+    E.out = PASS == PASS_ITER ? Yd : PASS == PASS_FINAL ? V.z : V.yfix;
+    E.phifix = V.phifix;
+    E.phi = V.phi;
+    E.phifix_out = V.phifix;
+    EpiCtx E1 = E;                 // FIX: the pending I rows go to ifix
+    E1.out = V.ifix;
 
     double dmax = 0.0, rmax = 0.0;
     const double* brow = op_s + g4 * C::LD + t4;
+    constexpr int NBP = PASS == PASS_FIX ? C::NB1 : C::NB0;      // blocks of the epilogue carried from tile to tile
+    double pend[2][NBP][2];
+#pragma unroll
+    for (int g = 0; g < 2; ++g)
+#pragma unroll
+        for (int t = 0; t < NBP; ++t) pend[g][t][0] = pend[g][t][1] = 0.0;
+    int64_t pj0 = my_tiles > 0 ? wid * RT_M : 0;
+    int prows = 0;                                                 // nothing pending yet: loads clamped, stores off
+
+    mbar_wait(op_bar, 0);
+
+    // reflecting ghost rows of y (reading S4) by the warp that owns the edge cell, once its stores are out
+    auto ghost_rows = [&](int64_t j0, int rows) {
+        if (PASS != PASS_ITER || rows == 0) return;
+        const bool gl = j0 == 0 && V.bcL == OCI_BC_REFLECTING;
+        const bool gr = j0 + rows == J && V.bcR == OCI_BC_REFLECTING;
+        if (gl || gr) {
+            __syncwarp();
+            __threadfence_block();
+            for (int q = lane; q < K2; q += 32) {
+                const int mir = mirror_q(q, N);
+                if (gl && q >= N) Yd[-(int64_t)K2 + q] = __ldcg(Yd + mir);
+                if (gr && q < N) Yd[J * K2 + q] = __ldcg(Yd + (J - 1) * K2 + mir);
+            }
+            __syncwarp();
+        }
+    };
 
     for (int it = 0; it < my_tiles; ++it) {
         const int s = it & 1;
         const int64_t j0 = (wid + (int64_t)it * nw) * RT_M;
         const int rows = (int)((J - j0 < RT_M) ? (J - j0) : RT_M);
         if (it + 1 < my_tiles) prefetch(it + 1);
-
-        // ---- global operands of the epilogue, requested now, consumed after the DMMAs
-        double2 fx[2][PASS == PASS_FIX ? 1 : K2 / 8];
-        double2 pf[2], po[2];
-        if (PASS != PASS_FIX) {
-            const double* __restrict__ fixp = PASS == PASS_FINAL ? V.ifix : V.yfix;
-#pragma unroll
-            for (int g = 0; g < 2; ++g) {
-                const int r = 8 * g + g4;
-                const int64_t j = (r < rows) ? j0 + r : j0;             // clamped: unconditional loads
-#pragma unroll
-                for (int t = 0; t < K2 / 8; ++t) fx[g][t] = *reinterpret_cast<const double2*>(fixp + j * K2 + 8 * t + 2 * t4);
-                if (PASS == PASS_ITER) {
-                    pf[g] = *reinterpret_cast<const double2*>(V.phifix + j * 4 + 2 * (t4 & 1));
-                    po[g] = *reinterpret_cast<const double2*>(V.phi + j * 4 + 2 * (t4 & 1));
-                }
-            }
-        }
 
         double acc[2][C::NB0][2];
 #pragma unroll
@@ -242,76 +326,45 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
             for (int t = 0; t < C::NB0; ++t) acc[g][t][0] = acc[g][t][1] = 0.0;
 
         mbar_wait(&my_full[s], (it >> 1) & 1);
-        const unsigned char* st = my_ring + (size_t)s * C::STAGE_BYTES;
-        tile_group<K2, PASS, C::NB0>(acc, st, brow, g4, t4);
-
-        // ---- epilogue of row group 0
-#pragma unroll
-        for (int g = 0; g < 2; ++g) {
-            const int r = 8 * g + g4;
-            const int64_t j = j0 + r;
-            if (r < rows) {
-                if (PASS == PASS_ITER) {
-#pragma unroll
-                    for (int t = 0; t < K2 / 8; ++t)
-                        *reinterpret_cast<double2*>(Yd + j * K2 + 8 * t + 2 * t4) =
-                            make_double2(fx[g][t].x + acc[g][t][0], fx[g][t].y + acc[g][t][1]);
-                    if (t4 < 2) {                                   // phi rows: columns 0..3 of the last block
-                        const double p0 = pf[g].x + acc[g][C::NB0 - 1][0], p1 = pf[g].y + acc[g][C::NB0 - 1][1];
-                        *reinterpret_cast<double2*>(V.phi + j * 4 + 2 * t4) = make_double2(p0, p1);
-                        dmax = fmax(dmax, fmax(fabs(p0 - po[g].x), fabs(p1 - po[g].y)));
-                        rmax = fmax(rmax, fmax(fabs(p0), fabs(p1)));
-                    }
-                } else if (PASS == PASS_FINAL) {
-#pragma unroll
-                    for (int t = 0; t < K2 / 8; ++t)
-                        *reinterpret_cast<double2*>(V.z + j * K2 + 8 * t + 2 * t4) =
-                            make_double2(fx[g][t].x + acc[g][t][0], fx[g][t].y + acc[g][t][1]);
-                } else {
-#pragma unroll
-                    for (int t = 0; t < K2 / 8; ++t)
-                        *reinterpret_cast<double2*>(V.yfix + j * K2 + 8 * t + 2 * t4) = make_double2(acc[g][t][0], acc[g][t][1]);
-                    if (t4 < 2)
-                        *reinterpret_cast<double2*>(V.phifix + j * 4 + 2 * t4) =
-                            make_double2(acc[g][C::NB0 - 1][0], acc[g][C::NB0 - 1][1]);
-                }
-            }
-        }
+        const double* st = reinterpret_cast<const double*>(my_ring + (size_t)s * C::STAGE_BYTES);
         if (PASS == PASS_FIX) {
-            // ---- row group 1: the I rows of Psi_fix from the same input tile
+            const double* pa = st + g4 * C::LDH + t4;
+            const double* pq = st + 2 * RT_M * C::LDH + g4 * 4 + t4;
+            // row group 0 (O rows + scalar flux) while the previous tile's I rows are stored
+            phase<K2, PASS, C::NB0, NBP, PK_FIX1, true>(acc, pa, pq, brow, pend, pj0, prows, E1, g4, t4, dmax, rmax);
+            // row group 1 (I rows) while this tile's O rows and scalar flux are stored
             constexpr int NB1 = C::NB1 > 0 ? C::NB1 : 1;
             double acc1[2][NB1][2];
 #pragma unroll
             for (int g = 0; g < 2; ++g)
 #pragma unroll
                 for (int t = 0; t < NB1; ++t) acc1[g][t][0] = acc1[g][t][1] = 0.0;
-            tile_group<K2, PASS, NB1>(acc1, st, brow + C::NB0 * 8 * C::LD, g4, t4);
+            phase<K2, PASS, NB1, C::NB0, PK_FIX0, true>(acc1, pa, pq, brow + C::NB0 * 8 * C::LD, acc, j0, rows, E, g4, t4, dmax, rmax);
 #pragma unroll
-            for (int g = 0; g < 2; ++g) {
-                const int r = 8 * g + g4;
-                const int64_t j = j0 + r;
-                if (r < rows) {
+            for (int g = 0; g < 2; ++g)
 #pragma unroll
-                    for (int t = 0; t < NB1; ++t)
-                        *reinterpret_cast<double2*>(V.ifix + j * K2 + 8 * t + 2 * t4) = make_double2(acc1[g][t][0], acc1[g][t][1]);
-                }
-            }
+                for (int t = 0; t < NBP; ++t) { pend[g][t][0] = acc1[g][t < NB1 ? t : 0][0]; pend[g][t][1] = acc1[g][t < NB1 ? t : 0][1]; }
+        } else {
+            const double* pa = st + g4 * C::LD + t4;
+            phase<K2, PASS, C::NB0, NBP, PASS == PASS_ITER ? PK_ITER : PK_FINAL, true>(acc, pa, pa, brow, pend, pj0, prows, E, g4, t4,
+                                                                                       dmax, rmax);
+            ghost_rows(pj0, prows);
+#pragma unroll
+            for (int g = 0; g < 2; ++g)
+#pragma unroll
+                for (int t = 0; t < NBP; ++t) { pend[g][t][0] = acc[g][t][0]; pend[g][t][1] = acc[g][t][1]; }
         }
-        __syncwarp();
-        // ---- reflecting ghost rows of y (reading S4) by the warp that owns the edge cell
-        if (PASS == PASS_ITER) {
-            const bool gl = j0 == 0 && V.bcL == OCI_BC_REFLECTING;
-            const bool gr = j0 + rows == J && V.bcR == OCI_BC_REFLECTING;
-            if (gl || gr) {
-                __threadfence_block();
-                for (int q = lane; q < K2; q += 32) {
-                    const int mir = mirror_q(q, N);
-                    if (gl && q >= N) Yd[-(int64_t)K2 + q] = __ldcg(Yd + mir);
-                    if (gr && q < N) Yd[J * K2 + q] = __ldcg(Yd + (J - 1) * K2 + mir);
-                }
-                __syncwarp();
-            }
-        }
+        pj0 = j0;
+        prows = rows;
+    }
+    // ---- drain the last pending epilogue
+    if (prows > 0) {
+        double dummy[2][1][2];
+        if (PASS == PASS_FIX) phase<K2, PASS, 1, NBP, PK_FIX1, false>(dummy, nullptr, nullptr, nullptr, pend, pj0, prows, E1, g4, t4, dmax, rmax);
+        else
+            phase<K2, PASS, 1, NBP, PASS == PASS_ITER ? PK_ITER : PK_FINAL, false>(dummy, nullptr, nullptr, nullptr, pend, pj0, prows, E,
+                                                                                   g4, t4, dmax, rmax);
+        ghost_rows(pj0, prows);
     }
     if (PASS == PASS_ITER) {
         dmax = warp_max(dmax);
@@ -328,11 +381,16 @@ bool oci_red_resident_supported(const DevView& V) { return V.nblk == 1 && (V.n =
 bool oci_red_resident_prepare(const DevView& V, RedResidentMaps* M)
 {
     const uint64_t K2 = (uint64_t)V.n / 2, N = (uint64_t)V.N, J = (uint64_t)V.J;
+    const uint32_t LD = (uint32_t)K2 + 4;
     for (int b = 0; b < 2; ++b)
-        if (!oci_encode_2d(&M->y_rows[b], V.y[b] - K2, J + 2, K2, RT_M + 2, (uint32_t)K2 + 4, false) ||
+        if (!oci_encode_2d(&M->y_rows[b], V.y[b] - K2, J + 2, K2, RT_M + 2, LD, false) ||
             !oci_encode_2d(&M->y_half[b], V.y[b] - K2, J + 2, K2, RT_M, (uint32_t)N + 4, false))
             return false;
-    return oci_encode_2d(&M->z_half, V.z, J, K2, RT_M, (uint32_t)N + 4, false) && oci_encode_2d(&M->q, V.Q, J, 4, RT_M, 4, false);
+    return oci_encode_2d(&M->z_half, V.z, J, K2, RT_M, (uint32_t)N + 4, false) && oci_encode_2d(&M->q, V.Q, J, 4, RT_M, 4, false) &&
+           oci_encode_2d(&M->rop, V.rop, K2 + 8, K2, (uint32_t)K2 + 8, LD, false) &&
+           oci_encode_2d(&M->fop, V.fop, K2, K2, (uint32_t)K2, LD, false) &&
+           oci_encode_2d(&M->xop_rows, V.xop, 2 * K2 + 8, K2 + 16, (uint32_t)K2, LD, false) &&
+           oci_encode_2d(&M->xop_phi, V.xop, 2 * K2 + 8, K2 + 16, 8, LD, false);
 }
 
 namespace {
@@ -358,8 +416,9 @@ void launch_rr(const DevView& V, const RedResidentMaps& M, int ybase, int slot, 
     const int b = ybase & 1;
     const CUtensorMap& ya = PASS == PASS_FIX ? M.y_half[b] : M.y_rows[b];
     const CUtensorMap& yb = PASS == PASS_FIX ? M.y_half[b ^ 1] : M.y_rows[b ^ 1];
-    oci_red_resident_kernel<K2, PASS><<<grid, RT_WARPS * 32, RCfg<K2, PASS>::SMEM, s>>>(V, ya, yb, M.z_half, M.q, ybase, slot, prev_slot,
-                                                                                        tol, cnt, force);
+    const CUtensorMap& op = PASS == PASS_FIX ? M.xop_rows : PASS == PASS_ITER ? M.rop : M.fop;
+    oci_red_resident_kernel<K2, PASS><<<grid, RT_WARPS * 32, RCfg<K2, PASS>::SMEM, s>>>(V, ya, yb, M.z_half, M.q, op, M.xop_phi, ybase,
+                                                                                        slot, prev_slot, tol, cnt, force);
 }
 
 template <int K2>
