@@ -318,6 +318,18 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
         const int64_t j0 = (wid + (int64_t)it * nw) * RT_M;
         const int rows = (int)((J - j0 < RT_M) ? (J - j0) : RT_M);
         if (it + 1 < my_tiles) prefetch(it + 1);
+        // the additive operands of THIS tile's epilogue (drained during the next phase) -> L2, so that the loads
+        // issued DIST k-steps ahead of their use see an L2 hit instead of a DRAM round trip
+        if (PASS != PASS_FIX) {
+            const char* f0 = reinterpret_cast<const char*>(E.fixp + j0 * K2);
+            const int bytes = rows * K2 * 8;
+            for (int o = lane * 128; o < bytes; o += 32 * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(f0 + o));
+            if (PASS == PASS_ITER && lane < 8) {
+                const char* p0 = reinterpret_cast<const char*>((lane < 4 ? E.phifix : E.phi) + j0 * 4);
+                const int o = (lane & 3) * 128;
+                if (o < rows * 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(p0 + o));
+            }
+        }
 
         double acc[2][C::NB0][2];
 #pragma unroll
