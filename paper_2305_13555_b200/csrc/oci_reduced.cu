@@ -179,128 +179,220 @@ int launch_unpack_yz(const DevView& V, int buf, int ybuf, cudaStream_t s)
     return 1;
 }
 
-// ---- the three passes as a batched GEMV, one CTA per cell (PASS_* of oci_internal.h).
+// ---- the three passes as a batched GEMV (PASS_* of oci_internal.h), HBM-bound when every cell has its own
+// operator.  EVERY WARP IS AN INDEPENDENT WORKER: the (cell, group of GR operator rows) pairs of the whole
+// problem form one long stream that is cut into equal contiguous pieces, one per warp; a warp keeps the
+// input vector of its current cell in a private strip of shared memory, streams its GR rows with 16-byte
+// non-allocating loads (all GR x 16 B per lane in flight together), reduces them by shuffle, and lane r
+// finishes row r.  No CTA barrier anywhere, so the 32 resident warps of an SM drift apart and HBM always
+// sees requests; equal pieces of a fine-grained stream leave no tail wave (config 5 is only 3.5 waves of
+// one-CTA-per-cell).
 // FIX  :  [yfix | ifix | phifix][j] = X_b [psi_{k-1/2}[j]; Q[j]],  psi_{k-1/2} from y[ybase][j], z[j]
 // ITER :  y^(l+1)[j] = yfix[j] + G_b inc,  phi^(l+1)[j] = phifix[j] + H_b inc, norms, ghost rows of y
 // FINAL:  z[j] = ifix[j] + F_b inc^(L-1); L is found on the device from the norm slots of the `cnt`
 //         queued iterations (`force`: this chunk ends at max_iters, finalise after cnt iterations if
 //         none converged); y^(L) is already in place.
-template <int PASS, int ROWS>
-__global__ void __launch_bounds__(256) oci_red_gemv_kernel(DevView V, int ybase, int slot, int prev_slot, double tol,
+template <int PASS, int GR>
+__global__ void __launch_bounds__(256, 2) oci_red_gemv_kernel(DevView V, int ybase, int slot, int prev_slot, double tol,
                                                            int cnt, int force)
 {
+    extern __shared__ double sm[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
     int ysrc = ybase;
     if (PASS == PASS_ITER) {
         if (step_done(V.norms, prev_slot, tol)) return;
     } else if (PASS == PASS_FINAL) {
-        int L = first_converged(V.norms, cnt, tol);
+        // the last iteration of this chunk of launches, with all loads of the scan in flight at once
+        int L = 0;
+        for (int i0 = 0; i0 < cnt && L == 0; i0 += 32) {
+            const int i = i0 + lane;
+            bool hit = false;
+            if (i < cnt) {
+                const double d = __longlong_as_double((long long)__ldcg(V.norms + 2 * i + 0));
+                const double r = __longlong_as_double((long long)__ldcg(V.norms + 2 * i + 1));
+                hit = converged(tol, d, r);
+            }
+            const unsigned m = __ballot_sync(0xffffffffu, hit);
+            if (m) L = i0 + __ffs(m);
+        }
         if (L == 0) {
             if (!force) return;
             L = cnt;
         }
         ysrc = (ybase + L - 1) & 1;
     }
-    extern __shared__ double sm[];
     const int n = V.n, N = V.N, K2 = n >> 1, N2 = N >> 1;
     const int K = PASS == PASS_FIX ? K2 + 4 : K2;                       // operator columns used
     const int ld = PASS == PASS_FIX ? K2 + 16 : K2;                     // operator row stride
     const int rows = PASS == PASS_FIX ? 2 * K2 + 4 : PASS == PASS_ITER ? K2 + 4 : K2;
-    double* in = sm;             // [K]
-    double* out = sm + K2 + 4;   // [rows]
-    const int64_t j = blockIdx.x, J = V.J;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int gpc = (rows + GR - 1) / GR;                               // row groups per cell
+    const int64_t J = V.J, G = J * gpc;
+    const int64_t wid = (int64_t)blockIdx.x * nwarp + warp, nw = (int64_t)gridDim.x * nwarp;
+    const int64_t g_begin = G * wid / nw, g_end = G * (wid + 1) / nw;
+    double* in = sm + (size_t)warp * (K2 + 8);                          // this warp's input vector [K] (+ zero pad)
     const double* __restrict__ Ys = V.y[ysrc];
     double* __restrict__ Yd = V.y[ysrc ^ 1];
+    double dmax = 0.0, rmax = 0.0;
+    int64_t jcur = -1;
 
-    if (PASS == PASS_FIX) {
-        for (int u = tid; u < K; u += 256) {
-            double v;
-            if (u < N) v = Ys[j * K2 + N2 + u];
-            else if (u < K2) v = V.z[j * K2 + N2 + (u - N)];
-            else v = V.Q[j * 4 + (u - K2)];
-            in[u] = v;
+    // The (row group, 64-column slice) steps of this warp form one flat sequence; the 16-byte loads of step
+    // s+1 are issued before step s is consumed, so a warp always has GR x 512 B of its stream in flight.
+    // FIX: the four Q columns are not worth a slice of their own: the lane that finishes a row adds them
+    const int KS_ = PASS == PASS_FIX ? K2 : K;                          // columns streamed in slices
+    const int KI = (KS_ + 63) / 64;                                     // column slices per row
+    const int64_t S = (g_end - g_begin) * KI;
+    auto op_base = [&](int64_t g) -> const double* {
+        const int64_t j = g / gpc;
+        const int i0 = (int)(g - j * gpc) * GR;
+        const int64_t b = V.blk[j];
+        return (PASS == PASS_FIX    ? V.xop + (size_t)b * (2 * K2 + 8) * ld
+                : PASS == PASS_ITER ? V.rop + (size_t)b * (K2 + 8) * ld
+                                    : V.fop + (size_t)b * K2 * ld) + (size_t)i0 * ld;
+    };
+    auto load_step = [&](double2 (&dst)[GR], int64_t g, int ki) {
+        const int64_t j = g / gpc;
+        const int i0 = (int)(g - j * gpc) * GR;
+        const double* __restrict__ M = op_base(g);
+        const int k = 2 * lane + 64 * ki;
+#pragma unroll
+        for (int r = 0; r < GR; ++r)
+            dst[r] = (i0 + r < rows && k < KS_) ? ldg_stream2(M + (size_t)r * ld + k) : make_double2(0.0, 0.0);
+    };
+    double2 cur[GR], nxt[GR];
+    double acc[GR];
+    double add = 0.0, old = 0.0;
+    double2 qc0 = make_double2(0.0, 0.0), qc1 = make_double2(0.0, 0.0);
+    if (S > 0) load_step(nxt, g_begin, 0);
+    int64_t g = g_begin;
+    int ki = 0;
+    for (int64_t st = 0; st < S; ++st) {
+#pragma unroll
+        for (int r = 0; r < GR; ++r) cur[r] = nxt[r];
+        {
+            int kin = ki + 1;
+            int64_t gn = g;
+            if (kin == KI) { kin = 0; ++gn; }
+            if (st + 1 < S) load_step(nxt, gn, kin);
         }
-    } else {
-        for (int q = tid; q < K2; q += 256) in[q] = Ys[(q < N ? j + 1 : j - 1) * K2 + q];
+        const int64_t j = g / gpc;
+        const int i0 = (int)(g - j * gpc) * GR;
+        const int i = i0 + lane;
+        const bool mine = lane < GR && i < rows;       // lane r < GR finishes row i0 + r
+        if (ki == 0) {
+            if (j != jcur) {
+                __syncwarp();
+                if (PASS == PASS_FIX) {
+                    for (int u = lane; u < K; u += 32)
+                        in[u] = u < N ? Ys[j * K2 + N2 + u] : u < K2 ? V.z[j * K2 + N2 + (u - N)] : V.Q[j * 4 + (u - K2)];
+                } else {
+                    for (int q = lane; q < K2; q += 32) in[q] = Ys[(q < N ? j + 1 : j - 1) * K2 + q];
+                }
+                if (lane < 4) in[K + lane] = 0.0;       // columns past K read as zero (the operator loads are zero there)
+                __syncwarp();
+                jcur = j;
+            }
+#pragma unroll
+            for (int r = 0; r < GR; ++r) acc[r] = 0.0;
+            // the additive operand of this lane's row, requested now, consumed after the last slice
+            add = 0.0;
+            if (mine) {
+                if (PASS == PASS_FIX) {
+                    const double* __restrict__ qrow = op_base(g) + (size_t)lane * ld + K2;
+                    qc0 = ldg_stream2(qrow);
+                    qc1 = ldg_stream2(qrow + 2);
+                }
+                if (PASS == PASS_FINAL) add = V.ifix[j * K2 + i];
+                if (PASS == PASS_ITER) {
+                    if (i < K2) add = V.yfix[j * K2 + i];
+                    else { add = V.phifix[j * 4 + (i - K2)]; old = V.phi[j * 4 + (i - K2)]; }
+                }
+            }
+        }
+        {
+            const int k = 2 * lane + 64 * ki;
+            const double2 c = k < KS_ ? *reinterpret_cast<const double2*>(in + k) : make_double2(0.0, 0.0);
+#pragma unroll
+            for (int r = 0; r < GR; ++r) acc[r] = fma(cur[r].y, c.y, fma(cur[r].x, c.x, acc[r]));
+        }
+        if (ki == KI - 1) {
+            double o = 0.0;
+#pragma unroll
+            for (int r = 0; r < GR; ++r) {
+#pragma unroll
+                for (int sh = 16; sh > 0; sh >>= 1) acc[r] += __shfl_xor_sync(0xffffffffu, acc[r], sh);
+                if (lane == r) o = acc[r];
+            }
+            if (mine) {
+                if (PASS == PASS_FIX) {
+                    o = fma(qc1.y, in[K2 + 3], fma(qc1.x, in[K2 + 2], fma(qc0.y, in[K2 + 1], fma(qc0.x, in[K2], o))));
+                    if (i < K2) V.yfix[j * K2 + i] = o;
+                    else if (i < 2 * K2) V.ifix[j * K2 + (i - K2)] = o;
+                    else V.phifix[j * 4 + (i - 2 * K2)] = o;
+                } else if (PASS == PASS_FINAL) {
+                    V.z[j * K2 + i] = add + o;
+                } else if (i < K2) {
+                    const double v = add + o;
+                    Yd[j * K2 + i] = v;
+                    // reflecting ghost rows (reading S4): the mirror image of the edge cell's outgoing flux
+                    if (j == 0 && i < N && V.bcL == OCI_BC_REFLECTING) Yd[-(int64_t)K2 + mirror_q(i, N)] = v;
+                    if (j == J - 1 && i >= N && V.bcR == OCI_BC_REFLECTING) Yd[J * K2 + mirror_q(i, N)] = v;
+                } else {
+                    const double a = add + o;
+                    V.phi[j * 4 + (i - K2)] = a;
+                    dmax = fmax(dmax, fabs(a - old));
+                    rmax = fmax(rmax, fabs(a));
+                }
+            }
+            ki = 0;
+            ++g;
+        } else {
+            ++ki;
+        }
     }
-    __syncthreads();
-
-    const int64_t b = V.blk[j];
-    const double* __restrict__ M = PASS == PASS_FIX    ? V.xop + (size_t)b * (2 * K2 + 8) * ld
-                                   : PASS == PASS_ITER ? V.rop + (size_t)b * (K2 + 8) * ld
-                                                       : V.fop + (size_t)b * K2 * ld;
-    for (int i0 = warp * ROWS; i0 < rows; i0 += 8 * ROWS) {
-        double acc[ROWS];
-#pragma unroll
-        for (int r = 0; r < ROWS; ++r) acc[r] = 0.0;
-        for (int k = 2 * lane; k < K; k += 64) {
-            const double c0 = in[k], c1 = in[k + 1];
-            double2 mrow[ROWS];
-#pragma unroll
-            for (int r = 0; r < ROWS; ++r)
-                mrow[r] = (i0 + r < rows) ? ldg_stream2(M + (size_t)(i0 + r) * ld + k) : make_double2(0.0, 0.0);
-#pragma unroll
-            for (int r = 0; r < ROWS; ++r) acc[r] = fma(mrow[r].y, c1, fma(mrow[r].x, c0, acc[r]));
+    if (PASS == PASS_ITER) {
+        dmax = warp_max(dmax);
+        rmax = warp_max(rmax);
+        if (lane == 0 && g_end > g_begin) {
+            atomic_max_nonneg(&V.norms[2 * slot + 0], dmax);
+            atomic_max_nonneg(&V.norms[2 * slot + 1], rmax);
         }
-#pragma unroll
-        for (int r = 0; r < ROWS; ++r) {
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) acc[r] += __shfl_xor_sync(0xffffffffu, acc[r], o);
-            if (lane == 0 && i0 + r < rows) out[i0 + r] = acc[r];
-        }
-    }
-    __syncthreads();
-
-    if (PASS == PASS_FIX) {
-        for (int i = tid; i < K2; i += 256) {
-            V.yfix[j * K2 + i] = out[i];
-            V.ifix[j * K2 + i] = out[K2 + i];
-        }
-        if (tid < 4) V.phifix[j * 4 + tid] = out[2 * K2 + tid];
-    } else if (PASS == PASS_ITER) {
-        for (int i = tid; i < K2; i += 256) {
-            const double v = V.yfix[j * K2 + i] + out[i];
-            out[i] = v;
-            Yd[j * K2 + i] = v;
-        }
-        if (warp == 0) {
-            double d = 0.0, r = 0.0;
-            if (lane < 4) {
-                const double a = V.phifix[j * 4 + lane] + out[K2 + lane];
-                const double old = V.phi[j * 4 + lane];
-                V.phi[j * 4 + lane] = a;
-                d = fabs(a - old);
-                r = fabs(a);
-            }
-            d = warp_max(d);
-            r = warp_max(r);
-            if (lane == 0) {
-                atomic_max_nonneg(&V.norms[2 * slot + 0], d);
-                atomic_max_nonneg(&V.norms[2 * slot + 1], r);
-            }
-        }
-        // reflecting ghost rows (reading S4): the mirror image of the edge cell's outgoing flux
-        const bool gl = j == 0 && V.bcL == OCI_BC_REFLECTING, gr = j == J - 1 && V.bcR == OCI_BC_REFLECTING;
-        if (gl || gr) {
-            __syncthreads();
-            for (int q = tid; q < K2; q += 256) {
-                if (gl && q >= N) Yd[-(int64_t)K2 + q] = out[mirror_q(q, N)];
-                if (gr && q < N) Yd[J * K2 + q] = out[mirror_q(q, N)];
-            }
-        }
-    } else {
-        for (int i = tid; i < K2; i += 256) V.z[j * K2 + i] = V.ifix[j * K2 + i] + out[i];
     }
 }
 
 int launch_red_gemv(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
                     cudaStream_t s)
 {
-    const size_t smem = sizeof(double) * (V.n / 2 + 4 + V.n + 4);
-    const unsigned grid = (unsigned)V.J;
-    if (pass == PASS_FIX) oci_red_gemv_kernel<PASS_FIX, 4><<<grid, 256, smem, s>>>(V, ybase, 0, -1, tol, 0, 0);
-    else if (pass == PASS_ITER) oci_red_gemv_kernel<PASS_ITER, 4><<<grid, 256, smem, s>>>(V, ybase, slot, prev_slot, tol, 0, 0);
-    else oci_red_gemv_kernel<PASS_FINAL, 4><<<grid, 256, smem, s>>>(V, ybase, 0, -1, tol, cnt, force);
+    constexpr int GR = 8;
+    const int K2 = V.n / 2;
+    const int rows = pass == PASS_FIX ? 2 * K2 + 4 : pass == PASS_ITER ? K2 + 4 : K2;
+    const int64_t G = V.J * ((rows + GR - 1) / GR);
+    // warps per CTA: 8 unless the private input vectors would not fit in shared memory (huge N)
+    int nwarp = 8;
+    while (nwarp > 1 && (size_t)nwarp * (K2 + 8) * 8 > 100 * 1024) nwarp >>= 1;
+    const size_t smem = sizeof(double) * (size_t)nwarp * (K2 + 8);
+    static bool attr = false;
+    static int sm_count = 148;
+    if (!attr) {
+        cudaFuncSetAttribute(oci_red_gemv_kernel<PASS_FIX, GR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+        cudaFuncSetAttribute(oci_red_gemv_kernel<PASS_ITER, GR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+        cudaFuncSetAttribute(oci_red_gemv_kernel<PASS_FINAL, GR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
+        attr = true;
+    }
+    // one wave: every CTA resident, the stream cut into equal pieces
+    int per_sm = 1;
+    if (pass == PASS_FIX) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, oci_red_gemv_kernel<PASS_FIX, GR>, nwarp * 32, smem);
+    else if (pass == PASS_ITER) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, oci_red_gemv_kernel<PASS_ITER, GR>, nwarp * 32, smem);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, oci_red_gemv_kernel<PASS_FINAL, GR>, nwarp * 32, smem);
+    if (per_sm < 1) per_sm = 1;
+    int64_t ctas = (G + nwarp - 1) / nwarp;                 // at least one row group per warp
+    if (ctas > (int64_t)sm_count * per_sm) ctas = (int64_t)sm_count * per_sm;
+    const unsigned grid = (unsigned)ctas, block = (unsigned)nwarp * 32;
+    if (pass == PASS_FIX) oci_red_gemv_kernel<PASS_FIX, GR><<<grid, block, smem, s>>>(V, ybase, 0, -1, tol, 0, 0);
+    else if (pass == PASS_ITER) oci_red_gemv_kernel<PASS_ITER, GR><<<grid, block, smem, s>>>(V, ybase, slot, prev_slot, tol, 0, 0);
+    else oci_red_gemv_kernel<PASS_FINAL, GR><<<grid, block, smem, s>>>(V, ybase, 0, -1, tol, cnt, force);
     return 1;
 }
 
