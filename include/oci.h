@@ -73,20 +73,26 @@ enum { OCI_KERNEL_GENERIC = 0, OCI_KERNEL_RESIDENT = 1, OCI_KERNEL_KTILED = 2, O
 /* Form of the OCI iteration inside oci_step (oci_set_iteration).  Both produce the iterates of
  * eq. (19), up to rounding order:
  * FULL    - every iteration applies the whole inverse, Psi^(l+1) = B^{-1} c^(l) (the paper's statement);
- * REDUCED - only the 2N RHS rows fed by incident fluxes change within a step (the (l) terms
- *           of eqs. 27,28), so per step: Psi_fix = B^{-1} c_fix once; per iteration the 2N
- *           outgoing rows and the 4 scalar-flux rows, y^(l+1) = yfix + G inc^(l), phi^(l+1) = phifix +
- *           H inc^(l) with G = B^{-1}[O,I] diag|mu| (2N x 2N), H = W B^{-1}[:,I] diag|mu| (4 x 2N); after
- *           the last iteration the other 2N rows from the same inc (F = B^{-1}[I,I] diag|mu|). */
+ * REDUCED - only the 2N RHS rows fed by incident fluxes change within a step (the (l) terms of
+ *           eqs. 27,28), so a step is three kinds of pass over packed state (O = the 2N rows
+ *           of Psi a neighbour reads, I = the other 2N, inc = the gathered neighbour values):
+ *             FIX   once:    [Psi_fix; W Psi_fix] = X [psi_{k-1/2}; Q]         (4N+4) x (2N+4)
+ *             ITER  L times: y^(l+1) = yfix + G inc^(l), phi^(l+1) = phifix + H inc^(l),
+ *                            G = B^{-1}[O,I] diag|mu| (2N x 2N), H = W B^{-1}[:,I] diag|mu| (4 x 2N)
+ *             FINAL once:    Psi^(L)[I] = ifix + F inc^(L-1), F = B^{-1}[I,I] diag|mu| (2N x 2N)
+ *           Every unknown of every cell is still computed every step; the state is kept in the packed
+ *           (O, I) order between steps and interleaved on demand (oci_get_angular_flux, si_step). */
 enum { OCI_ITERATION_FULL = 0, OCI_ITERATION_REDUCED = 1, OCI_ITERATION_AUTO = 2 };
 /* AUTO (the default) = REDUCED wherever a kernel of the reduced form is the faster one for this
  * problem: always on the PER_CELL path, on the SHARED path when a tensor-core kernel of the reduced
  * form serves the block size (or the block is small); FULL otherwise.  oci_get_info reports the
  * resolved form after oci_setup. */
 
-/* Kernel serving the REDUCED iteration: GEMV - batched GEMV, one operator per distinct block (any n);
- * RESIDENT - shared block, n in {64,128}: G, H resident in registers, fp64 tensor pipe;
- * KTILED - shared block, large n: operands streamed in K chunks by tensor-map TMA, fp64 tensor pipe. */
+/* Kernel family serving the REDUCED form (all three passes): GEMV - batched GEMV, one operator per
+ * distinct block (any n; HBM-bound on the PER_CELL path);
+ * RESIDENT - shared block, n in {64,128}: operators resident in shared memory, fp64 tensor pipe;
+ * KTILED - shared block, N a multiple of 64: operands streamed in K chunks by tensor-map TMA, fp64
+ *          tensor pipe. */
 enum { OCI_RKERNEL_GEMV = 0, OCI_RKERNEL_RESIDENT = 1, OCI_RKERNEL_KTILED = 2 };
 
 typedef struct {
@@ -172,9 +178,8 @@ int oci_get_block_inverse(const oci_ctx* ctx, int64_t blk, double* binv);
  * count since the last enable and resets them. */
 int oci_enable_kernel_timing(oci_ctx* ctx, int32_t on);
 int oci_get_kernel_time(oci_ctx* ctx, double* ms, int64_t* launches);
-/* REDUCED iteration only: the per-step Psi_fix pass (full apply + split) and the finalisation kernel,
- * accumulated like oci_get_kernel_time (which then counts the reduced iteration kernel). Any pointer
- * may be NULL. */
+/* REDUCED form only: the per-step FIX pass and FINAL pass, accumulated like oci_get_kernel_time
+ * (which then counts the ITER kernel).  Any pointer may be NULL. */
 int oci_get_aux_kernel_time(oci_ctx* ctx, double* fix_ms, int64_t* fix_launches, double* final_ms,
                             int64_t* final_launches);
 
