@@ -290,3 +290,23 @@ def test_mixing_schemes_and_iteration_forms_on_one_context(cfg, cells):
         assert rel(g.get_angular_flux(), o.angular_flux()) < 1e-12, (k, scheme, it)
         assert rel(g.get_scalar_flux(), o.scalar_flux()) < 1e-12, (k, scheme, it)
     g.close()
+
+
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_full_size_reduced_step_is_deterministic(cfg):
+    """Two runs of the same full-size REDUCED step must agree bit for bit: every reduction in the path is
+    order-fixed (max-norms, per-row dot products), so any difference is a race (this caught a missing
+    cross-proxy fence between LDS reads and the TMA refill of a stage in the K-tiled kernel)."""
+    import paper_2305_13555_b200 as P
+    p = make_problem(cfg)
+    out = []
+    for _ in range(2):
+        g = P.OCI.from_problem(p, iteration=REDUCED)
+        g.set_source(p.source(0))
+        assert g.oci_step(-1.0, 3)[:2] == (1, 3)
+        g.set_source(p.source(1))
+        assert g.oci_step(-1.0, 2)[:2] == (1, 2)
+        out.append((g.get_angular_flux().copy(), g.get_scalar_flux().copy()))
+        g.close()
+    assert np.array_equal(out[0][0], out[1][0])
+    assert np.array_equal(out[0][1], out[1][1])
