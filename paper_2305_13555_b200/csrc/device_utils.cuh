@@ -10,9 +10,19 @@ __device__ __forceinline__ bool step_done(const unsigned long long* __restrict__
                                           double tol)
 {
     if (prev_slot < 0) return false;
-    double d = __longlong_as_double((long long)norms[2 * prev_slot + 0]);
-    double r = __longlong_as_double((long long)norms[2 * prev_slot + 1]);
+    double d = __longlong_as_double((long long)__ldcg(norms + 2 * prev_slot + 0));
+    double r = __longlong_as_double((long long)__ldcg(norms + 2 * prev_slot + 1));
     return converged(tol, d, r);
+}
+
+// FIX pass of the reduced step (first kernel of every oci_step in that form): CTA 0 also clears the norm slots
+// and the grid-barrier counter the iteration launches of this step will use (saves two memsets per step).
+__device__ __forceinline__ void clear_step_state(const DevView& V)
+{
+    if (blockIdx.x == 0) {
+        for (int i = threadIdx.x; i < 2 * kNormSlots; i += blockDim.x) V.norms[i] = 0ull;
+        if (threadIdx.x == 0) V.flags[8] = 0;
+    }
 }
 
 // max over non-negative doubles through their (order-preserving) bit patterns: exact and

@@ -52,6 +52,7 @@ struct oci_ctx {
     bool yz_valid = false;             // ... when this is set (cleared by set_flux, si_step, a FULL-form oci_step)
     bool psi_valid = false;            // psi[cur] holds the current iterate in the full layout (cleared by a REDUCED step)
     int32_t red_kernel = OCI_RKERNEL_GEMV;
+    bool coop = false;                 // device supports cooperative launches
     int32_t predicted[2] = {0, 0};     // last iteration count of oci / si, sizes the launch chunk
     unsigned long long* h_norms = nullptr;   // pinned
     // timing
@@ -288,9 +289,20 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
         int32_t cnt = guess - done_iters;
         if (cnt < 4) cnt = 4;
         if (cnt > kNormSlots) cnt = kNormSlots;
+        if (red && ctx->red_kernel == OCI_RKERNEL_RESIDENT && ctx->coop) cnt = kNormSlots;   // the fused loop stops itself
         if (cnt > max_iters - done_iters) cnt = max_iters - done_iters;
-        CK(cudaMemsetAsync(V.norms, 0, sizeof(unsigned long long) * 2 * cnt, s));
-        for (int32_t i = 0; i < cnt; ++i) {
+        // (the FIX pass has already cleared the norm slots and the barrier counter for the first chunk)
+        if (!(red && done_iters == 0)) CK(cudaMemsetAsync(V.norms, 0, sizeof(unsigned long long) * 2 * cnt, s));
+        // the resident kernels of the reduced form run the whole chunk of iterations in ONE cooperative launch
+        // (grid-wide barrier + device-side stop between iterations): no launch gap, operator staged once
+        const bool fused_loop = red && ctx->red_kernel == OCI_RKERNEL_RESIDENT && ctx->coop && cnt > 1;
+        if (fused_loop) {
+            if (done_iters > 0) CK(cudaMemsetAsync(V.flags + 8, 0, 4, s));  // the grid barrier's arrival counter
+            if (timed) CK(cudaEventRecord(ctx->ev[0], s));
+            ctx->launches += launch_reduced_pass(ctx, PASS_ITER, (ctx->ycur + done_iters) & 1, 0, -1, tol, cnt, 0);
+            if (timed) CK(cudaEventRecord(ctx->ev[1], s));
+        }
+        for (int32_t i = 0; i < cnt && !fused_loop; ++i) {
             if (timed) CK(cudaEventRecord(ctx->ev[2 * i], s));
             if (si) ctx->launches += launch_si_iteration(V, ctx->cur, i, i - 1, tol, s);
             else if (red) ctx->launches += launch_reduced_pass(ctx, PASS_ITER, (ctx->ycur + done_iters + i) & 1, i, i - 1, tol, 0, 0);
@@ -313,8 +325,14 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
             std::memcpy(&r, &ctx->h_norms[2 * i + 1], 8);
             if (converged(tol, d, r)) { conv = true; executed = i + 1; break; }
         }
+        if (timed && fused_loop) {
+            float ms = 0.f;
+            CK(cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]));
+            ctx->kernel_ms += ms;                                           // one launch = `executed` iterations
+            ctx->kernel_launches += executed;
+        }
         if (timed) {
-            for (int32_t i = 0; i < executed; ++i) {
+            for (int32_t i = 0; i < executed && !fused_loop; ++i) {
                 float ms = 0.f;
                 CK(cudaEventElapsedTime(&ms, ctx->ev[2 * i], ctx->ev[2 * i + 1]));
                 ctx->kernel_ms += ms;
@@ -479,6 +497,12 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     ctx->red_kernel = (oci_red_resident_supported(V) && oci_red_resident_prepare(V, &ctx->rrmaps)) ? OCI_RKERNEL_RESIDENT
                       : (oci_red_ktiled_supported(V) && oci_red_ktiled_prepare(V, &ctx->rmaps)) ? OCI_RKERNEL_KTILED
                                                                                                  : OCI_RKERNEL_GEMV;
+    {
+        int dev = 0, coop = 0;
+        CK(cudaGetDevice(&dev));
+        CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+        ctx->coop = coop != 0;
+    }
     ctx->cur = 0;
     ctx->ycur = 0;
     ctx->yz_valid = false;

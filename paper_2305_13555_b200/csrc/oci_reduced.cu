@@ -221,6 +221,7 @@ __global__ void __launch_bounds__(256, 2) oci_red_gemv_kernel(DevView V, int yba
         }
         ysrc = (ybase + L - 1) & 1;
     }
+    if (PASS == PASS_FIX) clear_step_state(V);
     const int n = V.n, N = V.N, K2 = n >> 1, N2 = N >> 1;
     const int K = PASS == PASS_FIX ? K2 + 4 : K2;                       // operator columns used
     const int ld = PASS == PASS_FIX ? K2 + 16 : K2;                     // operator row stride

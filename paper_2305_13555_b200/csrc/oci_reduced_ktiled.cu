@@ -101,6 +101,7 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
         ysrc = (ybase + L - 1) & 1;
     }
     const CUtensorMap* my = (ysrc == ybase) ? &map_y : &map_y_alt;
+    if (PASS == PASS_FIX) clear_step_state(V);
 
     extern __shared__ unsigned char smem_raw[];
     // aligned up inside the shared window (pointer arithmetic on the array keeps the LDS/STS address space)

@@ -213,7 +213,10 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
         }
         ysrc = (ybase + L - 1) & 1;
     }
-    const CUtensorMap* my = (ysrc == ybase) ? &map_a : &map_a_alt;
+    // ITER: `cnt` iterations run inside this one (cooperative) launch, separated by a grid-wide barrier; iteration l
+    // reads y[(ybase + l) & 1], reports its norms in slot `slot + l`, and the loop ends at the first converged one
+    const int nloop = PASS == PASS_ITER ? (cnt > 1 ? cnt : 1) : 1;
+    if (PASS == PASS_FIX) clear_step_state(V);
 
     extern __shared__ unsigned char smem_raw[];
     // aligned up inside the shared window (pointer arithmetic on the array keeps the LDS/STS address space)
@@ -227,7 +230,6 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g4 = lane >> 2, t4 = lane & 3;
     const int64_t J = V.J;
-    double* __restrict__ Yd = V.y[ysrc ^ 1];
 
     const int64_t ntiles = (J + RT_M - 1) / RT_M;
     const int64_t wid = (int64_t)blockIdx.x * RT_WARPS + warp, nw = (int64_t)gridDim.x * RT_WARPS;
@@ -255,9 +257,11 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
     }
 
     // one lane requests a tile: tensor-map boxes straight into the warp's private ring
+    const CUtensorMap* my = nullptr;     // tensor map of this iteration's source y
+    int tc0 = 0;                         // tiles this warp has consumed in earlier iterations (ring position)
     auto prefetch = [&](int it) {
         if (lane == 0) {
-            const int s = it & 1;
+            const int s = (tc0 + it) & 1;
             const int j0 = (int)((wid + (int64_t)it * nw) * RT_M);
             unsigned char* st = my_ring + (size_t)s * C::STAGE_BYTES;
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -272,28 +276,19 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
         }
         __syncwarp();
     };
-    if (my_tiles > 0) prefetch(0);
 
     EpiCtx E;
     E.fixp = PASS == PASS_FINAL ? V.ifix : V.yfix;
-    E.out = PASS == PASS_ITER ? Yd : PASS == PASS_FINAL ? V.z : V.yfix;
+    E.out = PASS == PASS_FINAL ? V.z : V.yfix;          // ITER: set per iteration
     E.phifix = V.phifix;
     E.phi = V.phi;
     E.phifix_out = V.phifix;
     EpiCtx E1 = E;                 // FIX: the pending I rows go to ifix
     E1.out = V.ifix;
 
-    double dmax = 0.0, rmax = 0.0;
+    double* Yd = nullptr;
     const double* brow = op_s + g4 * C::LD + t4;
     constexpr int NBP = PASS == PASS_FIX ? C::NB1 : C::NB0;      // blocks of the epilogue carried from tile to tile
-    double pend[2][NBP][2];
-#pragma unroll
-    for (int g = 0; g < 2; ++g)
-#pragma unroll
-        for (int t = 0; t < NBP; ++t) pend[g][t][0] = pend[g][t][1] = 0.0;
-    int64_t pj0 = my_tiles > 0 ? wid * RT_M : 0;
-    int prows = 0;                                                 // nothing pending yet: loads clamped, stores off
-
     mbar_wait(op_bar, 0);
 
     // reflecting ghost rows of y (reading S4) by the warp that owns the edge cell, once its stores are out
@@ -313,8 +308,24 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
         }
     };
 
+  for (int l = 0; l < nloop; ++l) {
+    const int ysrc_l = PASS == PASS_ITER ? (ybase + l) & 1 : ysrc;
+    my = (ysrc_l == ybase) ? &map_a : &map_a_alt;
+    Yd = V.y[ysrc_l ^ 1];
+    if (PASS == PASS_ITER) E.out = Yd;
+    tc0 = l * my_tiles;
+    if (my_tiles > 0) prefetch(0);
+    double dmax = 0.0, rmax = 0.0;
+    double pend[2][NBP][2];
+#pragma unroll
+    for (int g = 0; g < 2; ++g)
+#pragma unroll
+        for (int t = 0; t < NBP; ++t) pend[g][t][0] = pend[g][t][1] = 0.0;
+    int64_t pj0 = my_tiles > 0 ? wid * RT_M : 0;
+    int prows = 0;                                                 // nothing pending yet: loads clamped, stores off
+
     for (int it = 0; it < my_tiles; ++it) {
-        const int s = it & 1;
+        const int s = (tc0 + it) & 1;
         const int64_t j0 = (wid + (int64_t)it * nw) * RT_M;
         const int rows = (int)((J - j0 < RT_M) ? (J - j0) : RT_M);
         if (it + 1 < my_tiles) prefetch(it + 1);
@@ -337,7 +348,7 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
 #pragma unroll
             for (int t = 0; t < C::NB0; ++t) acc[g][t][0] = acc[g][t][1] = 0.0;
 
-        mbar_wait(&my_full[s], (it >> 1) & 1);
+        mbar_wait(&my_full[s], ((tc0 + it) >> 1) & 1);
         const double* st = reinterpret_cast<const double*>(my_ring + (size_t)s * C::STAGE_BYTES);
         if (PASS == PASS_FIX) {
             const double* pa = st + g4 * C::LDH + t4;
@@ -382,10 +393,30 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
         dmax = warp_max(dmax);
         rmax = warp_max(rmax);
         if (lane == 0 && my_tiles > 0) {
-            atomic_max_nonneg(&V.norms[2 * slot + 0], dmax);
-            atomic_max_nonneg(&V.norms[2 * slot + 1], rmax);
+            atomic_max_nonneg(&V.norms[2 * (slot + l) + 0], dmax);
+            atomic_max_nonneg(&V.norms[2 * (slot + l) + 1], rmax);
+        }
+        if (nloop > 1) {
+            // ---- grid-wide barrier (cooperative launch: all CTAs are resident), then the stopping rule (a7)
+            // on the now final norms of this iteration: every CTA takes the same decision
+            __threadfence();
+            __syncthreads();
+            if (tid == 0) {
+                unsigned int* bar = reinterpret_cast<unsigned int*>(V.flags) + 8;
+                atomicAdd(bar, 1u);
+                const unsigned int target = (unsigned int)(l + 1) * gridDim.x;
+                unsigned int seen;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(bar) : "memory");
+                } while (seen < target);
+                // the y rows other CTAs have just stored are read next through the async proxy (TMA)
+                asm volatile("fence.proxy.async;" ::: "memory");
+            }
+            __syncthreads();
+            if (step_done(V.norms, slot + l, tol)) break;
         }
     }
+  }
 }
 
 bool oci_red_resident_supported(const DevView& V) { return V.nblk == 1 && (V.n == 128 || V.n == 64) && V.J + 18 < (int64_t)1 << 31; }
@@ -429,6 +460,15 @@ void launch_rr(const DevView& V, const RedResidentMaps& M, int ybase, int slot, 
     const CUtensorMap& ya = PASS == PASS_FIX ? M.y_half[b] : M.y_rows[b];
     const CUtensorMap& yb = PASS == PASS_FIX ? M.y_half[b ^ 1] : M.y_rows[b ^ 1];
     const CUtensorMap& op = PASS == PASS_FIX ? M.xop_rows : PASS == PASS_ITER ? M.rop : M.fop;
+    if (PASS == PASS_ITER && cnt > 1) {
+        // `cnt` iterations in one launch with a grid-wide barrier between them: every CTA must be resident
+        DevView Vv = V;
+        CUtensorMap a0 = ya, a1 = yb, a2 = M.z_half, a3 = M.q, a4 = op, a5 = M.xop_phi;
+        void* args[] = {&Vv, &a0, &a1, &a2, &a3, &a4, &a5, &ybase, &slot, &prev_slot, &tol, &cnt, &force};
+        cudaLaunchCooperativeKernel((const void*)oci_red_resident_kernel<K2, PASS>, dim3(grid), dim3(RT_WARPS * 32), args,
+                                    RCfg<K2, PASS>::SMEM, s);
+        return;
+    }
     oci_red_resident_kernel<K2, PASS><<<grid, RT_WARPS * 32, RCfg<K2, PASS>::SMEM, s>>>(V, ya, yb, M.z_half, M.q, op, M.xop_phi, ybase,
                                                                                         slot, prev_slot, tol, cnt, force);
 }
@@ -438,7 +478,7 @@ void launch_rr_pass(const DevView& V, const RedResidentMaps& M, int pass, int yb
                     int force, cudaStream_t s)
 {
     if (pass == PASS_FIX) launch_rr<K2, PASS_FIX>(V, M, ybase, 0, -1, tol, 0, 0, s);
-    else if (pass == PASS_ITER) launch_rr<K2, PASS_ITER>(V, M, ybase, slot, prev_slot, tol, 0, 0, s);
+    else if (pass == PASS_ITER) launch_rr<K2, PASS_ITER>(V, M, ybase, slot, prev_slot, tol, cnt, 0, s);   // cnt > 1: in-kernel loop
     else launch_rr<K2, PASS_FINAL>(V, M, ybase, 0, -1, tol, cnt, force, s);
 }
 }  // namespace
