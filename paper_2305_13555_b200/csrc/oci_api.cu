@@ -289,13 +289,13 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
         int32_t cnt = guess - done_iters;
         if (cnt < 4) cnt = 4;
         if (cnt > kNormSlots) cnt = kNormSlots;
-        if (red && ctx->red_kernel == OCI_RKERNEL_RESIDENT && ctx->coop) cnt = kNormSlots;   // the fused loop stops itself
+        if (red && ctx->red_kernel != OCI_RKERNEL_KTILED && ctx->coop) cnt = kNormSlots;   // the fused loop stops itself
         if (cnt > max_iters - done_iters) cnt = max_iters - done_iters;
         // (the FIX pass has already cleared the norm slots and the barrier counter for the first chunk)
         if (!(red && done_iters == 0)) CK(cudaMemsetAsync(V.norms, 0, sizeof(unsigned long long) * 2 * cnt, s));
-        // the resident kernels of the reduced form run the whole chunk of iterations in ONE cooperative launch
+        // the resident and GEMV kernels of the reduced form run the whole chunk of iterations in ONE cooperative launch
         // (grid-wide barrier + device-side stop between iterations): no launch gap, operator staged once
-        const bool fused_loop = red && ctx->red_kernel == OCI_RKERNEL_RESIDENT && ctx->coop && cnt > 1;
+        const bool fused_loop = red && ctx->red_kernel != OCI_RKERNEL_KTILED && ctx->coop && cnt > 1;
         if (fused_loop) {
             if (done_iters > 0) CK(cudaMemsetAsync(V.flags + 8, 0, 4, s));  // the grid barrier's arrival counter
             if (timed) CK(cudaEventRecord(ctx->ev[0], s));

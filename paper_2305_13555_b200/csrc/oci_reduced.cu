@@ -231,10 +231,11 @@ __global__ void __launch_bounds__(256, 2) oci_red_gemv_kernel(DevView V, int yba
     const int64_t wid = (int64_t)blockIdx.x * nwarp + warp, nw = (int64_t)gridDim.x * nwarp;
     const int64_t g_begin = G * wid / nw, g_end = G * (wid + 1) / nw;
     double* in = sm + (size_t)warp * (K2 + 8);                          // this warp's input vector [K] (+ zero pad)
-    const double* __restrict__ Ys = V.y[ysrc];
-    double* __restrict__ Yd = V.y[ysrc ^ 1];
-    double dmax = 0.0, rmax = 0.0;
-    int64_t jcur = -1;
+    // ITER: `cnt` > 1 iterations run inside this one (cooperative) launch, separated by a grid-wide barrier;
+    // iteration l reads y[(ybase + l) & 1] (through L2: other SMs wrote it) and reports its norms in slot + l
+    const int nloop = PASS == PASS_ITER ? (cnt > 1 ? cnt : 1) : 1;
+    const double* Ys = V.y[ysrc];
+    double* Yd = V.y[ysrc ^ 1];
 
     // The (row group, 64-column slice) steps of this warp form one flat sequence; the 16-byte loads of step
     // s+1 are issued before step s is consumed, so a warp always has GR x 512 B of its stream in flight.
@@ -264,6 +265,13 @@ __global__ void __launch_bounds__(256, 2) oci_red_gemv_kernel(DevView V, int yba
     double add = 0.0, old = 0.0;
     double2 qc0 = make_double2(0.0, 0.0), qc1 = make_double2(0.0, 0.0);
     if (S > 0) load_step(nxt, g_begin, 0);
+  for (int l = 0; l < nloop; ++l) {
+    if (PASS == PASS_ITER) {
+        Ys = V.y[(ybase + l) & 1];
+        Yd = V.y[(ybase + l + 1) & 1];
+    }
+    double dmax = 0.0, rmax = 0.0;
+    int64_t jcur = -1;
     int64_t g = g_begin;
     int ki = 0;
     for (int64_t st = 0; st < S; ++st) {
@@ -284,9 +292,9 @@ __global__ void __launch_bounds__(256, 2) oci_red_gemv_kernel(DevView V, int yba
                 __syncwarp();
                 if (PASS == PASS_FIX) {
                     for (int u = lane; u < K; u += 32)
-                        in[u] = u < N ? Ys[j * K2 + N2 + u] : u < K2 ? V.z[j * K2 + N2 + (u - N)] : V.Q[j * 4 + (u - K2)];
+                        in[u] = u < N ? __ldcg(Ys + j * K2 + N2 + u) : u < K2 ? V.z[j * K2 + N2 + (u - N)] : V.Q[j * 4 + (u - K2)];
                 } else {
-                    for (int q = lane; q < K2; q += 32) in[q] = Ys[(q < N ? j + 1 : j - 1) * K2 + q];
+                    for (int q = lane; q < K2; q += 32) in[q] = __ldcg(Ys + (q < N ? j + 1 : j - 1) * K2 + q);
                 }
                 if (lane < 4) in[K + lane] = 0.0;       // columns past K read as zero (the operator loads are zero there)
                 __syncwarp();
@@ -305,7 +313,7 @@ __global__ void __launch_bounds__(256, 2) oci_red_gemv_kernel(DevView V, int yba
                 if (PASS == PASS_FINAL) add = V.ifix[j * K2 + i];
                 if (PASS == PASS_ITER) {
                     if (i < K2) add = V.yfix[j * K2 + i];
-                    else { add = V.phifix[j * 4 + (i - K2)]; old = V.phi[j * 4 + (i - K2)]; }
+                    else { add = V.phifix[j * 4 + (i - K2)]; old = __ldcg(V.phi + j * 4 + (i - K2)); }
                 }
             }
         }
@@ -354,10 +362,29 @@ __global__ void __launch_bounds__(256, 2) oci_red_gemv_kernel(DevView V, int yba
         dmax = warp_max(dmax);
         rmax = warp_max(rmax);
         if (lane == 0 && g_end > g_begin) {
-            atomic_max_nonneg(&V.norms[2 * slot + 0], dmax);
-            atomic_max_nonneg(&V.norms[2 * slot + 1], rmax);
+            atomic_max_nonneg(&V.norms[2 * (slot + l) + 0], dmax);
+            atomic_max_nonneg(&V.norms[2 * (slot + l) + 1], rmax);
+        }
+        if (nloop > 1) {
+            // the operator does not depend on the iterate: the first step of the next iteration is requested
+            // before the grid-wide barrier, so HBM stays busy across it
+            if (l + 1 < nloop && S > 0) load_step(nxt, g_begin, 0);
+            __threadfence();
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                unsigned int* bar = reinterpret_cast<unsigned int*>(V.flags) + 8;
+                atomicAdd(bar, 1u);
+                const unsigned int target = (unsigned int)(l + 1) * gridDim.x;
+                unsigned int seen;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(bar) : "memory");
+                } while (seen < target);
+            }
+            __syncthreads();
+            if (step_done(V.norms, slot + l, tol)) break;      // a7: every CTA takes the same decision
         }
     }
+  }
 }
 
 int launch_red_gemv(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
@@ -392,7 +419,13 @@ int launch_red_gemv(const DevView& V, int pass, int ybase, int slot, int prev_sl
     if (ctas > (int64_t)sm_count * per_sm) ctas = (int64_t)sm_count * per_sm;
     const unsigned grid = (unsigned)ctas, block = (unsigned)nwarp * 32;
     if (pass == PASS_FIX) oci_red_gemv_kernel<PASS_FIX, GR><<<grid, block, smem, s>>>(V, ybase, 0, -1, tol, 0, 0);
-    else if (pass == PASS_ITER) oci_red_gemv_kernel<PASS_ITER, GR><<<grid, block, smem, s>>>(V, ybase, slot, prev_slot, tol, 0, 0);
+    else if (pass == PASS_ITER && cnt > 1) {
+        // `cnt` iterations in one launch with a grid-wide barrier between them: the grid is one resident wave
+        DevView Vv = V;
+        int zero = 0;
+        void* args[] = {&Vv, &ybase, &slot, &prev_slot, &tol, &cnt, &zero};
+        cudaLaunchCooperativeKernel((const void*)oci_red_gemv_kernel<PASS_ITER, GR>, dim3(grid), dim3(block), args, smem, s);
+    } else if (pass == PASS_ITER) oci_red_gemv_kernel<PASS_ITER, GR><<<grid, block, smem, s>>>(V, ybase, slot, prev_slot, tol, 0, 0);
     else oci_red_gemv_kernel<PASS_FINAL, GR><<<grid, block, smem, s>>>(V, ybase, 0, -1, tol, cnt, force);
     return 1;
 }

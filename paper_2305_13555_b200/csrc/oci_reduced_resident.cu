@@ -159,7 +159,7 @@ __device__ __forceinline__ void phase(double (&acc)[2][NBC][2], const double* __
 #pragma unroll
             for (int g = 0; g < 2; ++g) {
                 pf[g] = *reinterpret_cast<const double2*>(E.phifix + pj[g] * 4 + 2 * (t4 & 1));
-                po[g] = *reinterpret_cast<const double2*>(E.phi + pj[g] * 4 + 2 * (t4 & 1));
+                po[g] = __ldcg(reinterpret_cast<const double2*>(E.phi + pj[g] * 4 + 2 * (t4 & 1)));   // rewritten every iteration: L2
             }
         }
         // ---- pending epilogue: slice ks - DIST is added and stored
