@@ -38,7 +38,7 @@ constexpr int RK_A_BYTES = RK_M * RK_K * 8;   // 8 KB
 constexpr int RK_B_BYTES = RK_N * RK_K * 8;   // 16 KB
 constexpr int RK_P_BYTES = 8 * RK_K * 8;      // 1 KB: the scalar-flux rows (4 used)
 constexpr int RK_STAGE_BYTES = RK_A_BYTES + RK_B_BYTES + RK_P_BYTES + 1024;   // keeps every stage 2 KB-aligned
-constexpr size_t RK_SMEM = 1024 /*alignment slack*/ + (size_t)RK_STAGES * RK_STAGE_BYTES + 4 * RK_M * 4 * 8 /*phi_s*/ +
+constexpr size_t RK_SMEM = 1024 /*alignment slack*/ + (size_t)RK_STAGES * RK_STAGE_BYTES + 2 * 4 * RK_M * 4 * 8 /*phi_s, 2 buffers*/ +
                            2 * RK_STAGES * 8 + 64;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -107,8 +107,8 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
     // aligned up inside the shared window (pointer arithmetic on the array keeps the LDS/STS address space)
     unsigned char* base = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     unsigned char* stages = base;                                                    // [S][A 8K | B 16K | P 1K | pad]
-    double* phi_s = reinterpret_cast<double*>(base + (size_t)RK_STAGES * RK_STAGE_BYTES);   // [4 wn][64][4]
-    uint64_t* full = reinterpret_cast<uint64_t*>(phi_s + 4 * RK_M * 4);
+    double* phi_s2 = reinterpret_cast<double*>(base + (size_t)RK_STAGES * RK_STAGE_BYTES);  // [2][4 wn][64][4]
+    uint64_t* full = reinterpret_cast<uint64_t*>(phi_s2 + 2 * 4 * RK_M * 4);
     uint64_t* empty = full + RK_STAGES;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -214,6 +214,17 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
             }
         }
 
+        // scalar flux of this item's cells: thread tid will finish (cell tid/4, slot tid%4); its operands are
+        // requested now so that the epilogue has no dependent global load behind its barrier
+        double pfix = 0.0, pold = 0.0;
+        if (with_phi && PASS == PASS_ITER) {
+            int64_t j = j0 + (tid >> 2);
+            if (j >= J) j = J - 1;
+            pfix = V.phifix[j * 4 + (tid & 3)];
+            pold = V.phi[j * 4 + (tid & 3)];
+        }
+        double* phi_s = phi_s2 + (it & 1) * (4 * RK_M * 4);    // alternating buffers: one barrier per item
+
         double acc[4][4][2], accp[4][2];
 #pragma unroll
         for (int g = 0; g < 4; ++g) {
@@ -283,25 +294,21 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
                 phi_s[(wn * RK_M + r) * 4 + 2 * t4 + 1] = accp[g][1];
             }
         }
-        if (PASS != PASS_FINAL) {
+        if (with_phi) {                                              // uniform over the CTA
             named_bar_sync(1, 256);
-            if (with_phi) {
-                // thread tid owns (cell tid/4, slot tid%4) of the item
-                const int64_t j = j0 + (tid >> 2);
-                const double ssum = phi_s[0 * RK_M * 4 + tid] + phi_s[1 * RK_M * 4 + tid] + phi_s[2 * RK_M * 4 + tid] + phi_s[3 * RK_M * 4 + tid];
-                if (j < J) {
-                    if (PASS == PASS_FIX) {
-                        V.phifix[j * 4 + (tid & 3)] = ssum;
-                    } else {
-                        const double a = V.phifix[j * 4 + (tid & 3)] + ssum;
-                        const double old = V.phi[j * 4 + (tid & 3)];
-                        V.phi[j * 4 + (tid & 3)] = a;
-                        dmax = fmax(dmax, fabs(a - old));
-                        rmax = fmax(rmax, fabs(a));
-                    }
+            // thread tid owns (cell tid/4, slot tid%4) of the item
+            const int64_t j = j0 + (tid >> 2);
+            const double ssum = phi_s[0 * RK_M * 4 + tid] + phi_s[1 * RK_M * 4 + tid] + phi_s[2 * RK_M * 4 + tid] + phi_s[3 * RK_M * 4 + tid];
+            if (j < J) {
+                if (PASS == PASS_FIX) {
+                    V.phifix[j * 4 + (tid & 3)] = ssum;
+                } else {
+                    const double a = pfix + ssum;
+                    V.phi[j * 4 + (tid & 3)] = a;
+                    dmax = fmax(dmax, fabs(a - pold));
+                    rmax = fmax(rmax, fabs(a));
                 }
             }
-            named_bar_sync(1, 256);                                  // phi_s reusable
         }
     }
     if (PASS == PASS_ITER) {
