@@ -310,3 +310,26 @@ def test_full_size_reduced_step_is_deterministic(cfg):
         g.close()
     assert np.array_equal(out[0][0], out[1][0])
     assert np.array_equal(out[0][1], out[1][1])
+
+
+@pytest.mark.parametrize("N", [16, 32])
+def test_resident_fused_loop_many_iterations(N):
+    """The resident kernels run a whole chunk of up to 64 iterations in one cooperative launch (grid barrier and
+    device-side stop between iterations).  A problem that needs several chunks (thin cells, c = 0.999, long time
+    step, mirrors on both sides) exercises the re-arming of the barrier counter and of the norm slots."""
+    import paper_2305_13555_b200 as P
+    from oracle import Oracle
+    q = _custom(150, N, (REF, 0.0), (REF, 0.0), seed=11 + N, hetero=False, dt=50.0)
+    q.sigma_s[:] = q.sigma_t * 0.999
+    g, o = P.OCI.from_problem(q, iteration=REDUCED), Oracle.from_problem(q, threads=8)
+    assert g.get_info()["reduced_kernel"] == P.RKERNEL_RESIDENT
+    for x in (g, o):
+        x.set_source(q.source(0))
+    a, b = g.oci_step(1e-10, 100_000), o.oci_step(1e-10, 100_000)
+    assert a[0] == b[0] == 0 and abs(a[1] - b[1]) <= 1 and a[1] > 128, (a, b)
+    assert rel(g.get_scalar_flux(), o.scalar_flux()) < 1e-8
+    # and an exact count that ends in the middle of the second chunk
+    g.set_flux(q.psi0); o.set_flux(q.psi0)
+    assert g.oci_step(-1.0, 77)[:2] == (1, 77) == o.oci_step(-1.0, 77)[:2]
+    assert rel(g.get_angular_flux(), o.angular_flux()) < 1e-12
+    g.close()
