@@ -41,9 +41,10 @@ UNIT = "unknown-updates/s"
 NCU_TRAFFIC_BYTES = {(3, False): 374.17e6,    # profiles/r1_resident_cfg3_full.txt: 272.80 MB read + 101.37 MB written
                      (4, False): 178.67e6,    # profiles/r1_ktiled_cfg4_full.txt:   136.89 MB read +  41.78 MB written
                      (5, False): 2168.2e6,    # profiles/r1_percell_cfg5_full.txt:  2164.5 MB read +   3.8 MB written
-                     (3, True): 179.9e6,      # profiles/r1c_reduced_cfg3_full.txt: 143.2 MB read + 36.7 MB written (y stays partly in L2)
-                     (4, True): 75.5e6,       # profiles/r1c_reduced_cfg4_full.txt:  68.7 MB read +  6.8 MB written (y buffers fit in L2)
-                     (5, True): 567.5e6}      # profiles/r1c_reduced_cfg5_full.txt: 562.4 MB read +  5.1 MB written
+                     # reduced form, per ITERATION (resident and GEMV ITER launches run all iterations of a step: bytes / iterations)
+                     (3, True): 206.2e6,      # profiles/r1d_reduced_cfg3_full.txt: (846.0 MB read + 391.4 MB written) / 6 iterations
+                     (4, True): 75.6e6,       # profiles/r1d_reduced_cfg4_full.txt:  68.7 MB read +  6.9 MB written (y buffers fit in L2)
+                     (5, True): 558.6e6}      # profiles/r1d_reduced_cfg5_full.txt: (4447.6 MB read + 21.0 MB written) / 8 iterations
 
 
 def load_peaks():
