@@ -186,7 +186,9 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
     for (int ks = 0; ks < 4; ++ks) foff[ks] = (((ks + 4 * (t4 >> 1)) ^ g4) << 4) + ((t4 & 1) << 3);
     const int a_row = (wm * 32 + g4) * 128;              // + g*1024
     const int b_row = (wn * 32 + g4) * 128;              // + t*1024
-    const int p_off = g4 * 128 + foff[wn];               // scalar-flux block: this warp's k-step is ks = wn
+    // scalar-flux block: this warp's k-step is ks = wn (computed, not foff[wn]: a runtime index would push the
+    // whole foff array into local memory and put a local load in front of every fragment load)
+    const int p_off = g4 * 128 + (((wn + 4 * (t4 >> 1)) ^ g4) << 4) + ((t4 & 1) << 3);
 
     double* __restrict__ Yd = V.y[ysrc ^ 1];
     double dmax = 0.0, rmax = 0.0;
