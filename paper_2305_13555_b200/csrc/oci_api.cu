@@ -129,7 +129,7 @@ void gauss_legendre(int N, std::vector<double>& mu, std::vector<double>& w)
 
 struct Layout {
     int64_t binv, psi0, psi1, cfix, phi, Q, qs, dx, sig, sigs, blk, rep, mu, w, coef, ainv4, si_scan, phi_part, norms, tickets, flags,
-        xop, rop, fop, y0, y1, z, yfix, ifix, phifix, q16, total;
+        xop, rop, fop, y0, y1, z, yfix, ifix, phifix, q16, gitems, total;
 };
 
 int64_t align_up(int64_t x) { return (x + 255) & ~int64_t(255); }
@@ -175,7 +175,10 @@ Layout make_layout(int64_t J, int32_t N, int64_t nblk)
         L.yfix = take(J * K2 * 8);
         L.ifix = take(J * K2 * 8);
         L.phifix = take(J * 4 * 8);
-        L.q16 = take(nblk == 1 && N % 64 == 0 ? J * 16 * 8 : 0);
+        const bool grouped = nblk > 1 && nblk <= kMaxGroupedBlocks && N % 64 == 0;
+        L.q16 = take((nblk == 1 || grouped) && N % 64 == 0 ? J * 16 * 8 : 0);
+        // (cell tile, block) groups of the K-tiled kernels: at most min(nblk, 64) per tile of 64 cells
+        L.gitems = take(grouped ? ((J + 63) / 64) * (nblk < 64 ? nblk : 64) * 16 : 0);
     }
     L.total = o;
     return L;
@@ -449,6 +452,8 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     V.ifix = (double*)(base + L.ifix);
     V.phifix = (double*)(base + L.phifix);
     V.q16 = (double*)(base + L.q16);
+    V.gitems = nullptr;
+    V.ngroups = 0;
     V.v = ctx->v; V.dt = ctx->dt;
     V.bcL = ctx->bcL.kind; V.bcR = ctx->bcR.kind;
     V.bcLv = ctx->bcL.value; V.bcRv = ctx->bcR.value;
@@ -474,6 +479,32 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     CK(cudaMemcpyAsync(V.w, ctx->w.data(), ctx->N * 8, cudaMemcpyHostToDevice, s));
     CK(cudaMemcpyAsync(V.coef, coef.data(), n * 8, cudaMemcpyHostToDevice, s));
     CK(cudaStreamSynchronize(s));   // host vectors above are read by the async copies
+
+    if (ctx->nblk > 1 && ctx->nblk <= kMaxGroupedBlocks && ctx->N % 64 == 0) {
+        // row f2: list, tile by tile, the blocks present and which of the tile's 64 cells have each
+        std::vector<int32_t> items;
+        const int64_t nct = (ctx->J + 63) / 64;
+        for (int64_t ct = 0; ct < nct; ++ct) {
+            const int64_t j0 = ct * 64, j1 = j0 + 64 < ctx->J ? j0 + 64 : ctx->J;
+            for (int64_t ja = j0; ja < j1; ++ja) {
+                const int32_t b = ctx->blk[ja];
+                bool first = true;
+                for (int64_t jb = j0; jb < ja; ++jb) first = first && ctx->blk[jb] != b;
+                if (!first) continue;
+                uint64_t mask = 0;
+                for (int64_t jb = ja; jb < j1; ++jb)
+                    if (ctx->blk[jb] == b) mask |= 1ull << (jb - j0);
+                items.push_back((int32_t)ct);
+                items.push_back(b);
+                items.push_back((int32_t)(uint32_t)(mask & 0xffffffffull));
+                items.push_back((int32_t)(uint32_t)(mask >> 32));
+            }
+        }
+        V.gitems = (int32_t*)(base + L.gitems);
+        V.ngroups = (int64_t)items.size() / 4;
+        CK(cudaMemcpyAsync(V.gitems, items.data(), items.size() * 4, cudaMemcpyHostToDevice, s));
+        CK(cudaStreamSynchronize(s));
+    }
 
     ctx->launches += launch_form_and_invert(V, s);                       // a0, a1
     ctx->launches += launch_pack_operators(V, s);                        // f1: G, H, F

@@ -10,7 +10,8 @@
 namespace oci {
 
 constexpr int kNormSlots = 64;  // iterations launched between two host read-backs, at most
-constexpr int kScratchSlot = kNormSlots;   // norm slot nobody reads (the Psi_fix pass of the reduced iteration)
+constexpr int kScratchSlot = kNormSlots;
+constexpr int kMaxGroupedBlocks = 16;      // "a handful of materials": operators stay L2-resident, tensor-core path (row f2)   // norm slot nobody reads (the Psi_fix pass of the reduced iteration)
 
 // Device-side view of one problem.  Passed to kernels by value.
 // Psi buffers have one ghost row before row 0 and one after row J-1: psi[b]
@@ -52,6 +53,9 @@ struct DevView {
     double* ifix;               // [J][K2]  I rows of Psi_fix
     double* phifix;             // [J][4]   W Psi_fix
     double* q16;                // [J][16]  Q padded to one 128-byte row (K-tiled FIX pass only; else unused)
+    int32_t* gitems;            // [ngroups][4] = (cell tile, block, mask lo, mask hi): a handful of materials on the K-tiled
+                                // kernels (row f2); nullptr when all cells share one block (or have one each)
+    int64_t ngroups;
     double v, dt;
     int32_t bcL, bcR;
     double bcLv, bcRv;

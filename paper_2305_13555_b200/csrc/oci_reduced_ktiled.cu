@@ -21,7 +21,11 @@
 //     as one more 8-row operator box; MMA warp (wm, wn) takes their k-step ks = wn of every chunk (one
 //     extra DMMA per four), the four partial sums meet in shared memory in the epilogue;
 //   * epilogue from registers: + yfix / ifix (requested at the start of the item), 16-byte stores, the
-//     reflecting ghost rows of y, phi and the two max-norms.
+//     reflecting ghost rows of y, phi and the two max-norms;
+//   * a handful of materials (Reed-type slabs): the operators of all blocks are one tall
+//     matrix, so a block is a row offset of the same tensor map; the host lists (cell tile, block, mask of the
+//     tile's cells that have this block) groups, a tile that straddles an interface appears once per block it
+//     contains and stores only the masked cells.
 #include <cuda.h>
 
 #include "device_utils.cuh"
@@ -118,8 +122,21 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
     const int kch = K / RK_K;                                         // chunks per item
     const int ntn = (PASS == PASS_FIX ? 2 * K2 : K2) / RK_N;          // items per cell tile
     const int prow = PASS == PASS_FIX ? 2 * K2 : K2;                  // operator row of the scalar-flux block
+    const int rpb = PASS == PASS_FIX ? 2 * K2 + 8 : PASS == PASS_ITER ? K2 + 8 : K2;   // operator rows per block
     const int64_t nct = (J + RK_M - 1) / RK_M;
-    const int64_t nitems = nct * ntn;
+    const int64_t ngroups = V.gitems ? V.ngroups : nct;              // (cell tile, block) groups
+    const int64_t nitems = ngroups * ntn;
+    // item -> (cell tile, output tile, block, mask of the tile's cells that have this block)
+    auto decode = [&](int64_t item, int64_t& ct, int& nt, int& blk, unsigned& m0, unsigned& m1) {
+        const int64_t g = item / ntn;
+        nt = (int)(item - g * ntn);
+        if (V.gitems) {
+            const int4 e = __ldg(reinterpret_cast<const int4*>(V.gitems) + g);
+            ct = e.x; blk = e.y; m0 = (unsigned)e.z; m1 = (unsigned)e.w;
+        } else {
+            ct = g; blk = 0; m0 = m1 = 0xffffffffu;
+        }
+    };
     const int my_items = (int)((nitems - blockIdx.x + gridDim.x - 1) / gridDim.x);
 
     if (tid == 0) {
@@ -145,9 +162,12 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
             int q = 0;
             for (int it = 0; it < my_items; ++it) {
                 const int64_t item = (int64_t)blockIdx.x + (int64_t)it * gridDim.x;
-                const int j0 = (int)(item / ntn) * RK_M;
-                const int nt = (int)(item % ntn);
-                const int i0 = nt * RK_N;
+                int64_t ct;
+                int nt, blk;
+                unsigned m0, m1;
+                decode(item, ct, nt, blk, m0, m1);
+                const int j0 = (int)ct * RK_M;
+                const int i0 = blk * rpb + nt * RK_N;                // operator row in the tall matrix of all blocks
                 const bool with_phi = PASS != PASS_FINAL && nt == 0;
                 for (int kc = 0; kc < kch; ++kc, ++q) {
                     const int s = q % RK_STAGES;
@@ -168,7 +188,7 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
                         tma_load_2d(st, my, k0, j0 + 1 + (k0 < N ? 1 : -1), &full[s]);
                     }
                     tma_load_2d(st + RK_A_BYTES, &map_op, k0, i0, &full[s]);
-                    if (with_phi) tma_load_2d(st + RK_A_BYTES + RK_B_BYTES, &map_op8, k0, prow, &full[s]);
+                    if (with_phi) tma_load_2d(st + RK_A_BYTES + RK_B_BYTES, &map_op8, k0, blk * rpb + prow, &full[s]);
                 }
             }
         }
@@ -197,11 +217,14 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
     int q = 0;
     for (int it = 0; it < my_items; ++it) {
         const int64_t item = (int64_t)blockIdx.x + (int64_t)it * gridDim.x;
-        const int64_t ct = item / ntn;
-        const int nt = (int)(item % ntn);
+        int64_t ct;
+        int nt, blk;
+        unsigned m0, m1;
+        decode(item, ct, nt, blk, m0, m1);
         const int64_t j0 = ct * RK_M;
         const int i0 = nt * RK_N;
         const bool with_phi = PASS != PASS_FINAL && nt == 0;
+        const unsigned mw = wm ? m1 : m0;                            // this warp's 32 cells of the tile
 
         // ---- additive operand of the epilogue, requested now
         double2 fx[4][4];
@@ -267,7 +290,7 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
         for (int g = 0; g < 4; ++g) {
             const int r = wm * 32 + 8 * g + g4;
             const int64_t j = j0 + r;
-            if (j < J) {
+            if (j < J && ((mw >> (8 * g + g4)) & 1u)) {
 #pragma unroll
                 for (int t = 0; t < 4; ++t) {
                     const int i = i0 + wn * 32 + 8 * t + 2 * t4;
@@ -300,8 +323,9 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
             named_bar_sync(1, 256);
             // thread tid owns (cell tid/4, slot tid%4) of the item
             const int64_t j = j0 + (tid >> 2);
+            const bool mine = (((tid >> 7) ? m1 : m0) >> ((tid >> 2) & 31)) & 1u;
             const double ssum = phi_s[0 * RK_M * 4 + tid] + phi_s[1 * RK_M * 4 + tid] + phi_s[2 * RK_M * 4 + tid] + phi_s[3 * RK_M * 4 + tid];
-            if (j < J) {
+            if (j < J && mine) {
                 if (PASS == PASS_FIX) {
                     V.phifix[j * 4 + (tid & 3)] = ssum;
                 } else {
@@ -325,17 +349,17 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
 
 bool oci_red_ktiled_supported(const DevView& V)
 {
-    return V.nblk == 1 && V.N % 64 == 0 && V.n <= 2048 && V.J + 2 < (int64_t)1 << 31;
+    return (V.nblk == 1 || V.gitems != nullptr) && V.N % 64 == 0 && V.n <= 2048 && V.J + 2 < (int64_t)1 << 31;
 }
 
 bool oci_red_ktiled_prepare(const DevView& V, RedKtiledMaps* M)
 {
-    const uint64_t K2 = (uint64_t)V.n / 2, J = (uint64_t)V.J;
+    const uint64_t K2 = (uint64_t)V.n / 2, J = (uint64_t)V.J, nb = (uint64_t)V.nblk;
     return oci_encode_2d(&M->y[0], V.y[0] - K2, J + 2, K2, RK_M, RK_K, true) && oci_encode_2d(&M->y[1], V.y[1] - K2, J + 2, K2, RK_M, RK_K, true) &&
            oci_encode_2d(&M->z, V.z, J, K2, RK_M, RK_K, true) && oci_encode_2d(&M->q16, V.q16, J, 16, RK_M, RK_K, true) &&
-           oci_encode_2d(&M->xop, V.xop, 2 * K2 + 8, K2 + 16, RK_N, RK_K, true) && oci_encode_2d(&M->xop8, V.xop, 2 * K2 + 8, K2 + 16, 8, RK_K, true) &&
-           oci_encode_2d(&M->rop, V.rop, K2 + 8, K2, RK_N, RK_K, true) && oci_encode_2d(&M->rop8, V.rop, K2 + 8, K2, 8, RK_K, true) &&
-           oci_encode_2d(&M->fop, V.fop, K2, K2, RK_N, RK_K, true);
+           oci_encode_2d(&M->xop, V.xop, nb * (2 * K2 + 8), K2 + 16, RK_N, RK_K, true) && oci_encode_2d(&M->xop8, V.xop, nb * (2 * K2 + 8), K2 + 16, 8, RK_K, true) &&
+           oci_encode_2d(&M->rop, V.rop, nb * (K2 + 8), K2, RK_N, RK_K, true) && oci_encode_2d(&M->rop8, V.rop, nb * (K2 + 8), K2, 8, RK_K, true) &&
+           oci_encode_2d(&M->fop, V.fop, nb * K2, K2, RK_N, RK_K, true);
 }
 
 int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int ybase, int slot, int prev_slot, double tol, int cnt,
@@ -355,7 +379,7 @@ int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int yb
         attr = true;
     }
     const int K2 = V.n / 2;
-    const int64_t nitems = ((V.J + RK_M - 1) / RK_M) * ((pass == PASS_FIX ? 2 * K2 : K2) / RK_N);
+    const int64_t nitems = (V.gitems ? V.ngroups : (V.J + RK_M - 1) / RK_M) * ((pass == PASS_FIX ? 2 * K2 : K2) / RK_N);
     const unsigned grid = (unsigned)(nitems < sm_count ? nitems : sm_count);
     const CUtensorMap& ya = M.y[ybase & 1];
     const CUtensorMap& yb = M.y[(ybase & 1) ^ 1];

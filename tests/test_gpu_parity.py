@@ -333,3 +333,35 @@ def test_resident_fused_loop_many_iterations(N):
     assert g.oci_step(-1.0, 77)[:2] == (1, 77) == o.oci_step(-1.0, 77)[:2]
     assert rel(g.get_angular_flux(), o.angular_flux()) < 1e-12
     g.close()
+
+
+@pytest.mark.parametrize("J,N,bcL,bcR,bounds", [
+    (200, 64, (INC, 1.0), (VAC, 0.0), (0, 37, 101, 130, 200)),        # interfaces inside the 64-cell tiles
+    (130, 128, (REF, 0.0), (REF, 0.0), (0, 64, 65, 130)),            # a one-cell region, mirrors on both sides
+    (70, 64, (VAC, 0.0), (INC, 0.5), (0, 1, 3, 70)),
+])
+def test_grouped_materials_on_the_ktiled_kernels(J, N, bcL, bcR, bounds):
+    """a handful of materials (Reed-type slab).  The blocks are a row offset into one tall
+    operator matrix and a tile that straddles an interface is processed once per block with a cell mask, so the
+    tensor-core K-tiled kernels serve the problem instead of the per-cell GEMV."""
+    import paper_2305_13555_b200 as P
+    from workloads.configs import Problem
+    rng = np.random.default_rng(J + N)
+    mats = [(0.3, 2.0, 1.9), (0.11, 7.0, 0.7), (0.5, 0.4, 0.39), (0.2, 3.0, 2.0)]
+    dx, st, ss = np.empty(J), np.empty(J), np.empty(J)
+    for r in range(len(bounds) - 1):
+        m = mats[(r * 3) % len(mats)] if r != 2 else mats[0]          # region 2 repeats the first material
+        dx[bounds[r]:bounds[r + 1]], st[bounds[r]:bounds[r + 1]], ss[bounds[r]:bounds[r + 1]] = m
+    q = rng.uniform(0, 1, (J, 4))
+    p = Problem(0, "reed-like", N, J, dx, st, ss, 1.3, 0.09, 2, bcL, bcR, rng.uniform(0, 1, (J, N, 2)), _source=lambda step: q)
+    g = P.OCI.from_problem(p)
+    info = g.get_info()
+    assert 1 < info["n_blocks"] <= 4 and info["path"] == P.PATH_PER_CELL
+    assert info["reduced_kernel"] == P.RKERNEL_KTILED and info["iteration"] == P.ITERATION_REDUCED
+    g.close()
+    r = run_pair(p, "oci", steps=2, tol=-1.0, max_iters=4, threads=16, iteration=REDUCED)
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-12
+    assert rel(r["g_phi"], r["o_phi"]) < 1e-12
+    r = run_pair(p, "oci", steps=2, tol=1e-10, max_iters=10_000, threads=16)
+    assert r["g_iters"] == r["o_iters"]
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-9
