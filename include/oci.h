@@ -91,7 +91,7 @@ enum { OCI_ITERATION_FULL = 0, OCI_ITERATION_REDUCED = 1, OCI_ITERATION_AUTO = 2
 /* Kernel family serving the REDUCED form (all three passes): GEMV - batched GEMV, one operator per
  * distinct block (any n; HBM-bound on the PER_CELL path);
  * RESIDENT - shared block, n in {64,128}: operators resident in shared memory, fp64 tensor pipe;
- * KTILED - shared block, or 2..16 distinct blocks (a multi-region slab), N a multiple of 64: operands
+ * KTILED - shared block, or 2..16 distinct blocks (a multi-region slab), N a multiple of 16: operands
  *          streamed in K chunks by tensor-map TMA, fp64 tensor pipe; a block is a row offset into the
  *          stacked operators, a tile of cells that straddles an interface is done once per block. */
 enum { OCI_RKERNEL_GEMV = 0, OCI_RKERNEL_RESIDENT = 1, OCI_RKERNEL_KTILED = 2 };

@@ -175,8 +175,8 @@ Layout make_layout(int64_t J, int32_t N, int64_t nblk)
         L.yfix = take(J * K2 * 8);
         L.ifix = take(J * K2 * 8);
         L.phifix = take(J * 4 * 8);
-        const bool grouped = nblk > 1 && nblk <= kMaxGroupedBlocks && N % 64 == 0;
-        L.q16 = take((nblk == 1 || grouped) && N % 64 == 0 ? J * 16 * 8 : 0);
+        const bool grouped = nblk > 1 && nblk <= kMaxGroupedBlocks && N % 16 == 0;
+        L.q16 = take((nblk == 1 || grouped) && N % 16 == 0 ? J * 16 * 8 : 0);
         // (cell tile, block) groups of the K-tiled kernels: at most min(nblk, 64) per tile of 64 cells
         L.gitems = take(grouped ? ((J + 63) / 64) * (nblk < 64 ? nblk : 64) * 16 : 0);
     }
@@ -480,7 +480,7 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     CK(cudaMemcpyAsync(V.coef, coef.data(), n * 8, cudaMemcpyHostToDevice, s));
     CK(cudaStreamSynchronize(s));   // host vectors above are read by the async copies
 
-    if (ctx->nblk > 1 && ctx->nblk <= kMaxGroupedBlocks && ctx->N % 64 == 0) {
+    if (ctx->nblk > 1 && ctx->nblk <= kMaxGroupedBlocks && ctx->N % 16 == 0) {
         // row f2: list, tile by tile, the blocks present and which of the tile's 64 cells have each
         std::vector<int32_t> items;
         const int64_t nct = (ctx->J + 63) / 64;

@@ -1,5 +1,6 @@
-// Interface-reduced OCI step (oci_reduced.cu has the derivation), shared block, large blocks
-// (N a multiple of 64, i.e. K2 = 2N a multiple of 128; config 4: K2 = 256): the K-tiled fp64 tensor-core
+// Interface-reduced OCI step (oci_reduced.cu has the derivation), shared block or a handful of blocks, N a
+// multiple of 16 (config 4: N = 128, K2 = 2N = 256; the last 128-row item of a cell tile is partial when K2 is
+// not a multiple of 128): the K-tiled fp64 tensor-core
 // form of the three passes.  Each pass is a "gathered GEMM"
 //     out[j][i] = add[j][i] + sum_k Op[i][k] in_j[k]
 // whose input vector is a concatenation of row segments of arrays that already sit in HBM in the packed
@@ -120,7 +121,8 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
     const int64_t J = V.J;
     const int K = PASS == PASS_FIX ? K2 + RK_K : K2;
     const int kch = K / RK_K;                                         // chunks per item
-    const int ntn = (PASS == PASS_FIX ? 2 * K2 : K2) / RK_N;          // items per cell tile
+    const int orows = PASS == PASS_FIX ? 2 * K2 : K2;                 // output rows (without the scalar-flux block)
+    const int ntn = (orows + RK_N - 1) / RK_N;                        // items per cell tile (the last one may be partial)
     const int prow = PASS == PASS_FIX ? 2 * K2 : K2;                  // operator row of the scalar-flux block
     const int rpb = PASS == PASS_FIX ? 2 * K2 + 8 : PASS == PASS_ITER ? K2 + 8 : K2;   // operator rows per block
     const int64_t nct = (J + RK_M - 1) / RK_M;
@@ -235,7 +237,10 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
                 int64_t j = j0 + wm * 32 + 8 * g + g4;
                 if (j >= J) j = J - 1;
 #pragma unroll
-                for (int t = 0; t < 4; ++t) fx[g][t] = *reinterpret_cast<const double2*>(fixp + j * K2 + i0 + wn * 32 + 8 * t + 2 * t4);
+                for (int t = 0; t < 4; ++t) {
+                    const int i = i0 + wn * 32 + 8 * t + 2 * t4;
+                    fx[g][t] = i < orows ? *reinterpret_cast<const double2*>(fixp + j * K2 + i) : make_double2(0.0, 0.0);
+                }
             }
         }
 
@@ -294,6 +299,7 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
 #pragma unroll
                 for (int t = 0; t < 4; ++t) {
                     const int i = i0 + wn * 32 + 8 * t + 2 * t4;
+                    if (i >= orows) continue;                        // partial last item: rows of the phi block / the next block
                     if (PASS == PASS_ITER) {
                         const double v0 = fx[g][t].x + acc[g][t][0], v1 = fx[g][t].y + acc[g][t][1];
                         *reinterpret_cast<double2*>(Yd + j * K2 + i) = make_double2(v0, v1);
@@ -349,7 +355,8 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
 
 bool oci_red_ktiled_supported(const DevView& V)
 {
-    return (V.nblk == 1 || V.gitems != nullptr) && V.N % 64 == 0 && V.n <= 2048 && V.J + 2 < (int64_t)1 << 31;
+    // chunks of 16 k must not straddle the halves of the gather: N a multiple of 16
+    return (V.nblk == 1 || V.gitems != nullptr) && V.N % 16 == 0 && V.n <= 2048 && V.J + 2 < (int64_t)1 << 31;
 }
 
 bool oci_red_ktiled_prepare(const DevView& V, RedKtiledMaps* M)
@@ -379,7 +386,7 @@ int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int yb
         attr = true;
     }
     const int K2 = V.n / 2;
-    const int64_t nitems = (V.gitems ? V.ngroups : (V.J + RK_M - 1) / RK_M) * ((pass == PASS_FIX ? 2 * K2 : K2) / RK_N);
+    const int64_t nitems = (V.gitems ? V.ngroups : (V.J + RK_M - 1) / RK_M) * (((pass == PASS_FIX ? 2 * K2 : K2) + RK_N - 1) / RK_N);
     const unsigned grid = (unsigned)(nitems < sm_count ? nitems : sm_count);
     const CUtensorMap& ya = M.y[ybase & 1];
     const CUtensorMap& yb = M.y[(ybase & 1) ^ 1];

@@ -155,6 +155,8 @@ def test_edge_cases(J, N, bcL, bcR, hetero, scheme, iteration):
     (63, 24, (INC, 1.0), (REF, 0.0)),        # n = 96
     (64, 40, (REF, 0.0), (VAC, 0.0)),        # n = 160: two output tiles, the second ragged; exactly one cell tile
     (65, 64, (REF, 0.0), (REF, 0.0)),        # n = 256: cell tile + 1
+    (77, 48, (INC, 0.3), (REF, 0.0)),        # n = 192: reduced K-tiled kernel with one partial 128-row item
+    (129, 80, (REF, 0.0), (VAC, 0.0)),       # n = 320: two items, the second partial
     (200, 128, (VAC, 0.0), (INC, 0.7)),      # n = 512 (config-4 block size), 4 output tiles, ragged cells
     (130, 256, (REF, 0.0), (REF, 0.0)),      # n = 1024: the largest block the kernel takes
 ])
@@ -165,8 +167,9 @@ def test_ktiled_kernel_shapes(J, N, bcL, bcR, iteration):
     p = _custom(J, N, bcL, bcR, seed=J * 1000 + N, hetero=False)
     g = P.OCI.from_problem(p)
     assert g.get_info()["apply_kernel"] == P.KERNEL_KTILED
-    # the reduced form has a K-tiled tensor-core kernel of its own when N is a multiple of 64
-    assert g.get_info()["reduced_kernel"] == (P.RKERNEL_KTILED if N % 64 == 0 else P.RKERNEL_GEMV)
+    # the reduced form has a K-tiled tensor-core kernel of its own when N is a multiple of 16 (partial last item
+    # unless 2N is a multiple of 128)
+    assert g.get_info()["reduced_kernel"] == (P.RKERNEL_KTILED if N % 16 == 0 else P.RKERNEL_GEMV)
     g.close()
     r = run_pair(p, "oci", steps=2, tol=-1.0, max_iters=4, threads=16, iteration=iteration)
     assert rel(r["g_psi"], r["o_psi"]) < 1e-12
@@ -339,6 +342,8 @@ def test_resident_fused_loop_many_iterations(N):
     (200, 64, (INC, 1.0), (VAC, 0.0), (0, 37, 101, 130, 200)),        # interfaces inside the 64-cell tiles
     (130, 128, (REF, 0.0), (REF, 0.0), (0, 64, 65, 130)),            # a one-cell region, mirrors on both sides
     (70, 64, (VAC, 0.0), (INC, 0.5), (0, 1, 3, 70)),
+    (300, 32, (REF, 0.0), (VAC, 0.0), (0, 100, 131, 300)),           # S32 blocks: one partial item per tile
+    (90, 16, (INC, 2.0), (REF, 0.0), (0, 10, 64, 90)),
 ])
 def test_grouped_materials_on_the_ktiled_kernels(J, N, bcL, bcR, bounds):
     """a handful of materials (Reed-type slab).  The blocks are a row offset into one tall
