@@ -55,6 +55,8 @@ struct oci_ctx {
     bool coop = false;                 // device supports cooperative launches
     int32_t predicted[2] = {0, 0};     // last iteration count of oci / si, sizes the launch chunk
     unsigned long long* h_norms = nullptr;   // pinned
+    cudaStream_t stream2 = nullptr;          // side stream of the norm read-back (REDUCED form)
+    cudaEvent_t ev_norms = nullptr;
     // timing
     bool timing = false;
     std::vector<cudaEvent_t> ev;
@@ -312,6 +314,15 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
             else ctx->launches += launch_oci_iteration_any(ctx, (ctx->cur + done_iters + i) & 1, i, i - 1, tol);
             if (timed) CK(cudaEventRecord(ctx->ev[2 * i + 1], s));
         }
+        // The norms are final once the iteration launches are done.  REDUCED form: their read-back goes through a
+        // side stream, so the host gets the iteration count while the FINAL pass is still running and the host
+        // part of the next step (Python, three launches) overlaps it; everything else stays ordered on `s`.
+        const bool side_readback = red && !timed && ctx->stream2 != nullptr;
+        if (side_readback) {
+            CK(cudaEventRecord(ctx->ev_norms, s));
+            CK(cudaStreamWaitEvent(ctx->stream2, ctx->ev_norms, 0));
+            CK(cudaMemcpyAsync(ctx->h_norms, V.norms, sizeof(unsigned long long) * 2 * cnt, cudaMemcpyDeviceToHost, ctx->stream2));
+        }
         if (red) {
             // finalisation, queued before the read-back: finds the last iteration on the device and
             // does nothing if this chunk neither converged nor ends at max_iters
@@ -319,8 +330,12 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
             ctx->launches += launch_reduced_pass(ctx, PASS_FINAL, (ctx->ycur + done_iters) & 1, 0, -1, tol, cnt, done_iters + cnt >= max_iters);
             if (timed) CK(cudaEventRecord(ctx->ev_aux[3], s));
         }
-        CK(cudaMemcpyAsync(ctx->h_norms, V.norms, sizeof(unsigned long long) * 2 * cnt, cudaMemcpyDeviceToHost, s));
-        CK(cudaStreamSynchronize(s));                                       // the one read-back (a7)
+        if (side_readback) {
+            CK(cudaStreamSynchronize(ctx->stream2));                        // the one read-back (a7)
+        } else {
+            CK(cudaMemcpyAsync(ctx->h_norms, V.norms, sizeof(unsigned long long) * 2 * cnt, cudaMemcpyDeviceToHost, s));
+            CK(cudaStreamSynchronize(s));                                   // the one read-back (a7)
+        }
         CK(cudaGetLastError());
         int32_t executed = cnt;
         for (int32_t i = 0; i < cnt; ++i) {
@@ -518,6 +533,10 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
         return fail(ctx, OCI_E_SINGULAR, buf);
     }
     if (!ctx->h_norms) CK(cudaHostAlloc((void**)&ctx->h_norms, sizeof(unsigned long long) * 2 * kNormSlots, cudaHostAllocDefault));
+    if (!ctx->stream2) {
+        CK(cudaStreamCreateWithFlags(&ctx->stream2, cudaStreamNonBlocking));
+        CK(cudaEventCreateWithFlags(&ctx->ev_norms, cudaEventDisableTiming));
+    }
     if (ctx->ev.empty()) {
         ctx->ev.resize(2 * kNormSlots);
         for (auto& e : ctx->ev) CK(cudaEventCreate(&e));
@@ -725,6 +744,8 @@ void oci_destroy(oci_ctx* ctx)
 {
     if (!ctx) return;
     if (ctx->h_norms) cudaFreeHost(ctx->h_norms);
+    if (ctx->stream2) cudaStreamDestroy(ctx->stream2);
+    if (ctx->ev_norms) cudaEventDestroy(ctx->ev_norms);
     for (auto& e : ctx->ev) cudaEventDestroy(e);
     for (auto& e : ctx->ev_aux) if (e) cudaEventDestroy(e);
     delete ctx;
