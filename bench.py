@@ -401,6 +401,13 @@ def run_ours(args):
     del g
     torch.cuda.empty_cache()
 
+    # arrays a step streams: reduced form y (x2), z, yfix, ifix of J x 2N doubles each (+ one operator per cell on
+    # the per-cell path); full form the two Psi buffers and c_fix
+    ws = p.unknowns * 4.0 * 5 if reduced else p.unknowns * 8.0 * 3
+    if not shared:
+        ws += p.cells * (n // 2 + 4) * (n // 2) * 8.0 if reduced else p.cells * n * n * 8.0
+    l2_note = ("working set of a step %.0f MiB, larger than the 126 MB L2" % (ws / 2**20) if ws > 126e6 else
+               "working set of a step %.1f MiB fits L2 and is not flushed between steps (launch-latency-bound config)" % (ws / 2**20))
     line = None
     if rank == 0:
         per_cfg = per_config_table(torch, P) if (world == 1 and not args.no_table) else None
@@ -417,7 +424,7 @@ def run_ours(args):
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": p.name, "S_N": p.n_angles, "cells": p.cells, "unknowns": p.unknowns, "tol": p.tol,
                        "path": "shared" if shared else "per_cell", "parallelism": f"replicas x{world}" if world > 1 else "1 gpu",
-                       "l2": "working set larger than L2 (3 x %.0f MiB)" % (p.unknowns * 8 / 2**20) if p.unknowns * 24 > 126e6 else "flushed by per-step c_fix rewrite; working set fits L2"},
+                       "l2": l2_note},
             "iters_per_step": iters, "time_to_converge_ms_per_step": ms / args.steps,
             "roofline": roofline, "cpu_baseline": cpu,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
