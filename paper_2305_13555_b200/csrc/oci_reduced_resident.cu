@@ -232,7 +232,9 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
     const int64_t J = V.J;
 
     const int64_t ntiles = (J + RT_M - 1) / RT_M;
-    const int64_t wid = (int64_t)blockIdx.x * RT_WARPS + warp, nw = (int64_t)gridDim.x * RT_WARPS;
+    // warp-major numbering: warp 0 of every CTA first, so a small problem spreads over all SMs (one busy warp per SM
+    // partition has the DMMA pipe to itself) instead of filling the eight warps of a few CTAs
+    const int64_t wid = (int64_t)warp * gridDim.x + blockIdx.x, nw = (int64_t)gridDim.x * RT_WARPS;
     const int my_tiles = wid < ntiles ? (int)((ntiles - wid + nw - 1) / nw) : 0;
     unsigned char* my_ring = ring + (size_t)warp * RT_STAGES * C::STAGE_BYTES;
     uint64_t* my_full = full + warp * RT_STAGES;
@@ -454,8 +456,7 @@ void launch_rr(const DevView& V, const RedResidentMaps& M, int ybase, int slot, 
         attr = true;
     }
     const int64_t ntiles = (V.J + RT_M - 1) / RT_M;
-    const int64_t ctas = (ntiles + RT_WARPS - 1) / RT_WARPS;
-    const unsigned grid = (unsigned)(ctas < sm_count ? ctas : sm_count);
+    const unsigned grid = (unsigned)(ntiles < sm_count ? ntiles : sm_count);
     const int b = ybase & 1;
     const CUtensorMap& ya = PASS == PASS_FIX ? M.y_half[b] : M.y_rows[b];
     const CUtensorMap& yb = PASS == PASS_FIX ? M.y_half[b ^ 1] : M.y_rows[b ^ 1];
