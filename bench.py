@@ -280,7 +280,48 @@ def time_gpu_e2e(torch, g, p, steps):
     return updates / (ms * 1e-3), h2d / steps, d2h / steps
 
 
-def per_config_table(torch, P, skip=None):
+def iteration_roofline(P, p, info, cfg, kms, klaunch, aux, steps, peaks, peak_src, peak_live):
+    """Roofline of the OCI iteration kernel against the work it EXECUTES per launch (or, for the fused
+    loops, per iteration): the full apply is [n x n] per cell; the reduced iteration is
+    [(2N+4) x 2N] per cell (G and the four scalar-flux rows H); its FIX pass [(4N+4) x (2N+4)] and FINAL
+    pass [2N x 2N] run once per step and are listed in step_breakdown."""
+    shared = info["path"] == P.PATH_SHARED
+    n = info["block_dim"]
+    k_avg_ms = kms / max(klaunch, 1)
+    reduced = info["iteration"] == P.ITERATION_REDUCED
+    K2 = n // 2
+    M_op, K_op = (K2 + 4, K2) if reduced else (n, n)
+    fix_ms, fix_n, fin_ms, fin_n = aux["fix_ms"], aux["fix_launches"], aux["final_ms"], aux["final_launches"]
+    breakdown = {"iteration_kernel_ms": k_avg_ms, "iterations_per_step": klaunch / steps,
+                 "fix_pass_ms_per_step": fix_ms / max(fix_n, 1) if reduced else None,
+                 "final_pass_ms_per_step": fin_ms / max(fin_n, 1) if reduced else None,
+                 "operator_rows_x_cols": [M_op, K_op], "form": "reduced" if reduced else "full"}
+    if shared:
+        flops = 2.0 * M_op * K_op * p.cells
+        nominal_ratio = 45.0 / 2250.0        # guide: B200 fp64 tensor 45 TF vs bf16 2250 TF nominal
+        peak_scaled = peaks["bf16_tflops"] * nominal_ratio
+        peak = max(peak_live, peak_scaled)
+        achieved = flops / (k_avg_ms * 1e-3) * 1e-12
+        roofline = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                    "traffic": NCU_TRAFFIC_BYTES.get((cfg, reduced)),
+                    "kernel": "oci %s iteration (eq. 19), fp64 DMMA" % breakdown["form"], "algorithmic_flops_per_launch": flops,
+                    "avg_launch_ms": k_avg_ms, "launches_timed": klaunch,
+                    "peak_source": f"max(live DMMA issue-rate probe {peak_live:.2f}, MEASURED_PEAKS bf16 {peak_src} x 45/2250 = {peak_scaled:.2f})"}
+    else:
+        if reduced:   # operator + gathered half rows, yfix in, y out; phifix and old phi in, phi out
+            bytes_ = p.cells * (M_op * K_op * 8.0 + 3.0 * K2 * 8.0 + 96.0)
+        else:         # inverse + c_fix, 2 half rows, Psi out; phi
+            bytes_ = p.cells * (n * n * 8.0 + 4.0 * n * 8.0 + 64.0)
+        achieved = bytes_ / (k_avg_ms * 1e-3) * 1e-9
+        roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "frac": achieved / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get((cfg, reduced)),
+                    "kernel": "oci %s iteration (eq. 19), batched GEMV" % breakdown["form"], "algorithmic_bytes_per_launch": bytes_,
+                    "avg_launch_ms": k_avg_ms, "launches_timed": klaunch, "peak_source": f"MEASURED_PEAKS hbm_gbs ({peak_src})"}
+    roofline["step_breakdown"] = breakdown
+    return roofline
+
+
+def per_config_table(torch, P, peaks=None, peak_src=None, peak_live=None):
     """OCI vs the GPU SI comparator for every BASELINE config (each for its own number of steps)."""
     out = {}
     for cfg in (1, 2, 3, 4, 5):
@@ -296,6 +337,15 @@ def per_config_table(torch, P, skip=None):
             row[f"{scheme}_iters"] = iters
             row[f"{scheme}_updates_per_s"] = p.unknowns * sum(iters) / (ms * 1e-3)
         row["si_over_oci_time"] = row["si_ms_per_step"] / row["oci_ms_per_step"]
+        if cfg >= 3 and peaks is not None:       # cfg 1-2 are launch-latency bound: absolutes only
+            g.enable_kernel_timing(True)
+            time_gpu_steps(torch, g, p, p.n_steps, "oci")
+            kms, klaunch = g.get_kernel_time()
+            aux = g.get_aux_kernel_time()
+            g.enable_kernel_timing(False)
+            r = iteration_roofline(P, p, g.get_info(), cfg, kms, klaunch, aux, p.n_steps, peaks, peak_src, peak_live)
+            row["oci_iteration_roofline"] = {k: r[k] for k in ("bound", "achieved", "peak", "unit", "frac", "avg_launch_ms")}
+            row["oci_step_breakdown"] = r["step_breakdown"]
         out[f"cfg{cfg}"] = row
         g.close()
         del g
@@ -358,41 +408,9 @@ def run_ours(args):
     kms, klaunch = g.get_kernel_time()
     aux = g.get_aux_kernel_time()
     g.enable_kernel_timing(False)
-    k_avg_ms = kms / max(klaunch, 1)
-    # work the timed kernel EXECUTES per launch: the full apply is [n x n] per cell; the reduced
-    # iteration is [(2N+4) x 2N] per cell (G and the four scalar-flux rows H); its FIX pass
-    # [(4N+4) x (2N+4)] and FINAL pass [2N x 2N] run once per step and are listed in step_breakdown
+    peak_live = P.probe_fp64_tensor_tflops(f"cuda:{local}") if shared else None
+    roofline = iteration_roofline(P, p, info, args.config, kms, klaunch, aux, args.steps, peaks, peak_src, peak_live)
     reduced = info["iteration"] == P.ITERATION_REDUCED
-    K2 = n // 2
-    M_op, K_op = (K2 + 4, K2) if reduced else (n, n)
-    fix_ms, fix_n, fin_ms, fin_n = aux["fix_ms"], aux["fix_launches"], aux["final_ms"], aux["final_launches"]
-    breakdown = {"iteration_kernel_ms": k_avg_ms, "iterations_per_step": klaunch / args.steps,
-                 "fix_pass_ms_per_step": fix_ms / max(fix_n, 1) if reduced else None,
-                 "final_pass_ms_per_step": fin_ms / max(fin_n, 1) if reduced else None,
-                 "operator_rows_x_cols": [M_op, K_op], "form": "reduced" if reduced else "full"}
-    if shared:
-        flops = 2.0 * M_op * K_op * p.cells
-        peak_live = P.probe_fp64_tensor_tflops(f"cuda:{local}")
-        nominal_ratio = 45.0 / 2250.0        # guide: B200 fp64 tensor 45 TF vs bf16 2250 TF nominal
-        peak_scaled = peaks["bf16_tflops"] * nominal_ratio
-        peak = max(peak_live, peak_scaled)
-        achieved = flops / (k_avg_ms * 1e-3) * 1e-12
-        roofline = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                    "traffic": NCU_TRAFFIC_BYTES.get((args.config, reduced)),
-                    "kernel": "oci %s iteration (eq. 19), fp64 DMMA" % breakdown["form"], "algorithmic_flops_per_launch": flops,
-                    "avg_launch_ms": k_avg_ms, "launches_timed": klaunch,
-                    "peak_source": f"max(live DMMA issue-rate probe {peak_live:.2f}, MEASURED_PEAKS bf16 {peak_src} x 45/2250 = {peak_scaled:.2f})"}
-    else:
-        if reduced:   # operator + gathered half rows, yfix in, y out; phifix and old phi in, phi out
-            bytes_ = p.cells * (M_op * K_op * 8.0 + 3.0 * K2 * 8.0 + 96.0)
-        else:         # inverse + c_fix, 2 half rows, Psi out; phi
-            bytes_ = p.cells * (n * n * 8.0 + 4.0 * n * 8.0 + 64.0)
-        achieved = bytes_ / (k_avg_ms * 1e-3) * 1e-9
-        roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                    "frac": achieved / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get((args.config, reduced)),
-                    "kernel": "oci %s iteration (eq. 19), batched GEMV" % breakdown["form"], "algorithmic_bytes_per_launch": bytes_,
-                    "avg_launch_ms": k_avg_ms, "launches_timed": klaunch, "peak_source": f"MEASURED_PEAKS hbm_gbs ({peak_src})"}
-    roofline["step_breakdown"] = breakdown
 
     # ---- end to end through the C ABI with host buffers
     e2e_val, h2d, d2h = time_gpu_e2e(torch, g, p, args.steps)
@@ -410,7 +428,8 @@ def run_ours(args):
                "working set of a step %.1f MiB fits L2 and is not flushed between steps (launch-latency-bound config)" % (ws / 2**20))
     line = None
     if rank == 0:
-        per_cfg = per_config_table(torch, P) if (world == 1 and not args.no_table) else None
+        per_cfg = (per_config_table(torch, P, peaks, peak_src, peak_live or P.probe_fp64_tensor_tflops(f"cuda:{local}"))
+                   if (world == 1 and not args.no_table) else None)
         cpu = None
         if world == 1 and not args.no_cpu:
             from oracle import threads_available
