@@ -353,6 +353,302 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
     }
 }
 
+// ---- ping-pong variant of the same kernel, used when every CTA has at least one item per math group.
+// Two math groups of four warps share the SM, each warp 64 cells x 32 operator rows (32 accumulators), each group
+// with its own ring of RP_STAGES stages and its own producer thread; group 1 starts half an item behind group 0, so
+// one group's epilogue (global loads and stores, the scalar-flux barrier: 4 - 9 us of an item in the kernel above,
+// where all eight warps sit through it together) overlaps the other group's DMMA stream.  Measured at config 4:
+// FIX 0.176 -> 0.156 ms, ITER 0.107 -> 0.103 ms.  With fewer items than that an item would only get four warps,
+// which is slower (measured +20 % on a 70-item problem): the launcher then takes the kernel above.
+constexpr int RP_STAGES = 4;                  // per math group
+constexpr size_t RP_SMEM = 1024 /*alignment slack*/ + (size_t)2 * RP_STAGES * RK_STAGE_BYTES + 2 * 4 * RK_M * 4 * 8 /*phi_s, one per group*/ +
+                           (4 * RP_STAGES + 1) * 8 + 64;
+
+template <int PASS>
+__global__ void __launch_bounds__(384, 1)
+oci_red_ktiled_pp_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_y_alt,
+                      const __grid_constant__ CUtensorMap map_z, const __grid_constant__ CUtensorMap map_q,
+                      const __grid_constant__ CUtensorMap map_op, const __grid_constant__ CUtensorMap map_op8, int ybase, int slot,
+                      int prev_slot, double tol, int cnt, int force)
+{
+    // map_y = tensor map of y[ybase], map_y_alt = of y[ybase ^ 1]
+    int ysrc = ybase;
+    if (PASS == PASS_ITER) {
+        if (step_done(V.norms, prev_slot, tol)) return;
+    } else if (PASS == PASS_FINAL) {
+        int L = first_converged(V.norms, cnt, tol);
+        if (L == 0) {
+            if (!force) return;
+            L = cnt;
+        }
+        ysrc = (ybase + L - 1) & 1;
+    }
+    const CUtensorMap* my = (ysrc == ybase) ? &map_y : &map_y_alt;
+    if (PASS == PASS_FIX) clear_step_state(V);
+
+    extern __shared__ unsigned char smem_raw[];
+    // aligned up inside the shared window (pointer arithmetic on the array keeps the LDS/STS address space)
+    unsigned char* base = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    double* phi_all = reinterpret_cast<double*>(base + (size_t)2 * RP_STAGES * RK_STAGE_BYTES);   // [2 groups][4 wn][64][4]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(phi_all + 2 * 4 * RK_M * 4);
+    uint64_t* stagger = bars + 4 * RP_STAGES;    // group 0 -> group 1: "I am half way through my first item"
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int N = V.N, K2 = V.n >> 1, N2 = N >> 1;
+    const int64_t J = V.J;
+    const int K = PASS == PASS_FIX ? K2 + RK_K : K2;
+    const int kch = K / RK_K;                                         // chunks per item
+    const int orows = PASS == PASS_FIX ? 2 * K2 : K2;                 // output rows (without the scalar-flux block)
+    const int ntn = (orows + RK_N - 1) / RK_N;                        // items per cell tile (the last one may be partial)
+    const int prow = PASS == PASS_FIX ? 2 * K2 : K2;                  // operator row of the scalar-flux block
+    const int rpb = PASS == PASS_FIX ? 2 * K2 + 8 : PASS == PASS_ITER ? K2 + 8 : K2;   // operator rows per block
+    const int64_t nct = (J + RK_M - 1) / RK_M;
+    const int64_t ngroups = V.gitems ? V.ngroups : nct;              // (cell tile, block) groups
+    const int64_t nitems = ngroups * ntn;
+    // item -> (cell tile, output tile, block, mask of the tile's cells that have this block)
+    auto decode = [&](int64_t item, int64_t& ct, int& nt, int& blk, unsigned& m0, unsigned& m1) {
+        const int64_t g = item / ntn;
+        nt = (int)(item - g * ntn);
+        if (V.gitems) {
+            const int4 e = __ldg(reinterpret_cast<const int4*>(V.gitems) + g);
+            ct = e.x; blk = e.y; m0 = (unsigned)e.z; m1 = (unsigned)e.w;
+        } else {
+            ct = g; blk = 0; m0 = m1 = 0xffffffffu;
+        }
+    };
+    // Two math groups of four warps share the SM: group mg takes the items blockIdx.x + (2 it + mg) W.  Each has its
+    // own stage ring and producer thread, and group 1 starts half an item late, so while one group sits in its
+    // epilogue (loads, stores, the scalar-flux barrier) the other one keeps the DMMA pipe busy.
+    const int W = gridDim.x;
+    auto items_of = [&](int mg) { const int64_t first = (int64_t)blockIdx.x + (int64_t)mg * W;
+                                  return first < nitems ? (int)((nitems - first + 2 * W - 1) / (2 * W)) : 0; };
+
+    if (tid == 0) {
+        for (int s = 0; s < 2 * RP_STAGES; ++s) {
+            mbar_init(&bars[s], 1);                          // full[mg][s]
+            mbar_init(&bars[2 * RP_STAGES + s], 4);          // empty[mg][s]: the four warps of the group
+        }
+        mbar_init(stagger, 4);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp >= 8) {
+        // ============ auxiliary warpgroup: lane 0 of warps 8 and 9 = the TMA producers of ring 0 and ring 1 ============
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        if (warp < 10 && lane == 0) {
+            const int mg = warp - 8;
+            unsigned char* stages = base + (size_t)mg * RP_STAGES * RK_STAGE_BYTES;
+            uint64_t* full = bars + mg * RP_STAGES;
+            uint64_t* empty = bars + 2 * RP_STAGES + mg * RP_STAGES;
+            asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(my)) : "memory");
+            asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&map_op)) : "memory");
+            if (PASS != PASS_FINAL) asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&map_op8)) : "memory");
+            if (PASS == PASS_FIX) {
+                asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&map_z)) : "memory");
+                asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&map_q)) : "memory");
+            }
+            const int my_items = items_of(mg);
+            int q = 0;
+            for (int it = 0; it < my_items; ++it) {
+                const int64_t item = (int64_t)blockIdx.x + (int64_t)(2 * it + mg) * W;
+                int64_t ct;
+                int nt, blk;
+                unsigned m0, m1;
+                decode(item, ct, nt, blk, m0, m1);
+                const int j0 = (int)ct * RK_M;
+                const int i0 = blk * rpb + nt * RK_N;                // operator row in the tall matrix of all blocks
+                const bool with_phi = PASS != PASS_FINAL && nt == 0;
+                for (int kc = 0; kc < kch; ++kc, ++q) {
+                    const int s = q % RP_STAGES;
+                    if (q >= RP_STAGES) mbar_wait(&empty[s], ((q / RP_STAGES) - 1) & 1);
+                    unsigned char* st = stages + (size_t)s * RK_STAGE_BYTES;
+                    const int k0 = kc * RK_K;
+                    // the MMA warps read this stage through the generic proxy (LDS); order those reads, made
+                    // visible by the empty barrier, before the async-proxy write of the TMA unit
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    mbar_expect_tx(&full[s], RK_A_BYTES + RK_B_BYTES + (with_phi ? RK_P_BYTES : 0));
+                    if (PASS == PASS_FIX) {
+                        // y / z map rows: y carries the ghost row first (row = cell + 1), z and Q16 do not
+                        if (k0 < N) tma_load_2d(st, my, N2 + k0, j0 + 1, &full[s]);
+                        else if (k0 < K2) tma_load_2d(st, &map_z, N2 + k0 - N, j0, &full[s]);
+                        else tma_load_2d(st, &map_q, 0, j0, &full[s]);
+                    } else {
+                        // k < N (mu<0) comes from the right neighbour, else from the left one (row a3)
+                        tma_load_2d(st, my, k0, j0 + 1 + (k0 < N ? 1 : -1), &full[s]);
+                    }
+                    tma_load_2d(st + RK_A_BYTES, &map_op, k0, i0, &full[s]);
+                    if (with_phi) tma_load_2d(st + RK_A_BYTES + RK_B_BYTES, &map_op8, k0, blk * rpb + prow, &full[s]);
+                }
+            }
+        }
+        return;
+    }
+
+    // =========================== MMA warps: group mg = warp / 4, four warps x (64 cells x 32 rows) ===========================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");   // 8 x 32 x 208 + 4 x 32 x 56 registers: slack in every SM partition
+    const int g4 = lane >> 2, t4 = lane & 3;
+    const int mg = warp >> 2, wn = warp & 3;
+    const int gtid = tid & 127;                              // thread index inside the group
+    unsigned char* stages = base + (size_t)mg * RP_STAGES * RK_STAGE_BYTES;
+    uint64_t* full = bars + mg * RP_STAGES;
+    uint64_t* empty = bars + 2 * RP_STAGES + mg * RP_STAGES;
+    double* phi_s = phi_all + mg * (4 * RK_M * 4);           // [4 wn][64][4] k-partials of this group
+    // byte offset of this lane's fragment element inside a 128-byte swizzled row, per k-step:
+    // logical 16-byte unit ks + 4*(t4>>1), XOR row&7 (= g4), element t4&1
+    int foff[4];
+#pragma unroll
+    for (int ks = 0; ks < 4; ++ks) foff[ks] = (((ks + 4 * (t4 >> 1)) ^ g4) << 4) + ((t4 & 1) << 3);
+    const int a_row = g4 * 128;                              // + g*1024, g = 0..7: all 64 cells
+    const int b_row = (wn * 32 + g4) * 128;                  // + t*1024
+    // scalar-flux block: this warp's k-step is ks = wn (computed: a runtime index into foff would push it to local memory)
+    const int p_off = g4 * 128 + (((wn + 4 * (t4 >> 1)) ^ g4) << 4) + ((t4 & 1) << 3);
+
+    double* __restrict__ Yd = V.y[ysrc ^ 1];
+    const double* __restrict__ fixp = PASS == PASS_FINAL ? V.ifix : V.yfix;
+    double dmax = 0.0, rmax = 0.0;
+    const bool refl_l = V.bcL == OCI_BC_REFLECTING, refl_r = V.bcR == OCI_BC_REFLECTING;
+    const int my_items = items_of(mg);
+
+    if (mg == 1) mbar_wait(stagger, 0);                      // start half an item behind group 0
+
+    int q = 0;
+    for (int it = 0; it < my_items; ++it) {
+        const int64_t item = (int64_t)blockIdx.x + (int64_t)(2 * it + mg) * W;
+        int64_t ct;
+        int nt, blk;
+        unsigned m0, m1;
+        decode(item, ct, nt, blk, m0, m1);
+        const int64_t j0 = ct * RK_M;
+        const int i0 = nt * RK_N;
+        const bool with_phi = PASS != PASS_FINAL && nt == 0;
+
+        // scalar flux of this item's cells: thread gtid finishes (cell p/4, slot p%4) for p = gtid, gtid + 128; the
+        // operands are requested now so that nothing behind the barrier waits for global memory
+        double pfix[2] = {0.0, 0.0}, pold[2] = {0.0, 0.0};
+        if (with_phi && PASS == PASS_ITER) {
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int p = gtid + 128 * u;
+                int64_t j = j0 + (p >> 2);
+                if (j >= J) j = J - 1;
+                pfix[u] = V.phifix[j * 4 + (p & 3)];
+                pold[u] = V.phi[j * 4 + (p & 3)];
+            }
+        }
+
+        double acc[8][4][2], accp[8][2];
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+            accp[g][0] = accp[g][1] = 0.0;
+#pragma unroll
+            for (int t = 0; t < 4; ++t) acc[g][t][0] = acc[g][t][1] = 0.0;
+        }
+
+        for (int kc = 0; kc < kch; ++kc, ++q) {
+            const int s = q % RP_STAGES;
+            mbar_wait(&full[s], (q / RP_STAGES) & 1);
+            const unsigned char* st = stages + (size_t)s * RK_STAGE_BYTES;
+            const unsigned char* As = st + a_row;
+            const unsigned char* Bs = st + RK_A_BYTES + b_row;
+#pragma unroll
+            for (int ks = 0; ks < 4; ++ks) {
+                double a[8], b[4];
+#pragma unroll
+                for (int g = 0; g < 8; ++g) a[g] = *reinterpret_cast<const double*>(As + g * 1024 + foff[ks]);
+#pragma unroll
+                for (int t = 0; t < 4; ++t) b[t] = *reinterpret_cast<const double*>(Bs + t * 1024 + foff[ks]);
+#pragma unroll
+                for (int g = 0; g < 8; ++g)
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) dmma(acc[g][t][0], acc[g][t][1], a[g], b[t]);
+                if (with_phi && ks == wn) {
+                    const double bp = *reinterpret_cast<const double*>(st + RK_A_BYTES + RK_B_BYTES + p_off);
+#pragma unroll
+                    for (int g = 0; g < 8; ++g) dmma(accp[g][0], accp[g][1], a[g], bp);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(&empty[s]);
+                if (mg == 0 && it == 0 && kc == (kch >> 1)) mbar_arrive(stagger);
+            }
+        }
+        if (mg == 0 && it == 0 && kch < 2 && lane == 0) mbar_arrive(stagger);   // (kch >= 2 always; belt and braces)
+
+        // ---- epilogue: + additive operand (one cell block of 8 at a time), 16-byte stores, reflecting ghost rows
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+            const int r = 8 * g + g4;
+            const int64_t j = j0 + r;
+            const bool live = j < J && (((g < 4 ? m0 : m1) >> (r & 31)) & 1u);
+            double2 f[4];
+#pragma unroll
+            for (int t = 0; t < 4; ++t) {
+                const int i = i0 + wn * 32 + 8 * t + 2 * t4;
+                f[t] = (PASS != PASS_FIX && live && i < orows) ? *reinterpret_cast<const double2*>(fixp + j * K2 + i) : make_double2(0.0, 0.0);
+            }
+#pragma unroll
+            for (int t = 0; t < 4; ++t) {
+                const int i = i0 + wn * 32 + 8 * t + 2 * t4;
+                if (!live || i >= orows) continue;                   // partial last item: rows of the phi block / the next block
+                if (PASS == PASS_ITER) {
+                    const double v0 = f[t].x + acc[g][t][0], v1 = f[t].y + acc[g][t][1];
+                    *reinterpret_cast<double2*>(Yd + j * K2 + i) = make_double2(v0, v1);
+                    // reading S4: the mirror image of the edge cell's outgoing flux becomes the ghost row
+                    if (j == 0 && refl_l && i < N) {
+                        Yd[-(int64_t)K2 + mirror_q(i, N)] = v0;
+                        Yd[-(int64_t)K2 + mirror_q(i + 1, N)] = v1;
+                    }
+                    if (j == J - 1 && refl_r && i >= N) {
+                        Yd[J * K2 + mirror_q(i, N)] = v0;
+                        Yd[J * K2 + mirror_q(i + 1, N)] = v1;
+                    }
+                } else if (PASS == PASS_FINAL) {
+                    *reinterpret_cast<double2*>(V.z + j * K2 + i) = make_double2(f[t].x + acc[g][t][0], f[t].y + acc[g][t][1]);
+                } else {
+                    double* dst = i < K2 ? V.yfix + j * K2 + i : V.ifix + j * K2 + (i - K2);
+                    *reinterpret_cast<double2*>(dst) = make_double2(acc[g][t][0], acc[g][t][1]);
+                }
+            }
+            if (with_phi && t4 < 2) {     // columns 0..3 of the scalar-flux block: this warp's k-partial
+                phi_s[(wn * RK_M + r) * 4 + 2 * t4 + 0] = accp[g][0];
+                phi_s[(wn * RK_M + r) * 4 + 2 * t4 + 1] = accp[g][1];
+            }
+        }
+        if (with_phi) {                                              // uniform over the group
+            named_bar_sync(1 + mg, 128);
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int p = gtid + 128 * u;                        // (cell p/4, slot p%4)
+                const int r = p >> 2;
+                const int64_t j = j0 + r;
+                const double ssum = phi_s[0 * RK_M * 4 + p] + phi_s[1 * RK_M * 4 + p] + phi_s[2 * RK_M * 4 + p] + phi_s[3 * RK_M * 4 + p];
+                if (j < J && (((r < 32 ? m0 : m1) >> (r & 31)) & 1u)) {
+                    if (PASS == PASS_FIX) {
+                        V.phifix[j * 4 + (p & 3)] = ssum;
+                    } else {
+                        const double a = pfix[u] + ssum;
+                        V.phi[j * 4 + (p & 3)] = a;
+                        dmax = fmax(dmax, fabs(a - pold[u]));
+                        rmax = fmax(rmax, fabs(a));
+                    }
+                }
+            }
+            named_bar_sync(1 + mg, 128);                             // phi_s of this group reusable
+        }
+    }
+    if (mg == 0 && my_items == 0 && lane == 0) mbar_arrive(stagger);  // never leave group 1 waiting
+    if (PASS == PASS_ITER) {
+        dmax = warp_max(dmax);
+        rmax = warp_max(rmax);
+        if (lane == 0) {
+            atomic_max_nonneg(&V.norms[2 * slot + 0], dmax);
+            atomic_max_nonneg(&V.norms[2 * slot + 1], rmax);
+        }
+    }
+}
+
 bool oci_red_ktiled_supported(const DevView& V)
 {
     // chunks of 16 k must not straddle the halves of the gather: N a multiple of 16
@@ -390,6 +686,24 @@ int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int yb
     const unsigned grid = (unsigned)(nitems < sm_count ? nitems : sm_count);
     const CUtensorMap& ya = M.y[ybase & 1];
     const CUtensorMap& yb = M.y[(ybase & 1) ^ 1];
+    // ping-pong kernel when both math groups of every CTA get at least one item, else the eight-warp kernel
+    const bool pp = nitems >= 2 * (int64_t)grid;
+    if (pp) {
+        static bool attr_pp = false;
+        if (!attr_pp) {
+            cudaFuncSetAttribute(oci_red_ktiled_pp_kernel<PASS_FIX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RP_SMEM);
+            cudaFuncSetAttribute(oci_red_ktiled_pp_kernel<PASS_ITER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RP_SMEM);
+            cudaFuncSetAttribute(oci_red_ktiled_pp_kernel<PASS_FINAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RP_SMEM);
+            attr_pp = true;
+        }
+        if (pass == PASS_FIX)
+            oci_red_ktiled_pp_kernel<PASS_FIX><<<grid, 384, RP_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.xop, M.xop8, ybase, 0, -1, tol, 0, 0);
+        else if (pass == PASS_ITER)
+            oci_red_ktiled_pp_kernel<PASS_ITER><<<grid, 384, RP_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.rop, M.rop8, ybase, slot, prev_slot, tol, 0, 0);
+        else
+            oci_red_ktiled_pp_kernel<PASS_FINAL><<<grid, 384, RP_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.fop, M.fop, ybase, 0, -1, tol, cnt, force);
+        return 1;
+    }
     if (pass == PASS_FIX)
         oci_red_ktiled_kernel<PASS_FIX><<<grid, 384, RK_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.xop, M.xop8, ybase, 0, -1, tol, 0, 0);
     else if (pass == PASS_ITER)

@@ -370,3 +370,31 @@ def test_grouped_materials_on_the_ktiled_kernels(J, N, bcL, bcR, bounds):
     r = run_pair(p, "oci", steps=2, tol=1e-10, max_iters=10_000, threads=16)
     assert r["g_iters"] == r["o_iters"]
     assert rel(r["g_psi"], r["o_psi"]) < 1e-9
+
+
+@pytest.mark.parametrize("J,N,bcL,bcR,bounds", [
+    (20000, 64, (REF, 0.0), (REF, 0.0), (0, 7001, 7002, 13333, 20000)),   # 313+ items: ping-pong kernel, masks, mirrors
+    (19000, 48, (INC, 0.7), (REF, 0.0), (0, 19000)),                     # one block, partial 128-row items
+])
+def test_ktiled_pingpong_kernel(J, N, bcL, bcR, bounds):
+    """With at least two items per CTA the K-tiled passes run on the ping-pong kernel (two math groups of four
+    warps, two stage rings).  Fixed iterations against the oracle, then bit-reproducibility."""
+    import paper_2305_13555_b200 as P
+    from oracle import threads_available
+    from workloads.configs import Problem
+    rng = np.random.default_rng(J + N)
+    mats = [(0.3, 2.0, 1.9), (0.11, 7.0, 0.7), (0.5, 0.4, 0.39)]
+    dx, st, ss = np.empty(J), np.empty(J), np.empty(J)
+    for r in range(len(bounds) - 1):
+        dx[bounds[r]:bounds[r + 1]], st[bounds[r]:bounds[r + 1]], ss[bounds[r]:bounds[r + 1]] = mats[r % 3]
+    q = rng.uniform(0, 1, (J, 4))
+    p = Problem(0, "pp", N, J, dx, st, ss, 1.3, 0.09, 1, bcL, bcR, rng.uniform(0, 1, (J, N, 2)), _source=lambda step: q)
+    r = run_pair(p, "oci", steps=1, tol=-1.0, max_iters=3, threads=threads_available(), iteration=REDUCED)
+    assert r["info"]["reduced_kernel"] == P.RKERNEL_KTILED
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-12
+    assert rel(r["g_phi"], r["o_phi"]) < 1e-12
+    g = P.OCI.from_problem(p, iteration=REDUCED)
+    g.set_source(q)
+    g.oci_step(-1.0, 3)
+    assert np.array_equal(g.get_angular_flux(), r["g_psi"])
+    g.close()
