@@ -43,7 +43,7 @@ NCU_TRAFFIC_BYTES = {(3, False): 374.17e6,    # profiles/r1_resident_cfg3_full.t
                      (5, False): 2168.2e6,    # profiles/r1_percell_cfg5_full.txt:  2164.5 MB read +   3.8 MB written
                      # reduced form, per ITERATION (resident and GEMV ITER launches run all iterations of a step: bytes / iterations)
                      (3, True): 206.2e6,      # profiles/r1d_reduced_cfg3_full.txt: (846.0 MB read + 391.4 MB written) / 6 iterations
-                     (4, True): 75.6e6,       # profiles/r1d_reduced_cfg4_full.txt:  68.7 MB read +  6.9 MB written (y buffers fit in L2)
+                     (4, True): 75.6e6,       # profiles/r1e_reduced_cfg4_full.txt:  68.8 MB read +  6.8 MB written (y buffers fit in L2)
                      (5, True): 558.6e6}      # profiles/r1d_reduced_cfg5_full.txt: (4447.6 MB read + 21.0 MB written) / 8 iterations
 
 
