@@ -21,6 +21,10 @@
  *     form; pure absorber -> exp(-Sigma x/mu) at 2nd order
  *   - infinite-medium steady phi = Q/(Sigma-Sigma_s); OCI == SI; particle
  *     balance; LU vs numpy.linalg; spectral radii
+ *   - stopping rule: the (d, r) an iteration returns vs numpy max-norms of phi
+ *     re-formed from the angular fluxes (maxima placed in a k slot of an
+ *     interior cell), and the three branches of converged() with the d = tol r
+ *     boundary located by nextafter
  * Parity unpinned (no value printed in the paper): iteration counts and the
  * absolute flux values of the five BASELINE configs (oracle-vs-GPU only).
  *

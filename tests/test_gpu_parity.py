@@ -267,6 +267,34 @@ def test_full_size_si_fixed_iterations_cfg3():
     assert rel(r["g_phi"], r["o_phi"]) < 1e-12
 
 
+@pytest.mark.parametrize("scheme", ["oci", "si"])
+@pytest.mark.parametrize("cfg,steps", [(2, 3), (3, 1), (4, 2), (5, 1)])
+def test_full_size_converged_parity(cfg, steps, scheme):
+    """north_star's gate at BASELINE.json's full sizes, in the launch configuration bench.py times (the
+    library's default iteration form): converged steps to tol 1e-10 against the oracle on all host threads;
+    iteration counts within +-1 (equal in every run so far), Psi and phi within 10 x tol.  Config 4 runs two
+    steps so that a step with Q = 0 (the pulse is on during step 0 only, reading S6) is included."""
+    from oracle import threads_available
+    p = make_problem(cfg)
+    r = run_pair(p, scheme, steps=steps, tol=p.tol, max_iters=p.max_iters, threads=threads_available())
+    for a, b in zip(r["g_iters"], r["o_iters"]):
+        assert abs(a - b) <= 1, (r["g_iters"], r["o_iters"])
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-9
+    assert rel(r["g_phi"], r["o_phi"]) < 1e-9
+    if scheme == "oci":
+        import paper_2305_13555_b200 as P
+        assert r["info"]["iteration"] == P.ITERATION_REDUCED
+
+
+@pytest.mark.parametrize("cfg", [4, 5])
+def test_full_size_si_fixed_iterations(cfg):
+    from oracle import threads_available
+    p = make_problem(cfg)
+    r = run_pair(p, "si", steps=1, tol=-1.0, max_iters=2, threads=threads_available())
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-12
+    assert rel(r["g_phi"], r["o_phi"]) < 1e-12
+
+
 @pytest.mark.parametrize("cfg,cells", [(2, 150), (5, 40)])
 def test_mixing_schemes_and_iteration_forms_on_one_context(cfg, cells):
     """REDUCED keeps a packed copy of the outgoing rows between steps; every other way of changing the

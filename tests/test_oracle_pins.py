@@ -404,3 +404,95 @@ def test_fixed_iteration_mode_and_status():
         Oracle(np.ones(3), np.ones(3), np.zeros(3), 1.0, 1.0, 3)   # odd N
     with pytest.raises(ValueError):
         Oracle(-np.ones(3), np.ones(3), np.zeros(3), 1.0, 1.0, 2)  # dx <= 0
+
+
+# ----------------------------------------------------------------- stopping-rule arithmetic (reading S2)
+def _norm_problem(scheme_seed=0):
+    """Small heterogeneous slab whose source is concentrated in the k slots (0, 1) of one interior cell, so
+    that both max-norms of the first iterations sit in a k slot of an interior cell: a reduction over the
+    wrong slot range (k+1/2 only), over a sub-range of cells, or over phi_old instead of phi_new would miss it."""
+    rng = np.random.default_rng(2305 + scheme_seed)
+    N, J, v, dt = 4, 11, 1.1, 0.6
+    dx = rng.uniform(0.3, 0.9, J)
+    sig = rng.uniform(0.6, 2.5, J)
+    sigs = sig * rng.uniform(0.3, 0.9, J)
+    Q = np.full((J, 4), 1e-3)
+    Q[6, 0], Q[6, 1] = 40.0, 55.0                     # interior cell 6, slots (k,L), (k,R)
+    psi0 = rng.uniform(0.0, 0.05, (J, N, 2))
+    o = Oracle(dx, sig, sigs, v, dt, N, (INC, 0.3), (REF, 0.0))
+    o.setup()
+    o.set_flux(psi0)
+    o.set_source(Q)
+    return o, N, J
+
+
+@pytest.mark.parametrize("scheme", ["oci", "si"])
+def test_returned_norms_equal_their_definition(scheme):
+    """Reading S2 ("ceases changing"; north_star "tolerance on scalar flux"): after
+    an iteration d = max_{j,s}|phi^(l+1) - phi^(l)| and r = max_{j,s}|phi^(l+1)| over ALL cells and ALL four
+    slots, phi = sum_m w_m psi_m (eq. 18).  phi is re-formed here from the angular fluxes with
+    numpy.einsum and numpy's Gauss-Legendre weights, before and after each of several iterations."""
+    o, N, J = _norm_problem(0 if scheme == "oci" else 1)
+    _, w = np.polynomial.legendre.leggauss(N)
+    f = o.oci_iteration if scheme == "oci" else o.si_iteration
+    phi_old = np.einsum("m,jms->js", w, o.angular_flux())
+    seen_k_slot_interior = False
+    for it in range(6):
+        d, r = f()
+        phi_new = np.einsum("m,jms->js", w, o.angular_flux())
+        d_np, r_np = np.max(np.abs(phi_new - phi_old)), np.max(np.abs(phi_new))
+        assert abs(d - d_np) <= 4e-15 * r_np, (it, d, d_np)
+        assert abs(r - r_np) <= 4e-15 * r_np, (it, r, r_np)
+        assert np.max(np.abs(o.scalar_flux() - phi_new)) <= 4e-15 * r_np          # eq. (18) itself
+        jd, sd = np.unravel_index(np.argmax(np.abs(phi_new - phi_old)), phi_new.shape)
+        jr, sr = np.unravel_index(np.argmax(np.abs(phi_new)), phi_new.shape)
+        if it == 0:
+            # the construction works: both maxima in a k slot (0/1) of the interior cell
+            assert (jd, jr) == (6, 6) and sd in (0, 1) and sr in (0, 1)
+            seen_k_slot_interior = True
+            # ... and restricting either reduction to the k+1/2 slots, to the edge cells, or taking
+            # max|phi_old| for r would give a different number (so the pin can fail)
+            assert np.max(np.abs(phi_new[:, 2:] - phi_old[:, 2:])) < 0.9 * d
+            assert np.max(np.abs(phi_new[[0, -1]])) < 0.9 * r
+            assert np.max(np.abs(phi_old)) < 0.9 * r
+        phi_old = phi_new
+    assert seen_k_slot_interior
+
+
+@pytest.mark.parametrize("scheme", ["oci", "si"])
+def test_converged_branches(scheme):
+    """The three branches of the stopping rule (reading S2): tol < 0 never converges; r = 0 converges iff
+    d = 0; otherwise converged iff d <= tol * r, with equality counting (the boundary is found with
+    nextafter, so '<' instead of '<=' or a test against the previous r fails)."""
+    def fresh():
+        return _norm_problem(7)[0]
+
+    step = (lambda o, tol, mx: o.oci_step(tol, mx)) if scheme == "oci" else (lambda o, tol, mx: o.si_step(tol, mx))
+    o = fresh()
+    d, r = (o.oci_iteration if scheme == "oci" else o.si_iteration)()
+    assert d > 0 and r > 0
+    # smallest tol with tol * r >= d
+    t = d / r
+    while t * r < d:
+        t = np.nextafter(t, np.inf)
+    while np.nextafter(t, 0.0) * r >= d:
+        t = np.nextafter(t, 0.0)
+    st, it, res = step(fresh(), t, 50)
+    assert (st, it) == (0, 1) and res == d / r                       # d <= tol r holds with equality or by one ulp
+    st, it, _ = step(fresh(), np.nextafter(t, 0.0), 50)
+    assert it > 1                                                    # one ulp below: the first iterate is not accepted
+    # tol < 0: never, whatever d and r are; status 1 and exactly max_iters iterations
+    assert step(fresh(), -1.0, 4)[:2] == (1, 4)
+    assert step(fresh(), -0.0, 3)[0] in (0, 1)                       # -0.0 >= 0 is true: behaves as tol = 0
+    # tol = 0: converged only when the iterate stops changing bit for bit
+    o = fresh()
+    st, it, res = step(o, 0.0, 100_000)
+    assert st == 0 and res == 0.0 and it > 10                        # d == 0 exactly, reached only after many iterations
+    # r = 0 and d = 0 (all-zero problem): converged at the first iteration, resid = d = 0
+    z = Oracle(np.ones(3), np.ones(3), np.full(3, 0.5), 1.0, 1.0, 2)
+    z.setup()
+    z.set_flux(np.zeros((3, 2, 2)))
+    assert step(z, 1e-10, 100) == (0, 1, 0.0)
+    # r = 0 at tol = 0 as well (0 <= 0 * 0)
+    z.set_flux(np.zeros((3, 2, 2)))
+    assert step(z, 0.0, 100)[:2] == (0, 1)
