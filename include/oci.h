@@ -31,6 +31,13 @@
  * still committed); negative = failure, no state change:
  *   -1 invalid argument   -2 call order   -3 CUDA error
  *   -4 singular block     -5 workspace too small
+ *   -6 OCI_E_NONFINITE: the scalar flux became NaN or Inf inside a step (a
+ *      non-finite psi_edge or Q, or overflow); the iteration loop stops at
+ *      once on the device, the state is undefined, restart with oci_set_flux.
+ * Devices: the context belongs to the device its workspace lives on
+ * (oci_setup); every entry point makes that device current for the duration
+ * of the call and restores the caller's, so contexts on several devices can
+ * live in one process.
  * No exception crosses the ABI.  oci_last_error() describes the last failure.
  */
 #ifndef OCI_B200_H
@@ -45,7 +52,7 @@ extern "C" {
 typedef struct oci_ctx oci_ctx;
 
 enum { OCI_OK = 0, OCI_NOT_CONVERGED = 1, OCI_E_INVALID = -1, OCI_E_ORDER = -2, OCI_E_CUDA = -3,
-       OCI_E_SINGULAR = -4, OCI_E_WORKSPACE = -5 };
+       OCI_E_SINGULAR = -4, OCI_E_WORKSPACE = -5, OCI_E_NONFINITE = -6 };
 
 /* Boundary conditions (vacuum and reflecting P:31).
  * INCIDENT_ISOTROPIC: `value` is the incident ANGULAR flux psi_m for every
@@ -109,8 +116,9 @@ typedef struct {
 
 /* Problem statement (per-cell dx_j, Sigma_j, Sigma_s,j P:74-82).
  * dx, sigma_t, sigma_s: HOST [cells].  v = particle speed, dt = time step.
- * n_angles = N (even, >= 2).  Computes the Gauss-Legendre set on the host.
- * Errors: -1 if cells<1, N odd or <2, any dx<=0, Sigma<0, Sigma_s<0, v<=0,
+ * n_angles = N (even, 2 <= N <= 512: the setup and per-cell kernels stage O(4N)
+ * doubles per CTA in shared memory).  Computes the Gauss-Legendre set on the host.
+ * Errors: -1 if cells<1, N odd, <2 or >512, any dx<=0, Sigma<0, Sigma_s<0, v<=0,
  * dt<=0, a NULL pointer or an unknown BC kind. */
 int oci_create(oci_ctx** out, int64_t cells, const double* dx, const double* sigma_t,
                const double* sigma_s, double v, double dt, int32_t n_angles, oci_bc left,
@@ -147,7 +155,13 @@ int oci_set_source_dev(oci_ctx* ctx, const double* d_q);
  * step's psi_{k-1/2}.  tol < 0 never converges: exactly max_iters iterations.
  * iters (HOST, may be NULL): iterations done.  resid (HOST, may be NULL):
  * last d/r (d if r == 0).  One host read-back per call (per launch chunk).
- * Returns 0, 1 (OCI_NOT_CONVERGED), -1, -2, -3. */
+ * Stream order: everything is queued on the context's stream.  In the REDUCED
+ * form oci_step returns as soon as the iteration count is known, which is
+ * BEFORE its last kernel (the FINAL pass, which writes the I rows of Psi) has
+ * finished; every later call on this context is ordered behind it, but a
+ * caller that reads the workspace from ANOTHER stream must synchronise with
+ * the context's stream first.
+ * Returns 0, 1 (OCI_NOT_CONVERGED), -1, -2, -3, -6. */
 int oci_step(oci_ctx* ctx, double tol, int32_t max_iters, int32_t* iters, double* resid);
 int si_step(oci_ctx* ctx, double tol, int32_t max_iters, int32_t* iters, double* resid);
 
@@ -183,11 +197,6 @@ int oci_get_kernel_time(oci_ctx* ctx, double* ms, int64_t* launches);
  * (which then counts the ITER kernel).  Any pointer may be NULL. */
 int oci_get_aux_kernel_time(oci_ctx* ctx, double* fix_ms, int64_t* fix_launches, double* final_ms,
                             int64_t* final_launches);
-
-/* Roofline denominator for the SHARED path: sustained fp64 tensor-pipe (DMMA) issue rate of the
- * current device in TFLOP/s, measured by a registers-only probe kernel (about 0.1 s).
- * d_scratch: DEVICE, >= 8 bytes.  cuda_stream: cudaStream_t or NULL.  No context needed. */
-int oci_probe_fp64_tensor_tflops(void* d_scratch, void* cuda_stream, double* tflops);
 
 /* Number of kernels this library launched on this context so far. */
 int64_t oci_launch_count(const oci_ctx* ctx);

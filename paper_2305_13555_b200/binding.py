@@ -13,14 +13,13 @@ PATH_SHARED, PATH_PER_CELL = 0, 1
 KERNEL_GENERIC, KERNEL_RESIDENT, KERNEL_KTILED, KERNEL_PER_CELL = 0, 1, 2, 3
 ITERATION_FULL, ITERATION_REDUCED, ITERATION_AUTO = 0, 1, 2
 RKERNEL_GEMV, RKERNEL_RESIDENT, RKERNEL_KTILED = 0, 1, 2
-RKERNEL_GEMV, RKERNEL_RESIDENT, RKERNEL_KTILED = 0, 1, 2
 
 EXPORTED_SYMBOLS = [
     "oci_create", "oci_workspace_bytes", "oci_setup", "oci_set_flux", "oci_set_flux_dev", "oci_set_source",
     "oci_set_source_dev", "oci_step", "si_step", "oci_get_scalar_flux", "oci_get_angular_flux",
     "oci_get_scalar_flux_dev", "oci_get_angular_flux_dev", "oci_get_quadrature", "oci_get_info",
     "oci_get_block_inverse", "oci_enable_kernel_timing", "oci_get_kernel_time", "oci_get_aux_kernel_time", "oci_set_iteration", "oci_launch_count",
-    "oci_probe_fp64_tensor_tflops", "oci_last_error", "oci_destroy",
+    "oci_last_error", "oci_destroy",
 ]
 
 
@@ -90,8 +89,6 @@ def load_library():
     L.oci_get_aux_kernel_time.argtypes = [vp, _dp, C.POINTER(i64), _dp, C.POINTER(i64)]
     L.oci_set_iteration.restype = C.c_int
     L.oci_set_iteration.argtypes = [vp, i32]
-    L.oci_probe_fp64_tensor_tflops.restype = C.c_int
-    L.oci_probe_fp64_tensor_tflops.argtypes = [vp, vp, _dp]
     L.oci_launch_count.restype = i64
     L.oci_launch_count.argtypes = [vp]
     L.oci_last_error.restype = C.c_char_p
@@ -106,10 +103,20 @@ def _hp(a):
     return a.ctypes.data_as(_dp)
 
 
+_probe = None
+
+
 def probe_fp64_tensor_tflops(device="cuda:0") -> float:
-    """oci_probe_fp64_tensor_tflops on torch's current stream."""
+    """fp64 tensor-pipe (DMMA) issue rate of `device` in TFLOP/s, from the measurement probe liboci_probe.so
+    (not part of the product ABI), on torch's current stream."""
     import torch
-    L = load_library()
+    global _probe
+    if _probe is None:
+        _build.build()
+        _probe = C.CDLL(_build.PROBE_LIB)
+        _probe.oci_probe_fp64_tensor_tflops.restype = C.c_int
+        _probe.oci_probe_fp64_tensor_tflops.argtypes = [C.c_void_p, C.c_void_p, _dp]
+    L = _probe
     dev = torch.device(device)
     with torch.cuda.device(dev):
         scratch = torch.zeros(8, dtype=torch.float64, device=dev)

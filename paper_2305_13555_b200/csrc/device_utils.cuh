@@ -12,7 +12,7 @@ __device__ __forceinline__ bool step_done(const unsigned long long* __restrict__
     if (prev_slot < 0) return false;
     double d = __longlong_as_double((long long)__ldcg(norms + 2 * prev_slot + 0));
     double r = __longlong_as_double((long long)__ldcg(norms + 2 * prev_slot + 1));
-    return converged(tol, d, r);
+    return stop_now(tol, d, r);
 }
 
 // FIX pass of the reduced step (first kernel of every oci_step in that form): CTA 0 also clears the norm slots
@@ -25,6 +25,77 @@ __device__ __forceinline__ void clear_step_state(const DevView& V)
     }
 }
 
+// ---- shared-memory / mbarrier / TMA wrappers (one PTX instruction each), used by every TMA-fed kernel
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// 1-D bulk TMA global -> shared, completion on an mbarrier (SASS UBLKCP)
+__device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+// 2-D tensor-map TMA box global -> shared (SASS UTMALDG); c0 = column (inner), c1 = row of the box origin
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+            smem_u32(dst)),
+        "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(smem_u32(bar))
+        : "memory");
+}
+// the same with an L2 cache policy (createpolicy): which operand should stay in L2 and which should stream
+__device__ __forceinline__ void tma_load_2d_hint(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar, uint64_t policy)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;" ::"r"(
+            smem_u32(dst)),
+        "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(smem_u32(bar)), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_last()
+{
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first()
+{
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+// generic-proxy accesses of shared memory (LDS / STS) ordered before async-proxy ones (the TMA unit)
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void named_bar_sync(int id, int threads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+
 // max over non-negative doubles through their (order-preserving) bit patterns: exact and
 // independent of the reduction order, so host and device agree on the iteration count.
 __device__ __forceinline__ void atomic_max_nonneg(unsigned long long* addr, double v)
@@ -35,10 +106,19 @@ __device__ __forceinline__ void atomic_max_nonneg(unsigned long long* addr, doub
     if (bits > __ldcg(addr)) atomicMax(addr, bits);
 }
 
+// max of two values that are each non-negative (fabs applied) or NaN, taken on the bit patterns as integers:
+// the pattern of a non-negative double is monotone in its value, +inf sorts above every finite number and NaN
+// (0x7ff8...) above +inf, so a non-finite scalar flux reaches the host instead of being dropped the way fmax
+// drops a NaN.  Integer compare + select also keeps these off the fp64 pipe the DMMAs run on.
+__device__ __forceinline__ double nanmax(double a, double b)
+{
+    return __longlong_as_double(max(__double_as_longlong(a), __double_as_longlong(b)));
+}
+
 __device__ __forceinline__ double warp_max(double v)
 {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    for (int o = 16; o > 0; o >>= 1) v = nanmax(v, __shfl_xor_sync(0xffffffffu, v, o));
     return v;
 }
 
@@ -94,7 +174,7 @@ __device__ __forceinline__ int first_converged(const unsigned long long* __restr
     for (int i = 0; i < cnt; ++i) {
         const double d = __longlong_as_double((long long)__ldcg(norms + 2 * i + 0));
         const double r = __longlong_as_double((long long)__ldcg(norms + 2 * i + 1));
-        if (converged(tol, d, r)) return i + 1;
+        if (stop_now(tol, d, r)) return i + 1;
     }
     return 0;
 }

@@ -41,6 +41,7 @@ struct oci_ctx {
     alignas(64) RedKtiledMaps rmaps{};
     alignas(64) RedResidentMaps rrmaps{};
     bool use_ktiled = false;
+    int device = -1;                   // the device the workspace lives on; made current inside every entry point
     cudaStream_t stream = nullptr;
     void* ws = nullptr;
     int64_t ws_bytes = 0;
@@ -87,6 +88,30 @@ int cuda_fail(const oci_ctx* c, cudaError_t e, const char* where)
         cudaError_t e_ = (call);                                      \
         if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);      \
     } while (0)
+
+// a launcher returns the number of kernels it launched, or -1 when CUDA refused a launch
+#define LAUNCH(call)                                                  \
+    do {                                                              \
+        const int k_ = (call);                                        \
+        if (k_ < 0) return cuda_fail(ctx, cudaGetLastError(), #call); \
+        ctx->launches += k_;                                          \
+    } while (0)
+
+// Makes the context's device current for the duration of an entry point (the caller's current device need not
+// be the one the workspace lives on) and restores the previous one on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const oci_ctx* c)
+    {
+        if (c && c->device >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != c->device)
+            switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DeviceGuard()
+    {
+        if (switched) cudaSetDevice(prev);
+    }
+};
 
 // N-point Gauss-Legendre nodes and weights on [-1,1], ascending (weights sum to 2, the 1/2 of
 // eq. (1)).  Newton on P_N evaluated by the Bonnet recurrence, from the Tricomi initial guess;
@@ -158,10 +183,7 @@ Layout make_layout(int64_t J, int32_t N, int64_t nblk)
     L.w = take(N * 8);
     L.coef = take(n * 8);
     L.ainv4 = take(nblk * N * 16 * 8);
-    {
-        const int S = si_chunk_cells(J, N);
-        L.si_scan = take(((J + S - 1) / S) * N * 8 * 8);
-    }
+    L.si_scan = take(((J + 7) / 8) * N * 8 * 8);          // sized for the smallest chunk si_chunk_cells() can pick
     L.phi_part = take(nblk == 1 ? ((n + 127) / 128) * J * 4 * 8 : 0);
     L.norms = take((kNormSlots + 1) * 2 * 8);
     L.tickets = take(nblk == 1 ? ((J + 63) / 64) * 4 : 0);
@@ -229,9 +251,9 @@ int launch_oci_iteration_any(oci_ctx* ctx, int src, int slot, int prev_slot, dou
     if (ctx->path == OCI_PATH_PER_CELL) return launch_oci_percell(V, src, slot, prev_slot, tol, ctx->stream);
     if (oci_shared_fast_supported(V)) return launch_oci_shared_fast(V, src, slot, prev_slot, tol, ctx->stream);
     if (ctx->use_ktiled) return launch_oci_ktiled(V, ctx->maps, src, slot, prev_slot, tol, ctx->stream);
-    int k = launch_oci_generic(V, src, prev_slot, tol, ctx->stream);
-    k += launch_phi_norm(V, src ^ 1, slot, prev_slot, tol, true, ctx->stream);
-    return k;
+    const int k = launch_oci_generic(V, src, prev_slot, tol, ctx->stream);
+    const int k2 = launch_phi_norm(V, src ^ 1, slot, prev_slot, tol, true, ctx->stream);
+    return (k < 0 || k2 < 0) ? -1 : k + k2;
 }
 
 // AUTO: the reduced form wherever a kernel of that form is the faster one (oci.h)
@@ -256,8 +278,9 @@ int launch_reduced_pass(oci_ctx* ctx, int pass, int ybase, int slot, int prev_sl
 int ensure_psi(oci_ctx* ctx)
 {
     if (ctx->psi_valid) return 0;
-    ctx->psi_valid = true;
-    return launch_unpack_yz(ctx->V, ctx->cur, ctx->ycur, ctx->stream);
+    const int k = launch_unpack_yz(ctx->V, ctx->cur, ctx->ycur, ctx->stream);
+    if (k >= 0) ctx->psi_valid = true;
+    return k;
 }
 
 int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iters, double* resid)
@@ -266,6 +289,7 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
     if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "step before oci_setup");
     if (!ctx->have_flux) return fail(ctx, OCI_E_ORDER, "step before oci_set_flux");
     if (max_iters < 1 || tol != tol) return fail(ctx, OCI_E_INVALID, "max_iters < 1 or tol is NaN");
+    DeviceGuard guard(ctx);
     DevView& V = ctx->V;
     cudaStream_t s = ctx->stream;
     const bool red = !si && resolved_iteration(ctx) == OCI_ITERATION_REDUCED;
@@ -273,18 +297,18 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
 
     if (red) {
         if (!ctx->yz_valid) {
-            ctx->launches += launch_pack_yz(V, ctx->cur, 0, s);
+            LAUNCH(launch_pack_yz(V, ctx->cur, 0, s));
             ctx->ycur = 0;
             ctx->yz_valid = true;
         }
         ctx->psi_valid = false;
         if (timed) CK(cudaEventRecord(ctx->ev_aux[0], s));
-        ctx->launches += launch_reduced_pass(ctx, PASS_FIX, ctx->ycur, 0, -1, tol, 0, 0);   // a2 (+ a8 of the previous step)
+        LAUNCH(launch_reduced_pass(ctx, PASS_FIX, ctx->ycur, 0, -1, tol, 0, 0));   // a2 (+ a8 of the previous step)
         if (timed) CK(cudaEventRecord(ctx->ev_aux[1], s));
     } else {
-        ctx->launches += ensure_psi(ctx);
+        LAUNCH(ensure_psi(ctx));
         ctx->yz_valid = false;
-        ctx->launches += launch_cfix(V, ctx->cur, s);                      // a2 (+ a8 of the previous step)
+        LAUNCH(launch_cfix(V, ctx->cur, s));                      // a2 (+ a8 of the previous step)
     }
     int32_t done_iters = 0;
     bool conv = false;
@@ -304,14 +328,14 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
         if (fused_loop) {
             if (done_iters > 0) CK(cudaMemsetAsync(V.flags + 8, 0, 4, s));  // the grid barrier's arrival counter
             if (timed) CK(cudaEventRecord(ctx->ev[0], s));
-            ctx->launches += launch_reduced_pass(ctx, PASS_ITER, (ctx->ycur + done_iters) & 1, 0, -1, tol, cnt, 0);
+            LAUNCH(launch_reduced_pass(ctx, PASS_ITER, (ctx->ycur + done_iters) & 1, 0, -1, tol, cnt, 0));
             if (timed) CK(cudaEventRecord(ctx->ev[1], s));
         }
         for (int32_t i = 0; i < cnt && !fused_loop; ++i) {
             if (timed) CK(cudaEventRecord(ctx->ev[2 * i], s));
-            if (si) ctx->launches += launch_si_iteration(V, ctx->cur, i, i - 1, tol, s);
-            else if (red) ctx->launches += launch_reduced_pass(ctx, PASS_ITER, (ctx->ycur + done_iters + i) & 1, i, i - 1, tol, 0, 0);
-            else ctx->launches += launch_oci_iteration_any(ctx, (ctx->cur + done_iters + i) & 1, i, i - 1, tol);
+            if (si) LAUNCH(launch_si_iteration(V, ctx->cur, i, i - 1, tol, s));
+            else if (red) LAUNCH(launch_reduced_pass(ctx, PASS_ITER, (ctx->ycur + done_iters + i) & 1, i, i - 1, tol, 0, 0));
+            else LAUNCH(launch_oci_iteration_any(ctx, (ctx->cur + done_iters + i) & 1, i, i - 1, tol));
             if (timed) CK(cudaEventRecord(ctx->ev[2 * i + 1], s));
         }
         // The norms are final once the iteration launches are done.  REDUCED form: their read-back goes through a
@@ -327,7 +351,7 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
             // finalisation, queued before the read-back: finds the last iteration on the device and
             // does nothing if this chunk neither converged nor ends at max_iters
             if (timed) CK(cudaEventRecord(ctx->ev_aux[2], s));
-            ctx->launches += launch_reduced_pass(ctx, PASS_FINAL, (ctx->ycur + done_iters) & 1, 0, -1, tol, cnt, done_iters + cnt >= max_iters);
+            LAUNCH(launch_reduced_pass(ctx, PASS_FINAL, (ctx->ycur + done_iters) & 1, 0, -1, tol, cnt, done_iters + cnt >= max_iters));
             if (timed) CK(cudaEventRecord(ctx->ev_aux[3], s));
         }
         if (side_readback) {
@@ -341,7 +365,7 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
         for (int32_t i = 0; i < cnt; ++i) {
             std::memcpy(&d, &ctx->h_norms[2 * i], 8);
             std::memcpy(&r, &ctx->h_norms[2 * i + 1], 8);
-            if (converged(tol, d, r)) { conv = true; executed = i + 1; break; }
+            if (stop_now(tol, d, r)) { conv = true; executed = i + 1; break; }
         }
         if (timed && fused_loop) {
             float ms = 0.f;
@@ -375,6 +399,10 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
     else if (!si) ctx->cur = (ctx->cur + done_iters) & 1;                  // a8: pointer convention
     ctx->predicted[si ? 1 : 0] = done_iters;
     if (iters) *iters = done_iters;
+    if (!finite_norms(d, r)) {
+        if (resid) *resid = d;
+        return fail(ctx, OCI_E_NONFINITE, "the scalar flux became NaN or Inf (non-finite input or overflow); restart with oci_set_flux");
+    }
     if (resid) *resid = (r > 0.0) ? d / r : d;
     return conv ? OCI_OK : OCI_NOT_CONVERGED;
 }
@@ -389,7 +417,7 @@ int oci_create(oci_ctx** out, int64_t cells, const double* dx, const double* sig
     if (!out) return OCI_E_INVALID;
     *out = nullptr;
     if (cells < 1 || !dx || !sigma_t || !sigma_s) return OCI_E_INVALID;
-    if (n_angles < 2 || (n_angles & 1) || n_angles > 4096) return OCI_E_INVALID;
+    if (n_angles < 2 || (n_angles & 1) || n_angles > 512) return OCI_E_INVALID;   // oci.h: kernels stage O(4N) doubles per CTA
     if (!(v > 0.0) || !(dt > 0.0) || !std::isfinite(v) || !std::isfinite(dt)) return OCI_E_INVALID;
     if (!bc_ok(left) || !bc_ok(right) || !std::isfinite(left.value) || !std::isfinite(right.value))
         return OCI_E_INVALID;
@@ -429,6 +457,15 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     if (bytes < L.total) return fail(ctx, OCI_E_WORKSPACE, "workspace too small");
     ctx->ready = false;
     ctx->have_flux = false;
+    {
+        // the device the workspace lives on is the context's device from here on
+        cudaPointerAttributes pa{};
+        CK(cudaPointerGetAttributes(&pa, d_workspace));
+        if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)
+            return fail(ctx, OCI_E_INVALID, "workspace is not device memory");
+        ctx->device = pa.device;
+    }
+    DeviceGuard guard(ctx);
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->ws = d_workspace;
     ctx->ws_bytes = bytes;
@@ -472,6 +509,19 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     V.v = ctx->v; V.dt = ctx->dt;
     V.bcL = ctx->bcL.kind; V.bcR = ctx->bcR.kind;
     V.bcLv = ctx->bcL.value; V.bcRv = ctx->bcR.value;
+    {
+        int sms = 0, coop = 0;
+        CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device));
+        CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device));
+        V.sm_count = sms;
+        ctx->coop = coop != 0;
+        // more than 48 KB of dynamic shared memory is a per-device, per-kernel opt-in
+        CK(oci_shared_fast_opt_in());
+        CK(oci_ktiled_opt_in());
+        CK(oci_red_gemv_opt_in());
+        CK(oci_red_ktiled_opt_in());
+        CK(oci_red_resident_opt_in());
+    }
 
     cudaStream_t s = ctx->stream;
     // coef[4m+s] = |mu_m| on the rows that take an incident flux (eqs. 27,28), else 0
@@ -521,8 +571,8 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
         CK(cudaStreamSynchronize(s));
     }
 
-    ctx->launches += launch_form_and_invert(V, s);                       // a0, a1
-    ctx->launches += launch_pack_operators(V, s);                        // f1: G, H, F
+    LAUNCH(launch_form_and_invert(V, s));                                // a0, a1
+    LAUNCH(launch_pack_operators(V, s));                                 // f1: G, H, F
     int32_t flag = 0;
     CK(cudaMemcpyAsync(&flag, V.flags, 4, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
@@ -547,12 +597,6 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     ctx->red_kernel = (oci_red_resident_supported(V) && oci_red_resident_prepare(V, &ctx->rrmaps)) ? OCI_RKERNEL_RESIDENT
                       : (oci_red_ktiled_supported(V) && oci_red_ktiled_prepare(V, &ctx->rmaps)) ? OCI_RKERNEL_KTILED
                                                                                                  : OCI_RKERNEL_GEMV;
-    {
-        int dev = 0, coop = 0;
-        CK(cudaGetDevice(&dev));
-        CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
-        ctx->coop = coop != 0;
-    }
     ctx->cur = 0;
     ctx->ycur = 0;
     ctx->yz_valid = false;
@@ -564,11 +608,11 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
 
 static int set_flux_common(oci_ctx* ctx, const double* d_edge)
 {
-    ctx->launches += launch_set_flux(ctx->V, d_edge, 0, ctx->stream);
+    LAUNCH(launch_set_flux(ctx->V, d_edge, 0, ctx->stream));
     ctx->cur = 0;
     ctx->yz_valid = false;
     ctx->psi_valid = true;
-    ctx->launches += launch_phi_norm(ctx->V, 0, 0, -1, -1.0, false, ctx->stream);   // phi^(0), ghost rows
+    LAUNCH(launch_phi_norm(ctx->V, 0, 0, -1, -1.0, false, ctx->stream));   // phi^(0), ghost rows
     CK(cudaStreamSynchronize(ctx->stream));
     CK(cudaGetLastError());
     ctx->have_flux = true;
@@ -579,6 +623,7 @@ int oci_set_flux(oci_ctx* ctx, const double* psi_edge)
 {
     if (!ctx || !psi_edge) return fail(ctx, OCI_E_INVALID, "NULL argument");
     if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_set_flux before oci_setup");
+    DeviceGuard guard(ctx);
     // stage through c_fix (recomputed at the start of every step, and at least as large)
     CK(cudaMemcpyAsync(ctx->V.cfix, psi_edge, (size_t)ctx->J * ctx->N * 2 * 8, cudaMemcpyHostToDevice, ctx->stream));
     return set_flux_common(ctx, ctx->V.cfix);
@@ -588,6 +633,7 @@ int oci_set_flux_dev(oci_ctx* ctx, const double* d_psi_edge)
 {
     if (!ctx || !d_psi_edge) return fail(ctx, OCI_E_INVALID, "NULL argument");
     if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_set_flux_dev before oci_setup");
+    DeviceGuard guard(ctx);
     return set_flux_common(ctx, d_psi_edge);
 }
 
@@ -603,6 +649,7 @@ int oci_set_source(oci_ctx* ctx, const double* q)
 {
     if (!ctx) return OCI_E_INVALID;
     if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_set_source before oci_setup");
+    DeviceGuard guard(ctx);
     if (q) CK(cudaMemcpyAsync(ctx->V.Q, q, (size_t)ctx->J * 4 * 8, cudaMemcpyHostToDevice, ctx->stream));
     else CK(cudaMemsetAsync(ctx->V.Q, 0, (size_t)ctx->J * 4 * 8, ctx->stream));
     if (int rc = refresh_q16(ctx)) return rc;
@@ -614,6 +661,7 @@ int oci_set_source_dev(oci_ctx* ctx, const double* d_q)
 {
     if (!ctx) return OCI_E_INVALID;
     if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_set_source_dev before oci_setup");
+    DeviceGuard guard(ctx);
     if (d_q) CK(cudaMemcpyAsync(ctx->V.Q, d_q, (size_t)ctx->J * 4 * 8, cudaMemcpyDeviceToDevice, ctx->stream));
     else CK(cudaMemsetAsync(ctx->V.Q, 0, (size_t)ctx->J * 4 * 8, ctx->stream));
     return refresh_q16(ctx);
@@ -629,10 +677,19 @@ int si_step(oci_ctx* ctx, double tol, int32_t max_iters, int32_t* iters, double*
     return run_step(ctx, true, tol, max_iters, iters, resid);
 }
 
+static int unpack_for_get(oci_ctx* ctx)
+{
+    if (!ctx || !ctx->ready) return OCI_OK;          // get_common reports these
+    DeviceGuard guard(ctx);
+    LAUNCH(ensure_psi(ctx));
+    return OCI_OK;
+}
+
 static int get_common(const oci_ctx* ctx, double* dst, const double* src, size_t bytes, cudaMemcpyKind kind, bool sync)
 {
     if (!ctx || !dst) return fail(ctx, OCI_E_INVALID, "NULL argument");
     if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "get before oci_setup");
+    DeviceGuard guard(ctx);
     CK(cudaMemcpyAsync(dst, src, bytes, kind, ctx->stream));
     if (sync) CK(cudaStreamSynchronize(ctx->stream));
     return OCI_OK;
@@ -644,7 +701,7 @@ int oci_get_scalar_flux(const oci_ctx* ctx, double* phi)
 }
 int oci_get_angular_flux(const oci_ctx* ctx, double* psi)
 {
-    if (ctx && ctx->ready) const_cast<oci_ctx*>(ctx)->launches += ensure_psi(const_cast<oci_ctx*>(ctx));
+    if (int rc = unpack_for_get(const_cast<oci_ctx*>(ctx))) return rc;
     return get_common(ctx, psi, ctx ? ctx->V.psi[ctx->cur] : nullptr, ctx ? (size_t)ctx->J * ctx->n * 8 : 0,
                       cudaMemcpyDeviceToHost, true);
 }
@@ -654,7 +711,7 @@ int oci_get_scalar_flux_dev(const oci_ctx* ctx, double* d_phi)
 }
 int oci_get_angular_flux_dev(const oci_ctx* ctx, double* d_psi)
 {
-    if (ctx && ctx->ready) const_cast<oci_ctx*>(ctx)->launches += ensure_psi(const_cast<oci_ctx*>(ctx));
+    if (int rc = unpack_for_get(const_cast<oci_ctx*>(ctx))) return rc;
     return get_common(ctx, d_psi, ctx ? ctx->V.psi[ctx->cur] : nullptr, ctx ? (size_t)ctx->J * ctx->n * 8 : 0,
                       cudaMemcpyDeviceToDevice, false);
 }
@@ -689,6 +746,7 @@ int oci_get_block_inverse(const oci_ctx* ctx, int64_t blk, double* binv)
     if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_get_block_inverse before oci_setup");
     if (blk < 0 || blk >= ctx->nblk) return fail(ctx, OCI_E_INVALID, "block index out of range");
     const size_t nn = (size_t)ctx->n * ctx->n;
+    DeviceGuard guard(ctx);
     CK(cudaMemcpyAsync(binv, ctx->V.binv + (size_t)blk * nn, nn * 8, cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     return OCI_OK;
@@ -743,6 +801,7 @@ const char* oci_last_error(const oci_ctx* ctx) { return ctx ? ctx->err.c_str() :
 void oci_destroy(oci_ctx* ctx)
 {
     if (!ctx) return;
+    DeviceGuard guard(ctx);
     if (ctx->h_norms) cudaFreeHost(ctx->h_norms);
     if (ctx->stream2) cudaStreamDestroy(ctx->stream2);
     if (ctx->ev_norms) cudaEventDestroy(ctx->ev_norms);

@@ -59,6 +59,7 @@ struct DevView {
     double v, dt;
     int32_t bcL, bcR;
     double bcLv, bcRv;
+    int32_t sm_count;           // SMs of the device the workspace lives on (queried once in oci_setup)
 };
 
 // Tensor maps of the K-tiled shared-block kernel (oci_iter_shared_ktiled.cu), encoded once in oci_setup.
@@ -84,19 +85,32 @@ struct RedResidentMaps {
 
 // The stopping rule (reading S2), evaluated identically on host and device.
 __host__ __device__ inline bool converged(double tol, double d, double r) { return tol >= 0.0 && d <= tol * r; }
+// A NaN or Inf scalar flux (non-finite input, overflow) also ends the iteration loop, on the device as on the
+// host: the step then returns OCI_E_NONFINITE instead of running to max_iters on garbage.
+__host__ __device__ inline bool finite_norms(double d, double r) { return d <= 1.7976931348623157e308 && r <= 1.7976931348623157e308; }
+__host__ __device__ inline bool stop_now(double tol, double d, double r) { return converged(tol, d, r) || !finite_norms(d, r); }
 
 // Cells per chunk of the SI scan (si_sweep.cu): one chunk for tiny slabs (launch-latency bound), else
 // the largest of 64, 32, 16, 8 that still gives every SM about 8 warps of (chunk, angle) threads.
-inline int si_chunk_cells(int64_t J, int32_t N)
+inline int si_chunk_cells(int64_t J, int32_t N, int sm_count = 148)
 {
     if (J <= 32) return (int)J;
     const int64_t lanes = N >= 32 ? (N + 31) / 32 * 32 : N;
     for (int S = 64; S > 8; S >>= 1)
-        if (((J + S - 1) / S) * lanes >= (int64_t)148 * 8 * 32) return S;
+        if (((J + S - 1) / S) * lanes >= (int64_t)sm_count * 8 * 32) return S;
     return 8;
 }
 
-// ---- launchers (each returns the number of kernels it launched) ----
+// ---- launchers: each returns the number of kernels it launched, or -1 when a launch was refused (the CUDA
+// error stays readable through cudaGetLastError)
+inline int launched(int k) { return cudaPeekAtLastError() == cudaSuccess ? k : -1; }
+// Opt-in to more than 48 KB of dynamic shared memory for every kernel of a file that needs it.  The attribute is
+// per device, so oci_setup calls these with the context's device current (no per-process caching).
+cudaError_t oci_shared_fast_opt_in();
+cudaError_t oci_ktiled_opt_in();
+cudaError_t oci_red_gemv_opt_in();
+cudaError_t oci_red_ktiled_opt_in();
+cudaError_t oci_red_resident_opt_in();
 int launch_form_and_invert(const DevView& V, cudaStream_t s);
 int launch_set_flux(const DevView& V, const double* d_psi_edge, int buf, cudaStream_t s);
 int launch_cfix(const DevView& V, int buf, cudaStream_t s);

@@ -91,7 +91,7 @@ int launch_oci_generic(const DevView& V, int src, int prev_slot, double tol, cud
 {
     dim3 grid((unsigned)((V.J + TM - 1) / TM), (unsigned)((V.n + TN - 1) / TN));
     oci_iter_generic_kernel<<<grid, 256, 0, s>>>(V, src, prev_slot, tol);
-    return 1;
+    return launched(1);
 }
 
 }  // namespace oci

@@ -96,7 +96,7 @@ int launch_oci_percell(const DevView& V, int src, int slot, int prev_slot, doubl
 {
     size_t smem = sizeof(double) * 2 * V.n;
     oci_iter_percell_kernel<4><<<(unsigned)V.J, 256, smem, s>>>(V, src, slot, prev_slot, tol);
-    return 1;
+    return launched(1);
 }
 
 }  // namespace oci

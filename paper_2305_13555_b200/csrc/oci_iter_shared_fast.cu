@@ -28,46 +28,6 @@ constexpr int TM = 32;        // cells per tile
 constexpr int CSLOTS = 4;    // RHS tiles in flight (loaded / assembled / in the DMMAs)
 constexpr int PSLOTS = 2;    // neighbour half-row tiles in flight (dead once the RHS is assembled)
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-// 1-D bulk TMA global -> shared, completion on an mbarrier (SASS UBLKCP)
-__device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-// 16-byte asynchronous copy global -> shared (SASS LDGSTS), L2-cached only
-__device__ __forceinline__ void fence_proxy_async()
-{
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-}
-
 #ifdef OCI_DBG_TRACE
 #define TRACE(slotidx)                                                                        \
     do {                                                                                      \
@@ -228,8 +188,8 @@ oci_iter_resident_kernel(DevView V, int src, int slot, int prev_slot, double tol
             for (int w8 = 0; w8 < 8; ++w8) s += pp[w8 * TM * 4];
             const bool ok = valid && tid < TM * 4 && (tid >> 2) < tile_rows(it);
             if (ok) V.phi[tile_j0(it) * 4 + tid] = s;
-            dmax = ok ? fmax(dmax, fabs(s - old)) : dmax;
-            rmax = ok ? fmax(rmax, fabs(s)) : rmax;
+            dmax = ok ? nanmax(dmax, fabs(s - old)) : dmax;
+            rmax = ok ? nanmax(rmax, fabs(s)) : rmax;
         };
         auto load_phi_old = [&](int it) {
             return (it < my_tiles && tid < TM * 4 && (tid >> 2) < tile_rows(it)) ? V.phi[tile_j0(it) * 4 + tid] : 0.0;
@@ -349,30 +309,22 @@ bool oci_shared_fast_supported(const DevView& V) { return V.nblk == 1 && (V.n ==
 
 int launch_oci_shared_fast(const DevView& V, int src, int slot, int prev_slot, double tol, cudaStream_t s)
 {
-    static int sm_count = 0;
-    if (sm_count == 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
-    }
+    const int sm_count = V.sm_count;
     const int64_t ntiles = (V.J + TM - 1) / TM;
     const unsigned grid = (unsigned)(ntiles < sm_count ? ntiles : sm_count);
     if (V.n == 128) {
-        static bool attr = false;
-        if (!attr) {
-            cudaFuncSetAttribute(oci_iter_resident_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<128>::SMEM);
-            attr = true;
-        }
         oci_iter_resident_kernel<128><<<grid, 384, Cfg<128>::SMEM, s>>>(V, src, slot, prev_slot, tol);
     } else {
-        static bool attr = false;
-        if (!attr) {
-            cudaFuncSetAttribute(oci_iter_resident_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<64>::SMEM);
-            attr = true;
-        }
         oci_iter_resident_kernel<64><<<grid, 384, Cfg<64>::SMEM, s>>>(V, src, slot, prev_slot, tol);
     }
-    return 1;
+    return launched(1);
+}
+
+cudaError_t oci_shared_fast_opt_in()
+{
+    cudaError_t e = cudaFuncSetAttribute(oci_iter_resident_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<128>::SMEM);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(oci_iter_resident_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<64>::SMEM);
 }
 
 }  // namespace oci

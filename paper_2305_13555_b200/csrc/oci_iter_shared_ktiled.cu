@@ -40,43 +40,6 @@ constexpr int KT_MAX_N = 1024;
 constexpr size_t KT_SMEM = 1024 /*alignment slack*/ + (size_t)KT_STAGES * KT_STAGE_BYTES + 4 * KT_M * 4 * 8 /*phi_s*/ +
                            KT_MAX_N * 8 /*coef*/ + 3 * KT_STAGES * 8 + 64;
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
-            smem_u32(dst)),
-        "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(smem_u32(bar))
-        : "memory");
-}
-__device__ __forceinline__ void named_bar_sync(int id, int threads)
-{
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
-}
 
 }  // namespace
 
@@ -279,8 +242,8 @@ oci_iter_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_cfix, 
             if (last && j < J) {
                 const double old = V.phi[j * 4 + (tid & 3)];
                 V.phi[j * 4 + (tid & 3)] = ssum;
-                dmax = fmax(dmax, fabs(ssum - old));
-                rmax = fmax(rmax, fabs(ssum));
+                dmax = nanmax(dmax, fabs(ssum - old));
+                rmax = nanmax(rmax, fabs(ssum));
             }
             named_bar_sync(1, 256);                                  // phi_s / ticket_s reusable
         }
@@ -346,21 +309,16 @@ bool oci_ktiled_prepare(const DevView& V, KtiledMaps* M)
 
 int launch_oci_ktiled(const DevView& V, const KtiledMaps& M, int src, int slot, int prev_slot, double tol, cudaStream_t s)
 {
-    static int sm_count = 0;
-    static bool attr = false;
-    if (sm_count == 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
-    }
-    if (!attr) {
-        cudaFuncSetAttribute(oci_iter_ktiled_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)KT_SMEM);
-        attr = true;
-    }
+    const int sm_count = V.sm_count;
     const int64_t nitems = ((V.J + KT_M - 1) / KT_M) * ((V.n + KT_N - 1) / KT_N);
     const unsigned grid = (unsigned)(nitems < sm_count ? nitems : sm_count);
     oci_iter_ktiled_kernel<<<grid, 288, KT_SMEM, s>>>(V, M.cfix, M.psi[src], M.binv, src, slot, prev_slot, tol);
-    return 1;
+    return launched(1);
+}
+
+cudaError_t oci_ktiled_opt_in()
+{
+    return cudaFuncSetAttribute(oci_iter_ktiled_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)KT_SMEM);
 }
 
 }  // namespace oci

@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(256) pack_operators_kernel(DevView V)
 int launch_pack_operators(const DevView& V, cudaStream_t s)
 {
     pack_operators_kernel<<<(unsigned)V.nblk, 256, 0, s>>>(V);
-    return 1;
+    return launched(1);
 }
 
 // ---- (y[ybuf], z) <- Psi[buf], ghost rows of y included (after set_flux / si_step / a FULL-form step)
@@ -153,7 +153,7 @@ int launch_pack_yz(const DevView& V, int buf, int ybuf, cudaStream_t s)
 {
     const int64_t tot = (V.J + 2) * (V.n >> 1);
     pack_yz_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, s>>>(V, buf, ybuf);
-    return 1;
+    return launched(1);
 }
 
 // ---- Psi[buf] <- (y[ybuf], z): the full layout on demand; the ghost rows of Psi take the O entries
@@ -176,7 +176,7 @@ int launch_unpack_yz(const DevView& V, int buf, int ybuf, cudaStream_t s)
 {
     const int64_t tot = (V.J + 2) * (V.n >> 1);
     unpack_yz_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, s>>>(V, buf, ybuf);
-    return 1;
+    return launched(1);
 }
 
 // ---- the three passes as a batched GEMV (PASS_* of oci_internal.h), HBM-bound when every cell has its own
@@ -210,7 +210,7 @@ __global__ void __launch_bounds__(256, 2) oci_red_gemv_kernel(DevView V, int yba
             if (i < cnt) {
                 const double d = __longlong_as_double((long long)__ldcg(V.norms + 2 * i + 0));
                 const double r = __longlong_as_double((long long)__ldcg(V.norms + 2 * i + 1));
-                hit = converged(tol, d, r);
+                hit = stop_now(tol, d, r);
             }
             const unsigned m = __ballot_sync(0xffffffffu, hit);
             if (m) L = i0 + __ffs(m);
@@ -348,8 +348,8 @@ __global__ void __launch_bounds__(256, 2) oci_red_gemv_kernel(DevView V, int yba
                 } else {
                     const double a = add + o;
                     V.phi[j * 4 + (i - K2)] = a;
-                    dmax = fmax(dmax, fabs(a - old));
-                    rmax = fmax(rmax, fabs(a));
+                    dmax = nanmax(dmax, fabs(a - old));
+                    rmax = nanmax(rmax, fabs(a));
                 }
             }
             ki = 0;
@@ -398,17 +398,7 @@ int launch_red_gemv(const DevView& V, int pass, int ybase, int slot, int prev_sl
     int nwarp = 8;
     while (nwarp > 1 && (size_t)nwarp * (K2 + 8) * 8 > 100 * 1024) nwarp >>= 1;
     const size_t smem = sizeof(double) * (size_t)nwarp * (K2 + 8);
-    static bool attr = false;
-    static int sm_count = 148;
-    if (!attr) {
-        cudaFuncSetAttribute(oci_red_gemv_kernel<PASS_FIX, GR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
-        cudaFuncSetAttribute(oci_red_gemv_kernel<PASS_ITER, GR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
-        cudaFuncSetAttribute(oci_red_gemv_kernel<PASS_FINAL, GR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
-        attr = true;
-    }
+    const int sm_count = V.sm_count;
     // one wave: every CTA resident, the stream cut into equal pieces
     int per_sm = 1;
     if (pass == PASS_FIX) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, oci_red_gemv_kernel<PASS_FIX, GR>, nwarp * 32, smem);
@@ -427,7 +417,19 @@ int launch_red_gemv(const DevView& V, int pass, int ybase, int slot, int prev_sl
         cudaLaunchCooperativeKernel((const void*)oci_red_gemv_kernel<PASS_ITER, GR>, dim3(grid), dim3(block), args, smem, s);
     } else if (pass == PASS_ITER) oci_red_gemv_kernel<PASS_ITER, GR><<<grid, block, smem, s>>>(V, ybase, slot, prev_slot, tol, 0, 0);
     else oci_red_gemv_kernel<PASS_FINAL, GR><<<grid, block, smem, s>>>(V, ybase, 0, -1, tol, cnt, force);
-    return 1;
+    return launched(1);
+}
+
+cudaError_t oci_red_gemv_opt_in()
+{
+    constexpr int GR = 8;
+    cudaError_t e = cudaSuccess;
+    const auto at = cudaFuncAttributeMaxDynamicSharedMemorySize;
+    if ((e = cudaFuncSetAttribute(oci_red_gemv_kernel<PASS_FIX, GR>, at, 100 * 1024)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(oci_red_gemv_kernel<PASS_ITER, GR>, at, 100 * 1024)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(oci_red_gemv_kernel<PASS_FINAL, GR>, at, 100 * 1024)) != cudaSuccess)
+        return e;
+    return e;
 }
 
 }  // namespace oci

@@ -46,44 +46,6 @@ constexpr int RK_STAGE_BYTES = RK_A_BYTES + RK_B_BYTES + RK_P_BYTES + 1024;   //
 constexpr size_t RK_SMEM = 1024 /*alignment slack*/ + (size_t)RK_STAGES * RK_STAGE_BYTES + 2 * 4 * RK_M * 4 * 8 /*phi_s, 2 buffers*/ +
                            2 * RK_STAGES * 8 + 64;
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
-            smem_u32(dst)),
-        "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(smem_u32(bar))
-        : "memory");
-}
-__device__ __forceinline__ void named_bar_sync(int id, int threads)
-{
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
-}
-
 }  // namespace
 
 template <int PASS>
@@ -337,8 +299,8 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
                 } else {
                     const double a = pfix + ssum;
                     V.phi[j * 4 + (tid & 3)] = a;
-                    dmax = fmax(dmax, fabs(a - pold));
-                    rmax = fmax(rmax, fabs(a));
+                    dmax = nanmax(dmax, fabs(a - pold));
+                    rmax = nanmax(rmax, fabs(a));
                 }
             }
         }
@@ -630,8 +592,8 @@ oci_red_ktiled_pp_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, c
                     } else {
                         const double a = pfix[u] + ssum;
                         V.phi[j * 4 + (p & 3)] = a;
-                        dmax = fmax(dmax, fabs(a - pold[u]));
-                        rmax = fmax(rmax, fabs(a));
+                        dmax = nanmax(dmax, fabs(a - pold[u]));
+                        rmax = nanmax(rmax, fabs(a));
                     }
                 }
             }
@@ -668,19 +630,7 @@ bool oci_red_ktiled_prepare(const DevView& V, RedKtiledMaps* M)
 int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int ybase, int slot, int prev_slot, double tol, int cnt,
                       int force, cudaStream_t s)
 {
-    static int sm_count = 0;
-    static bool attr = false;
-    if (sm_count == 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
-    }
-    if (!attr) {
-        cudaFuncSetAttribute(oci_red_ktiled_kernel<PASS_FIX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RK_SMEM);
-        cudaFuncSetAttribute(oci_red_ktiled_kernel<PASS_ITER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RK_SMEM);
-        cudaFuncSetAttribute(oci_red_ktiled_kernel<PASS_FINAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RK_SMEM);
-        attr = true;
-    }
+    const int sm_count = V.sm_count;
     const int K2 = V.n / 2;
     const int64_t nitems = (V.gitems ? V.ngroups : (V.J + RK_M - 1) / RK_M) * (((pass == PASS_FIX ? 2 * K2 : K2) + RK_N - 1) / RK_N);
     const unsigned grid = (unsigned)(nitems < sm_count ? nitems : sm_count);
@@ -689,20 +639,13 @@ int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int yb
     // ping-pong kernel when both math groups of every CTA get at least one item, else the eight-warp kernel
     const bool pp = nitems >= 2 * (int64_t)grid;
     if (pp) {
-        static bool attr_pp = false;
-        if (!attr_pp) {
-            cudaFuncSetAttribute(oci_red_ktiled_pp_kernel<PASS_FIX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RP_SMEM);
-            cudaFuncSetAttribute(oci_red_ktiled_pp_kernel<PASS_ITER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RP_SMEM);
-            cudaFuncSetAttribute(oci_red_ktiled_pp_kernel<PASS_FINAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RP_SMEM);
-            attr_pp = true;
-        }
         if (pass == PASS_FIX)
             oci_red_ktiled_pp_kernel<PASS_FIX><<<grid, 384, RP_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.xop, M.xop8, ybase, 0, -1, tol, 0, 0);
         else if (pass == PASS_ITER)
             oci_red_ktiled_pp_kernel<PASS_ITER><<<grid, 384, RP_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.rop, M.rop8, ybase, slot, prev_slot, tol, 0, 0);
         else
             oci_red_ktiled_pp_kernel<PASS_FINAL><<<grid, 384, RP_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.fop, M.fop, ybase, 0, -1, tol, cnt, force);
-        return 1;
+        return launched(1);
     }
     if (pass == PASS_FIX)
         oci_red_ktiled_kernel<PASS_FIX><<<grid, 384, RK_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.xop, M.xop8, ybase, 0, -1, tol, 0, 0);
@@ -710,7 +653,21 @@ int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int yb
         oci_red_ktiled_kernel<PASS_ITER><<<grid, 384, RK_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.rop, M.rop8, ybase, slot, prev_slot, tol, 0, 0);
     else
         oci_red_ktiled_kernel<PASS_FINAL><<<grid, 384, RK_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.fop, M.fop, ybase, 0, -1, tol, cnt, force);
-    return 1;
+    return launched(1);
+}
+
+cudaError_t oci_red_ktiled_opt_in()
+{
+    cudaError_t e = cudaSuccess;
+    const auto at = cudaFuncAttributeMaxDynamicSharedMemorySize;
+    if ((e = cudaFuncSetAttribute(oci_red_ktiled_kernel<PASS_FIX>, at, (int)RK_SMEM)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(oci_red_ktiled_kernel<PASS_ITER>, at, (int)RK_SMEM)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(oci_red_ktiled_kernel<PASS_FINAL>, at, (int)RK_SMEM)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(oci_red_ktiled_pp_kernel<PASS_FIX>, at, (int)RP_SMEM)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(oci_red_ktiled_pp_kernel<PASS_ITER>, at, (int)RP_SMEM)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(oci_red_ktiled_pp_kernel<PASS_FINAL>, at, (int)RP_SMEM)) != cudaSuccess)
+        return e;
+    return e;
 }
 
 }  // namespace oci

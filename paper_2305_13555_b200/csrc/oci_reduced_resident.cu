@@ -35,37 +35,6 @@ constexpr int RT_M = 16;       // cells per warp tile
 constexpr int RT_WARPS = 8;
 constexpr int RT_STAGES = 2;
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
-            smem_u32(dst)),
-        "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(smem_u32(bar))
-        : "memory");
-}
-
-
 template <int K2, int PASS>
 struct RCfg {
     static constexpr int N = K2 / 2;
@@ -179,8 +148,8 @@ __device__ __forceinline__ void phase(double (&acc)[2][NBC][2], const double* __
                     if (PK == PK_ITER) {
                         const double p0 = pf[g].x + pend[g][NBP - 1][0], p1 = pf[g].y + pend[g][NBP - 1][1];
                         *reinterpret_cast<double2*>(E.phi + pj[g] * 4 + 2 * t4) = make_double2(p0, p1);
-                        dmax = fmax(dmax, fmax(fabs(p0 - po[g].x), fabs(p1 - po[g].y)));
-                        rmax = fmax(rmax, fmax(fabs(p0), fabs(p1)));
+                        dmax = nanmax(dmax, nanmax(fabs(p0 - po[g].x), fabs(p1 - po[g].y)));
+                        rmax = nanmax(rmax, nanmax(fabs(p0), fabs(p1)));
                     } else {
                         *reinterpret_cast<double2*>(E.phifix_out + pj[g] * 4 + 2 * t4) = make_double2(pend[g][NBP - 1][0], pend[g][NBP - 1][1]);
                     }
@@ -443,18 +412,7 @@ template <int K2, int PASS>
 void launch_rr(const DevView& V, const RedResidentMaps& M, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
                cudaStream_t s)
 {
-    static int sm_count = 0;
-    static bool attr = false;
-    if (sm_count == 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
-    }
-    if (!attr) {
-        cudaFuncSetAttribute(oci_red_resident_kernel<K2, PASS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)RCfg<K2, PASS>::SMEM);
-        attr = true;
-    }
+    const int sm_count = V.sm_count;
     const int64_t ntiles = (V.J + RT_M - 1) / RT_M;
     const unsigned grid = (unsigned)(ntiles < sm_count ? ntiles : sm_count);
     const int b = ybase & 1;
@@ -467,7 +425,7 @@ void launch_rr(const DevView& V, const RedResidentMaps& M, int ybase, int slot, 
         CUtensorMap a0 = ya, a1 = yb, a2 = M.z_half, a3 = M.q, a4 = op, a5 = M.xop_phi;
         void* args[] = {&Vv, &a0, &a1, &a2, &a3, &a4, &a5, &ybase, &slot, &prev_slot, &tol, &cnt, &force};
         cudaLaunchCooperativeKernel((const void*)oci_red_resident_kernel<K2, PASS>, dim3(grid), dim3(RT_WARPS * 32), args,
-                                    RCfg<K2, PASS>::SMEM, s);
+                                    RCfg<K2, PASS>::SMEM, s);     // a refused launch is picked up by launched()
         return;
     }
     oci_red_resident_kernel<K2, PASS><<<grid, RT_WARPS * 32, RCfg<K2, PASS>::SMEM, s>>>(V, ya, yb, M.z_half, M.q, op, M.xop_phi, ybase,
@@ -489,7 +447,25 @@ int launch_red_resident(const DevView& V, const RedResidentMaps& M, int pass, in
 {
     if (V.n == 128) launch_rr_pass<64>(V, M, pass, ybase, slot, prev_slot, tol, cnt, force, s);
     else launch_rr_pass<32>(V, M, pass, ybase, slot, prev_slot, tol, cnt, force, s);
-    return 1;
+    return launched(1);
+}
+
+namespace {
+template <int K2, int PASS>
+cudaError_t opt_in_rr()
+{
+    return cudaFuncSetAttribute(oci_red_resident_kernel<K2, PASS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RCfg<K2, PASS>::SMEM);
+}
+}  // namespace
+
+cudaError_t oci_red_resident_opt_in()
+{
+    cudaError_t e = cudaSuccess;
+    if ((e = opt_in_rr<64, PASS_FIX>()) != cudaSuccess || (e = opt_in_rr<64, PASS_ITER>()) != cudaSuccess ||
+        (e = opt_in_rr<64, PASS_FINAL>()) != cudaSuccess || (e = opt_in_rr<32, PASS_FIX>()) != cudaSuccess ||
+        (e = opt_in_rr<32, PASS_ITER>()) != cudaSuccess || (e = opt_in_rr<32, PASS_FINAL>()) != cudaSuccess)
+        return e;
+    return e;
 }
 
 }  // namespace oci

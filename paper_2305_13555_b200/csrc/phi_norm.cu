@@ -76,8 +76,8 @@ __global__ void __launch_bounds__(256, 2) phi_norm_kernel(DevView V, int buf, in
             if (j < V.J) {
                 if (lane < 2) {
                     *reinterpret_cast<double2*>(V.phi + j * 4 + 2 * lane) = make_double2(a0[c], a1[c]);
-                    dmax = fmax(dmax, fmax(fabs(a0[c] - oldv[c].x), fabs(a1[c] - oldv[c].y)));
-                    rmax = fmax(rmax, fmax(fabs(a0[c]), fabs(a1[c])));
+                    dmax = nanmax(dmax, nanmax(fabs(a0[c] - oldv[c].x), fabs(a1[c] - oldv[c].y)));
+                    rmax = nanmax(rmax, nanmax(fabs(a0[c]), fabs(a1[c])));
                 }
                 if (j == 0 || j == V.J - 1) refresh_ghost_rows(V, P, j, lane);
             }
@@ -90,7 +90,7 @@ __global__ void __launch_bounds__(256, 2) phi_norm_kernel(DevView V, int buf, in
         if (lane == 0) { sd[warp] = dmax; sr[warp] = rmax; }
         __syncthreads();
         if (threadIdx.x == 0) {
-            for (int q = 1; q < 8; ++q) { dmax = fmax(dmax, sd[q]); rmax = fmax(rmax, sr[q]); }
+            for (int q = 1; q < 8; ++q) { dmax = nanmax(dmax, sd[q]); rmax = nanmax(rmax, sr[q]); }
             atomic_max_nonneg(&V.norms[2 * slot + 0], dmax);
             atomic_max_nonneg(&V.norms[2 * slot + 1], rmax);
         }
@@ -101,10 +101,10 @@ int launch_phi_norm(const DevView& V, int buf, int slot, int prev_slot, double t
                     cudaStream_t s)
 {
     int64_t blocks = (V.J + 63) / 64;
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > (int64_t)V.sm_count * 16) blocks = (int64_t)V.sm_count * 16;
     if (with_norms) phi_norm_kernel<true><<<(unsigned)blocks, 256, 0, s>>>(V, buf, slot, prev_slot, tol);
     else phi_norm_kernel<false><<<(unsigned)blocks, 256, 0, s>>>(V, buf, slot, prev_slot, tol);
-    return 1;
+    return launched(1);
 }
 
 }  // namespace oci

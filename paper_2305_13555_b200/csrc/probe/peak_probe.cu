@@ -3,9 +3,18 @@
 // 16 warps x 2 CTAs per SM, 8 independent accumulator chains per warp, registers only.
 #include <cstdio>
 
-#include "device_utils.cuh"
+#include <cuda_runtime.h>
+#include <stdint.h>
 
-namespace oci {
+namespace oci_probe {
+
+// D(8x8) += A(8x4, row) * B(4x8, col), fp64 tensor pipe (SASS DMMA.8x8x4)
+__device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
 
 __global__ void __launch_bounds__(512) dmma_issue_kernel(double* out, int iters, double a0, double b0)
 {
@@ -23,24 +32,25 @@ __global__ void __launch_bounds__(512) dmma_issue_kernel(double* out, int iters,
     if (s == 123.456) out[0] = s;   // keep the chains alive without a store in the common case
 }
 
-}  // namespace oci
+}  // namespace oci_probe
 
+// Returns 0, -1 (NULL argument) or -3 (CUDA error).  d_scratch: DEVICE, 8 doubles; tflops: HOST.
 extern "C" int oci_probe_fp64_tensor_tflops(void* d_scratch, void* cuda_stream, double* tflops)
 {
-    if (!tflops || !d_scratch) return OCI_E_INVALID;
+    if (!tflops || !d_scratch) return -1;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return OCI_E_CUDA;
-    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return OCI_E_CUDA;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -3;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -3;
     cudaEvent_t e0, e1;
-    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return OCI_E_CUDA;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return -3;
     const int iters = 40000, grid = sms * 2;
     double best = 0.0;
     for (int rep = 0; rep < 4; ++rep) {
         cudaEventRecord(e0, s);
-        oci::dmma_issue_kernel<<<grid, 512, 0, s>>>((double*)d_scratch, iters, 1.0000001, 0.9999999);
+        oci_probe::dmma_issue_kernel<<<grid, 512, 0, s>>>((double*)d_scratch, iters, 1.0000001, 0.9999999);
         cudaEventRecord(e1, s);
-        if (cudaEventSynchronize(e1) != cudaSuccess) return OCI_E_CUDA;
+        if (cudaEventSynchronize(e1) != cudaSuccess) return -3;
         float ms = 0.f;
         cudaEventElapsedTime(&ms, e0, e1);
         const double fl = 2.0 * 256.0 * 8.0 * (double)iters * 16.0 * grid;
@@ -49,7 +59,7 @@ extern "C" int oci_probe_fp64_tensor_tflops(void* d_scratch, void* cuda_stream, 
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    if (cudaGetLastError() != cudaSuccess) return OCI_E_CUDA;
+    if (cudaGetLastError() != cudaSuccess) return -3;
     *tflops = best;
-    return OCI_OK;
+    return 0;
 }

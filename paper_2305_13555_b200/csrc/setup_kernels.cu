@@ -191,7 +191,7 @@ int launch_form_and_invert(const DevView& V, cudaStream_t s)
     invert_blocks_kernel<T><<<(unsigned)V.nblk, T, smem, s>>>(V);
     int64_t tot = V.nblk * V.N;
     ainv4_kernel<<<(unsigned)((tot + 127) / 128), 128, 0, s>>>(V);
-    return 3;
+    return launched(3);
 }
 
 // set_flux: seed the iterate from the corner values at the previous time edge (reading S3):
@@ -222,7 +222,7 @@ int launch_set_flux(const DevView& V, const double* d_psi_edge, int buf, cudaStr
 {
     int64_t tot = V.J * V.n;
     set_flux_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, s>>>(V, d_psi_edge, buf);
-    return 1;
+    return launched(1);
 }
 
 // a2: c_fix[j][4m+s] = (h/4) Q[j][s] + (s<2 ? alpha * psi_{k-1/2}[j][m][s] : 0), where psi_{k-1/2} is the
@@ -248,7 +248,7 @@ int launch_cfix(const DevView& V, int buf, cudaStream_t s)
 {
     int64_t tot = V.J * V.N;
     cfix_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, s>>>(V, buf);
-    return 1;
+    return launched(1);
 }
 
 }  // namespace oci

@@ -212,24 +212,24 @@ __global__ void __launch_bounds__(256) si_carry_kernel(DevView V, int buf, int p
 
 int launch_si_iteration(const DevView& V, int buf, int slot, int prev_slot, double tol, cudaStream_t s)
 {
-    const int S = si_chunk_cells(V.J, V.N);
+    const int S = si_chunk_cells(V.J, V.N, V.sm_count);
     const int C = (int)((V.J + S - 1) / S);
     int Nr = 32;
     if (V.N >= 32) Nr = (V.N + 31) / 32 * 32;
     else while (Nr / 2 >= V.N) Nr /= 2;
     const int64_t threads = (int64_t)C * Nr;
     const unsigned blocks = (unsigned)((threads + 127) / 128);
-    int launched = 0;
+    int nlaunch = 0;
     if (C > 1) {
         if (V.nblk == 1) si_chunk_kernel<8, true, 1><<<blocks, 128, 0, s>>>(V, buf, prev_slot, tol, S, C, Nr);
         else si_chunk_kernel<4, false, 1><<<blocks, 128, 0, s>>>(V, buf, prev_slot, tol, S, C, Nr);
         si_carry_kernel<<<(unsigned)V.N, 256, 0, s>>>(V, buf, prev_slot, tol, C);
-        launched += 2;
+        nlaunch += 2;
     }
     if (V.nblk == 1) si_chunk_kernel<8, true, 3><<<blocks, 128, 0, s>>>(V, buf, prev_slot, tol, S, C, Nr);
     else si_chunk_kernel<4, false, 3><<<blocks, 128, 0, s>>>(V, buf, prev_slot, tol, S, C, Nr);
-    launched += 1 + launch_phi_norm(V, buf, slot, prev_slot, tol, true, s);
-    return launched;
+    nlaunch += 1 + launch_phi_norm(V, buf, slot, prev_slot, tol, true, s);
+    return launched(nlaunch);
 }
 
 }  // namespace oci

@@ -32,7 +32,7 @@ def test_library_exports_every_declared_symbol():
 
 def test_binding_methods_follow_the_header_names():
     for nm in declared_symbols():
-        if nm in ("oci_create", "oci_destroy", "oci_last_error", "oci_probe_fp64_tensor_tflops"):
+        if nm in ("oci_create", "oci_destroy", "oci_last_error"):
             continue
         meth = nm if nm in ("oci_step", "si_step") else nm[len("oci_"):]
         assert hasattr(P.OCI, meth), meth
@@ -51,7 +51,7 @@ def test_device_library_quadrature_matches_numpy(N):
 
 @pytest.mark.parametrize("kw", [
     dict(dx=[0.0, 1.0]), dict(dx=[-1.0, 1.0]), dict(st=[-0.1, 1.0]), dict(ss=[1.0, -2.0]), dict(v=0.0), dict(dt=0.0),
-    dict(dt=float("nan")), dict(N=3), dict(N=0), dict(N=1), dict(bcL=(7, 0.0)), dict(bcR=(1, float("inf"))),
+    dict(dt=float("nan")), dict(N=3), dict(N=0), dict(N=1), dict(N=514), dict(bcL=(7, 0.0)), dict(bcR=(1, float("inf"))),
     dict(dx=[float("nan"), 1.0]),
 ])
 def test_create_rejects_invalid_arguments(kw):

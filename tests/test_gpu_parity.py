@@ -234,6 +234,20 @@ def test_api_errors_on_device():
     assert e.value.code == -1
     assert g.oci_step()[0] == 0
     g.close()
+    # a non-finite input must surface as OCI_E_NONFINITE (-6), not as a "converged" step with a NaN flux
+    for bad in (np.nan, np.inf):
+        for scheme in ("oci", "si"):
+            h = P.OCI(np.ones(40), np.ones(40), np.full(40, 0.5), 1.0, 0.1, 4)
+            h.setup()
+            e0 = np.ones((40, 4, 2))
+            e0[17, 2, 1] = bad
+            h.set_flux(e0)
+            with pytest.raises(P.OCIError) as e:
+                (h.oci_step if scheme == "oci" else h.si_step)(1e-10, 10_000)
+            assert e.value.code == -6, (bad, scheme)
+            h.set_flux(np.ones((40, 4, 2)))                  # restart with finite data works
+            assert (h.oci_step if scheme == "oci" else h.si_step)(1e-10, 10_000)[0] == 0
+            h.close()
     # singular block: Sigma = 0, dt = huge, reflecting-free pure streaming is still non-singular, so
     # build a genuinely singular one: Sigma_s = Sigma with dt -> infinity (infinite medium, c = 1)
     s = P.OCI(np.ones(2), np.ones(2), np.ones(2), 1.0, 1e300, 2)
