@@ -100,8 +100,11 @@ enum { OCI_ITERATION_FULL = 0, OCI_ITERATION_REDUCED = 1, OCI_ITERATION_AUTO = 2
  * RESIDENT - shared block, n in {64,128}: operators resident in shared memory, fp64 tensor pipe;
  * KTILED - shared block, or 2..16 distinct blocks (a multi-region slab), N a multiple of 16: operands
  *          streamed in K chunks by tensor-map TMA, fp64 tensor pipe; a block is a row offset into the
- *          stacked operators, a tile of cells that straddles an interface is done once per block. */
-enum { OCI_RKERNEL_GEMV = 0, OCI_RKERNEL_RESIDENT = 1, OCI_RKERNEL_KTILED = 2 };
+ *          stacked operators, a tile of cells that straddles an interface is done once per block;
+ * OPREG - ONE shared block, N in {64, 128} (config 4): each CTA keeps 64 operator rows as DMMA fragments in
+ *          registers for the whole launch and only the cell rows stream (tensor-map TMA); fp64 tensor pipe.
+ * oci_setup picks RESIDENT, else OPREG, else KTILED, else GEMV; oci_set_reduced_kernel overrides. */
+enum { OCI_RKERNEL_AUTO = -1, OCI_RKERNEL_GEMV = 0, OCI_RKERNEL_RESIDENT = 1, OCI_RKERNEL_KTILED = 2, OCI_RKERNEL_OPREG = 3 };
 
 typedef struct {
     int64_t cells;        /* J */
@@ -168,6 +171,11 @@ int si_step(oci_ctx* ctx, double tol, int32_t max_iters, int32_t* iters, double*
 /* Select the form of the OCI iteration (default OCI_ITERATION_AUTO).  May be called at any time
  * after oci_create; takes effect at the next oci_step.  Errors: -1. */
 int oci_set_iteration(oci_ctx* ctx, int32_t iteration);
+
+/* Force the kernel family of the REDUCED form (default OCI_RKERNEL_AUTO).  Call BEFORE oci_setup; oci_setup
+ * returns -1 if the forced family does not serve this problem (block size, number of blocks).  For tests and
+ * for comparing families on shapes more than one serves.  Errors: -1 (unknown family). */
+int oci_set_reduced_kernel(oci_ctx* ctx, int32_t kernel);
 
 /* Results of the current state.  phi: [cells][4] (eq. 18);
  * psi: [cells][N][4].  HOST pointers; _dev variants take DEVICE pointers and

@@ -12,13 +12,13 @@ BC_VACUUM, BC_INCIDENT_ISOTROPIC, BC_REFLECTING = 0, 1, 2
 PATH_SHARED, PATH_PER_CELL = 0, 1
 KERNEL_GENERIC, KERNEL_RESIDENT, KERNEL_KTILED, KERNEL_PER_CELL = 0, 1, 2, 3
 ITERATION_FULL, ITERATION_REDUCED, ITERATION_AUTO = 0, 1, 2
-RKERNEL_GEMV, RKERNEL_RESIDENT, RKERNEL_KTILED = 0, 1, 2
+RKERNEL_AUTO, RKERNEL_GEMV, RKERNEL_RESIDENT, RKERNEL_KTILED, RKERNEL_OPREG = -1, 0, 1, 2, 3
 
 EXPORTED_SYMBOLS = [
     "oci_create", "oci_workspace_bytes", "oci_setup", "oci_set_flux", "oci_set_flux_dev", "oci_set_source",
     "oci_set_source_dev", "oci_step", "si_step", "oci_get_scalar_flux", "oci_get_angular_flux",
     "oci_get_scalar_flux_dev", "oci_get_angular_flux_dev", "oci_get_quadrature", "oci_get_info",
-    "oci_get_block_inverse", "oci_enable_kernel_timing", "oci_get_kernel_time", "oci_get_aux_kernel_time", "oci_set_iteration", "oci_launch_count",
+    "oci_get_block_inverse", "oci_enable_kernel_timing", "oci_get_kernel_time", "oci_get_aux_kernel_time", "oci_set_iteration", "oci_set_reduced_kernel", "oci_launch_count",
     "oci_last_error", "oci_destroy",
 ]
 
@@ -89,6 +89,8 @@ def load_library():
     L.oci_get_aux_kernel_time.argtypes = [vp, _dp, C.POINTER(i64), _dp, C.POINTER(i64)]
     L.oci_set_iteration.restype = C.c_int
     L.oci_set_iteration.argtypes = [vp, i32]
+    L.oci_set_reduced_kernel.restype = C.c_int
+    L.oci_set_reduced_kernel.argtypes = [vp, i32]
     L.oci_launch_count.restype = i64
     L.oci_launch_count.argtypes = [vp]
     L.oci_last_error.restype = C.c_char_p
@@ -149,10 +151,12 @@ class OCI:
         self._ws = None
 
     @classmethod
-    def from_problem(cls, p, device="cuda:0", set_flux=True, iteration=None):
+    def from_problem(cls, p, device="cuda:0", set_flux=True, iteration=None, reduced_kernel=None):
         o = cls(p.dx, p.sigma_t, p.sigma_s, p.v, p.dt, p.n_angles, p.bc_left, p.bc_right)
         if iteration is not None:
             o.set_iteration(iteration)
+        if reduced_kernel is not None:
+            o.set_reduced_kernel(reduced_kernel)
         o.setup(device)
         if set_flux:
             o.set_flux(p.psi0)
@@ -277,6 +281,9 @@ class OCI:
 
     def set_iteration(self, iteration):
         self._check(self._L.oci_set_iteration(self._h, int(iteration)))
+
+    def set_reduced_kernel(self, kernel):
+        self._check(self._L.oci_set_reduced_kernel(self._h, int(kernel)))
 
     def launch_count(self):
         return int(self._L.oci_launch_count(self._h))

@@ -40,7 +40,9 @@ struct oci_ctx {
     alignas(64) KtiledMaps maps{};
     alignas(64) RedKtiledMaps rmaps{};
     alignas(64) RedResidentMaps rrmaps{};
+    alignas(64) RedOpregMaps romaps{};
     bool use_ktiled = false;
+    int32_t forced_rkernel = OCI_RKERNEL_AUTO;   // oci_set_reduced_kernel
     int device = -1;                   // the device the workspace lives on; made current inside every entry point
     cudaStream_t stream = nullptr;
     void* ws = nullptr;
@@ -269,6 +271,8 @@ int launch_reduced_pass(oci_ctx* ctx, int pass, int ybase, int slot, int prev_sl
 {
     if (ctx->red_kernel == OCI_RKERNEL_KTILED)
         return launch_red_ktiled(ctx->V, ctx->rmaps, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
+    if (ctx->red_kernel == OCI_RKERNEL_OPREG)
+        return launch_red_opreg(ctx->V, ctx->romaps, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
     if (ctx->red_kernel == OCI_RKERNEL_RESIDENT)
         return launch_red_resident(ctx->V, ctx->rrmaps, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
     return launch_red_gemv(ctx->V, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
@@ -521,6 +525,7 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
         CK(oci_red_gemv_opt_in());
         CK(oci_red_ktiled_opt_in());
         CK(oci_red_resident_opt_in());
+        CK(oci_red_opreg_opt_in());
     }
 
     cudaStream_t s = ctx->stream;
@@ -594,9 +599,20 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     }
     ctx->use_ktiled = ctx->path == OCI_PATH_SHARED && !oci_shared_fast_supported(V) && oci_ktiled_supported(V) &&
                       oci_ktiled_prepare(V, &ctx->maps);
-    ctx->red_kernel = (oci_red_resident_supported(V) && oci_red_resident_prepare(V, &ctx->rrmaps)) ? OCI_RKERNEL_RESIDENT
-                      : (oci_red_ktiled_supported(V) && oci_red_ktiled_prepare(V, &ctx->rmaps)) ? OCI_RKERNEL_KTILED
-                                                                                                 : OCI_RKERNEL_GEMV;
+    {
+        const int32_t want = ctx->forced_rkernel;
+        auto may = [&](int32_t k) { return want == OCI_RKERNEL_AUTO || want == k; };
+        if (may(OCI_RKERNEL_RESIDENT) && oci_red_resident_supported(V) && oci_red_resident_prepare(V, &ctx->rrmaps))
+            ctx->red_kernel = OCI_RKERNEL_RESIDENT;
+        else if (may(OCI_RKERNEL_OPREG) && oci_red_opreg_supported(V) && oci_red_opreg_prepare(V, &ctx->romaps))
+            ctx->red_kernel = OCI_RKERNEL_OPREG;
+        else if (may(OCI_RKERNEL_KTILED) && oci_red_ktiled_supported(V) && oci_red_ktiled_prepare(V, &ctx->rmaps))
+            ctx->red_kernel = OCI_RKERNEL_KTILED;
+        else if (may(OCI_RKERNEL_GEMV))
+            ctx->red_kernel = OCI_RKERNEL_GEMV;
+        else
+            return fail(ctx, OCI_E_INVALID, "the kernel family forced with oci_set_reduced_kernel does not serve this problem");
+    }
     ctx->cur = 0;
     ctx->ycur = 0;
     ctx->yz_valid = false;
@@ -640,7 +656,7 @@ int oci_set_flux_dev(oci_ctx* ctx, const double* d_psi_edge)
 // Q padded to one 128-byte row per cell for the K-tiled FIX pass (a strided copy, the pad stays zero)
 static int refresh_q16(oci_ctx* ctx)
 {
-    if (ctx->red_kernel != OCI_RKERNEL_KTILED) return OCI_OK;
+    if (ctx->red_kernel != OCI_RKERNEL_KTILED && ctx->red_kernel != OCI_RKERNEL_OPREG) return OCI_OK;
     CK(cudaMemcpy2DAsync(ctx->V.q16, 128, ctx->V.Q, 32, 32, (size_t)ctx->J, cudaMemcpyDeviceToDevice, ctx->stream));
     return OCI_OK;
 }
@@ -781,6 +797,14 @@ int oci_set_iteration(oci_ctx* ctx, int32_t iteration)
     if (iteration != OCI_ITERATION_FULL && iteration != OCI_ITERATION_REDUCED && iteration != OCI_ITERATION_AUTO)
         return fail(ctx, OCI_E_INVALID, "unknown iteration form");
     ctx->iteration = iteration;
+    return OCI_OK;
+}
+
+int oci_set_reduced_kernel(oci_ctx* ctx, int32_t kernel)
+{
+    if (!ctx) return OCI_E_INVALID;
+    if (kernel < OCI_RKERNEL_AUTO || kernel > OCI_RKERNEL_OPREG) return fail(ctx, OCI_E_INVALID, "unknown kernel family");
+    ctx->forced_rkernel = kernel;
     return OCI_OK;
 }
 

@@ -72,6 +72,11 @@ struct RedKtiledMaps {
     CUtensorMap y[2], z, q16, xop, xop8, rop, rop8, fop;
 };
 
+// Tensor maps of the operator-in-registers kernels of the reduced step (oci_reduced_opreg.cu): boxes of 64 rows x 16 columns
+struct RedOpregMaps {
+    CUtensorMap y[2], z, q16, yfix, ifix;
+};
+
 // Tensor maps of the resident kernels of the reduced step (oci_reduced_resident.cu)
 struct RedResidentMaps {
     CUtensorMap y_rows[2];   // box (K2+4) x 18: whole rows j0-1 .. j0+16 of y, padded pitch (ITER, FINAL)
@@ -111,6 +116,7 @@ cudaError_t oci_ktiled_opt_in();
 cudaError_t oci_red_gemv_opt_in();
 cudaError_t oci_red_ktiled_opt_in();
 cudaError_t oci_red_resident_opt_in();
+cudaError_t oci_red_opreg_opt_in();
 int launch_form_and_invert(const DevView& V, cudaStream_t s);
 int launch_set_flux(const DevView& V, const double* d_psi_edge, int buf, cudaStream_t s);
 int launch_cfix(const DevView& V, int buf, cudaStream_t s);
@@ -136,6 +142,10 @@ bool oci_red_ktiled_supported(const DevView& V);
 bool oci_red_ktiled_prepare(const DevView& V, RedKtiledMaps* M);
 int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int ybase, int slot, int prev_slot, double tol,
                       int cnt, int force, cudaStream_t s);
+bool oci_red_opreg_supported(const DevView& V);
+bool oci_red_opreg_prepare(const DevView& V, RedOpregMaps* M);
+int launch_red_opreg(const DevView& V, const RedOpregMaps& M, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
+                     cudaStream_t s);
 bool oci_red_resident_supported(const DevView& V);
 bool oci_red_resident_prepare(const DevView& V, RedResidentMaps* M);
 int launch_red_resident(const DevView& V, const RedResidentMaps& M, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,

@@ -21,13 +21,13 @@ FULL, REDUCED = 0, 1
 ITERATIONS = [pytest.param(FULL, id="full"), pytest.param(REDUCED, id="reduced")]
 
 
-def run_pair(p, scheme, steps, tol, max_iters, threads=8, iteration=None):
+def run_pair(p, scheme, steps, tol, max_iters, threads=8, iteration=None, reduced_kernel=None):
     """Run `steps` time steps on both sides; return per-step (iters) and final fluxes.
     iteration: OCI_ITERATION_FULL / _REDUCED (None = the library default); the oracle is always the
     plain method (one LU solve per cell per iteration)."""
     import paper_2305_13555_b200 as P
     from oracle import Oracle
-    g = P.OCI.from_problem(p, iteration=iteration)
+    g = P.OCI.from_problem(p, iteration=iteration, reduced_kernel=reduced_kernel)
     o = Oracle.from_problem(p, threads=threads)
     gi, oi = [], []
     for k in range(steps):
@@ -165,18 +165,73 @@ def test_ktiled_kernel_shapes(J, N, bcL, bcR, iteration):
     mirrors, the cross-CTA scalar-flux ticket (n > 128)."""
     import paper_2305_13555_b200 as P
     p = _custom(J, N, bcL, bcR, seed=J * 1000 + N, hetero=False)
-    g = P.OCI.from_problem(p)
-    assert g.get_info()["apply_kernel"] == P.KERNEL_KTILED
     # the reduced form has a K-tiled tensor-core kernel of its own when N is a multiple of 16 (partial last item
-    # unless 2N is a multiple of 128)
+    # unless 2N is a multiple of 128); N = 64, 128 default to the operator-in-registers family, so the K-tiled one is
+    # forced here (test_opreg_kernel_shapes covers the default)
+    forced = P.RKERNEL_KTILED if N % 16 == 0 else None
+    g = P.OCI.from_problem(p, reduced_kernel=forced)
+    assert g.get_info()["apply_kernel"] == P.KERNEL_KTILED
     assert g.get_info()["reduced_kernel"] == (P.RKERNEL_KTILED if N % 16 == 0 else P.RKERNEL_GEMV)
     g.close()
-    r = run_pair(p, "oci", steps=2, tol=-1.0, max_iters=4, threads=16, iteration=iteration)
+    r = run_pair(p, "oci", steps=2, tol=-1.0, max_iters=4, threads=16, iteration=iteration, reduced_kernel=forced)
     assert rel(r["g_psi"], r["o_psi"]) < 1e-12
     assert rel(r["g_phi"], r["o_phi"]) < 1e-12
-    r = run_pair(p, "oci", steps=2, tol=1e-10, max_iters=10_000, threads=16, iteration=iteration)
+    r = run_pair(p, "oci", steps=2, tol=1e-10, max_iters=10_000, threads=16, iteration=iteration, reduced_kernel=forced)
     assert r["g_iters"] == r["o_iters"]
     assert rel(r["g_psi"], r["o_psi"]) < 1e-9
+
+
+@pytest.mark.parametrize("J,N,bcL,bcR", [
+    (1, 64, (REF, 0.0), (REF, 0.0)),         # one cell between two mirrors: both ghost rows come from the same tile
+    (63, 64, (INC, 1.0), (REF, 0.0)),        # one ragged tile
+    (64, 128, (REF, 0.0), (VAC, 0.0)),       # exactly one tile, config-4 block size
+    (65, 128, (VAC, 0.0), (REF, 0.0)),       # tile + 1 cell
+    (200, 128, (VAC, 0.0), (INC, 0.7)),
+    (2500, 64, (REF, 0.0), (REF, 0.0)),      # 40 tiles: more tiles than CTAs of one row group (K2 = 128: 2 / 4 groups)
+    (5000, 128, (INC, 0.4), (REF, 0.0)),     # 79 tiles: several tiles per CTA (ITER: 37 CTAs per row group, FIX: 18)
+])
+def test_opreg_kernel_shapes(J, N, bcL, bcR):
+    """One shared block with N = 64 or 128 (config 4's block size): the reduced step on the operator-in-registers
+    kernels (every CTA keeps 64 operator rows as DMMA fragments, cell tiles stream by TMA): ragged tiles, both
+    mirrors, more tiles than CTAs, the row group that owns the scalar-flux rows rotating from tile to tile."""
+    import paper_2305_13555_b200 as P
+    from oracle import threads_available
+    p = _custom(J, N, bcL, bcR, seed=J * 7 + N, hetero=False)
+    th = threads_available()
+    r = run_pair(p, "oci", steps=2, tol=-1.0, max_iters=4, threads=th)
+    assert r["info"]["reduced_kernel"] == P.RKERNEL_OPREG and r["info"]["iteration"] == P.ITERATION_REDUCED
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-12
+    assert rel(r["g_phi"], r["o_phi"]) < 1e-12
+    r = run_pair(p, "oci", steps=2, tol=1e-10, max_iters=10_000, threads=th)
+    assert r["g_iters"] == r["o_iters"]
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-9
+    # forcing a family that does not serve the problem is an error at setup, not a silent fallback
+    g = P.OCI(p.dx, p.sigma_t, p.sigma_s, p.v, p.dt, p.n_angles, p.bc_left, p.bc_right)
+    g.set_reduced_kernel(P.RKERNEL_RESIDENT)
+    with pytest.raises(P.OCIError) as e:
+        g.setup()
+    assert e.value.code == -1
+    g.close()
+
+
+def test_opreg_fused_loop_many_iterations():
+    """The operator-in-registers ITER kernel runs a whole chunk of up to 64 iterations in one cooperative launch;
+    a problem that needs several chunks re-arms the barrier counter, the norm slots and the producer hand-off."""
+    import paper_2305_13555_b200 as P
+    from oracle import Oracle
+    q = _custom(150, 64, (REF, 0.0), (REF, 0.0), seed=77, hetero=False, dt=50.0)
+    q.sigma_s[:] = q.sigma_t * 0.999
+    g, o = P.OCI.from_problem(q), Oracle.from_problem(q, threads=8)
+    assert g.get_info()["reduced_kernel"] == P.RKERNEL_OPREG
+    for x in (g, o):
+        x.set_source(q.source(0))
+    a, b = g.oci_step(1e-10, 100_000), o.oci_step(1e-10, 100_000)
+    assert a[0] == b[0] == 0 and abs(a[1] - b[1]) <= 1 and a[1] > 128, (a, b)
+    assert rel(g.get_scalar_flux(), o.scalar_flux()) < 1e-8
+    g.set_flux(q.psi0); o.set_flux(q.psi0)
+    assert g.oci_step(-1.0, 77)[:2] == (1, 77) == o.oci_step(-1.0, 77)[:2]
+    assert rel(g.get_angular_flux(), o.angular_flux()) < 1e-12
+    g.close()
 
 
 def test_apply_kernel_selection():
@@ -186,7 +241,7 @@ def test_apply_kernel_selection():
         g = P.OCI.from_problem(make_problem(cfg, cells=cells))
         assert g.get_info()["apply_kernel"] == want, cfg
         assert g.get_info()["reduced_kernel"] == {1: P.RKERNEL_GEMV, 2: P.RKERNEL_RESIDENT, 3: P.RKERNEL_RESIDENT,
-                                                  4: P.RKERNEL_KTILED, 5: P.RKERNEL_GEMV}[cfg], cfg
+                                                  4: P.RKERNEL_OPREG, 5: P.RKERNEL_GEMV}[cfg], cfg
         assert g.get_info()["iteration"] == P.ITERATION_REDUCED, cfg      # AUTO resolves to the reduced form on all five
         g.close()
 
