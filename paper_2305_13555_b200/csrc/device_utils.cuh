@@ -51,6 +51,18 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
         "DONE_%=:\n"
         "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
+// non-blocking test of a phase (the predicate is consumed later, so the latency of the test overlaps other work)
+__device__ __forceinline__ uint32_t mbar_test(uint64_t* bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return ok;
+}
 // 1-D bulk TMA global -> shared, completion on an mbarrier (SASS UBLKCP)
 __device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
 {
@@ -129,6 +141,32 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                  : "+d"(c0), "+d"(c1)
                  : "d"(a), "d"(b));
+}
+
+// The same under a warp-uniform predicate, and a predicated 8-byte shared-memory load: work that only some tiles
+// need (the scalar-flux rows) without a branch, so that the surrounding DMMA stream stays one basic block and the
+// compiler can software-pipeline the fragment loads across k-steps.
+__device__ __forceinline__ void dmma_if(double& c0, double& c1, double a, double b, int pred)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.s32 p, %4, 0;\n"
+        "@p mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+        "}\n"
+        : "+d"(c0), "+d"(c1)
+        : "d"(a), "d"(b), "r"(pred));
+}
+__device__ __forceinline__ void lds_if(double& v, uint32_t saddr, int pred)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.s32 p, %2, 0;\n"
+        "@p ld.shared.f64 %0, [%1];\n"
+        "}\n"
+        : "+d"(v)
+        : "r"(saddr), "r"(pred));
 }
 
 // ---- packed interface layout of the reduced step (oci_reduced.cu has the definition)

@@ -28,6 +28,8 @@
 // global memory with the same permutation.
 #include <cuda.h>
 
+#include <type_traits>
+
 #include "device_utils.cuh"
 
 namespace oci {
@@ -55,7 +57,7 @@ struct OCfg {
     static constexpr int OPLD = PASS == PASS_FIX ? K2 + 16 : K2;         // row stride of the operator in global memory
     static constexpr int PROW = PASS == PASS_FIX ? 2 * K2 : K2;          // operator row of the scalar-flux block
     static constexpr size_t SMEM = 1024 /*alignment slack*/ + (size_t)RO_RING * RO_STAGE_BYTES + (ADD ? 2 * RO_FX_BYTES : 0) +
-                                   (PHI ? 8 * PLD * 8 : 0) + (2 * RO_RING + 6) * 8 + 64;
+                                   (PHI ? 8 * PLD * 8 : 0) + (2 * RO_RING + 8) * 8 + 64;
 };
 
 }  // namespace
@@ -93,7 +95,8 @@ oci_red_opreg_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, const
     uint64_t* fx_full = empty + RO_RING;      // [2]
     uint64_t* fx_empty = fx_full + 2;         // [2]
     uint64_t* iter_bar = fx_empty + 2;        // MMA warps -> producer: "the grid barrier after iteration l has been passed"
-    volatile int* go_s = reinterpret_cast<volatile int*>(iter_bar + 1);   // ... and whether another iteration follows
+    uint64_t* stagger = iter_bar + 1;         // warps 0-3 -> warps 4-7: "one stage into this iteration"
+    volatile int* go_s = reinterpret_cast<volatile int*>(stagger + 1);   // ... and whether another iteration follows
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t J = V.J;
@@ -113,6 +116,7 @@ oci_red_opreg_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, const
             mbar_init(&fx_empty[s], 8);
         }
         mbar_init(iter_bar, 1);
+        mbar_init(stagger, 4);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     // the scalar-flux operator rows -> shared memory (plain loads: once per launch)
@@ -214,6 +218,10 @@ oci_red_opreg_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, const
         const int ysrc_l = PASS == PASS_ITER ? (ybase + l) & 1 : ysrc;
         double* __restrict__ Yd = V.y[ysrc_l ^ 1];
         double dmax = 0.0, rmax = 0.0;
+        // The two warps of every SM partition (w and w + 4) run one stage apart, so that the epilogue of one (shared-
+        // memory loads, adds, stores: about the time of the 64 DMMAs of a stage) overlaps the other one's DMMA stream
+        // instead of idling the pipe in lock step; the grid barrier re-aligns them, so the offset is set up per iteration.
+        if (warp >= 4 && my_tiles > 0) mbar_wait(stagger, l & 1);
         for (int it = 0; it < my_tiles; ++it) {
             const int tile = t0 + it * G;
             const int64_t j0 = (int64_t)tile * RO_M;
@@ -223,33 +231,50 @@ oci_red_opreg_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, const
 #pragma unroll
             for (int g = 0; g < 8; ++g) acc[g][0] = acc[g][1] = 0.0;
 
+            uint32_t ready = mbar_test(&full[q & (RO_RING - 1)], (q / RO_RING) & 1);
+            // The k loop of a tile exists twice: without the scalar-flux rows (three tiles of four run this one: nothing
+            // but the fragment loads and the DMMA stream) and with them (one more fragment pair and DMMA per k-step).
+            // A branch or a predicate per k-step instead costs every tile about 15 % (measured): it breaks the stream up.
+            auto tile_mma = [&](auto phi_tag) {
+                constexpr bool WP = decltype(phi_tag)::value;
 #pragma unroll
-            for (int s = 0; s < C::MAIN_STAGES; ++s) {
-                const int st = (q + s) & (RO_RING - 1);
-                mbar_wait(&full[st], ((q + s) / RO_RING) & 1);
-                const unsigned char* As = ring + (size_t)st * RO_STAGE_BYTES + a_row;
+                for (int s = 0; s < C::MAIN_STAGES; ++s) {
+                    const int st = (q + s) & (RO_RING - 1);
+                    if (!ready) mbar_wait(&full[st], ((q + s) / RO_RING) & 1);
+                    // the next stage's barrier is tested now and looked at after this stage's DMMAs (FIX: the Q16 stage last)
+                    if (s + 1 < C::SPT) ready = mbar_test(&full[(q + s + 1) & (RO_RING - 1)], ((q + s + 1) / RO_RING) & 1);
+                    const unsigned char* As = ring + (size_t)st * RO_STAGE_BYTES + a_row;
+                    const unsigned char* Ap = As + warp * 1024;              // this warp's own cell block (scalar flux)
 #pragma unroll
-                for (int k8 = 0; k8 < 8; ++k8) {
-                    const int kk = 8 * s + k8;                               // k-step of the gathered vector
-                    const unsigned char* Ab = As + (k8 >> 2) * RO_BOX_BYTES + foff[k8 & 3];
-                    double a[8];
+                    for (int k8 = 0; k8 < 8; ++k8) {
+                        const int kk = 8 * s + k8;                           // k-step of the gathered vector
+                        const int ko = (k8 >> 2) * RO_BOX_BYTES + foff[k8 & 3];
+                        double a[8];
 #pragma unroll
-                    for (int g = 0; g < 8; ++g) a[g] = *reinterpret_cast<const double*>(Ab + g * 1024);
+                        for (int g = 0; g < 8; ++g) a[g] = *reinterpret_cast<const double*>(As + ko + g * 1024);
 #pragma unroll
-                    for (int g = 0; g < 8; ++g) dmma(acc[g][0], acc[g][1], a[g], bfr[kk]);
-                    if (with_phi) {
-                        // this warp's cell block (g = warp) against the scalar-flux rows
-                        const double ap = *reinterpret_cast<const double*>(Ab + warp * 1024);
-                        dmma(accp[0], accp[1], ap, pfr[16 * (kk >> 2) + 2 * (kk & 3)]);
+                        for (int g = 0; g < 8; ++g) dmma(acc[g][0], acc[g][1], a[g], bfr[kk]);
+                        if (WP) {
+                            // cell block g = warp against the scalar-flux rows (a[warp] would be a runtime register index)
+                            const double ap = *reinterpret_cast<const double*>(Ap + ko);
+                            const double bp = pfr[16 * (kk >> 2) + 2 * (kk & 3)];
+                            dmma(accp[0], accp[1], ap, bp);
+                        }
+                    }
+                    __syncwarp();
+                    if (lane == 0) {
+                        mbar_arrive(&empty[st]);
+                        // group 0 (warps 0-3) tells group 1 (warps 4-7) that it is one stage into the iteration
+                        if (s == 0 && it == 0 && warp < 4) mbar_arrive(stagger);
                     }
                 }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&empty[st]);
-            }
+            };
+            if (with_phi) tile_mma(std::true_type{});
+            else tile_mma(std::false_type{});
             if (PASS == PASS_FIX) {
                 // the source columns: box Q16 (columns 0..3 used), k-steps 0 and 1 of its chunk
                 const int st = (q + C::MAIN_STAGES) & (RO_RING - 1);
-                mbar_wait(&full[st], ((q + C::MAIN_STAGES) / RO_RING) & 1);
+                if (!ready) mbar_wait(&full[st], ((q + C::MAIN_STAGES) / RO_RING) & 1);
                 const unsigned char* As = ring + (size_t)st * RO_STAGE_BYTES + a_row;
 #pragma unroll
                 for (int ks = 0; ks < 2; ++ks) {
