@@ -101,6 +101,18 @@ __device__ __forceinline__ uint64_t l2_policy_evict_first()
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
+// 16-byte global load / store / L2 prefetch with an L2 eviction policy
+__device__ __forceinline__ double2 ldg2_hint(const double* p, uint64_t policy)
+{
+    double2 r;
+    asm volatile("ld.global.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(policy));
+    return r;
+}
+__device__ __forceinline__ void stg2_hint(double* p, double2 v, uint64_t policy)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(policy) : "memory");
+}
+__device__ __forceinline__ void prefetch_l2_evict_last(const void* p) { asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(p)); }
 // generic-proxy accesses of shared memory (LDS / STS) ordered before async-proxy ones (the TMA unit)
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void named_bar_sync(int id, int threads)

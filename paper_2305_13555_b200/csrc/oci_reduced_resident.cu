@@ -81,6 +81,8 @@ struct EpiCtx {
     const double* __restrict__ phifix;
     double* __restrict__ phi;
     double* __restrict__ phifix_out;
+    uint64_t pol_keep;                 // L2 policy of the additive operand (re-read every iteration: evict_last)
+    uint64_t pol_out;                  // L2 policy of the FIX pass's stores (yfix: evict_last, ifix: evict_first)
 };
 
 // One phase = all k-steps of one row group of one tile (NBC n8 blocks, accumulators acc) with the epilogue of
@@ -122,7 +124,7 @@ __device__ __forceinline__ void phase(double (&acc)[2][NBC][2], const double* __
         // ---- pending epilogue: loads of slice ks
         if (LOADS && ks < NSL) {
 #pragma unroll
-            for (int g = 0; g < 2; ++g) fxw[ks][g] = *reinterpret_cast<const double2*>(E.fixp + pj[g] * K2 + 8 * ks + 2 * t4);
+            for (int g = 0; g < 2; ++g) fxw[ks][g] = ldg2_hint(E.fixp + pj[g] * K2 + 8 * ks + 2 * t4, E.pol_keep);
         }
         if (PK == PK_ITER && ks == NSL) {
 #pragma unroll
@@ -138,7 +140,10 @@ __device__ __forceinline__ void phase(double (&acc)[2][NBC][2], const double* __
             for (int g = 0; g < 2; ++g) {
                 double2 v = make_double2(pend[g][t][0], pend[g][t][1]);
                 if (LOADS) { v.x += fxw[t][g].x; v.y += fxw[t][g].y; }
-                if (ok[g]) *reinterpret_cast<double2*>(E.out + pj[g] * K2 + 8 * t + 2 * t4) = v;
+                if (ok[g]) {
+                    if (LOADS) *reinterpret_cast<double2*>(E.out + pj[g] * K2 + 8 * t + 2 * t4) = v;
+                    else stg2_hint(E.out + pj[g] * K2 + 8 * t + 2 * t4, v, E.pol_out);
+                }
             }
         }
         if ((PK == PK_ITER || PK == PK_FIX0) && ks == NSL + DIST) {     // scalar-flux block: columns 0..3 of block NSL
@@ -227,13 +232,22 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
         }
     }
 
+    // L2 residency (126 MB): the additive operand (yfix: J x 2N doubles, 64 MB at config 3) is re-read by every
+    // iteration of the step and is asked to stay (evict_last); the iterate streams: a row of y is dead once its tile
+    // and the two neighbouring tiles have read it (evict_first), and y^(l+1) is written with the default priority so
+    // that its most recently written part is still in L2 when iteration l+1 reads it - which is why odd iterations
+    // walk the tiles in the opposite order (`rev`).  ifix is only read by the FINAL pass: written evict_first.
+    const uint64_t pol_last = l2_policy_evict_last(), pol_first = l2_policy_evict_first();
+    bool rev = false;                    // this iteration walks the warp's tiles from the last one down
+    auto tile_at = [&](int it) -> int64_t { return wid + (int64_t)(rev ? my_tiles - 1 - it : it) * nw; };
+
     // one lane requests a tile: tensor-map boxes straight into the warp's private ring
     const CUtensorMap* my = nullptr;     // tensor map of this iteration's source y
     int tc0 = 0;                         // tiles this warp has consumed in earlier iterations (ring position)
     auto prefetch = [&](int it) {
         if (lane == 0) {
             const int s = (tc0 + it) & 1;
-            const int j0 = (int)((wid + (int64_t)it * nw) * RT_M);
+            const int j0 = (int)(tile_at(it) * RT_M);
             unsigned char* st = my_ring + (size_t)s * C::STAGE_BYTES;
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             mbar_expect_tx(&my_full[s], C::TX_BYTES);
@@ -242,7 +256,7 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
                 tma_load_2d(st + RT_M * C::LDH * 8, &map_z, N2, j0, &my_full[s]);
                 tma_load_2d(st + 2 * RT_M * C::LDH * 8, &map_q, 0, j0, &my_full[s]);
             } else {
-                tma_load_2d(st, my, 0, j0, &my_full[s]);                                          // rows j0-1 .. j0+16
+                tma_load_2d_hint(st, my, 0, j0, &my_full[s], pol_first);                          // rows j0-1 .. j0+16
             }
         }
         __syncwarp();
@@ -254,8 +268,11 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
     E.phifix = V.phifix;
     E.phi = V.phi;
     E.phifix_out = V.phifix;
+    E.pol_keep = pol_last;
+    E.pol_out = pol_last;          // FIX: yfix stays for the iterations
     EpiCtx E1 = E;                 // FIX: the pending I rows go to ifix
     E1.out = V.ifix;
+    E1.pol_out = pol_first;
 
     double* Yd = nullptr;
     const double* brow = op_s + g4 * C::LD + t4;
@@ -284,6 +301,7 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
     my = (ysrc_l == ybase) ? &map_a : &map_a_alt;
     Yd = V.y[ysrc_l ^ 1];
     if (PASS == PASS_ITER) E.out = Yd;
+    rev = PASS == PASS_ITER && ((slot + l) & 1);
     tc0 = l * my_tiles;
     if (my_tiles > 0) prefetch(0);
     double dmax = 0.0, rmax = 0.0;
@@ -292,12 +310,12 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
     for (int g = 0; g < 2; ++g)
 #pragma unroll
         for (int t = 0; t < NBP; ++t) pend[g][t][0] = pend[g][t][1] = 0.0;
-    int64_t pj0 = my_tiles > 0 ? wid * RT_M : 0;
+    int64_t pj0 = my_tiles > 0 ? tile_at(0) * RT_M : 0;
     int prows = 0;                                                 // nothing pending yet: loads clamped, stores off
 
     for (int it = 0; it < my_tiles; ++it) {
         const int s = (tc0 + it) & 1;
-        const int64_t j0 = (wid + (int64_t)it * nw) * RT_M;
+        const int64_t j0 = tile_at(it) * RT_M;
         const int rows = (int)((J - j0 < RT_M) ? (J - j0) : RT_M);
         if (it + 1 < my_tiles) prefetch(it + 1);
         // the additive operands of THIS tile's epilogue (drained during the next phase) -> L2, so that the loads
@@ -305,7 +323,7 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
         if (PASS != PASS_FIX) {
             const char* f0 = reinterpret_cast<const char*>(E.fixp + j0 * K2);
             const int bytes = rows * K2 * 8;
-            for (int o = lane * 128; o < bytes; o += 32 * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(f0 + o));
+            for (int o = lane * 128; o < bytes; o += 32 * 128) prefetch_l2_evict_last(f0 + o);
             if (PASS == PASS_ITER && lane < 8) {
                 const char* p0 = reinterpret_cast<const char*>((lane < 4 ? E.phifix : E.phi) + j0 * 4);
                 const int o = (lane & 3) * 128;
