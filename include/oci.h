@@ -206,6 +206,11 @@ int oci_get_kernel_time(oci_ctx* ctx, double* ms, int64_t* launches);
 int oci_get_aux_kernel_time(oci_ctx* ctx, double* fix_ms, int64_t* fix_launches, double* final_ms,
                             int64_t* final_launches);
 
+/* Device time of the last oci_setup on this context (forming and inverting the blocks, packing the
+ * operators of the reduced step): milliseconds between CUDA events on the context's stream.  Reported
+ * once, separately from the per-step times.  Errors: -1, -2 (before oci_setup). */
+int oci_get_setup_time(const oci_ctx* ctx, double* ms);
+
 /* Number of kernels this library launched on this context so far. */
 int64_t oci_launch_count(const oci_ctx* ctx);
 

@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = [
     "oci_create", "oci_workspace_bytes", "oci_setup", "oci_set_flux", "oci_set_flux_dev", "oci_set_source",
     "oci_set_source_dev", "oci_step", "si_step", "oci_get_scalar_flux", "oci_get_angular_flux",
     "oci_get_scalar_flux_dev", "oci_get_angular_flux_dev", "oci_get_quadrature", "oci_get_info",
-    "oci_get_block_inverse", "oci_enable_kernel_timing", "oci_get_kernel_time", "oci_get_aux_kernel_time", "oci_set_iteration", "oci_set_reduced_kernel", "oci_launch_count",
+    "oci_get_block_inverse", "oci_enable_kernel_timing", "oci_get_kernel_time", "oci_get_aux_kernel_time", "oci_set_iteration", "oci_set_reduced_kernel", "oci_get_setup_time", "oci_launch_count",
     "oci_last_error", "oci_destroy",
 ]
 
@@ -91,6 +91,8 @@ def load_library():
     L.oci_set_iteration.argtypes = [vp, i32]
     L.oci_set_reduced_kernel.restype = C.c_int
     L.oci_set_reduced_kernel.argtypes = [vp, i32]
+    L.oci_get_setup_time.restype = C.c_int
+    L.oci_get_setup_time.argtypes = [vp, _dp]
     L.oci_launch_count.restype = i64
     L.oci_launch_count.argtypes = [vp]
     L.oci_last_error.restype = C.c_char_p
@@ -284,6 +286,11 @@ class OCI:
 
     def set_reduced_kernel(self, kernel):
         self._check(self._L.oci_set_reduced_kernel(self._h, int(kernel)))
+
+    def get_setup_time(self) -> float:
+        ms = C.c_double(0.0)
+        self._check(self._L.oci_get_setup_time(self._h, C.byref(ms)))
+        return ms.value
 
     def launch_count(self):
         return int(self._L.oci_launch_count(self._h))

@@ -65,6 +65,7 @@ struct oci_ctx {
     std::vector<cudaEvent_t> ev;
     cudaEvent_t ev_aux[4] = {nullptr, nullptr, nullptr, nullptr};
     double kernel_ms = 0.0;
+    double setup_ms = 0.0;             // device time of form + invert + pack in the last oci_setup
     int64_t kernel_launches = 0;
     double aux_ms[2] = {0.0, 0.0};     // reduced iteration: Psi_fix pass, finalisation
     int64_t aux_launches[2] = {0, 0};
@@ -158,7 +159,7 @@ void gauss_legendre(int N, std::vector<double>& mu, std::vector<double>& w)
 
 struct Layout {
     int64_t binv, psi0, psi1, cfix, phi, Q, qs, dx, sig, sigs, blk, rep, mu, w, coef, ainv4, si_scan, phi_part, norms, tickets, flags,
-        xop, rop, fop, y0, y1, z, yfix, ifix, phifix, q16, gitems, total;
+        xop, rop, fop, y0, y1, z, yfix, ifix, phifix, q16, gitems, perm, team_bar, total;
 };
 
 int64_t align_up(int64_t x) { return (x + 255) & ~int64_t(255); }
@@ -206,6 +207,8 @@ Layout make_layout(int64_t J, int32_t N, int64_t nblk)
         // (cell tile, block) groups of the K-tiled kernels: at most min(nblk, 64) per tile of 64 cells
         L.gitems = take(grouped ? ((J + 63) / 64) * (nblk < 64 ? nblk : 64) * 16 : 0);
     }
+    L.perm = take(nblk * n * 4);
+    L.team_bar = take(4096 * 4);
     L.total = o;
     return L;
 }
@@ -510,6 +513,8 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     V.q16 = (double*)(base + L.q16);
     V.gitems = nullptr;
     V.ngroups = 0;
+    V.perm = (int32_t*)(base + L.perm);
+    V.team_bar = (int32_t*)(base + L.team_bar);
     V.v = ctx->v; V.dt = ctx->dt;
     V.bcL = ctx->bcL.kind; V.bcR = ctx->bcR.kind;
     V.bcLv = ctx->bcL.value; V.bcRv = ctx->bcR.value;
@@ -520,6 +525,7 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
         V.sm_count = sms;
         ctx->coop = coop != 0;
         // more than 48 KB of dynamic shared memory is a per-device, per-kernel opt-in
+        CK(oci_setup_opt_in());
         CK(oci_shared_fast_opt_in());
         CK(oci_ktiled_opt_in());
         CK(oci_red_gemv_opt_in());
@@ -576,12 +582,24 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
         CK(cudaStreamSynchronize(s));
     }
 
+    if (ctx->ev.empty()) {
+        ctx->ev.resize(2 * kNormSlots);
+        for (auto& e : ctx->ev) CK(cudaEventCreate(&e));
+        for (auto& e : ctx->ev_aux) CK(cudaEventCreate(&e));
+    }
+    CK(cudaEventRecord(ctx->ev[0], s));
     LAUNCH(launch_form_and_invert(V, s));                                // a0, a1
     LAUNCH(launch_pack_operators(V, s));                                 // f1: G, H, F
+    CK(cudaEventRecord(ctx->ev[1], s));
     int32_t flag = 0;
     CK(cudaMemcpyAsync(&flag, V.flags, 4, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
     CK(cudaGetLastError());
+    {
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]));
+        ctx->setup_ms = ms;
+    }
     if (flag != 0) {
         char buf[96];
         std::snprintf(buf, sizeof buf, "block %d is singular", flag - 1);
@@ -591,11 +609,6 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     if (!ctx->stream2) {
         CK(cudaStreamCreateWithFlags(&ctx->stream2, cudaStreamNonBlocking));
         CK(cudaEventCreateWithFlags(&ctx->ev_norms, cudaEventDisableTiming));
-    }
-    if (ctx->ev.empty()) {
-        ctx->ev.resize(2 * kNormSlots);
-        for (auto& e : ctx->ev) CK(cudaEventCreate(&e));
-        for (auto& e : ctx->ev_aux) CK(cudaEventCreate(&e));
     }
     ctx->use_ktiled = ctx->path == OCI_PATH_SHARED && !oci_shared_fast_supported(V) && oci_ktiled_supported(V) &&
                       oci_ktiled_prepare(V, &ctx->maps);
@@ -815,6 +828,14 @@ int oci_get_kernel_time(oci_ctx* ctx, double* ms, int64_t* launches)
     if (launches) *launches = ctx->kernel_launches;
     ctx->kernel_ms = 0.0;
     ctx->kernel_launches = 0;
+    return OCI_OK;
+}
+
+int oci_get_setup_time(const oci_ctx* ctx, double* ms)
+{
+    if (!ctx || !ms) return fail(ctx, OCI_E_INVALID, "NULL argument");
+    if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_get_setup_time before oci_setup");
+    *ms = ctx->setup_ms;
     return OCI_OK;
 }
 

@@ -42,7 +42,9 @@ struct DevView {
     double* phi_part;           // [ceil(n/128)][J][4]  per-item scalar-flux partials (K-tiled kernel)
     int32_t* tickets;           // [ceil(J/64)]  arrival counters of the K-tiled kernel's cell tiles (0 between launches)
     unsigned long long* norms;  // [kNormSlots][2]  bit patterns of (d, r), atomicMax targets
-    int32_t* flags;             // [0] = 1 + index of a singular block, 0 if none
+    int32_t* flags;             // [0] = 1 + index of a singular block, 0 if none; [8] grid-barrier counter of the fused loops
+    int32_t* perm;              // [nblk][n]  pivot rows of the blocked inversion (setup)
+    int32_t* team_bar;          // [min(nblk, SMs)]  team-barrier counters of the blocked inversion (setup)
     // ---- interface-reduced step (oci_reduced.cu), K2 = 2N
     double* xop;                // [nblk][2*K2+8][K2+16]  FIX operator X (rows: O, I, scalar flux; zero padded)
     double* rop;                // [nblk][K2+8][K2]  rows 0..K2-1: G = B^{-1}[O,I] diag|mu|; K2..K2+3: H = W B^{-1}[:,I] diag|mu|; rest 0
@@ -111,6 +113,7 @@ inline int si_chunk_cells(int64_t J, int32_t N, int sm_count = 148)
 inline int launched(int k) { return cudaPeekAtLastError() == cudaSuccess ? k : -1; }
 // Opt-in to more than 48 KB of dynamic shared memory for every kernel of a file that needs it.  The attribute is
 // per device, so oci_setup calls these with the context's device current (no per-process caching).
+cudaError_t oci_setup_opt_in();
 cudaError_t oci_shared_fast_opt_in();
 cudaError_t oci_ktiled_opt_in();
 cudaError_t oci_red_gemv_opt_in();

@@ -63,7 +63,7 @@ __device__ __forceinline__ double2 ldg_stream2(const double* p)
 
 }  // namespace
 
-// ---- setup: X, G, H, F of every distinct block from its inverse (one CTA per block)
+// ---- setup: X, G, H, F of every distinct block from its inverse (gridDim.x = blocks, gridDim.y CTAs share a block)
 __global__ void __launch_bounds__(256) pack_operators_kernel(DevView V)
 {
     const int n = V.n, N = V.N, K2 = n >> 1, MO = K2 + 8, MF = 2 * K2 + 8, KF = K2 + 16;
@@ -74,7 +74,8 @@ __global__ void __launch_bounds__(256) pack_operators_kernel(DevView V)
     double* __restrict__ X = V.xop + (size_t)b * MF * KF;
     const double h = V.dx[V.rep[b]];
     const double al = h / (2.0 * V.v * V.dt), q4 = 0.25 * h;
-    for (int e = threadIdx.x; e < MO * K2; e += blockDim.x) {
+    const int tid = blockIdx.y * blockDim.x + threadIdx.x, nth = gridDim.y * blockDim.x;
+    for (int e = tid; e < MO * K2; e += nth) {
         const int r = e / K2, p = e - r * K2;
         const int ip = o_row(p, N) ^ 1;
         const double cf = V.coef[ip];
@@ -92,7 +93,7 @@ __global__ void __launch_bounds__(256) pack_operators_kernel(DevView V)
     }
     // X: rows [0,K2) = O rows, [K2,2K2) = I rows, [2K2,2K2+4) = the scalar-flux rows W B^{-1}, rest 0;
     // columns [0,K2) = alpha * B^{-1}[.][fix_col_row(u)], [K2,K2+4) = (h/4) sum_m B^{-1}[.][4m+s], rest 0
-    for (int e = threadIdx.x; e < MF * KF; e += blockDim.x) {
+    for (int e = tid; e < MF * KF; e += nth) {
         const int r = e / KF, u = e - r * KF;
         double val = 0.0;
         if (r < 2 * K2 + 4 && u < K2 + 4) {
@@ -128,7 +129,8 @@ __global__ void __launch_bounds__(256) pack_operators_kernel(DevView V)
 
 int launch_pack_operators(const DevView& V, cudaStream_t s)
 {
-    pack_operators_kernel<<<(unsigned)V.nblk, 256, 0, s>>>(V);
+    const unsigned fy = V.nblk >= V.sm_count ? 1u : (unsigned)((2 * V.sm_count + V.nblk - 1) / V.nblk);
+    pack_operators_kernel<<<dim3((unsigned)V.nblk, fy), 256, 0, s>>>(V);
     return launched(1);
 }
 

@@ -79,6 +79,36 @@ def test_setup_block_inverse_matches_oracle(cfg, cells):
     g.close()
 
 
+@pytest.mark.parametrize("N,nblk", [(2, 1), (2, 300), (4, 5), (6, 2), (10, 1), (10, 200), (48, 3), (64, 150), (128, 1), (128, 2), (256, 1), (512, 1)])
+def test_blocked_inversion_shapes(N, nblk):
+    """Kernel (a1): the blocked Gauss-Jordan inversion over its panel widths (n <= 512: 32, n <= 1024: 16, else 8),
+    partial last panels (n = 24, 40), one CTA per block and teams of CTAs per block (fewer blocks than SMs), against
+    the oracle's LU applied to the identity and against B B^{-1} = I.  Small dt makes the -dx/(v dt) sub-diagonal
+    entries dominate, so about half of all rows are interchanged."""
+    import paper_2305_13555_b200 as P
+    from oracle import cell_matrix, gauss_legendre, lu_factor, lu_solve
+    rng = np.random.default_rng(N * 1000 + nblk)
+    J = nblk
+    dx, st = rng.uniform(0.05, 1.0, J), rng.uniform(0.2, 8.0, J)
+    ss = st * rng.uniform(0.1, 0.99, J)
+    v, dt = 1.3, 0.02
+    g = P.OCI(dx, st, ss, v, dt, N)
+    g.setup()
+    assert g.get_info()["n_blocks"] == nblk and g.get_setup_time() > 0.0
+    mu, w = gauss_legendre(N)
+    n = 4 * N
+    for b in sorted({0, nblk // 2, nblk - 1}):
+        B = cell_matrix(mu, w, dx[b], st[b], ss[b], v, dt)
+        LU, piv, bad = lu_factor(B)
+        assert bad == 0 and np.sum(piv != np.arange(n)) > n // 8      # pivoting really happens
+        got = g.get_block_inverse(b)
+        assert np.max(np.abs(B @ got - np.eye(n))) < 1e-12
+        if n <= 512:
+            ref = np.column_stack([lu_solve(LU, piv, e) for e in np.eye(n)])
+            assert rel(got, ref) < 1e-12
+    g.close()
+
+
 SCHEMES = [pytest.param("oci", FULL, id="oci-full"), pytest.param("oci", REDUCED, id="oci-reduced"),
            pytest.param("si", None, id="si")]
 
