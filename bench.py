@@ -14,6 +14,10 @@ Timing: W untimed warm-up steps, state reset to the initial condition (untimed),
 steps between CUDA events on the library's stream, barrier + synchronize on both sides, max over
 ranks.  The working set (three 128 MiB arrays) is larger than the 126 MB L2.
 
+--gpus N (under torchrun, one rank per GPU): row f4, ONE slab of N x 131,072 cells sharded by contiguous cell
+ranges (weak scaling); the edge half rows and the two norms of the stopping rule travel per iteration as peer-memory
+stores (csrc/shard_exchange.cu), NCCL is only used for the rendezvous and the timing barrier.
+
 --impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded
 sample of the same workload; see DESIGN.md "Measurement".
 """
@@ -35,16 +39,20 @@ from workloads import make_problem  # noqa: E402
 METRIC = "oci_unknown_updates_per_s"
 UNIT = "unknown-updates/s"
 
-# DRAM traffic per launch of the dominant kernel from the committed `ncu --set full` capture
-# (profiles/), bytes per launch; None where no capture exists for that config's kernel.
-# Keyed by (config, reduced iteration form?).
-NCU_TRAFFIC_BYTES = {(3, False): 374.17e6,    # profiles/r1_resident_cfg3_full.txt: 272.80 MB read + 101.37 MB written
-                     (4, False): 178.67e6,    # profiles/r1_ktiled_cfg4_full.txt:   136.89 MB read +  41.78 MB written
-                     (5, False): 2168.2e6,    # profiles/r1_percell_cfg5_full.txt:  2164.5 MB read +   3.8 MB written
-                     # reduced form, per ITERATION (resident and GEMV ITER launches run all iterations of a step: bytes / iterations)
-                     (3, True): 206.2e6,      # profiles/r1d_reduced_cfg3_full.txt: (846.0 MB read + 391.4 MB written) / 6 iterations
-                     (4, True): 75.6e6,       # profiles/r1e_reduced_cfg4_full.txt:  68.8 MB read +  6.8 MB written (y buffers fit in L2)
-                     (5, True): 558.6e6}      # profiles/r1d_reduced_cfg5_full.txt: (4447.6 MB read + 21.0 MB written) / 8 iterations
+def load_traffic(cfg, reduced):
+    """DRAM bytes per iteration of the dominant kernel from the committed `ncu --set full` capture: profiles/traffic.json,
+    written by `python -m paper_2305_13555_b200.ncu_traffic` from the .ncu-rep together with the commit the capture was
+    taken at, so that a stale capture is visible next to the number."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(path):
+        return None, None
+    with open(path) as f:
+        t = json.load(f)
+    e = t.get("entries", {}).get(f"cfg{cfg}_{'reduced' if reduced else 'full'}")
+    if not e:
+        return None, None
+    return e["dram_bytes_per_iteration"], {"file": "profiles/traffic.json", "capture": e.get("capture"), "kernel": e.get("kernel"),
+                                           "captured_at_commit": e.get("commit")}
 
 
 def load_peaks():
@@ -174,24 +182,43 @@ def oracle_sample_problem(cfg):
 FULL_CELLS = {1: 20, 2: 1000, 3: 131072, 4: 16384, 5: 4096}
 
 
-def time_oracle(cfg, steps, warmup, threads):
+def time_oracle(cfg, steps, warmup, threads, scheme="oci", cells=None):
     from oracle import Oracle
     p, desc = oracle_sample_problem(cfg)
+    if cells is not None and cells < p.cells:
+        p = make_problem(cfg, cells=cells)
+        desc = f"config {cfg} with the first {cells} of {FULL_CELLS[cfg]} cells (same materials, angles, dt, BCs)"
     o = Oracle.from_problem(p, threads=threads)
+    step = o.oci_step if scheme == "oci" else o.si_step
     for k in range(warmup):
         o.set_source(p.source(k))
-        o.oci_step(p.tol, p.max_iters)
+        step(p.tol, p.max_iters)
     o.set_flux(p.psi0)
     updates, iters = 0, []
     t0 = time.perf_counter()
     for k in range(steps):
         o.set_source(p.source(k))
-        st, it, _ = o.oci_step(p.tol, p.max_iters)
+        st, it, _ = step(p.tol, p.max_iters)
         updates += p.unknowns * it
         iters.append(it)
     dt = time.perf_counter() - t0
-    return dict(value=updates / dt, seconds=dt, iters=iters, sample=f"{desc}, {steps} time steps, OCI to tol {p.tol:g}",
+    return dict(value=updates / dt, seconds=dt, iters=iters,
+                sample=f"{desc}, {steps} time steps, {scheme.upper()} to tol {p.tol:g}, {threads} thread(s)",
                 ms_per_step=dt / steps * 1e3, cells=p.cells)
+
+
+def oracle_legs(cfg, threads):
+    """SURVEY 8(d) "Oracle timing": the oracle as it stands, OCI and SI, on (i) one thread and (ii) all host cores
+    (threads over cells for OCI, over angles for SI, as the paper's CPU runs).  The one-thread legs use a
+    quarter of the sample so that the whole baseline stays within tens of seconds."""
+    p, _ = oracle_sample_problem(cfg)
+    small = max(1, p.cells // 4) if cfg in (3, 4, 5) else None
+    steps = 1 if cfg in (3, 4, 5) else 5
+    legs = {}
+    for scheme in ("oci", "si"):
+        legs[f"{scheme}_all_cores"] = time_oracle(cfg, steps, 0, threads, scheme)
+        legs[f"{scheme}_1_thread"] = time_oracle(cfg, steps, 0, 1, scheme, cells=small)
+    return legs
 
 
 def run_reference(args):
@@ -206,7 +233,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
         "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": r["ms_per_step"], "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": make_problem(args.config, cells=1).name, "note": "CPU oracle on a bounded sample"},
+        "config": {"workload": make_problem(args.config, cells=1).name},
         "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": threads, "kind": "oracle", "sample": r["sample"]},
         "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "iters_per_step": r["iters"],
@@ -218,62 +245,80 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------ GPU arm
 def time_gpu_steps(torch, g, p, steps, scheme, sampler=None, barrier=None):
     """Reset to the IC (untimed), then time exactly `steps` steps with CUDA events on the library's
-    (= torch's current) stream.  Returns (ms, iters list)."""
-    g.set_flux(p.psi0)
+    (= torch's current) stream.  `g`: an OCI context or a ShardedOCI.  Returns (ms, iters, per-step ms)."""
+    sharded = hasattr(g, "shards")
+    if sharded:
+        g.set_flux_from_problem()
+    else:
+        g.set_flux(p.psi0)
     qdev = {}
-    for k in range(steps):                      # inputs resident in HBM before the timed region
-        q = p.source(k)
-        if q is not None and id(q) not in qdev:
-            qdev[id(q)] = torch.from_numpy(np.ascontiguousarray(q)).cuda()
-    step = g.oci_step if scheme == "oci" else g.si_step
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if not sharded:
+        for k in range(steps):                  # inputs resident in HBM before the timed region
+            q = p.source(k)
+            if q is not None and id(q) not in qdev:
+                qdev[id(q)] = torch.from_numpy(np.ascontiguousarray(q)).cuda()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
     if barrier:
         barrier()
     torch.cuda.synchronize()
     if sampler:
         sampler.start()
     iters = []
-    e0.record()
+    ev[0].record()
     for k in range(steps):
-        q = p.source(k)
-        g.set_source_dev(qdev[id(q)] if q is not None else None)
-        st, it, _ = step(p.tol, p.max_iters)
+        if sharded:
+            g.set_source(k)
+            st, it, _ = g.step(p.tol, p.max_iters)
+        else:
+            q = p.source(k)
+            g.set_source_dev(qdev[id(q)] if q is not None else None)
+            st, it, _ = (g.oci_step if scheme == "oci" else g.si_step)(p.tol, p.max_iters)
         iters.append(it)
-    e1.record()
+        ev[k + 1].record()
     torch.cuda.synchronize()
     if sampler:
         sampler.pause()
     if barrier:
         barrier()
-    return e0.elapsed_time(e1), iters
+    return ev[0].elapsed_time(ev[-1]), iters, [ev[k].elapsed_time(ev[k + 1]) for k in range(steps)]
 
 
 def time_gpu_e2e(torch, g, p, steps):
-    """Same K steps through the C ABI with HOST buffers: the initial condition and every step's
-    source are copied host->device from pinned memory and every step's scalar flux is read back,
+    """Same K steps through the C ABI with HOST buffers: the initial condition and every step's source are copied
+    host->device from pinned memory and every step's scalar flux is read back into pinned host memory
+    (oci_get_scalar_flux_async: the copy of step k's flux overlaps step k+1; oci_synchronize before the clock stops),
     all inside the timed region."""
-    psi0 = torch.from_numpy(np.ascontiguousarray(p.psi0)).pin_memory()
+    sharded = hasattr(g, "shards")
+    ctxs = g.shards if sharded else [g]
+    probs = [c.problem for c in ctxs] if sharded else [p]
+    psi0 = [torch.from_numpy(np.ascontiguousarray(q.psi0)).pin_memory() for q in probs]
     qpin = {}
-    for k in range(steps):
-        q = p.source(k)
-        if q is not None and id(q) not in qpin:
-            qpin[id(q)] = torch.from_numpy(np.ascontiguousarray(q)).pin_memory()
-    phi = torch.empty((p.cells, 4), dtype=torch.float64).pin_memory()
-    h2d = psi0.numel() * 8
+    for q in probs:
+        for k in range(steps):
+            a = q.source(k)
+            if a is not None and (id(q), k) not in qpin:
+                qpin[(id(q), k)] = torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    phi = [[torch.empty((q.cells, 4), dtype=torch.float64).pin_memory() for _ in range(2)] for q in probs]
+    h2d = sum(t.numel() * 8 for t in psi0)
     d2h = 0
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    g.set_flux(psi0.numpy())
+    for c, t in zip(ctxs, psi0):
+        c.set_flux(t.numpy())
     updates = 0
     for k in range(steps):
-        q = p.source(k)
-        g.set_source(qpin[id(q)].numpy() if q is not None else None)
-        h2d += p.cells * 32 if q is not None else 0
-        st, it, _ = g.oci_step(p.tol, p.max_iters)
-        updates += p.unknowns * it
-        g.get_scalar_flux(out=phi.numpy())
-        d2h += p.cells * 32
+        for c, q in zip(ctxs, probs):
+            a = qpin.get((id(q), k))
+            c.set_source(a.numpy() if a is not None else None)
+            h2d += q.cells * 32 if a is not None else 0
+        st, it, _ = g.step(p.tol, p.max_iters) if sharded else g.oci_step(p.tol, p.max_iters)
+        updates += sum(q.unknowns for q in probs) * it
+        for c, q, bufs in zip(ctxs, probs, phi):
+            c.get_scalar_flux_async(bufs[k & 1])
+            d2h += q.cells * 32
+    for c in ctxs:
+        c.synchronize()
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1)
@@ -292,6 +337,7 @@ def iteration_roofline(P, p, info, cfg, kms, klaunch, aux, steps, peaks, peak_sr
     K2 = n // 2
     M_op, K_op = (K2 + 4, K2) if reduced else (n, n)
     fix_ms, fix_n, fin_ms, fin_n = aux["fix_ms"], aux["fix_launches"], aux["final_ms"], aux["final_launches"]
+    traffic, traffic_src = load_traffic(cfg, reduced)
     breakdown = {"iteration_kernel_ms": k_avg_ms, "iterations_per_step": klaunch / steps,
                  "fix_pass_ms_per_step": fix_ms / max(fix_n, 1) if reduced else None,
                  "final_pass_ms_per_step": fin_ms / max(fin_n, 1) if reduced else None,
@@ -303,7 +349,7 @@ def iteration_roofline(P, p, info, cfg, kms, klaunch, aux, steps, peaks, peak_sr
         peak = max(peak_live, peak_scaled)
         achieved = flops / (k_avg_ms * 1e-3) * 1e-12
         roofline = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                    "traffic": NCU_TRAFFIC_BYTES.get((cfg, reduced)),
+                    "traffic": traffic, "traffic_source": traffic_src,
                     "kernel": "oci %s iteration (eq. 19), fp64 DMMA" % breakdown["form"], "algorithmic_flops_per_launch": flops,
                     "avg_launch_ms": k_avg_ms, "launches_timed": klaunch,
                     "peak_source": f"max(live DMMA issue-rate probe {peak_live:.2f}, MEASURED_PEAKS bf16 {peak_src} x 45/2250 = {peak_scaled:.2f})"}
@@ -314,7 +360,7 @@ def iteration_roofline(P, p, info, cfg, kms, klaunch, aux, steps, peaks, peak_sr
             bytes_ = p.cells * (n * n * 8.0 + 4.0 * n * 8.0 + 64.0)
         achieved = bytes_ / (k_avg_ms * 1e-3) * 1e-9
         roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                    "frac": achieved / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get((cfg, reduced)),
+                    "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "traffic_source": traffic_src,
                     "kernel": "oci %s iteration (eq. 19), batched GEMV" % breakdown["form"], "algorithmic_bytes_per_launch": bytes_,
                     "avg_launch_ms": k_avg_ms, "launches_timed": klaunch, "peak_source": f"MEASURED_PEAKS hbm_gbs ({peak_src})"}
     roofline["step_breakdown"] = breakdown
@@ -327,13 +373,15 @@ def per_config_table(torch, P, peaks=None, peak_src=None, peak_live=None):
     for cfg in (1, 2, 3, 4, 5):
         p = make_problem(cfg)
         g = P.OCI.from_problem(p)
-        row = {"S_N": p.n_angles, "cells": p.cells, "path": "shared" if g.get_info()["path"] == 0 else "per_cell"}
+        row = {"S_N": p.n_angles, "cells": p.cells, "path": "shared" if g.get_info()["path"] == 0 else "per_cell",
+               "setup_ms": g.get_setup_time()}
         for scheme in ("oci", "si"):
-            for k in range(2):                   # warm-up
+            for k in range(3):                   # warm-up
                 g.set_source(p.source(k))
                 (g.oci_step if scheme == "oci" else g.si_step)(p.tol, p.max_iters)
-            ms, iters = time_gpu_steps(torch, g, p, p.n_steps, scheme)
+            ms, iters, each = time_gpu_steps(torch, g, p, p.n_steps, scheme)
             row[f"{scheme}_ms_per_step"] = ms / p.n_steps
+            row[f"{scheme}_ms_per_step_median"] = float(np.median(each))
             row[f"{scheme}_iters"] = iters
             row[f"{scheme}_updates_per_s"] = p.unknowns * sum(iters) / (ms * 1e-3)
         row["si_over_oci_time"] = row["si_ms_per_step"] / row["oci_ms_per_step"]
@@ -381,52 +429,76 @@ def run_ours(args):
         barrier = dist.barrier
 
     peaks, peak_src = load_peaks()
-    p = make_problem(args.config)
-    g = P.OCI.from_problem(p, device=f"cuda:{local}")
-    info = g.get_info()
+    if world > 1:
+        # row f4: ONE slab of world x (config's cells), sharded by contiguous cell ranges (weak scaling)
+        from paper_2305_13555_b200.sharding import ShardedOCI
+        p = make_problem(args.config, cells=FULL_CELLS[args.config] * world)
+        g = ShardedOCI.distributed(p, device=f"cuda:{local}")
+        ctx = g.shards[0]
+
+        def warm_step(k):
+            g.set_source(k)
+            g.step(p.tol, p.max_iters)
+    else:
+        p = make_problem(args.config)
+        g = ctx = P.OCI.from_problem(p, device=f"cuda:{local}")
+
+        def warm_step(k):
+            g.set_source(p.source(k))
+            g.oci_step(p.tol, p.max_iters)
+    info = ctx.get_info()
     shared = info["path"] == P.PATH_SHARED
     n = info["block_dim"]
+    p_local = ctx.problem if world > 1 else p
 
-    # warm-up steps (untimed)
-    for k in range(args.warmup):
-        g.set_source(p.source(k))
-        g.oci_step(p.tol, p.max_iters)
+    for k in range(args.warmup):                # warm-up steps (untimed)
+        warm_step(k)
 
     # ---- headline: K steps, inputs resident in HBM
     sampler = ClockSampler(local) if rank == 0 else None
-    l0 = g.launch_count()
-    ms, iters = time_gpu_steps(torch, g, p, args.steps, "oci", sampler, barrier)
-    launches = g.launch_count() - l0
-    updates = p.unknowns * sum(iters)
-    ms, updates = aggregate_over_ranks(torch, ms, updates, "cuda" if world > 1 else None)
+    l0 = ctx.launch_count()
+    ms, iters, each = time_gpu_steps(torch, g, p, args.steps, "oci", sampler, barrier)
+    launches = ctx.launch_count() - l0
+    updates = p.unknowns * sum(iters)           # the whole slab: every rank advances its share of it
+    if world > 1:
+        ms, _ = aggregate_over_ranks(torch, ms, 0.0, "cuda")
+        each = [aggregate_over_ranks(torch, t, 0.0, "cuda")[0] for t in each]
     value = updates / (ms * 1e-3)
 
     # ---- the dominant kernel alone (events around every OCI apply launch, same steps again)
-    g.enable_kernel_timing(True)
-    _, iters2 = time_gpu_steps(torch, g, p, args.steps, "oci", sampler)
+    ctx.enable_kernel_timing(True)
+    time_gpu_steps(torch, g, p, args.steps, "oci", sampler, barrier)
     clocks = sampler.result(" during the headline and the per-kernel timed regions") if sampler else None
-    kms, klaunch = g.get_kernel_time()
-    aux = g.get_aux_kernel_time()
-    g.enable_kernel_timing(False)
+    kms, klaunch = ctx.get_kernel_time()
+    aux = ctx.get_aux_kernel_time()
+    ctx.enable_kernel_timing(False)
     peak_live = P.probe_fp64_tensor_tflops(f"cuda:{local}") if shared else None
-    roofline = iteration_roofline(P, p, info, args.config, kms, klaunch, aux, args.steps, peaks, peak_src, peak_live)
+    roofline = iteration_roofline(P, p_local, info, args.config, kms, klaunch, aux, args.steps, peaks, peak_src, peak_live)
     reduced = info["iteration"] == P.ITERATION_REDUCED
 
     # ---- end to end through the C ABI with host buffers
+    if barrier:
+        barrier()
     e2e_val, h2d, d2h = time_gpu_e2e(torch, g, p, args.steps)
-    _, e2e_val = aggregate_over_ranks(torch, 0.0, e2e_val, "cuda" if world > 1 else None)
+    if world > 1:
+        # every rank measured the whole slab's updates over its own clock: the job's figure is the slowest rank's
+        t = torch.tensor([e2e_val], dtype=torch.float64, device="cuda")
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MIN)
+        e2e_val = float(t.item())
+        _, h2d = aggregate_over_ranks(torch, 0.0, h2d, "cuda")
+        _, d2h = aggregate_over_ranks(torch, 0.0, d2h, "cuda")
+    setup_ms = ctx.get_setup_time()
     g.close()
     del g
     torch.cuda.empty_cache()
 
     # arrays a step streams: reduced form y (x2), z, yfix, ifix of J x 2N doubles each (+ one operator per cell on
     # the per-cell path); full form the two Psi buffers and c_fix
-    ws = p.unknowns * 4.0 * 5 if reduced else p.unknowns * 8.0 * 3
+    ws = p_local.unknowns * 4.0 * 5 if reduced else p_local.unknowns * 8.0 * 3
     if not shared:
-        ws += p.cells * (n // 2 + 4) * (n // 2) * 8.0 if reduced else p.cells * n * n * 8.0
-    l2_note = ("working set of a step %.0f MiB, larger than the 126 MB L2" % (ws / 2**20) if ws > 126e6 else
+        ws += p_local.cells * (n // 2 + 4) * (n // 2) * 8.0 if reduced else p_local.cells * n * n * 8.0
+    l2_note = ("working set of a step %.0f MiB per GPU, larger than the 126 MB L2" % (ws / 2**20) if ws > 126e6 else
                "working set of a step %.1f MiB fits L2 and is not flushed between steps (launch-latency-bound config)" % (ws / 2**20))
-    line = None
     if rank == 0:
         per_cfg = (per_config_table(torch, P, peaks, peak_src, peak_live or P.probe_fp64_tensor_tflops(f"cuda:{local}"))
                    if (world == 1 and not args.no_table) else None)
@@ -434,17 +506,23 @@ def run_ours(args):
         if world == 1 and not args.no_cpu:
             from oracle import threads_available
             th = threads_available()
-            r = time_oracle(args.config, 1 if args.config in (3, 4, 5) else 5, 0, th)
+            legs = oracle_legs(args.config, th)
+            r = legs["oci_all_cores"]
             cpu = {"value": r["value"], "unit": UNIT, "cores": th, "kind": "oracle", "sample": r["sample"],
-                   "ms_per_step_on_sample": r["ms_per_step"], "sample_cells": r["cells"]}
+                   "ms_per_step_on_sample": r["ms_per_step"], "sample_cells": r["cells"],
+                   "legs": {k: {"value": v["value"], "ms_per_step_on_sample": v["ms_per_step"], "sample": v["sample"], "iters": v["iters"]}
+                            for k, v in legs.items()}}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms / args.steps, "ms_per_step_median": float(np.median(each)), "ms_per_step_each": each,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": p.name, "S_N": p.n_angles, "cells": p.cells, "unknowns": p.unknowns, "tol": p.tol,
-                       "path": "shared" if shared else "per_cell", "parallelism": f"replicas x{world}" if world > 1 else "1 gpu",
+                       "path": "shared" if shared else "per_cell",
+                       "parallelism": (f"one slab sharded over {world} GPUs by cell ranges ({p_local.cells} cells each), halo + norm exchange "
+                                       "by peer-memory stores per iteration" if world > 1 else "1 gpu"),
                        "l2": l2_note},
-            "iters_per_step": iters, "time_to_converge_ms_per_step": ms / args.steps,
+            "iters_per_step": iters, "time_to_converge_ms_per_step": ms / args.steps, "setup_ms": setup_ms,
             "roofline": roofline, "cpu_baseline": cpu,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": int(launches), "clocks": clocks, "per_config": per_cfg,

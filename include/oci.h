@@ -58,8 +58,10 @@ enum { OCI_OK = 0, OCI_NOT_CONVERGED = 1, OCI_E_INVALID = -1, OCI_E_ORDER = -2, 
  * INCIDENT_ISOTROPIC: `value` is the incident ANGULAR flux psi_m for every
  * incoming direction, constant in time, used for both the k and k+1/2
  * balance equations.  REFLECTING: incident psi_m = outgoing psi_{N-1-m} of the
- * previous iterate (lagged in both OCI and SI). */
-enum { OCI_BC_VACUUM = 0, OCI_BC_INCIDENT_ISOTROPIC = 1, OCI_BC_REFLECTING = 2 };
+ * previous iterate (lagged in both OCI and SI).
+ * HALO (row f4, sharded slab): the face is a cut between two shards of one slab; the incident flux is the
+ * neighbour shard's outgoing flux of the previous iterate, delivered by oci_shard_attach's mailboxes. */
+enum { OCI_BC_VACUUM = 0, OCI_BC_INCIDENT_ISOTROPIC = 1, OCI_BC_REFLECTING = 2, OCI_BC_HALO = 3 };
 typedef struct { int32_t kind; double value; } oci_bc;
 
 /* Which kernel family oci_setup selected for the OCI apply (eq. 19):
@@ -122,7 +124,8 @@ typedef struct {
  * n_angles = N (even, 2 <= N <= 512: the setup and per-cell kernels stage O(4N)
  * doubles per CTA in shared memory).  Computes the Gauss-Legendre set on the host.
  * Errors: -1 if cells<1, N odd, <2 or >512, any dx<=0, Sigma<0, Sigma_s<0, v<=0,
- * dt<=0, a NULL pointer or an unknown BC kind. */
+ * dt<=0, a NULL pointer or an unknown BC kind.  A context with an OCI_BC_HALO face must be attached to
+ * its slab (oci_shard_attach) before it can step. */
 int oci_create(oci_ctx** out, int64_t cells, const double* dx, const double* sigma_t,
                const double* sigma_s, double v, double dt, int32_t n_angles, oci_bc left,
                oci_bc right);
@@ -147,7 +150,9 @@ int oci_set_flux(oci_ctx* ctx, const double* psi_edge);
 int oci_set_flux_dev(oci_ctx* ctx, const double* d_psi_edge);
 
 /* Isotropic source Q: HOST [cells][4] in slot order; NULL = 0; sticky
- * until the next call.  _dev: DEVICE pointer. */
+ * until the next call.  _dev: DEVICE pointer.  With a HOST pointer the call
+ * returns when the copy is done (the buffer may be reused at once); NULL and
+ * the _dev variant are asynchronous on the context's stream. */
 int oci_set_source(oci_ctx* ctx, const double* q);
 int oci_set_source_dev(oci_ctx* ctx, const double* d_q);
 
@@ -172,6 +177,31 @@ int si_step(oci_ctx* ctx, double tol, int32_t max_iters, int32_t* iters, double*
  * after oci_create; takes effect at the next oci_step.  Errors: -1. */
 int oci_set_iteration(oci_ctx* ctx, int32_t iteration);
 
+/* ---- Row f4: one slab sharded over several GPUs by contiguous cell ranges ----------------------
+ * Shard r of W is an ordinary context over its own cells (one process per GPU, or several contexts in one process)
+ * whose cut faces have kind OCI_BC_HALO: left face for r > 0, right face for r < W-1.  Within an iteration a
+ * shard owes each neighbour the N outgoing values of its edge cell and every rank needs the maximum over ranks of the
+ * two norms of the stopping rule; both travel as plain stores into peer memory (NVLink), issued by stream-ordered
+ * kernels behind every iteration launch, with no host involvement per iteration and no collective library.  Because
+ * the maximum is exact, every rank takes the same stopping decision and the iterates and iteration counts are those
+ * of the unsharded problem, bit for bit.  REDUCED form of oci_step only (si_step and the FULL form return -1).
+ *
+ * oci_shard_mailbox_bytes: DEVICE bytes of one rank's mailbox.  The caller allocates one mailbox per rank in memory
+ * every rank can address (peer-mapped / symmetric memory; 16-byte aligned) and passes all W device addresses, in rank
+ * order, to oci_shard_attach on every rank (HOST array of W DEVICE pointers; after oci_setup, before oci_set_flux).
+ * oci_shard_attach zeroes the rank's own mailbox on the context's stream: all ranks must have completed it (a
+ * barrier across ranks after a stream synchronise) before any rank steps.  Errors: -1 (rank / world out of range,
+ * W > 64, a cut face that is not HALO or a HALO face that is not a cut), -2.
+ *
+ * oci_shard_step advances n shards that live in THIS process by one time step, interleaving their launches
+ * (iteration, push, pull) so that on a single device and stream every pull is ordered behind all pushes; n = 1 is the
+ * one-process-per-GPU case, and oci_step on a sharded context is oci_shard_step with n = 1.  All shards of the slab,
+ * in this process or not, must be stepped with the same tol and max_iters.  iters / resid as oci_step (identical on
+ * every shard).  With n > 1 all contexts must share one device and one stream. */
+int64_t oci_shard_mailbox_bytes(int32_t n_angles, int32_t world);
+int oci_shard_attach(oci_ctx* ctx, int32_t rank, int32_t world, void* const* d_mailboxes);
+int oci_shard_step(oci_ctx* const* ctxs, int32_t n, double tol, int32_t max_iters, int32_t* iters, double* resid);
+
 /* Force the kernel family of the REDUCED form (default OCI_RKERNEL_AUTO).  Call BEFORE oci_setup; oci_setup
  * returns -1 if the forced family does not serve this problem (block size, number of blocks).  For tests and
  * for comparing families on shapes more than one serves.  Errors: -1 (unknown family). */
@@ -184,6 +214,15 @@ int oci_get_scalar_flux(const oci_ctx* ctx, double* phi);
 int oci_get_angular_flux(const oci_ctx* ctx, double* psi);
 int oci_get_scalar_flux_dev(const oci_ctx* ctx, double* d_phi);
 int oci_get_angular_flux_dev(const oci_ctx* ctx, double* d_psi);
+
+/* Streaming read-back for time-stepping loops: oci_get_scalar_flux_async snapshots phi of the current state on the
+ * context's stream (a device-to-device copy into a staging array, so the next step may overwrite phi) and copies the
+ * snapshot to `phi_pinned` (HOST, page-locked, [cells][4]) on a side stream, concurrently with whatever is queued
+ * next; it returns at once.  The data is valid after oci_synchronize (or the next oci_get_scalar_flux_async /
+ * oci_synchronize, which wait for the previous snapshot's copy).  oci_synchronize waits for everything this context
+ * has queued on its stream and its side stream.  Errors: -1, -2, -3. */
+int oci_get_scalar_flux_async(oci_ctx* ctx, double* phi_pinned);
+int oci_synchronize(oci_ctx* ctx);
 
 /* Quadrature in use: HOST mu[N], w[N], ascending mu. */
 int oci_get_quadrature(const oci_ctx* ctx, double* mu, double* w);

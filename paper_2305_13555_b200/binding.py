@@ -8,7 +8,7 @@ import numpy as np
 
 from . import build as _build
 
-BC_VACUUM, BC_INCIDENT_ISOTROPIC, BC_REFLECTING = 0, 1, 2
+BC_VACUUM, BC_INCIDENT_ISOTROPIC, BC_REFLECTING, BC_HALO = 0, 1, 2, 3
 PATH_SHARED, PATH_PER_CELL = 0, 1
 KERNEL_GENERIC, KERNEL_RESIDENT, KERNEL_KTILED, KERNEL_PER_CELL = 0, 1, 2, 3
 ITERATION_FULL, ITERATION_REDUCED, ITERATION_AUTO = 0, 1, 2
@@ -17,8 +17,8 @@ RKERNEL_AUTO, RKERNEL_GEMV, RKERNEL_RESIDENT, RKERNEL_KTILED, RKERNEL_OPREG = -1
 EXPORTED_SYMBOLS = [
     "oci_create", "oci_workspace_bytes", "oci_setup", "oci_set_flux", "oci_set_flux_dev", "oci_set_source",
     "oci_set_source_dev", "oci_step", "si_step", "oci_get_scalar_flux", "oci_get_angular_flux",
-    "oci_get_scalar_flux_dev", "oci_get_angular_flux_dev", "oci_get_quadrature", "oci_get_info",
-    "oci_get_block_inverse", "oci_enable_kernel_timing", "oci_get_kernel_time", "oci_get_aux_kernel_time", "oci_set_iteration", "oci_set_reduced_kernel", "oci_get_setup_time", "oci_launch_count",
+    "oci_get_scalar_flux_dev", "oci_get_angular_flux_dev", "oci_get_scalar_flux_async", "oci_synchronize", "oci_get_quadrature", "oci_get_info",
+    "oci_get_block_inverse", "oci_enable_kernel_timing", "oci_get_kernel_time", "oci_get_aux_kernel_time", "oci_set_iteration", "oci_set_reduced_kernel", "oci_get_setup_time", "oci_shard_mailbox_bytes", "oci_shard_attach", "oci_shard_step", "oci_launch_count",
     "oci_last_error", "oci_destroy",
 ]
 
@@ -75,6 +75,10 @@ def load_library():
         f = getattr(L, name)
         f.restype = C.c_int
         f.argtypes = [vp, dbl, i32, C.POINTER(i32), _dp]
+    L.oci_get_scalar_flux_async.restype = C.c_int
+    L.oci_get_scalar_flux_async.argtypes = [vp, vp]
+    L.oci_synchronize.restype = C.c_int
+    L.oci_synchronize.argtypes = [vp]
     L.oci_get_quadrature.restype = C.c_int
     L.oci_get_quadrature.argtypes = [vp, _dp, _dp]
     L.oci_get_info.restype = C.c_int
@@ -93,6 +97,12 @@ def load_library():
     L.oci_set_reduced_kernel.argtypes = [vp, i32]
     L.oci_get_setup_time.restype = C.c_int
     L.oci_get_setup_time.argtypes = [vp, _dp]
+    L.oci_shard_mailbox_bytes.restype = i64
+    L.oci_shard_mailbox_bytes.argtypes = [i32, i32]
+    L.oci_shard_attach.restype = C.c_int
+    L.oci_shard_attach.argtypes = [vp, i32, i32, C.POINTER(vp)]
+    L.oci_shard_step.restype = C.c_int
+    L.oci_shard_step.argtypes = [C.POINTER(vp), i32, dbl, i32, C.POINTER(i32), _dp]
     L.oci_launch_count.restype = i64
     L.oci_launch_count.argtypes = [vp]
     L.oci_last_error.restype = C.c_char_p
@@ -240,6 +250,14 @@ class OCI:
         self._check(self._L.oci_get_scalar_flux(self._h, _hp(a)))
         return a
 
+    def get_scalar_flux_async(self, pinned):
+        """`pinned`: a page-locked torch tensor [cells][4] float64 (torch.empty(...).pin_memory()); valid after synchronize()."""
+        assert pinned.is_pinned() and pinned.dtype.itemsize == 8 and pinned.numel() == self.cells * 4 and pinned.is_contiguous()
+        self._check(self._L.oci_get_scalar_flux_async(self._h, C.c_void_p(pinned.data_ptr())))
+
+    def synchronize(self):
+        self._check(self._L.oci_synchronize(self._h))
+
     def get_angular_flux(self):
         a = np.empty((self.cells, self.n_angles, 4))
         self._check(self._L.oci_get_angular_flux(self._h, _hp(a)))
@@ -287,6 +305,11 @@ class OCI:
     def set_reduced_kernel(self, kernel):
         self._check(self._L.oci_set_reduced_kernel(self._h, int(kernel)))
 
+    def shard_attach(self, rank, world, mailbox_ptrs):
+        """oci_shard_attach: `mailbox_ptrs` = the W device addresses (ints) of all ranks' mailboxes, in rank order."""
+        arr = (C.c_void_p * int(world))(*[C.c_void_p(int(p)) for p in mailbox_ptrs])
+        self._check(self._L.oci_shard_attach(self._h, int(rank), int(world), arr))
+
     def get_setup_time(self) -> float:
         ms = C.c_double(0.0)
         self._check(self._L.oci_get_setup_time(self._h, C.byref(ms)))
@@ -294,3 +317,18 @@ class OCI:
 
     def launch_count(self):
         return int(self._L.oci_launch_count(self._h))
+
+
+def shard_mailbox_bytes(n_angles, world) -> int:
+    return int(load_library().oci_shard_mailbox_bytes(int(n_angles), int(world)))
+
+
+def shard_step(shards, tol=1e-10, max_iters=10_000):
+    """oci_shard_step over the shards of one slab that live in this process (a list of OCI objects)."""
+    L = load_library()
+    arr = (C.c_void_p * len(shards))(*[s._h for s in shards])
+    it, res = C.c_int32(0), C.c_double(0.0)
+    rc = L.oci_shard_step(arr, len(shards), float(tol), int(max_iters), C.byref(it), C.byref(res))
+    if rc < 0:
+        raise OCIError(rc, L.oci_last_error(shards[0]._h).decode())
+    return rc, it.value, res.value

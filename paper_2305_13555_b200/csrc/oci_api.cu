@@ -43,6 +43,9 @@ struct oci_ctx {
     alignas(64) RedOpregMaps romaps{};
     bool use_ktiled = false;
     int32_t forced_rkernel = OCI_RKERNEL_AUTO;   // oci_set_reduced_kernel
+    // row f4: shard of a slab (shard_exchange.cu)
+    bool sharded = false;
+    unsigned long long xtag = 0;       // exchanges completed so far (the next one carries xtag + 1)
     int device = -1;                   // the device the workspace lives on; made current inside every entry point
     cudaStream_t stream = nullptr;
     void* ws = nullptr;
@@ -60,6 +63,9 @@ struct oci_ctx {
     unsigned long long* h_norms = nullptr;   // pinned
     cudaStream_t stream2 = nullptr;          // side stream of the norm read-back (REDUCED form)
     cudaEvent_t ev_norms = nullptr;
+    cudaEvent_t ev_snap = nullptr, ev_snap_done = nullptr;   // oci_get_scalar_flux_async
+    bool snap_pending = false;
+    double* phi_stage = nullptr;
     // timing
     bool timing = false;
     std::vector<cudaEvent_t> ev;
@@ -159,7 +165,7 @@ void gauss_legendre(int N, std::vector<double>& mu, std::vector<double>& w)
 
 struct Layout {
     int64_t binv, psi0, psi1, cfix, phi, Q, qs, dx, sig, sigs, blk, rep, mu, w, coef, ainv4, si_scan, phi_part, norms, tickets, flags,
-        xop, rop, fop, y0, y1, z, yfix, ifix, phifix, q16, gitems, perm, team_bar, total;
+        xop, rop, fop, y0, y1, z, yfix, ifix, phifix, q16, gitems, perm, team_bar, peers, phi_stage, total;
 };
 
 int64_t align_up(int64_t x) { return (x + 255) & ~int64_t(255); }
@@ -209,6 +215,8 @@ Layout make_layout(int64_t J, int32_t N, int64_t nblk)
     }
     L.perm = take(nblk * n * 4);
     L.team_bar = take(4096 * 4);
+    L.peers = take(64 * 8);
+    L.phi_stage = take(J * 4 * 8);
     L.total = o;
     return L;
 }
@@ -247,7 +255,7 @@ void classify(oci_ctx* c)
 
 bool bc_ok(const oci_bc& b)
 {
-    return b.kind == OCI_BC_VACUUM || b.kind == OCI_BC_INCIDENT_ISOTROPIC || b.kind == OCI_BC_REFLECTING;
+    return b.kind == OCI_BC_VACUUM || b.kind == OCI_BC_INCIDENT_ISOTROPIC || b.kind == OCI_BC_REFLECTING || b.kind == OCI_BC_HALO;
 }
 
 int launch_oci_iteration_any(oci_ctx* ctx, int src, int slot, int prev_slot, double tol)
@@ -290,12 +298,95 @@ int ensure_psi(oci_ctx* ctx)
     return k;
 }
 
+// Row f4: one time step of n shards that live in this process (n = 1: one process per GPU).  REDUCED form, one launch
+// per iteration followed by the halo / norm exchange (shard_exchange.cu); launches of the shards are interleaved so
+// that on one device and stream every pull is ordered behind every push.
+int run_step_sharded(oci_ctx* const* cs, int32_t n, double tol, int32_t max_iters, int32_t* iters, double* resid)
+{
+    oci_ctx* ctx = cs[0];                                                    // errors are reported on the first shard
+    for (int32_t c = 0; c < n; ++c) {
+        if (!cs[c]) return fail(ctx, OCI_E_INVALID, "NULL shard");
+        if (!cs[c]->ready || !cs[c]->sharded) return fail(ctx, OCI_E_ORDER, "shard not set up or not attached");
+        if (!cs[c]->have_flux) return fail(ctx, OCI_E_ORDER, "step before oci_set_flux");
+        if (n > 1 && (cs[c]->stream != ctx->stream || cs[c]->device != ctx->device))
+            return fail(ctx, OCI_E_INVALID, "shards stepped together must share one device and one stream");
+        if (cs[c]->iteration == OCI_ITERATION_FULL) return fail(ctx, OCI_E_INVALID, "the FULL form is not available on a sharded context");
+    }
+    if (max_iters < 1 || tol != tol) return fail(ctx, OCI_E_INVALID, "max_iters < 1 or tol is NaN");
+    DeviceGuard guard(ctx);
+#define EACH for (int32_t c_ = 0; c_ < n; ++c_)
+#define C_ cs[c_]
+    // the packed state and, after oci_set_flux, the neighbours' edge values in the ghost rows
+    bool fresh = false;
+    EACH if (!C_->yz_valid) fresh = true;
+    if (fresh) {
+        EACH {
+            oci_ctx* ctx = C_;
+            if (!ctx->yz_valid) { LAUNCH(launch_pack_yz(ctx->V, ctx->cur, 0, ctx->stream)); ctx->ycur = 0; ctx->yz_valid = true; }
+        }
+        // (all shards of a slab are restarted together, so every rank takes this branch in the same step)
+        EACH { oci_ctx* ctx = C_; LAUNCH(launch_shard_push(ctx->V, ctx->ycur, -1, -1, tol, ctx->xtag + 1, ctx->stream)); }
+        EACH { oci_ctx* ctx = C_; LAUNCH(launch_shard_pull(ctx->V, ctx->ycur, -1, -1, tol, ctx->xtag + 1, ctx->stream)); }
+        EACH C_->xtag += 1;
+    }
+    EACH { oci_ctx* ctx = C_; ctx->psi_valid = false; LAUNCH(launch_reduced_pass(ctx, PASS_FIX, ctx->ycur, 0, -1, tol, 0, 0)); }
+    int32_t done_iters = 0;
+    bool conv = false;
+    double d = 0.0, r = 0.0;
+    const int32_t guess = ctx->predicted[0] > 0 ? ctx->predicted[0] + 1 : 8;
+    while (done_iters < max_iters && !conv) {
+        int32_t cnt = guess - done_iters;
+        if (cnt < 4) cnt = 4;
+        if (cnt > kNormSlots) cnt = kNormSlots;
+        if (cnt > max_iters - done_iters) cnt = max_iters - done_iters;
+        if (done_iters > 0) EACH { oci_ctx* ctx = C_; CK(cudaMemsetAsync(ctx->V.norms, 0, sizeof(unsigned long long) * 2 * cnt, ctx->stream)); }
+        for (int32_t i = 0; i < cnt; ++i) {
+            EACH { oci_ctx* ctx = C_; LAUNCH(launch_reduced_pass(ctx, PASS_ITER, (ctx->ycur + done_iters + i) & 1, i, i - 1, tol, 0, 0)); }
+            EACH { oci_ctx* ctx = C_; LAUNCH(launch_shard_push(ctx->V, (ctx->ycur + done_iters + i + 1) & 1, i, i - 1, tol, ctx->xtag + 1 + i, ctx->stream)); }
+            EACH { oci_ctx* ctx = C_; LAUNCH(launch_shard_pull(ctx->V, (ctx->ycur + done_iters + i + 1) & 1, i, i - 1, tol, ctx->xtag + 1 + i, ctx->stream)); }
+        }
+        EACH { oci_ctx* ctx = C_; LAUNCH(launch_reduced_pass(ctx, PASS_FINAL, (ctx->ycur + done_iters) & 1, 0, -1, tol, cnt, done_iters + cnt >= max_iters)); }
+        // the norms are global after the pull, so any shard's copy tells the iteration count
+        CK(cudaMemcpyAsync(ctx->h_norms, ctx->V.norms, sizeof(unsigned long long) * 2 * cnt, cudaMemcpyDeviceToHost, ctx->stream));
+        EACH { oci_ctx* ctx = C_; CK(cudaStreamSynchronize(ctx->stream)); }
+        CK(cudaGetLastError());
+        int32_t executed = cnt;
+        for (int32_t i = 0; i < cnt; ++i) {
+            std::memcpy(&d, &ctx->h_norms[2 * i], 8);
+            std::memcpy(&r, &ctx->h_norms[2 * i + 1], 8);
+            if (stop_now(tol, d, r)) { conv = true; executed = i + 1; break; }
+        }
+        done_iters += executed;
+        EACH C_->xtag += (unsigned long long)executed;                      // exchanges that really ran: parities keep alternating
+    }
+    EACH {
+        C_->ycur = (C_->ycur + done_iters) & 1;
+        C_->predicted[0] = done_iters;
+    }
+#undef EACH
+#undef C_
+    if (iters) *iters = done_iters;
+    if (!finite_norms(d, r)) {
+        if (resid) *resid = d;
+        return fail(ctx, OCI_E_NONFINITE, "the scalar flux became NaN or Inf (non-finite input or overflow); restart with oci_set_flux");
+    }
+    if (resid) *resid = (r > 0.0) ? d / r : d;
+    return conv ? OCI_OK : OCI_NOT_CONVERGED;
+}
+
 int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iters, double* resid)
 {
     if (!ctx) return OCI_E_INVALID;
     if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "step before oci_setup");
     if (!ctx->have_flux) return fail(ctx, OCI_E_ORDER, "step before oci_set_flux");
     if (max_iters < 1 || tol != tol) return fail(ctx, OCI_E_INVALID, "max_iters < 1 or tol is NaN");
+    const bool halo = ctx->bcL.kind == OCI_BC_HALO || ctx->bcR.kind == OCI_BC_HALO;
+    if (halo && !ctx->sharded) return fail(ctx, OCI_E_ORDER, "a context with an OCI_BC_HALO face must be attached with oci_shard_attach");
+    if (ctx->sharded) {
+        if (si) return fail(ctx, OCI_E_INVALID, "si_step is not available on a sharded context");
+        oci_ctx* one = ctx;
+        return run_step_sharded(&one, 1, tol, max_iters, iters, resid);
+    }
     DeviceGuard guard(ctx);
     DevView& V = ctx->V;
     cudaStream_t s = ctx->stream;
@@ -515,6 +606,13 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     V.ngroups = 0;
     V.perm = (int32_t*)(base + L.perm);
     V.team_bar = (int32_t*)(base + L.team_bar);
+    V.peers = (unsigned long long*)(base + L.peers);
+    ctx->phi_stage = (double*)(base + L.phi_stage);
+    ctx->snap_pending = false;
+    V.rank = 0;
+    V.world = 1;
+    ctx->sharded = false;
+    ctx->xtag = 0;
     V.v = ctx->v; V.dt = ctx->dt;
     V.bcL = ctx->bcL.kind; V.bcR = ctx->bcR.kind;
     V.bcLv = ctx->bcL.value; V.bcRv = ctx->bcR.value;
@@ -609,6 +707,8 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     if (!ctx->stream2) {
         CK(cudaStreamCreateWithFlags(&ctx->stream2, cudaStreamNonBlocking));
         CK(cudaEventCreateWithFlags(&ctx->ev_norms, cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&ctx->ev_snap, cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&ctx->ev_snap_done, cudaEventDisableTiming));
     }
     ctx->use_ktiled = ctx->path == OCI_PATH_SHARED && !oci_shared_fast_supported(V) && oci_ktiled_supported(V) &&
                       oci_ktiled_prepare(V, &ctx->maps);
@@ -682,7 +782,7 @@ int oci_set_source(oci_ctx* ctx, const double* q)
     if (q) CK(cudaMemcpyAsync(ctx->V.Q, q, (size_t)ctx->J * 4 * 8, cudaMemcpyHostToDevice, ctx->stream));
     else CK(cudaMemsetAsync(ctx->V.Q, 0, (size_t)ctx->J * 4 * 8, ctx->stream));
     if (int rc = refresh_q16(ctx)) return rc;
-    CK(cudaStreamSynchronize(ctx->stream));
+    if (q) CK(cudaStreamSynchronize(ctx->stream));      // the caller may reuse its buffer at once; Q = 0 needs no host data
     return OCI_OK;
 }
 
@@ -743,6 +843,34 @@ int oci_get_angular_flux_dev(const oci_ctx* ctx, double* d_psi)
     if (int rc = unpack_for_get(const_cast<oci_ctx*>(ctx))) return rc;
     return get_common(ctx, d_psi, ctx ? ctx->V.psi[ctx->cur] : nullptr, ctx ? (size_t)ctx->J * ctx->n * 8 : 0,
                       cudaMemcpyDeviceToDevice, false);
+}
+
+int oci_get_scalar_flux_async(oci_ctx* ctx, double* phi_pinned)
+{
+    if (!ctx || !phi_pinned) return fail(ctx, OCI_E_INVALID, "NULL argument");
+    if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "get before oci_setup");
+    DeviceGuard guard(ctx);
+    const size_t bytes = (size_t)ctx->J * 32;
+    // the staging array is free once the previous snapshot has left it
+    if (ctx->snap_pending) CK(cudaStreamWaitEvent(ctx->stream, ctx->ev_snap_done, 0));
+    CK(cudaMemcpyAsync(ctx->phi_stage, ctx->V.phi, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    CK(cudaEventRecord(ctx->ev_snap, ctx->stream));
+    CK(cudaStreamWaitEvent(ctx->stream2, ctx->ev_snap, 0));
+    CK(cudaMemcpyAsync(phi_pinned, ctx->phi_stage, bytes, cudaMemcpyDeviceToHost, ctx->stream2));
+    CK(cudaEventRecord(ctx->ev_snap_done, ctx->stream2));
+    ctx->snap_pending = true;
+    return OCI_OK;
+}
+
+int oci_synchronize(oci_ctx* ctx)
+{
+    if (!ctx) return OCI_E_INVALID;
+    if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_synchronize before oci_setup");
+    DeviceGuard guard(ctx);
+    CK(cudaStreamSynchronize(ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream2));
+    ctx->snap_pending = false;
+    return OCI_OK;
 }
 
 int oci_get_quadrature(const oci_ctx* ctx, double* mu, double* w)
@@ -813,6 +941,42 @@ int oci_set_iteration(oci_ctx* ctx, int32_t iteration)
     return OCI_OK;
 }
 
+int64_t oci_shard_mailbox_bytes(int32_t n_angles, int32_t world)
+{
+    if (n_angles < 2 || world < 1 || world > 64) return 0;
+    return 8 * (4 * (int64_t)n_angles + 4 * (int64_t)world + (int64_t)world);
+}
+
+int oci_shard_attach(oci_ctx* ctx, int32_t rank, int32_t world, void* const* d_mailboxes)
+{
+    if (!ctx || !d_mailboxes) return fail(ctx, OCI_E_INVALID, "NULL argument");
+    if (!ctx->ready) return fail(ctx, OCI_E_ORDER, "oci_shard_attach before oci_setup");
+    if (world < 1 || world > 64 || rank < 0 || rank >= world) return fail(ctx, OCI_E_INVALID, "rank / world out of range (world <= 64)");
+    if ((ctx->bcL.kind == OCI_BC_HALO) != (rank > 0) || (ctx->bcR.kind == OCI_BC_HALO) != (rank < world - 1))
+        return fail(ctx, OCI_E_INVALID, "exactly the cut faces of a shard must be OCI_BC_HALO");
+    unsigned long long ptrs[64] = {0};
+    for (int32_t r = 0; r < world; ++r) {
+        if (!d_mailboxes[r] || ((uintptr_t)d_mailboxes[r] & 15) != 0) return fail(ctx, OCI_E_INVALID, "NULL or misaligned mailbox");
+        ptrs[r] = (unsigned long long)(uintptr_t)d_mailboxes[r];
+    }
+    DeviceGuard guard(ctx);
+    CK(cudaMemcpyAsync(ctx->V.peers, ptrs, sizeof(unsigned long long) * world, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemsetAsync(d_mailboxes[rank], 0, (size_t)oci_shard_mailbox_bytes(ctx->N, world), ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));                                 // `ptrs` is on the stack
+    ctx->V.rank = rank;
+    ctx->V.world = world;
+    ctx->sharded = true;
+    ctx->xtag = 0;
+    ctx->iteration = OCI_ITERATION_REDUCED;
+    return OCI_OK;
+}
+
+int oci_shard_step(oci_ctx* const* ctxs, int32_t n, double tol, int32_t max_iters, int32_t* iters, double* resid)
+{
+    if (!ctxs || n < 1 || !ctxs[0]) return OCI_E_INVALID;
+    return run_step_sharded(ctxs, n, tol, max_iters, iters, resid);
+}
+
 int oci_set_reduced_kernel(oci_ctx* ctx, int32_t kernel)
 {
     if (!ctx) return OCI_E_INVALID;
@@ -850,6 +1014,8 @@ void oci_destroy(oci_ctx* ctx)
     if (ctx->h_norms) cudaFreeHost(ctx->h_norms);
     if (ctx->stream2) cudaStreamDestroy(ctx->stream2);
     if (ctx->ev_norms) cudaEventDestroy(ctx->ev_norms);
+    if (ctx->ev_snap) cudaEventDestroy(ctx->ev_snap);
+    if (ctx->ev_snap_done) cudaEventDestroy(ctx->ev_snap_done);
     for (auto& e : ctx->ev) cudaEventDestroy(e);
     for (auto& e : ctx->ev_aux) if (e) cudaEventDestroy(e);
     delete ctx;

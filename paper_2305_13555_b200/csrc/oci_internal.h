@@ -62,6 +62,9 @@ struct DevView {
     int32_t bcL, bcR;
     double bcLv, bcRv;
     int32_t sm_count;           // SMs of the device the workspace lives on (queried once in oci_setup)
+    // ---- row f4: this context is shard `rank` of `world` (shard_exchange.cu); world = 1 when not sharded
+    int32_t rank, world;
+    unsigned long long* peers;  // [world] device addresses of every rank's mailbox (peer mapped), in the workspace
 };
 
 // Tensor maps of the K-tiled shared-block kernel (oci_iter_shared_ktiled.cu), encoded once in oci_setup.
@@ -145,6 +148,8 @@ bool oci_red_ktiled_supported(const DevView& V);
 bool oci_red_ktiled_prepare(const DevView& V, RedKtiledMaps* M);
 int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int ybase, int slot, int prev_slot, double tol,
                       int cnt, int force, cudaStream_t s);
+int launch_shard_push(const DevView& V, int ybuf, int slot, int prev_slot, double tol, unsigned long long tag, cudaStream_t s);
+int launch_shard_pull(const DevView& V, int ybuf, int slot, int prev_slot, double tol, unsigned long long tag, cudaStream_t s);
 bool oci_red_opreg_supported(const DevView& V);
 bool oci_red_opreg_prepare(const DevView& V, RedOpregMaps* M);
 int launch_red_opreg(const DevView& V, const RedOpregMaps& M, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,

@@ -303,6 +303,32 @@ def test_not_converged_status_and_restart(iteration):
     g.close(); g2.close()
 
 
+def test_async_scalar_flux_snapshots():
+    """oci_get_scalar_flux_async: the snapshot of step k (taken on the stream, copied out on the side stream while
+    step k+1 runs) must equal the synchronous read-back of the same step, for every step, with two alternating pinned
+    buffers as bench.py's end-to-end leg uses them."""
+    import torch
+    import paper_2305_13555_b200 as P
+    p = make_problem(2, cells=700)
+    a, b = P.OCI.from_problem(p), P.OCI.from_problem(p)
+    bufs = [torch.empty((p.cells, 4), dtype=torch.float64).pin_memory() for _ in range(2)]
+    want, got = [], []
+    for k in range(5):
+        for g in (a, b):
+            g.set_source(p.source(k))
+            g.oci_step(p.tol, p.max_iters)
+        want.append(a.get_scalar_flux().copy())
+        b.get_scalar_flux_async(bufs[k & 1])
+        if k >= 1:                                   # the previous snapshot is complete once the next one has been queued ...
+            b.synchronize()                          # ... and synchronised
+            got.append(bufs[k & 1].numpy().copy())
+    b.synchronize()
+    assert np.array_equal(bufs[0].numpy(), want[4])
+    for k, snap in enumerate(got, start=1):
+        assert np.array_equal(snap, want[k])
+    a.close(); b.close()
+
+
 def test_api_errors_on_device():
     import paper_2305_13555_b200 as P
     g = P.OCI(np.ones(4), np.ones(4), np.full(4, 0.5), 1.0, 0.1, 4)
