@@ -165,7 +165,7 @@ void gauss_legendre(int N, std::vector<double>& mu, std::vector<double>& w)
 
 struct Layout {
     int64_t binv, psi0, psi1, cfix, phi, Q, qs, dx, sig, sigs, blk, rep, mu, w, coef, ainv4, si_scan, phi_part, norms, tickets, flags,
-        xop, rop, fop, y0, y1, z, yfix, ifix, phifix, q16, gitems, perm, team_bar, peers, phi_stage, total;
+        xop, rop, fop, y0, y1, z, yfix, ifix, phifix, q16, gitems, perm, team_bar, peers, phi_stage, si_part, si_inflow, si_src1, total;
 };
 
 int64_t align_up(int64_t x) { return (x + 255) & ~int64_t(255); }
@@ -217,6 +217,9 @@ Layout make_layout(int64_t J, int32_t N, int64_t nblk)
     L.team_bar = take(4096 * 4);
     L.peers = take(64 * 8);
     L.phi_stage = take(J * 4 * 8);
+    L.si_part = take((N / 32 > 2 ? N / 32 : 2) * J * 4 * 8);
+    L.si_inflow = take(2 * N * 2 * 8);
+    L.si_src1 = take(J * 4 * 8);
     L.total = o;
     return L;
 }
@@ -392,6 +395,7 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
     cudaStream_t s = ctx->stream;
     const bool red = !si && resolved_iteration(ctx) == OCI_ITERATION_REDUCED;
     const bool timed = ctx->timing && !si;
+    const bool si_fast = si && si_fast_supported(V);                     // phi-only iterations, Psi once at the end
 
     if (red) {
         if (!ctx->yz_valid) {
@@ -406,7 +410,8 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
     } else {
         LAUNCH(ensure_psi(ctx));
         ctx->yz_valid = false;
-        LAUNCH(launch_cfix(V, ctx->cur, s));                      // a2 (+ a8 of the previous step)
+        if (si_fast) LAUNCH(launch_si_fast_begin(V, ctx->cur, s));          // psi_{k-1/2}, compact (+ a8 of the previous step)
+        else LAUNCH(launch_cfix(V, ctx->cur, s));                 // a2 (+ a8 of the previous step)
     }
     int32_t done_iters = 0;
     bool conv = false;
@@ -431,7 +436,8 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
         }
         for (int32_t i = 0; i < cnt && !fused_loop; ++i) {
             if (timed) CK(cudaEventRecord(ctx->ev[2 * i], s));
-            if (si) LAUNCH(launch_si_iteration(V, ctx->cur, i, i - 1, tol, s));
+            if (si_fast) LAUNCH(launch_si_fast_iteration(V, ctx->cur, done_iters + i, i, i - 1, tol, s));
+            else if (si) LAUNCH(launch_si_iteration(V, ctx->cur, i, i - 1, tol, s));
             else if (red) LAUNCH(launch_reduced_pass(ctx, PASS_ITER, (ctx->ycur + done_iters + i) & 1, i, i - 1, tol, 0, 0));
             else LAUNCH(launch_oci_iteration_any(ctx, (ctx->cur + done_iters + i) & 1, i, i - 1, tol));
             if (timed) CK(cudaEventRecord(ctx->ev[2 * i + 1], s));
@@ -452,6 +458,7 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
             LAUNCH(launch_reduced_pass(ctx, PASS_FINAL, (ctx->ycur + done_iters) & 1, 0, -1, tol, cnt, done_iters + cnt >= max_iters));
             if (timed) CK(cudaEventRecord(ctx->ev_aux[3], s));
         }
+        if (si_fast) LAUNCH(launch_si_fast_final(V, ctx->cur, done_iters, tol, cnt, done_iters + cnt >= max_iters, s));
         if (side_readback) {
             CK(cudaStreamSynchronize(ctx->stream2));                        // the one read-back (a7)
         } else {
@@ -608,6 +615,10 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     V.team_bar = (int32_t*)(base + L.team_bar);
     V.peers = (unsigned long long*)(base + L.peers);
     ctx->phi_stage = (double*)(base + L.phi_stage);
+    V.si_prev = V.cfix;
+    V.si_part = (double*)(base + L.si_part);
+    V.si_inflow = (double*)(base + L.si_inflow);
+    V.si_src1 = (double*)(base + L.si_src1);
     ctx->snap_pending = false;
     V.rank = 0;
     V.world = 1;

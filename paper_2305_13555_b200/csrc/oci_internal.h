@@ -39,6 +39,10 @@ struct DevView {
     double* coef;               // [n]  |mu_m| on the rows that take an incident flux, else 0
     double* ainv4;              // [nblk][N][16]  (A_m)^{-1} for SI
     double* si_scan;            // [chunks][N][8]  SI scan: chunk maps (P, z) and chunk inflows (si_sweep.cu)
+    double* si_prev;            // [J][N][2]  psi_{k-1/2}, compact (si_sweep_fast.cu; aliases c_fix, which SI then does not use)
+    double* si_part;            // [max(2, N/32)][J][4]  scalar-flux partials per lane group (si_sweep_fast.cu)
+    double* si_src1;            // [J][4]  second buffer of the SI scattering source (the first is qs), by iteration parity
+    double* si_inflow;          // [2][N][2]  boundary inflow of every angle, by iteration parity (si_sweep_fast.cu)
     double* phi_part;           // [ceil(n/128)][J][4]  per-item scalar-flux partials (K-tiled kernel)
     int32_t* tickets;           // [ceil(J/64)]  arrival counters of the K-tiled kernel's cell tiles (0 between launches)
     unsigned long long* norms;  // [kNormSlots][2]  bit patterns of (d, r), atomicMax targets
@@ -131,6 +135,11 @@ int launch_phi_norm(const DevView& V, int buf, int slot, int prev_slot, double t
 int launch_oci_iteration(const DevView& V, int path, int src, int slot, int prev_slot, double tol,
                          cudaStream_t s);
 int launch_si_iteration(const DevView& V, int buf, int slot, int prev_slot, double tol, cudaStream_t s);
+// fast form (si_sweep_fast.cu): N/2 a power of two
+bool si_fast_supported(const DevView& V);
+int launch_si_fast_begin(const DevView& V, int buf, cudaStream_t s);
+int launch_si_fast_iteration(const DevView& V, int buf, int it, int slot, int prev_slot, double tol, cudaStream_t s);
+int launch_si_fast_final(const DevView& V, int buf, int it0, double tol, int cnt, int force, cudaStream_t s);
 // interface-reduced step (oci_reduced.cu, oci_reduced_resident.cu, oci_reduced_ktiled.cu)
 enum { PASS_FIX = 0, PASS_ITER = 1, PASS_FINAL = 2 };
 int launch_pack_operators(const DevView& V, cudaStream_t s);

@@ -496,3 +496,23 @@ def test_converged_branches(scheme):
     # r = 0 at tol = 0 as well (0 <= 0 * 0)
     z.set_flux(np.zeros((3, 2, 2)))
     assert step(z, 0.0, 100)[:2] == (0, 1)
+
+
+# ----------------------------------------------------------------- Fig. 1-style map, row f4's second half
+def test_rho_map_trends_and_stored_table():
+    """`python -m oracle.rho_map` (steady S4, reflecting): what P:31 and P:37 state must hold over the whole grid -
+    rho_OCI falls monotonically as the cell optical thickness grows, rho_SI "depends strongly on the scattering ratio
+    and is nearly independent of cell optical thickness" (within a few per cent of c once cells are >= 0.5 mfp), OCI
+    loses to SI on thin cells and wins on thick ones - and the committed table is what the script writes."""
+    import os
+    from oracle import rho_map
+    txt, grid = rho_map.table(24)
+    for c in rho_map.CS:
+        oci = [grid[(th, c)][0] for th in rho_map.THICK]
+        assert all(a > b for a, b in zip(oci, oci[1:])), (c, oci)
+        for th in rho_map.THICK:
+            if th >= 0.5:
+                assert abs(grid[(th, c)][1] - c) < 0.09 * c, (th, c, grid[(th, c)])
+        assert grid[(0.05, c)][0] > grid[(0.05, c)][1] and grid[(10.0, c)][0] < grid[(10.0, c)][1]
+    stored = open(os.path.join(os.path.dirname(rho_map.__file__), "rho_map_S4.txt")).read()
+    assert stored == txt
