@@ -221,6 +221,100 @@ def oracle_legs(cfg, threads):
     return legs
 
 
+class CpuBlasReduced:
+    """A TUNED CPU restatement of the algorithm the GPU arm runs, for a fair CPU figure next to the (deliberately
+    plain) oracle: shared block, the block inverse formed once with LAPACK, and the interface-reduced iteration of
+    DESIGN.md 6.7 - y^(l+1) = yfix + inc G^T, phi^(l+1) = phifix + inc H^T - as two threaded BLAS dgemms per
+    iteration at the FULL cell count.  The matrix B comes from the oracle's `cell_matrix` (this is bench.py's CPU
+    leg, the one place outside tests/ that may call oracle/); everything else is numpy.  Not used for parity."""
+
+    def __init__(self, p):
+        from oracle import cell_matrix, gauss_legendre
+        assert np.all(p.dx == p.dx[0]) and np.all(p.sigma_t == p.sigma_t[0]) and np.all(p.sigma_s == p.sigma_s[0])
+        self.p, N, J = p, p.n_angles, p.cells
+        self.mu, self.w = gauss_legendre(N)
+        h = float(p.dx[0])
+        Binv = np.linalg.inv(cell_matrix(self.mu, self.w, h, float(p.sigma_t[0]), float(p.sigma_s[0]), p.v, p.dt))
+        m = np.arange(N)
+        neg = self.mu < 0
+        # I: rows that receive an incident flux (k slot, then k+1/2 slot); O = the partner slots a neighbour reads
+        self.I = np.concatenate([4 * m + np.where(neg, 1, 0), 4 * m + np.where(neg, 3, 2)])
+        self.O = self.I ^ 1
+        self.from_right = np.concatenate([neg, neg])                 # mu < 0: the value comes from cell j+1
+        amu = np.abs(np.concatenate([self.mu, self.mu]))
+        W = np.zeros((4, 4 * N))
+        for s_ in range(4):
+            W[s_, 4 * m + s_] = self.w
+        self.G = np.ascontiguousarray((Binv[np.ix_(self.O, self.I)] * amu).T)        # [2N][2N], applied as inc @ G
+        self.H = np.ascontiguousarray(((W @ Binv)[:, self.I] * amu).T)               # [2N][4]
+        self.Binv, self.W, self.alpha, self.h = Binv, W, h / (2 * p.v * p.dt), h
+        self.mirror = np.concatenate([N - 1 - m, N + (N - 1 - m)])   # packed index of the mirror angle, same time slot
+        self.Y = np.zeros((J + 2, 2 * N))                            # O rows of the iterate with ghost rows 0 and J+1
+        psi = np.empty((J, N, 4))
+        psi[:, :, 0] = psi[:, :, 2] = p.psi0[:, :, 0]
+        psi[:, :, 1] = psi[:, :, 3] = p.psi0[:, :, 1]
+        self.Psi = psi.reshape(J, 4 * N)
+        self.phi = self.Psi @ W.T
+
+    def _ghosts(self):
+        p, Y = self.p, self.Y
+        for side, bc, row, src in ((0, p.bc_left, 0, 1), (1, p.bc_right, -1, -2)):
+            if bc[0] == 2:
+                Y[row] = Y[src][self.mirror]
+            else:
+                Y[row] = bc[1] if bc[0] == 1 else 0.0
+
+    def step(self, q, tol, max_iters):
+        p, J, N = self.p, self.p.cells, self.p.n_angles
+        cfix = np.zeros((J, 4 * N))
+        if q is not None:
+            cfix += 0.25 * self.h * np.tile(q, (1, N))
+        prev = self.Psi.reshape(J, N, 4)[:, :, 2:]
+        cfix.reshape(J, N, 4)[:, :, :2] += self.alpha * prev
+        fix = cfix @ self.Binv.T                                       # Psi_fix, once per step
+        yfix, phifix = np.ascontiguousarray(fix[:, self.O]), fix @ self.W.T
+        self.Y[1:-1] = self.Psi[:, self.O]
+        inc = np.empty((J, 2 * N))
+        it, d, r = 0, 0.0, 0.0
+        while it < max_iters:
+            self._ghosts()
+            inc[:, self.from_right] = self.Y[2:, self.from_right]
+            inc[:, ~self.from_right] = self.Y[:-2, ~self.from_right]
+            ynew = yfix + inc @ self.G
+            phinew = phifix + inc @ self.H
+            d, r = np.max(np.abs(phinew - self.phi)), np.max(np.abs(phinew))
+            self.Y[1:-1], self.phi = ynew, phinew
+            it += 1
+            if tol >= 0 and d <= tol * r:
+                break
+        # the I rows of the converged iterate from the last gathered inc (the FINAL pass)
+        F = (self.Binv[np.ix_(self.I, self.I)] * np.abs(np.concatenate([self.mu, self.mu]))).T
+        self.Psi[:, self.O] = self.Y[1:-1]
+        self.Psi[:, self.I] = fix[:, self.I] + inc @ F
+        return it
+
+
+def time_cpu_blas(cfg, steps):
+    """Unknown-updates/s of the tuned CPU restatement (CpuBlasReduced) at the config's FULL size; None for per-cell
+    configs (a batched GEMV over 2 GiB of inverses is not a BLAS-3 problem)."""
+    if cfg == 5:
+        return None
+    p = make_problem(cfg)
+    c = CpuBlasReduced(p)
+    c.step(p.source(0), p.tol, p.max_iters)                            # warm-up (BLAS thread pool, page faults)
+    updates, t0 = 0, time.perf_counter()
+    for k in range(1, 1 + steps):
+        updates += p.unknowns * c.step(p.source(k), p.tol, p.max_iters)
+    dt = time.perf_counter() - t0
+    try:
+        import threadpoolctl
+        th = max([i.get("num_threads", 1) for i in threadpoolctl.threadpool_info()] + [1])
+    except Exception:
+        th = os.cpu_count()
+    return {"value": updates / dt, "unit": UNIT, "ms_per_step": dt / steps * 1e3, "threads": th, "cells": p.cells,
+            "kind": "numpy + threaded BLAS, pre-inverted block, interface-reduced iteration (same algorithm as the GPU arm), full size"}
+
+
 def run_reference(args):
     rank, world, _ = dist_env()
     if rank != 0:
@@ -511,7 +605,8 @@ def run_ours(args):
             cpu = {"value": r["value"], "unit": UNIT, "cores": th, "kind": "oracle", "sample": r["sample"],
                    "ms_per_step_on_sample": r["ms_per_step"], "sample_cells": r["cells"],
                    "legs": {k: {"value": v["value"], "ms_per_step_on_sample": v["ms_per_step"], "sample": v["sample"], "iters": v["iters"]}
-                            for k, v in legs.items()}}
+                            for k, v in legs.items()},
+                   "tuned_same_algorithm": time_cpu_blas(args.config, 2)}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "ms_per_step_median": float(np.median(each)), "ms_per_step_each": each,
