@@ -103,7 +103,7 @@ enum { OCI_ITERATION_FULL = 0, OCI_ITERATION_REDUCED = 1, OCI_ITERATION_AUTO = 2
  * KTILED - shared block, or 2..16 distinct blocks (a multi-region slab), N a multiple of 16: operands
  *          streamed in K chunks by tensor-map TMA, fp64 tensor pipe; a block is a row offset into the
  *          stacked operators, a tile of cells that straddles an interface is done once per block;
- * OPREG - ONE shared block, N in {64, 128} (config 4): each CTA keeps 64 operator rows as DMMA fragments in
+ * OPREG - ONE shared block, N in {32, 64, 128} (config 4; N = 32 only when forced): each CTA keeps 64 operator rows as DMMA fragments in
  *          registers for the whole launch and only the cell rows stream (tensor-map TMA); fp64 tensor pipe.
  * oci_setup picks RESIDENT, else OPREG, else KTILED, else GEMV; oci_set_reduced_kernel overrides. */
 enum { OCI_RKERNEL_AUTO = -1, OCI_RKERNEL_GEMV = 0, OCI_RKERNEL_RESIDENT = 1, OCI_RKERNEL_KTILED = 2, OCI_RKERNEL_OPREG = 3 };

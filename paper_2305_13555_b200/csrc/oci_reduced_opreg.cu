@@ -387,7 +387,7 @@ oci_red_opreg_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, const
 
 bool oci_red_opreg_supported(const DevView& V)
 {
-    return V.nblk == 1 && (V.n == 512 || V.n == 256) && V.J + 2 < (int64_t)1 << 31 && V.sm_count >= 8;
+    return V.nblk == 1 && (V.n == 512 || V.n == 256 || V.n == 128) && V.J + 2 < (int64_t)1 << 31 && V.sm_count >= 8;
 }
 
 bool oci_red_opreg_prepare(const DevView& V, RedOpregMaps* M)
@@ -441,7 +441,8 @@ int launch_red_opreg(const DevView& V, const RedOpregMaps& M, int pass, int ybas
                      cudaStream_t s)
 {
     if (V.n == 512) return launch_ro_pass<256>(V, M, pass, ybase, slot, prev_slot, tol, cnt, force, s);
-    return launch_ro_pass<128>(V, M, pass, ybase, slot, prev_slot, tol, cnt, force, s);
+    if (V.n == 256) return launch_ro_pass<128>(V, M, pass, ybase, slot, prev_slot, tol, cnt, force, s);
+    return launch_ro_pass<64>(V, M, pass, ybase, slot, prev_slot, tol, cnt, force, s);
 }
 
 cudaError_t oci_red_opreg_opt_in()
@@ -449,7 +450,9 @@ cudaError_t oci_red_opreg_opt_in()
     cudaError_t e = cudaSuccess;
     if ((e = opt_in_ro<256, PASS_FIX>()) != cudaSuccess || (e = opt_in_ro<256, PASS_ITER>()) != cudaSuccess ||
         (e = opt_in_ro<256, PASS_FINAL>()) != cudaSuccess || (e = opt_in_ro<128, PASS_FIX>()) != cudaSuccess ||
-        (e = opt_in_ro<128, PASS_ITER>()) != cudaSuccess || (e = opt_in_ro<128, PASS_FINAL>()) != cudaSuccess)
+        (e = opt_in_ro<128, PASS_ITER>()) != cudaSuccess || (e = opt_in_ro<128, PASS_FINAL>()) != cudaSuccess ||
+        (e = opt_in_ro<64, PASS_FIX>()) != cudaSuccess || (e = opt_in_ro<64, PASS_ITER>()) != cudaSuccess ||
+        (e = opt_in_ro<64, PASS_FINAL>()) != cudaSuccess)
         return e;
     return e;
 }

@@ -244,6 +244,19 @@ def test_opreg_kernel_shapes(J, N, bcL, bcR):
     g.close()
 
 
+def test_opreg_kernels_at_config3_block_size():
+    """N = 32 (config 3) defaults to the resident kernels; the operator-in-registers family serves it too when forced
+    (one row group, the scalar-flux rows on every tile) and must give the same iterates."""
+    import paper_2305_13555_b200 as P
+    from oracle import threads_available
+    p = make_problem(3, cells=1500)
+    r = run_pair(p, "oci", steps=2, tol=-1.0, max_iters=4, threads=threads_available(), reduced_kernel=P.RKERNEL_OPREG)
+    assert r["info"]["reduced_kernel"] == P.RKERNEL_OPREG
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-12 and rel(r["g_phi"], r["o_phi"]) < 1e-12
+    r = run_pair(p, "oci", steps=2, tol=p.tol, max_iters=p.max_iters, threads=threads_available(), reduced_kernel=P.RKERNEL_OPREG)
+    assert r["g_iters"] == r["o_iters"] and rel(r["g_psi"], r["o_psi"]) < 1e-9
+
+
 def test_opreg_fused_loop_many_iterations():
     """The operator-in-registers ITER kernel runs a whole chunk of up to 64 iterations in one cooperative launch;
     a problem that needs several chunks re-arms the barrier counter, the norm slots and the producer hand-off."""
