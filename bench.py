@@ -479,6 +479,8 @@ def per_config_table(torch, P, peaks=None, peak_src=None, peak_live=None):
             row[f"{scheme}_iters"] = iters
             row[f"{scheme}_updates_per_s"] = p.unknowns * sum(iters) / (ms * 1e-3)
         row["si_over_oci_time"] = row["si_ms_per_step"] / row["oci_ms_per_step"]
+        row["oci_woodbury"] = woodbury_row(torch, P, p, peaks)
+        row["si_over_oci_woodbury_time"] = row["si_ms_per_step"] / row["oci_woodbury"]["ms_per_step"]
         if cfg >= 3 and peaks is not None:       # cfg 1-2 are launch-latency bound: absolutes only
             g.enable_kernel_timing(True)
             time_gpu_steps(torch, g, p, p.n_steps, "oci")
@@ -492,6 +494,37 @@ def per_config_table(torch, P, peaks=None, peak_src=None, peak_live=None):
         g.close()
         del g
         torch.cuda.empty_cache()
+    return out
+
+
+def woodbury_row(torch, P, p, peaks):
+    """The same time steps with the O(N) apply through the rank-4 scattering matrix (row f3, second half; selected with
+    oci_set_reduced_kernel): time to converge, and the iteration kernel against the HBM roofline - its algorithmic bytes
+    per iteration are the state only, J (6N doubles of y in / yfix in / y out + 96 B of scalar flux), plus 16N doubles of
+    4x4 pieces, one row of M and the block index per cell when every cell has its own block."""
+    g = P.OCI.from_problem(p, reduced_kernel=P.RKERNEL_WOODBURY)
+    for k in range(3):
+        g.set_source(p.source(k))
+        g.oci_step(p.tol, p.max_iters)
+    ms, iters, each = time_gpu_steps(torch, g, p, p.n_steps, "oci")
+    g.enable_kernel_timing(True)
+    time_gpu_steps(torch, g, p, p.n_steps, "oci")
+    kms, klaunch = g.get_kernel_time()
+    aux = g.get_aux_kernel_time()
+    g.enable_kernel_timing(False)
+    N = p.n_angles
+    per_cell = g.get_info()["path"] == P.PATH_PER_CELL
+    bytes_ = p.cells * (48.0 * N + 96.0 + ((128.0 * N + 132.0) if per_cell else 0.0))
+    k_avg = kms / max(klaunch, 1)
+    out = {"ms_per_step": ms / p.n_steps, "ms_per_step_median": float(np.median(each)), "iters": iters,
+           "updates_per_s": p.unknowns * sum(iters) / (ms * 1e-3), "iteration_kernel_ms": k_avg,
+           "fix_pass_ms_per_step": aux["fix_ms"] / max(aux["fix_launches"], 1),
+           "final_pass_ms_per_step": aux["final_ms"] / max(aux["final_launches"], 1)}
+    if peaks is not None and p.cfg >= 3:
+        ach = bytes_ / (k_avg * 1e-3) * 1e-9
+        out["iteration_roofline"] = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
+                                     "algorithmic_bytes_per_iteration": bytes_}
+    g.close()
     return out
 
 

@@ -105,8 +105,13 @@ enum { OCI_ITERATION_FULL = 0, OCI_ITERATION_REDUCED = 1, OCI_ITERATION_AUTO = 2
  *          stacked operators, a tile of cells that straddles an interface is done once per block;
  * OPREG - ONE shared block, N in {32, 64, 128} (config 4; N = 32 only when forced): each CTA keeps 64 operator rows as DMMA fragments in
  *          registers for the whole launch and only the cell rows stream (tensor-map TMA); fp64 tensor pipe.
+ * WOODBURY - any problem: B^{-1} is never applied as a dense matrix.  The scattering matrix of eq. (22), has
+ *          rank 4 (isotropic, one group), so B^{-1} c = t + kappa A^{-1} (1 (x) phi), t = A^{-1} c a 4x4 apply per angle,
+ *          phi = (I_4 - kappa sum_m w_m A_m^{-1})^{-1} sum_m w_m t_m: O(N) work and bytes per cell instead of O(N^2);
+ *          HBM-bound.  Same iterates up to rounding order.  Selected only on request.
  * oci_setup picks RESIDENT, else OPREG, else KTILED, else GEMV; oci_set_reduced_kernel overrides. */
-enum { OCI_RKERNEL_AUTO = -1, OCI_RKERNEL_GEMV = 0, OCI_RKERNEL_RESIDENT = 1, OCI_RKERNEL_KTILED = 2, OCI_RKERNEL_OPREG = 3 };
+enum { OCI_RKERNEL_AUTO = -1, OCI_RKERNEL_GEMV = 0, OCI_RKERNEL_RESIDENT = 1, OCI_RKERNEL_KTILED = 2, OCI_RKERNEL_OPREG = 3,
+       OCI_RKERNEL_WOODBURY = 4 };
 
 typedef struct {
     int64_t cells;        /* J */

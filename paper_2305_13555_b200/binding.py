@@ -12,7 +12,7 @@ BC_VACUUM, BC_INCIDENT_ISOTROPIC, BC_REFLECTING, BC_HALO = 0, 1, 2, 3
 PATH_SHARED, PATH_PER_CELL = 0, 1
 KERNEL_GENERIC, KERNEL_RESIDENT, KERNEL_KTILED, KERNEL_PER_CELL = 0, 1, 2, 3
 ITERATION_FULL, ITERATION_REDUCED, ITERATION_AUTO = 0, 1, 2
-RKERNEL_AUTO, RKERNEL_GEMV, RKERNEL_RESIDENT, RKERNEL_KTILED, RKERNEL_OPREG = -1, 0, 1, 2, 3
+RKERNEL_AUTO, RKERNEL_GEMV, RKERNEL_RESIDENT, RKERNEL_KTILED, RKERNEL_OPREG, RKERNEL_WOODBURY = -1, 0, 1, 2, 3, 4
 
 EXPORTED_SYMBOLS = [
     "oci_create", "oci_workspace_bytes", "oci_setup", "oci_set_flux", "oci_set_flux_dev", "oci_set_source",

@@ -165,7 +165,7 @@ void gauss_legendre(int N, std::vector<double>& mu, std::vector<double>& w)
 
 struct Layout {
     int64_t binv, psi0, psi1, cfix, phi, Q, qs, dx, sig, sigs, blk, rep, mu, w, coef, ainv4, si_scan, phi_part, norms, tickets, flags,
-        xop, rop, fop, y0, y1, z, yfix, ifix, phifix, q16, gitems, perm, team_bar, peers, phi_stage, si_part, si_inflow, si_src1, total;
+        xop, rop, fop, y0, y1, z, yfix, ifix, phifix, q16, gitems, perm, team_bar, peers, phi_stage, si_part, si_inflow, si_src1, wba, wbd, wbm, total;
 };
 
 int64_t align_up(int64_t x) { return (x + 255) & ~int64_t(255); }
@@ -220,6 +220,9 @@ Layout make_layout(int64_t J, int32_t N, int64_t nblk)
     L.si_part = take((N / 32 > 2 ? N / 32 : 2) * J * 4 * 8);
     L.si_inflow = take(2 * N * 2 * 8);
     L.si_src1 = take(J * 4 * 8);
+    L.wba = take(nblk * 16 * N * 8);
+    L.wbd = take(nblk * 16 * N * 8);
+    L.wbm = take(nblk * 32 * 8);
     L.total = o;
     return L;
 }
@@ -287,6 +290,8 @@ int launch_reduced_pass(oci_ctx* ctx, int pass, int ybase, int slot, int prev_sl
         return launch_red_ktiled(ctx->V, ctx->rmaps, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
     if (ctx->red_kernel == OCI_RKERNEL_OPREG)
         return launch_red_opreg(ctx->V, ctx->romaps, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
+    if (ctx->red_kernel == OCI_RKERNEL_WOODBURY)
+        return launch_red_woodbury(ctx->V, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
     if (ctx->red_kernel == OCI_RKERNEL_RESIDENT)
         return launch_red_resident(ctx->V, ctx->rrmaps, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
     return launch_red_gemv(ctx->V, pass, ybase, slot, prev_slot, tol, cnt, force, ctx->stream);
@@ -619,6 +624,9 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     V.si_part = (double*)(base + L.si_part);
     V.si_inflow = (double*)(base + L.si_inflow);
     V.si_src1 = (double*)(base + L.si_src1);
+    V.wba = (double*)(base + L.wba);
+    V.wbd = (double*)(base + L.wbd);
+    V.wbm = (double*)(base + L.wbm);
     ctx->snap_pending = false;
     V.rank = 0;
     V.world = 1;
@@ -699,6 +707,7 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     CK(cudaEventRecord(ctx->ev[0], s));
     LAUNCH(launch_form_and_invert(V, s));                                // a0, a1
     LAUNCH(launch_pack_operators(V, s));                                 // f1: G, H, F
+    LAUNCH(launch_woodbury_setup(V, s));                                 // f3: per-angle inverses element-major, M
     CK(cudaEventRecord(ctx->ev[1], s));
     int32_t flag = 0;
     CK(cudaMemcpyAsync(&flag, V.flags, 4, cudaMemcpyDeviceToHost, s));
@@ -726,7 +735,9 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     {
         const int32_t want = ctx->forced_rkernel;
         auto may = [&](int32_t k) { return want == OCI_RKERNEL_AUTO || want == k; };
-        if (may(OCI_RKERNEL_RESIDENT) && oci_red_resident_supported(V) && oci_red_resident_prepare(V, &ctx->rrmaps))
+        if (want == OCI_RKERNEL_WOODBURY)                 // only on request: the dense families are the general method
+            ctx->red_kernel = OCI_RKERNEL_WOODBURY;
+        else if (may(OCI_RKERNEL_RESIDENT) && oci_red_resident_supported(V) && oci_red_resident_prepare(V, &ctx->rrmaps))
             ctx->red_kernel = OCI_RKERNEL_RESIDENT;
         else if (may(OCI_RKERNEL_OPREG) && oci_red_opreg_supported(V) && oci_red_opreg_prepare(V, &ctx->romaps))
             ctx->red_kernel = OCI_RKERNEL_OPREG;
@@ -991,7 +1002,7 @@ int oci_shard_step(oci_ctx* const* ctxs, int32_t n, double tol, int32_t max_iter
 int oci_set_reduced_kernel(oci_ctx* ctx, int32_t kernel)
 {
     if (!ctx) return OCI_E_INVALID;
-    if (kernel < OCI_RKERNEL_AUTO || kernel > OCI_RKERNEL_OPREG) return fail(ctx, OCI_E_INVALID, "unknown kernel family");
+    if (kernel < OCI_RKERNEL_AUTO || kernel > OCI_RKERNEL_WOODBURY) return fail(ctx, OCI_E_INVALID, "unknown kernel family");
     ctx->forced_rkernel = kernel;
     return OCI_OK;
 }

@@ -59,6 +59,10 @@ struct DevView {
     double* ifix;               // [J][K2]  I rows of Psi_fix
     double* phifix;             // [J][4]   W Psi_fix
     double* q16;                // [J][16]  Q padded to one 128-byte row (K-tiled FIX pass only; else unused)
+    // ---- O(N) apply through the rank-4 scattering matrix (oci_reduced_woodbury.cu)
+    double* wba;                // [nblk][16][N]  (A_m)^{-1}, element-major (coalesced over the angles)
+    double* wbd;                // [nblk][16][N]  kappa (A_m)^{-1} M, element-major
+    double* wbm;                // [nblk][32]     M = (I_4 - kappa sum_m w_m A_m^{-1})^{-1} (16), kappa = dx Sigma_s / 4, padding
     int32_t* gitems;            // [ngroups][4] = (cell tile, block, mask lo, mask hi): a handful of materials on the K-tiled
                                 // kernels (row f2); nullptr when all cells share one block (or have one each)
     int64_t ngroups;
@@ -163,6 +167,8 @@ bool oci_red_opreg_supported(const DevView& V);
 bool oci_red_opreg_prepare(const DevView& V, RedOpregMaps* M);
 int launch_red_opreg(const DevView& V, const RedOpregMaps& M, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
                      cudaStream_t s);
+int launch_woodbury_setup(const DevView& V, cudaStream_t s);
+int launch_red_woodbury(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s);
 bool oci_red_resident_supported(const DevView& V);
 bool oci_red_resident_prepare(const DevView& V, RedResidentMaps* M);
 int launch_red_resident(const DevView& V, const RedResidentMaps& M, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,

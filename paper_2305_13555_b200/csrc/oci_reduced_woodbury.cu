@@ -1,0 +1,548 @@
+// O(N) apply of the one-cell inverse through the rank-4 structure of the scattering matrix (SURVEY §8(f) row f3,
+// second half; eq. (22)): B = A - S with A = blockdiag(A_m) (eqs. 20,21) and
+// S = U V,  U = kappa (1_N (x) I_4)  [4N x 4],  V = (w^T (x) I_4)  [4 x 4N],  kappa = dx Sigma_s / 4   (reading G5),
+// so by the Sherman-Morrison-Woodbury identity
+//     B^{-1} c = t + A^{-1} U (I_4 - V A^{-1} U)^{-1} V t,      t = A^{-1} c  (one 4x4 apply per angle)
+// With s = V t = sum_m w_m t_m (a 4-vector per cell) and M = (I_4 - kappa sum_m w_m A_m^{-1})^{-1}:
+//     phi = V B^{-1} c = M s            (the scalar flux of the result, eq. 18)
+//     Psi_m = t_m + kappa A_m^{-1} phi  (every angle sees the same self-consistent scattering source)
+// about 50 N multiply-adds and 16 N doubles of operator per cell instead of (4N)^2 of each.  It holds because the
+// scattering of eq. (1) is isotropic and one-group; the dense kernels remain the general method (and the roofline
+// target), this family is selected only on request (oci_set_reduced_kernel(OCI_RKERNEL_WOODBURY)).
+//
+// The family serves the interface-reduced step of oci_reduced.cu with the same packed state (y, z, yfix, ifix,
+// phifix), the same three passes and the same loop control, so everything around the kernels (fused cooperative
+// iteration loop, device-side stop, sharding, layout conversion) is shared with the dense families:
+//   FIX  :  c = c_fix (eqs. 27,28 without the (l) terms)            -> yfix, ifix, phifix
+//   ITER :  c = |mu| inc^(l) on the two incident rows of each angle -> y^(l+1) = yfix + Psi[O], phi^(l+1) = phifix + phi
+//   FINAL:  the same from inc^(L-1)                                 -> z = ifix + Psi[I]
+// Thread = (cell, angle); the 4-vector s is summed over the angles of a cell by warp shuffles (N a power of two)
+// and, across the warps of a cell or for other N, through shared memory in a fixed order (deterministic).
+// HBM-bound: per cell and iteration 6N doubles of state (+ 16N + 17 of operator when every cell has its own block).
+#include "device_utils.cuh"
+
+namespace oci {
+
+namespace {
+
+// inverse of a 4x4 by Gauss-Jordan with partial pivoting, in place on [A | I]; returns false on a zero pivot
+__device__ bool invert4(double (&A)[16], double (&I)[16])
+{
+#pragma unroll
+    for (int i = 0; i < 16; ++i) I[i] = (i % 5 == 0) ? 1.0 : 0.0;
+    bool ok = true;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        int p = k;
+        double best = fabs(A[4 * k + k]);
+#pragma unroll
+        for (int i = k + 1; i < 4; ++i) {
+            const double a = fabs(A[4 * i + k]);
+            if (a > best) { best = a; p = i; }
+        }
+#pragma unroll
+        for (int i = k + 1; i < 4; ++i) {
+            if (i == p) {
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const double t1 = A[4 * k + c]; A[4 * k + c] = A[4 * i + c]; A[4 * i + c] = t1;
+                    const double t2 = I[4 * k + c]; I[4 * k + c] = I[4 * i + c]; I[4 * i + c] = t2;
+                }
+            }
+        }
+        if (!(best > 0.0)) ok = false;
+        const double pinv = 1.0 / A[4 * k + k];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) { A[4 * k + c] *= pinv; I[4 * k + c] *= pinv; }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            if (i != k) {
+                const double f = A[4 * i + k];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) { A[4 * i + c] -= f * A[4 * k + c]; I[4 * i + c] -= f * I[4 * k + c]; }
+            }
+        }
+    }
+    return ok;
+}
+
+}  // namespace
+
+// ---- setup: one warp per distinct block.  Element-major copies (so that the threads of a cell read them coalesced)
+// of the per-angle inverses of ainv4_kernel and of their product with the 4x4 that closes the scattering source:
+//     wba[b][e][m] = A_m^{-1}[e/4][e%4],   wbd[b][e][m] = (kappa A_m^{-1} M)[e/4][e%4],
+//     wbm[b] = [ M (16) | kappa ],   M = (I_4 - kappa sum_m w_m A_m^{-1})^{-1},
+// so that Psi_m = t_m + D_m s and phi = M s with s = sum_m w_m t_m.
+__global__ void __launch_bounds__(128) woodbury_setup_kernel(DevView V)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t b = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (b >= V.nblk) return;
+    const int N = V.N;
+    const int64_t r = V.rep[b];
+    const double kappa = 0.25 * V.dx[r] * V.sigs[r];
+    double K[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) K[e] = 0.0;
+    for (int m = lane; m < N; m += 32) {
+        const double* __restrict__ a = V.ainv4 + ((size_t)b * N + m) * 16;
+        const double wm = V.w[m];
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const double v = a[e];
+            V.wba[((size_t)b * 16 + e) * N + m] = v;
+            K[e] = fma(wm, v, K[e]);
+        }
+    }
+#pragma unroll
+    for (int e = 0; e < 16; ++e)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) K[e] += __shfl_xor_sync(0xffffffffu, K[e], o);
+    double T[16], M[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) T[e] = ((e % 5 == 0) ? 1.0 : 0.0) - kappa * K[e];
+    const bool ok = invert4(T, M);                                        // every lane (all hold the same K)
+    if (lane == 0) {
+        if (!ok) atomicCAS(V.flags, 0, (int)b + 1);                      // singular exactly when B is (reported like a1)
+        double* out = V.wbm + (size_t)b * 32;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) out[e] = M[e];
+        out[16] = kappa;
+    }
+    for (int m = lane; m < N; m += 32) {
+        const double* __restrict__ a = V.ainv4 + ((size_t)b * N + m) * 16;
+#pragma unroll
+        for (int rr = 0; rr < 4; ++rr)
+#pragma unroll
+            for (int cc = 0; cc < 4; ++cc) {
+                double d = 0.0;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) d = fma(a[4 * rr + k], M[4 * k + cc], d);
+                V.wbd[((size_t)b * 16 + 4 * rr + cc) * N + m] = kappa * d;
+            }
+    }
+}
+
+int launch_woodbury_setup(const DevView& V, cudaStream_t s)
+{
+    const int64_t threads = V.nblk * 32;
+    woodbury_setup_kernel<<<(unsigned)((threads + 127) / 128), 128, 0, s>>>(V);
+    return launched(1);
+}
+
+namespace {
+
+// Sum of p over the angles of this thread's cell, delivered to every thread of the cell.  The order of the additions is
+// fixed by the geometry alone and the same for every lane, so a step is reproducible bit for bit and does not depend on
+// where in a CTA a cell lands.  `sm` = this call's half of a double buffer (consecutive calls alternate halves, which
+// makes one CTA barrier per call enough).
+// W = 0: any N - every term goes through shared memory and is summed in angle order.
+// W = 8, 16, 32 (N a power of two, W = min(N, 32)): a transposing butterfly - the first level exchanges two of the four
+// values and keeps two, the second exchanges one and keeps one, the remaining levels reduce a single value: 6 shuffles
+// instead of 20 for a full warp, after which the lane with bits (hi, hi2) holds the total of slot 2 hi + hi2.  N <= 32:
+// the four totals are broadcast by four more shuffles; N > 32: the partials of the cell's N/32 warps meet in shared memory.
+template <int W>
+__device__ __forceinline__ void cell_sum(double (&p)[4], int N, int cell_slot, double* __restrict__ sm)
+{
+    if (W == 0) {
+        *reinterpret_cast<double4*>(sm + threadIdx.x * 4) = make_double4(p[0], p[1], p[2], p[3]);
+        __syncthreads();
+        const double* __restrict__ q = sm + (size_t)cell_slot * N * 4;
+        p[0] = p[1] = p[2] = p[3] = 0.0;
+        for (int k = 0; k < N; ++k) {
+            const double4 a = *reinterpret_cast<const double4*>(q + k * 4);
+            p[0] += a.x; p[1] += a.y; p[2] += a.z; p[3] += a.w;
+        }
+        return;
+    }
+    const int lane = threadIdx.x & 31;
+    constexpr int H = W > 0 ? W / 2 : 1, Q4 = W > 0 ? W / 4 : 1;
+    const bool hi = (lane & H) != 0;
+    double k0 = hi ? p[2] : p[0], k1 = hi ? p[3] : p[1];
+    k0 += __shfl_xor_sync(0xffffffffu, hi ? p[0] : p[2], H);
+    k1 += __shfl_xor_sync(0xffffffffu, hi ? p[1] : p[3], H);
+    const bool hi2 = (lane & Q4) != 0;
+    double keep = hi2 ? k1 : k0;
+    keep += __shfl_xor_sync(0xffffffffu, hi2 ? k0 : k1, Q4);
+#pragma unroll
+    for (int o = Q4 / 2; o > 0; o >>= 1) keep += __shfl_xor_sync(0xffffffffu, keep, o);
+    if (N <= 32) {
+        const int base = lane & ~(W - 1);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) p[i] = __shfl_sync(0xffffffffu, keep, base + (i >> 1) * H + (i & 1) * Q4);
+        return;
+    }
+    const int warp = threadIdx.x >> 5, wpc = N >> 5;
+    if ((lane & 7) == 0) sm[warp * 4 + (lane >> 3)] = keep;               // lanes 0, 8, 16, 24 hold slots 0..3
+    __syncthreads();
+    const double* __restrict__ q = sm + (warp / wpc) * wpc * 4;
+    p[0] = p[1] = p[2] = p[3] = 0.0;
+    for (int w = 0; w < wpc; ++w) {
+        const double4 a = *reinterpret_cast<const double4*>(q + w * 4);
+        p[0] += a.x; p[1] += a.y; p[2] += a.z; p[3] += a.w;
+    }
+}
+
+// what a thread reads for one (cell, angle): FIX - the k+1/2 entries of y and z, and Q; ITER / FINAL - the two
+// gathered neighbour values and the two entries of the additive operand; pf / po: phifix and the old scalar flux of
+// slot m & 3 (threads of angles 0..3 only).  Everything an item consumes is requested one item ahead, so that no
+// instruction of the current item waits on a scoreboard the loads of the next item are counted on.
+struct WbRaw {
+    double a, b, c, d, pf, po;
+    double4 q;
+};
+
+// the 4x4 pieces a pass needs for one (block, angle), scaled once.  ITER / FINAL, with a, b the two gathered values:
+//   w t_m = pk a + pe b        pk, pe = w |mu| (the two columns of A_m^{-1} that the incident rows feed)
+//   stored rows = [g0 a + g1 b, g2 a + g3 b] + [dk; de] s      g = |mu| (those rows of the two columns), dk, de = rows of D_m
+// FIX: t = A_m^{-1} c with all four columns (pk, pe, pk2, pe2 = columns 0..3, unscaled) and all of D_m
+template <int PASS>
+struct WbOps {
+    double pk[4], pe[4], dk[4], de[4];
+    double g[PASS == PASS_FIX ? 1 : 4];
+    double pk2[PASS == PASS_FIX ? 4 : 1], pe2[PASS == PASS_FIX ? 4 : 1], dk2[PASS == PASS_FIX ? 4 : 1], de2[PASS == PASS_FIX ? 4 : 1];
+};
+
+template <int PASS>
+__device__ __forceinline__ void load_ops(WbOps<PASS>& O, const double* __restrict__ a, const double* __restrict__ d, int N, int half,
+                                         double amu, double wm)
+{
+    // a, d: wba / wbd of this block at this thread's angle; element e of the 4x4 is e * N doubles further
+    if (PASS == PASS_FIX) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            O.pk[r] = a[(size_t)(4 * r + 0) * N];
+            O.pe[r] = a[(size_t)(4 * r + 1) * N];
+            O.pk2[r] = a[(size_t)(4 * r + 2) * N];
+            O.pe2[r] = a[(size_t)(4 * r + 3) * N];
+            O.dk[r] = d[(size_t)(0 + r) * N];
+            O.de[r] = d[(size_t)(4 + r) * N];
+            O.dk2[r] = d[(size_t)(8 + r) * N];
+            O.de2[r] = d[(size_t)(12 + r) * N];
+        }
+    } else {
+        // incident rows (eqs. 27,28): (m,1),(m,3) for mu < 0 (half 0), (m,0),(m,2) for mu > 0; the pass stores the O rows
+        // (the other two, ITER) or the I rows themselves (FINAL)
+        const int Ik = half ? 0 : 1;
+        const int Rk = PASS == PASS_ITER ? (Ik ^ 1) : Ik;
+        const double* __restrict__ ac = a + (size_t)Ik * N;
+        const double* __restrict__ dr = d + (size_t)(4 * Rk) * N;
+        double ck[4], ce[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            ck[r] = ac[(size_t)(4 * r) * N];
+            ce[r] = ac[(size_t)(4 * r + 2) * N];
+            O.dk[r] = dr[(size_t)r * N];
+            O.de[r] = dr[(size_t)(8 + r) * N];
+        }
+        O.g[0] = amu * (Rk ? ck[1] : ck[0]);
+        O.g[1] = amu * (Rk ? ce[1] : ce[0]);
+        O.g[2] = amu * (Rk ? ck[3] : ck[2]);
+        O.g[3] = amu * (Rk ? ce[3] : ce[2]);
+        const double wa = wm * amu;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) { O.pk[r] = wa * ck[r]; O.pe[r] = wa * ce[r]; }
+    }
+}
+
+}  // namespace
+
+// ---- the three passes.  SHARED: all cells share one block, whose 4x4 pieces for this thread's angle live in registers
+// for the whole launch; otherwise they are streamed per cell (coalesced over the angles).  A CTA of TPB threads takes
+// TPB / N whole cells at a time (thread = (cell slot, angle)), groups of cells strided over the grid.
+// IDX: the type of cell and element indices (int32_t when (J + 2) * 2N fits, which keeps the address arithmetic of the
+// six streams of an item to one instruction each).
+template <int PASS, bool SHARED, int TPB, int W, typename IDX>
+__global__ void __launch_bounds__(TPB, TPB == 256 ? 2 : 1)
+oci_red_woodbury_kernel(DevView V, int ybase, int slot, int prev_slot, double tol, int cnt, int force)
+{
+    extern __shared__ __align__(32) double wsm[];
+    const int lane = threadIdx.x & 31;
+    int ysrc = ybase;
+    if (PASS == PASS_ITER) {
+        if (step_done(V.norms, prev_slot, tol)) return;
+    } else if (PASS == PASS_FINAL) {
+        // the last executed iteration of this chunk of launches (all loads of the scan in flight at once)
+        int L = 0;
+        for (int i0 = 0; i0 < cnt && L == 0; i0 += 32) {
+            const int i = i0 + lane;
+            bool hit = false;
+            if (i < cnt) {
+                const double d = __longlong_as_double((long long)__ldcg(V.norms + 2 * i + 0));
+                const double r = __longlong_as_double((long long)__ldcg(V.norms + 2 * i + 1));
+                hit = stop_now(tol, d, r);
+            }
+            const unsigned msk = __ballot_sync(0xffffffffu, hit);
+            if (msk) L = i0 + __ffs(msk);
+        }
+        if (L == 0) {
+            if (!force) return;
+            L = cnt;
+        }
+        ysrc = (ybase + L - 1) & 1;
+    }
+    if (PASS == PASS_FIX) clear_step_state(V);
+
+    const int N = V.N, K2 = 2 * N, N2 = N >> 1;
+    const IDX J = (IDX)V.J;
+    const int cpb = TPB / N;                                               // cells a CTA handles at a time
+    const int cs = threadIdx.x / N;                                        // this thread's cell slot ...
+    const bool active = W > 0 || cs < cpb;                                 // (idle threads when N does not divide TPB)
+    const int m = active ? threadIdx.x - cs * N : 0;                       // ... and angle
+    const int cslot = active ? cs : 0;
+    constexpr int sm_half = W == 0 ? 4 * TPB : 4 * (TPB / 32);
+
+    // packed positions of this angle's two outgoing entries (k slot, k+1/2 slot)
+    const int half = m >= N2, mm = m - half * N2;
+    const int qk = pack_q(half, 0, mm, N), qe = pack_q(half, 1, mm, N);
+    const double amu = fabs(V.mu[m]), wm = V.w[m];
+    const int nbr = half ? -K2 : K2;                 // row offset of the neighbour the inflow comes from
+    const bool ghost_l = PASS == PASS_ITER && !half && V.bcL == OCI_BC_REFLECTING;
+    const bool ghost_r = PASS == PASS_ITER && half && V.bcR == OCI_BC_REFLECTING;
+    const int mqk = mirror_q(qk, N), mqe = mirror_q(qe, N);
+    // the scalar flux phi = M s (eq. 18): slot m & 3 by the threads of angles 0..3 (N = 2: slots m and m + 2)
+    const bool phi_lane = PASS != PASS_FINAL && active && m < 4;
+    const int psl = m & 3;
+
+    WbOps<PASS> O;
+    double alpha = 0.0, q4 = 0.0, mrow[4] = {0.0, 0.0, 0.0, 0.0};
+    if (SHARED) {
+        load_ops<PASS>(O, V.wba + m, V.wbd + m, N, half, amu, wm);
+        const double h = V.dx[V.rep[0]];
+        alpha = h / (2.0 * V.v * V.dt);
+        q4 = 0.25 * h;
+#pragma unroll
+        for (int cc = 0; cc < 4; ++cc) mrow[cc] = V.wbm[4 * psl + cc];
+    }
+
+    const IDX ngroups = (J + cpb - 1) / cpb;
+    const IDX jstep = (IDX)gridDim.x * cpb;
+    const int nloop = PASS == PASS_ITER ? (cnt > 1 ? cnt : 1) : 1;
+    int flip = 0;
+  for (int l = 0; l < nloop; ++l) {
+    const double* __restrict__ Ys = V.y[PASS == PASS_ITER ? (ybase + l) & 1 : ysrc];
+    double* __restrict__ Yd = V.y[PASS == PASS_ITER ? (ybase + l + 1) & 1 : ysrc ^ 1];
+    // per-thread column pointers; j * K2 walks the cells of this thread
+    const double* __restrict__ in_k = PASS == PASS_FIX ? Ys + qe : Ys + nbr + qk;
+    const double* __restrict__ in_e = PASS == PASS_FIX ? V.z + qe : Ys + nbr + qe;
+    const double* __restrict__ fx_k = (PASS == PASS_ITER ? V.yfix : V.ifix) + qk;
+    const double* __restrict__ fx_e = (PASS == PASS_ITER ? V.yfix : V.ifix) + qe;
+    double* __restrict__ out_k = (PASS == PASS_ITER ? Yd : PASS == PASS_FINAL ? V.z : V.yfix) + qk;
+    double* __restrict__ out_e = (PASS == PASS_ITER ? Yd : PASS == PASS_FINAL ? V.z : V.yfix) + qe;
+    // (the loaded values are not touched before the item that consumes them: a select right behind a load would make
+    // the prefetch wait for its own data)
+    auto load_raw = [&](IDX jc, IDX o) {
+        WbRaw R;
+        // ITER / FINAL: inc^(l), the neighbour's outgoing flux of the previous iterate (ghost rows at the domain faces),
+        // through L2: other SMs wrote it in the previous iteration of this launch
+        R.a = __ldcg(in_k + o);
+        R.b = PASS == PASS_FIX ? in_e[o] : __ldcg(in_e + o);
+        R.c = R.d = R.pf = R.po = 0.0;
+        R.q = make_double4(0.0, 0.0, 0.0, 0.0);
+        if (PASS == PASS_FIX) {
+            R.q = *reinterpret_cast<const double4*>(V.Q + jc * 4);
+        } else {
+            R.c = fx_k[o];
+            R.d = fx_e[o];
+            if (PASS == PASS_ITER && phi_lane) {
+                R.pf = V.phifix[jc * 4 + psl];
+                R.po = __ldcg(V.phi + jc * 4 + psl);
+            }
+        }
+        return R;
+    };
+    double dmax = 0.0, rmax = 0.0;
+    IDX j = (IDX)blockIdx.x * cpb + cs, off = j * K2;
+    const IDX ostep = jstep * K2;
+    WbRaw nxt = (active && j < J) ? load_raw(j, off) : load_raw(0, 0);     // clamped: unconditional loads
+    for (IDX grp = blockIdx.x; grp < ngroups; grp += gridDim.x, j += jstep, off += ostep) {
+        WbRaw R = nxt;
+        const bool valid = active && j < J;
+        if (grp + gridDim.x < ngroups) {
+            const bool okn = active && j + jstep < J;
+            nxt = load_raw(okn ? j + jstep : 0, okn ? off + ostep : 0);
+        }
+        if (!valid) R.a = R.b = 0.0;                                       // an idle thread adds nothing to the cell sums
+        int64_t b = 0;
+        if (!SHARED) {
+            b = V.blk[valid ? j : 0];
+            load_ops<PASS>(O, V.wba + (size_t)b * 16 * N + m, V.wbd + (size_t)b * 16 * N + m, N, half, amu, wm);
+            if (PASS == PASS_FIX) {
+                const double h = V.dx[valid ? j : 0];
+                alpha = h / (2.0 * V.v * V.dt);
+                q4 = 0.25 * h;
+            }
+            if (phi_lane) {
+#pragma unroll
+                for (int cc = 0; cc < 4; ++cc) mrow[cc] = __ldg(V.wbm + (size_t)b * 32 + 4 * psl + cc);
+            }
+        }
+        // ---- s = sum_m w_m t_m (over the cell), t = A_m^{-1} c; what is stored = t + D_m s
+        double t[4], p[4];
+        if (PASS == PASS_FIX) {
+            // c_fix of eqs. (27),(28): psi_{k-1/2} = the k+1/2 entries of the committed state (row a8) and Q
+            const double pL = half ? R.b : R.a, pR = half ? R.a : R.b;     // slots (k+1/2,L), (k+1/2,R)
+            const double c0 = fma(alpha, pL, q4 * R.q.x), c1 = fma(alpha, pR, q4 * R.q.y), c2 = q4 * R.q.z, c3 = q4 * R.q.w;
+            const double wv = valid ? wm : 0.0;
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                t[r] = fma(O.pe2[r], c3, fma(O.pk2[r], c2, fma(O.pe[r], c1, O.pk[r] * c0)));
+                p[r] = wv * t[r];
+            }
+        } else {
+#pragma unroll
+            for (int r = 0; r < 4; ++r) p[r] = fma(O.pe[r], R.b, O.pk[r] * R.a);
+        }
+        cell_sum<W>(p, N, cslot, wsm + (flip ? sm_half : 0));
+        flip ^= 1;
+        if (!valid) continue;
+        if (phi_lane) {
+            const double ph = fma(mrow[3], p[3], fma(mrow[2], p[2], fma(mrow[1], p[1], mrow[0] * p[0])));
+            if (PASS == PASS_FIX) V.phifix[j * 4 + psl] = ph;
+            if (PASS == PASS_ITER) {
+                // a6: phi^(l+1) = phifix + phi and the two max-norms of the stopping rule
+                const double nw = R.pf + ph;
+                V.phi[j * 4 + psl] = nw;
+                dmax = nanmax(dmax, fabs(nw - R.po));
+                rmax = nanmax(rmax, fabs(nw));
+            }
+            if (N == 2) {                                                  // two angles: slots 2, 3 as well
+                const double* __restrict__ Mb = V.wbm + (size_t)b * 32 + 4 * (psl + 2);
+                const double ph2 = fma(Mb[3], p[3], fma(Mb[2], p[2], fma(Mb[1], p[1], Mb[0] * p[0])));
+                if (PASS == PASS_FIX) V.phifix[j * 4 + psl + 2] = ph2;
+                if (PASS == PASS_ITER) {
+                    const double nw = V.phifix[j * 4 + psl + 2] + ph2, old = __ldcg(V.phi + j * 4 + psl + 2);
+                    V.phi[j * 4 + psl + 2] = nw;
+                    dmax = nanmax(dmax, fabs(nw - old));
+                    rmax = nanmax(rmax, fabs(nw));
+                }
+            }
+        }
+        if (PASS == PASS_FIX) {
+            double psi[4];
+            psi[0] = fma(O.dk[3], p[3], fma(O.dk[2], p[2], fma(O.dk[1], p[1], fma(O.dk[0], p[0], t[0]))));
+            psi[1] = fma(O.de[3], p[3], fma(O.de[2], p[2], fma(O.de[1], p[1], fma(O.de[0], p[0], t[1]))));
+            psi[2] = fma(O.dk2[3], p[3], fma(O.dk2[2], p[2], fma(O.dk2[1], p[1], fma(O.dk2[0], p[0], t[2]))));
+            psi[3] = fma(O.de2[3], p[3], fma(O.de2[2], p[2], fma(O.de2[1], p[1], fma(O.de2[0], p[0], t[3]))));
+            out_k[off] = half ? psi[1] : psi[0];                           // yfix: O rows (a neighbour reads them)
+            out_e[off] = half ? psi[3] : psi[2];
+            V.ifix[off + qk] = half ? psi[0] : psi[1];                     // I rows
+            V.ifix[off + qe] = half ? psi[2] : psi[3];
+        } else {
+            // rows (Rk, Rk + 2) of Psi_m: the O rows for ITER, the I rows for FINAL
+            const double tk = fma(O.g[1], R.b, O.g[0] * R.a), te = fma(O.g[3], R.b, O.g[2] * R.a);
+            const double vk = R.c + fma(O.dk[3], p[3], fma(O.dk[2], p[2], fma(O.dk[1], p[1], fma(O.dk[0], p[0], tk))));
+            const double ve = R.d + fma(O.de[3], p[3], fma(O.de[2], p[2], fma(O.de[1], p[1], fma(O.de[0], p[0], te))));
+            out_k[off] = vk;
+            out_e[off] = ve;
+            // reflecting ghost rows (reading S4): the mirror image of the edge cell's outgoing flux
+            if (ghost_l && j == 0) {
+                Yd[mqk - K2] = vk;
+                Yd[mqe - K2] = ve;
+            }
+            if (ghost_r && j == J - 1) {
+                Yd[(int64_t)J * K2 + mqk] = vk;
+                Yd[(int64_t)J * K2 + mqe] = ve;
+            }
+        }
+    }
+    if (PASS == PASS_ITER) {
+        dmax = warp_max(dmax);
+        rmax = warp_max(rmax);
+        if (lane == 0) {
+            atomic_max_nonneg(&V.norms[2 * (slot + l) + 0], dmax);
+            atomic_max_nonneg(&V.norms[2 * (slot + l) + 1], rmax);
+        }
+        if (nloop > 1) {
+            // grid-wide barrier (cooperative launch), then the stopping rule on the now final norms (a7)
+            __threadfence();
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                unsigned int* bar = reinterpret_cast<unsigned int*>(V.flags) + 8;
+                atomicAdd(bar, 1u);
+                const unsigned int target = (unsigned int)(l + 1) * gridDim.x;
+                unsigned int seen;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(bar) : "memory");
+                } while (seen < target);
+            }
+            __syncthreads();
+            if (step_done(V.norms, slot + l, tol)) break;
+        }
+    }
+  }
+}
+
+namespace {
+struct WbLaunch { unsigned grid; size_t smem; };
+
+template <int PASS, bool SHARED, int TPB, int W, typename IDX>
+WbLaunch wb_config(const DevView& V)
+{
+    WbLaunch c{};
+    c.smem = 2 * sizeof(double) * 4 * (W == 0 ? TPB : TPB / 32);
+    const int cpb = TPB / V.N;
+    const int64_t groups = (V.J + cpb - 1) / cpb;
+    int per_sm = 1;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, oci_red_woodbury_kernel<PASS, SHARED, TPB, W, IDX>, TPB, c.smem);
+    if (per_sm < 1) per_sm = 1;
+    const int64_t cap = (int64_t)V.sm_count * per_sm;                     // one resident wave (the fused loop needs it)
+    c.grid = (unsigned)(groups < cap ? groups : cap);
+    return c;
+}
+
+template <int PASS, bool SHARED, int TPB, int W, typename IDX>
+void launch_wb_i(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
+{
+    const WbLaunch c = wb_config<PASS, SHARED, TPB, W, IDX>(V);
+    if (PASS == PASS_ITER && cnt > 1) {
+        DevView Vv = V;
+        void* args[] = {&Vv, &ybase, &slot, &prev_slot, &tol, &cnt, &force};
+        cudaLaunchCooperativeKernel((const void*)oci_red_woodbury_kernel<PASS, SHARED, TPB, W, IDX>, dim3(c.grid), dim3(TPB), args, c.smem, s);
+        return;
+    }
+    oci_red_woodbury_kernel<PASS, SHARED, TPB, W, IDX><<<c.grid, TPB, c.smem, s>>>(V, ybase, slot, prev_slot, tol, cnt, force);
+}
+
+template <int PASS, bool SHARED, int TPB, int W>
+void launch_wb_w(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
+{
+    // 32-bit indices when every element offset (ghost rows and one grid stride past the end included) fits
+    const int64_t lim = (V.J + 2 + (int64_t)V.sm_count * 8 * (TPB / V.N + 1)) * 2 * V.N;
+    if (lim < ((int64_t)1 << 31)) launch_wb_i<PASS, SHARED, TPB, W, int32_t>(V, ybase, slot, prev_slot, tol, cnt, force, s);
+    else launch_wb_i<PASS, SHARED, TPB, W, int64_t>(V, ybase, slot, prev_slot, tol, cnt, force, s);
+}
+
+// CTAs of 256 threads (one or more whole cells each) unless a cell has more angles than that; the butterfly for
+// power-of-two N >= 8, the shared-memory sum otherwise
+template <int PASS, bool SHARED>
+void launch_wb(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
+{
+    const int N = V.N;
+    const bool pow2 = (N & (N - 1)) == 0 && N >= 8;
+    if (N > 256) {
+        if (pow2) launch_wb_w<PASS, SHARED, 512, 32>(V, ybase, slot, prev_slot, tol, cnt, force, s);
+        else launch_wb_w<PASS, SHARED, 512, 0>(V, ybase, slot, prev_slot, tol, cnt, force, s);
+    } else if (!pow2) launch_wb_w<PASS, SHARED, 256, 0>(V, ybase, slot, prev_slot, tol, cnt, force, s);
+    else if (N == 8) launch_wb_w<PASS, SHARED, 256, 8>(V, ybase, slot, prev_slot, tol, cnt, force, s);
+    else if (N == 16) launch_wb_w<PASS, SHARED, 256, 16>(V, ybase, slot, prev_slot, tol, cnt, force, s);
+    else launch_wb_w<PASS, SHARED, 256, 32>(V, ybase, slot, prev_slot, tol, cnt, force, s);
+}
+
+template <bool SHARED>
+void launch_wb_pass(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
+{
+    if (pass == PASS_FIX) launch_wb<PASS_FIX, SHARED>(V, ybase, 0, -1, tol, 0, 0, s);
+    else if (pass == PASS_ITER) launch_wb<PASS_ITER, SHARED>(V, ybase, slot, prev_slot, tol, cnt, 0, s);
+    else launch_wb<PASS_FINAL, SHARED>(V, ybase, 0, -1, tol, cnt, force, s);
+}
+}  // namespace
+
+int launch_red_woodbury(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
+{
+    if (V.nblk == 1) launch_wb_pass<true>(V, pass, ybase, slot, prev_slot, tol, cnt, force, s);
+    else launch_wb_pass<false>(V, pass, ybase, slot, prev_slot, tol, cnt, force, s);
+    return launched(1);
+}
+
+}  // namespace oci

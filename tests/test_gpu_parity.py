@@ -564,3 +564,86 @@ def test_ktiled_pingpong_kernel(J, N, bcL, bcR, bounds):
     g.oci_step(-1.0, 3)
     assert np.array_equal(g.get_angular_flux(), r["g_psi"])
     g.close()
+
+
+# ---- O(N) apply through the rank-4 scattering matrix (row f3, second half; oci_reduced_woodbury.cu)
+@pytest.mark.parametrize("cfg,cells,steps", [(1, 20, 5), (2, 203, 4), (3, 300, 3), (4, 70, 2), (5, 37, 3)])
+def test_woodbury_parity_small(cfg, cells, steps):
+    """The Woodbury family against the oracle (which LU-solves the dense block): fixed iteration count 1e-12,
+    converged 1e-9 and iteration counts, on every config's materials, angles and BCs."""
+    import paper_2305_13555_b200 as P
+    p = make_problem(cfg, cells=cells)
+    r = run_pair(p, "oci", steps=2, tol=-1.0, max_iters=5, reduced_kernel=P.RKERNEL_WOODBURY)
+    assert r["info"]["reduced_kernel"] == P.RKERNEL_WOODBURY and r["info"]["iteration"] == P.ITERATION_REDUCED
+    assert r["g_iters"] == [5, 5] == r["o_iters"]
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-12
+    assert rel(r["g_phi"], r["o_phi"]) < 1e-12
+    r = run_pair(p, "oci", steps=steps, tol=p.tol, max_iters=p.max_iters, reduced_kernel=P.RKERNEL_WOODBURY)
+    assert r["g_iters"] == r["o_iters"]
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-9
+    assert rel(r["g_phi"], r["o_phi"]) < 1e-9
+
+
+@pytest.mark.parametrize("J,N,bcL,bcR,hetero", [
+    (1, 2, (VAC, 0.0), (VAC, 0.0), False),        # one cell, S2: one thread pair per cell
+    (1, 4, (REF, 0.0), (REF, 0.0), False),        # one cell between two mirrors
+    (2, 2, (INC, 0.5), (REF, 0.0), True),
+    (33, 6, (REF, 0.0), (INC, 2.0), False),       # N not a power of two: the shared-memory sum, idle threads in the CTA
+    (65, 10, (INC, 1.0), (INC, 0.25), True),
+    (257, 8, (REF, 0.0), (VAC, 0.0), True),       # 32 cells per CTA, several CTAs, ragged last group
+    (31, 48, (VAC, 0.0), (REF, 0.0), False),      # 5 cells per CTA, 16 idle threads
+    (40, 64, (REF, 0.0), (REF, 0.0), True),       # two warps per cell: shuffles + partials
+    (19, 256, (INC, 0.7), (REF, 0.0), False),     # one cell per CTA of 256
+    (5, 512, (REF, 0.0), (VAC, 0.0), True),       # the largest N: CTA of 512
+    (3, 300, (VAC, 0.0), (INC, 1.0), False),      # N > 256, not a power of two
+])
+def test_woodbury_shapes(J, N, bcL, bcR, hetero):
+    import paper_2305_13555_b200 as P
+    p = _custom(J, N, bcL, bcR, seed=J * 100 + N, hetero=hetero)
+    r = run_pair(p, "oci", steps=2, tol=-1.0, max_iters=4, reduced_kernel=P.RKERNEL_WOODBURY)
+    assert r["info"]["reduced_kernel"] == P.RKERNEL_WOODBURY
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-12
+    assert rel(r["g_phi"], r["o_phi"]) < 1e-12
+    r = run_pair(p, "oci", steps=2, tol=1e-10, max_iters=10_000, reduced_kernel=P.RKERNEL_WOODBURY)
+    for a, b in zip(r["g_iters"], r["o_iters"]):
+        assert abs(a - b) <= 1
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-9
+
+
+@pytest.mark.parametrize("cfg,steps", [(3, 1), (4, 2), (5, 1)])
+def test_woodbury_full_size(cfg, steps):
+    """BASELINE size: the Woodbury family against the oracle (converged, iteration counts) and, bit for bit, against
+    itself (the sums over angles have a fixed order)."""
+    import paper_2305_13555_b200 as P
+    from oracle import threads_available
+    p = make_problem(cfg)
+    r = run_pair(p, "oci", steps=steps, tol=p.tol, max_iters=p.max_iters, threads=threads_available(), reduced_kernel=P.RKERNEL_WOODBURY)
+    assert r["g_iters"] == r["o_iters"]
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-9
+    assert rel(r["g_phi"], r["o_phi"]) < 1e-9
+    g = P.OCI.from_problem(p, reduced_kernel=P.RKERNEL_WOODBURY)
+    for k in range(steps):
+        g.set_source(p.source(k))
+        g.oci_step(p.tol, p.max_iters)
+    assert np.array_equal(g.get_angular_flux(), r["g_psi"])
+    g.close()
+
+
+def test_woodbury_agrees_with_the_dense_families_on_a_sharded_slab():
+    """The family shares the packed state and the loop control with the dense kernels: a slab cut into three shards
+    (emulated ranks on one GPU) gives the unsharded Woodbury result bit for bit."""
+    import paper_2305_13555_b200 as P
+    from paper_2305_13555_b200.sharding import ShardedOCI
+    p = make_problem(3, cells=700)
+    g = P.OCI.from_problem(p, reduced_kernel=P.RKERNEL_WOODBURY)
+    s = ShardedOCI.local(p, 3, reduced_kernel=P.RKERNEL_WOODBURY)
+    s.set_flux_from_problem()
+    for k in range(2):
+        g.set_source(p.source(k))
+        s.set_source(k)
+        a = g.oci_step(p.tol, p.max_iters)
+        b = s.step(p.tol, p.max_iters)
+        assert a[:2] == b[:2]
+    assert np.array_equal(g.get_angular_flux(), s.get_angular_flux())
+    g.close()
+    s.close()
