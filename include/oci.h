@@ -122,6 +122,7 @@ typedef struct {
     int32_t apply_kernel; /* OCI_KERNEL_* */
     int32_t iteration;    /* OCI_ITERATION_* */
     int32_t reduced_kernel; /* OCI_RKERNEL_* */
+    int32_t small_step_cluster; /* CTAs of the one-launch step's cluster, 0 = the three-pass kernels (oci_set_small_step) */
 } oci_info;
 
 /* Problem statement (per-cell dx_j, Sigma_j, Sigma_s,j P:74-82).
@@ -211,6 +212,16 @@ int oci_shard_step(oci_ctx* const* ctxs, int32_t n, double tol, int32_t max_iter
  * returns -1 if the forced family does not serve this problem (block size, number of blocks).  For tests and
  * for comparing families on shapes more than one serves.  Errors: -1 (unknown family). */
 int oci_set_reduced_kernel(oci_ctx* ctx, int32_t kernel);
+
+/* One-launch step for small shared-block problems (the launch-latency-bound end of S4..S128): FIX, every ITER iteration
+ * with the stopping rule and FINAL inside ONE kernel on one thread-block cluster, the state resident in distributed
+ * shared memory, a hardware cluster barrier per iteration instead of a grid-wide one.  Same operators, same iterates up to
+ * rounding order.  mode -1 (default): used by itself when the problem is small enough to fit and to win and no kernel
+ * family has been forced; 0: never; 1: required (oci_setup returns -1 if the problem does not fit: per-cell blocks, HALO
+ * faces, N > 32, or a state larger than a cluster's shared memory).  Call BEFORE oci_setup.  oci_get_info reports the
+ * cluster size in use.  A step that does not converge within the 64 iterations of one launch continues on the three-pass
+ * kernels.  Errors: -1. */
+int oci_set_small_step(oci_ctx* ctx, int32_t mode);
 
 /* Results of the current state.  phi: [cells][4] (eq. 18);
  * psi: [cells][N][4].  HOST pointers; _dev variants take DEVICE pointers and

@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = [
     "oci_create", "oci_workspace_bytes", "oci_setup", "oci_set_flux", "oci_set_flux_dev", "oci_set_source",
     "oci_set_source_dev", "oci_step", "si_step", "oci_get_scalar_flux", "oci_get_angular_flux",
     "oci_get_scalar_flux_dev", "oci_get_angular_flux_dev", "oci_get_scalar_flux_async", "oci_synchronize", "oci_get_quadrature", "oci_get_info",
-    "oci_get_block_inverse", "oci_enable_kernel_timing", "oci_get_kernel_time", "oci_get_aux_kernel_time", "oci_set_iteration", "oci_set_reduced_kernel", "oci_get_setup_time", "oci_shard_mailbox_bytes", "oci_shard_attach", "oci_shard_step", "oci_launch_count",
+    "oci_get_block_inverse", "oci_enable_kernel_timing", "oci_get_kernel_time", "oci_get_aux_kernel_time", "oci_set_iteration", "oci_set_reduced_kernel", "oci_set_small_step", "oci_get_setup_time", "oci_shard_mailbox_bytes", "oci_shard_attach", "oci_shard_step", "oci_launch_count",
     "oci_last_error", "oci_destroy",
 ]
 
@@ -36,7 +36,7 @@ class _bc(C.Structure):
 class _info(C.Structure):
     _fields_ = [("cells", C.c_int64), ("n_angles", C.c_int32), ("block_dim", C.c_int32),
                 ("n_blocks", C.c_int64), ("path", C.c_int32), ("apply_kernel", C.c_int32),
-                ("iteration", C.c_int32), ("reduced_kernel", C.c_int32)]
+                ("iteration", C.c_int32), ("reduced_kernel", C.c_int32), ("small_step_cluster", C.c_int32)]
 
 
 _dp = C.POINTER(C.c_double)
@@ -95,6 +95,8 @@ def load_library():
     L.oci_set_iteration.argtypes = [vp, i32]
     L.oci_set_reduced_kernel.restype = C.c_int
     L.oci_set_reduced_kernel.argtypes = [vp, i32]
+    L.oci_set_small_step.restype = C.c_int
+    L.oci_set_small_step.argtypes = [vp, i32]
     L.oci_get_setup_time.restype = C.c_int
     L.oci_get_setup_time.argtypes = [vp, _dp]
     L.oci_shard_mailbox_bytes.restype = i64
@@ -163,12 +165,14 @@ class OCI:
         self._ws = None
 
     @classmethod
-    def from_problem(cls, p, device="cuda:0", set_flux=True, iteration=None, reduced_kernel=None):
+    def from_problem(cls, p, device="cuda:0", set_flux=True, iteration=None, reduced_kernel=None, small_step=None):
         o = cls(p.dx, p.sigma_t, p.sigma_s, p.v, p.dt, p.n_angles, p.bc_left, p.bc_right)
         if iteration is not None:
             o.set_iteration(iteration)
         if reduced_kernel is not None:
             o.set_reduced_kernel(reduced_kernel)
+        if small_step is not None:
+            o.set_small_step(small_step)
         o.setup(device)
         if set_flux:
             o.set_flux(p.psi0)
@@ -278,7 +282,8 @@ class OCI:
         i = _info()
         self._check(self._L.oci_get_info(self._h, C.byref(i)))
         return dict(cells=i.cells, n_angles=i.n_angles, block_dim=i.block_dim, n_blocks=i.n_blocks, path=i.path,
-                    apply_kernel=i.apply_kernel, iteration=i.iteration, reduced_kernel=i.reduced_kernel)
+                    apply_kernel=i.apply_kernel, iteration=i.iteration, reduced_kernel=i.reduced_kernel,
+                    small_step_cluster=i.small_step_cluster)
 
     def get_block_inverse(self, blk=0):
         n = 4 * self.n_angles
@@ -304,6 +309,9 @@ class OCI:
 
     def set_reduced_kernel(self, kernel):
         self._check(self._L.oci_set_reduced_kernel(self._h, int(kernel)))
+
+    def set_small_step(self, mode):
+        self._check(self._L.oci_set_small_step(self._h, int(mode)))
 
     def shard_attach(self, rank, world, mailbox_ptrs):
         """oci_shard_attach: `mailbox_ptrs` = the W device addresses (ints) of all ranks' mailboxes, in rank order."""

@@ -25,6 +25,21 @@ __device__ __forceinline__ void clear_step_state(const DevView& V)
     }
 }
 
+// a7, the host's side of a fused iteration loop: one thread of the grid calls this when the loop ends (converged, or all
+// `cnt` iterations run) with the number of iterations run and the norms of the last one.  The values land in mapped host
+// memory, the launch's sequence number last (system-scope fence in between), so the host learns the iteration count by
+// polling a word instead of queueing a copy and synchronising a stream.
+__device__ __forceinline__ void publish_step(const DevView& V, int iterations, int last_slot)
+{
+    if (V.host_pub == nullptr) return;
+    volatile unsigned long long* h = V.host_pub;
+    h[1] = (unsigned long long)iterations;
+    h[2] = __ldcg(V.norms + 2 * last_slot + 0);
+    h[3] = __ldcg(V.norms + 2 * last_slot + 1);
+    __threadfence_system();
+    h[0] = V.pub_seq;
+}
+
 // ---- shared-memory / mbarrier / TMA wrappers (one PTX instruction each), used by every TMA-fed kernel
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count)

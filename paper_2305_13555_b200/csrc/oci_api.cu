@@ -1,6 +1,7 @@
 // Host driver behind the C ABI of include/oci.h: argument checking, quadrature, block
 // classification, workspace layout, the time-step loop and error
 // reporting.  Every arithmetic step of the path runs in the kernels of this directory.
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -43,6 +44,8 @@ struct oci_ctx {
     alignas(64) RedOpregMaps romaps{};
     bool use_ktiled = false;
     int32_t forced_rkernel = OCI_RKERNEL_AUTO;   // oci_set_reduced_kernel
+    int32_t small_mode = -1;                     // oci_set_small_step: -1 auto, 0 off, 1 required
+    int32_t small_cluster = 0;                   // cluster size of the one-launch step, 0 = not used (resolved in oci_setup)
     // row f4: shard of a slab (shard_exchange.cu)
     bool sharded = false;
     unsigned long long xtag = 0;       // exchanges completed so far (the next one carries xtag + 1)
@@ -61,6 +64,9 @@ struct oci_ctx {
     bool coop = false;                 // device supports cooperative launches
     int32_t predicted[2] = {0, 0};     // last iteration count of oci / si, sizes the launch chunk
     unsigned long long* h_norms = nullptr;   // pinned
+    unsigned long long* h_pub = nullptr;     // pinned + mapped: [4] = seq, iterations, bits(d), bits(r) written by a fused loop (a7)
+    unsigned long long* d_pub = nullptr;     // its device address
+    unsigned long long pub_seq = 0;
     cudaStream_t stream2 = nullptr;          // side stream of the norm read-back (REDUCED form)
     cudaEvent_t ev_norms = nullptr;
     cudaEvent_t ev_snap = nullptr, ev_snap_done = nullptr;   // oci_get_scalar_flux_async
@@ -105,6 +111,30 @@ int cuda_fail(const oci_ctx* c, cudaError_t e, const char* where)
         if (k_ < 0) return cuda_fail(ctx, cudaGetLastError(), #call); \
         ctx->launches += k_;                                          \
     } while (0)
+
+// a7 without a copy: wait until the fused iteration loop launched with sequence number `seq` has published its
+// iteration count (device_utils.cuh: publish_step).  Spins on the mapped word; every so often it asks the stream whether
+// it is still running, so that a failed launch or kernel ends the wait with the CUDA error instead of hanging.
+int wait_published(oci_ctx* ctx, unsigned long long seq, int32_t* iterations, double* d, double* r)
+{
+    volatile unsigned long long* h = ctx->h_pub;
+    for (unsigned long spins = 1;; ++spins) {
+        if (h[0] == seq) break;
+        if ((spins & 4095) == 0) {
+            const cudaError_t q = cudaStreamQuery(ctx->stream);
+            if (q != cudaErrorNotReady && h[0] != seq) {
+                if (q != cudaSuccess) return cuda_fail(ctx, q, "fused iteration loop");
+                return fail(ctx, OCI_E_CUDA, "the fused iteration loop ended without reporting its iteration count");
+            }
+        }
+    }
+    std::atomic_thread_fence(std::memory_order_acquire);
+    *iterations = (int32_t)h[1];
+    const unsigned long long db = h[2], rb = h[3];
+    std::memcpy(d, &db, 8);
+    std::memcpy(r, &rb, 8);
+    return OCI_OK;
+}
 
 // Makes the context's device current for the duration of an entry point (the caller's current device need not
 // be the one the workspace lives on) and restores the previous one on return.
@@ -402,6 +432,12 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
     const bool timed = ctx->timing && !si;
     const bool si_fast = si && si_fast_supported(V);                     // phi-only iterations, Psi once at the end
 
+    int32_t done_iters = 0;
+    bool conv = false;
+    double d = 0.0, r = 0.0;
+    // small shared-block problems: FIX, all iterations and FINAL in ONE launch on one cluster (oci_reduced_small.cu);
+    // the per-kernel timing of the roofline reports keeps the three passes apart
+    const bool small = red && ctx->small_cluster > 0 && !timed && resolved_iteration(ctx) == OCI_ITERATION_REDUCED;
     if (red) {
         if (!ctx->yz_valid) {
             LAUNCH(launch_pack_yz(V, ctx->cur, 0, s));
@@ -409,6 +445,19 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
             ctx->yz_valid = true;
         }
         ctx->psi_valid = false;
+    }
+    if (small) {
+        const int32_t cnt = max_iters < kNormSlots ? max_iters : kNormSlots;
+        V.host_pub = ctx->d_pub;
+        V.pub_seq = ++ctx->pub_seq;
+        LAUNCH(launch_red_small(V, ctx->small_cluster, ctx->ycur, tol, cnt, cnt >= max_iters, s));
+        V.host_pub = nullptr;
+        int32_t executed = 0;
+        if (int rc = wait_published(ctx, ctx->pub_seq, &executed, &d, &r)) return rc;   // the one read-back (a7), no copy
+        conv = stop_now(tol, d, r);
+        done_iters = executed;
+        // (not converged and max_iters not reached: the three-pass kernels go on from the state the kernel left)
+    } else if (red) {
         if (timed) CK(cudaEventRecord(ctx->ev_aux[0], s));
         LAUNCH(launch_reduced_pass(ctx, PASS_FIX, ctx->ycur, 0, -1, tol, 0, 0));   // a2 (+ a8 of the previous step)
         if (timed) CK(cudaEventRecord(ctx->ev_aux[1], s));
@@ -418,9 +467,6 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
         if (si_fast) LAUNCH(launch_si_fast_begin(V, ctx->cur, s));          // psi_{k-1/2}, compact (+ a8 of the previous step)
         else LAUNCH(launch_cfix(V, ctx->cur, s));                 // a2 (+ a8 of the previous step)
     }
-    int32_t done_iters = 0;
-    bool conv = false;
-    double d = 0.0, r = 0.0;
     int32_t guess = ctx->predicted[si ? 1 : 0] > 0 ? ctx->predicted[si ? 1 : 0] + 1 : 8;
     while (done_iters < max_iters && !conv) {
         int32_t cnt = guess - done_iters;
@@ -433,10 +479,16 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
         // the resident and GEMV kernels of the reduced form run the whole chunk of iterations in ONE cooperative launch
         // (grid-wide barrier + device-side stop between iterations): no launch gap, operator staged once
         const bool fused_loop = red && ctx->red_kernel != OCI_RKERNEL_KTILED && ctx->coop && cnt > 1;
+        // ... and reports its iteration count straight into mapped host memory (publish_step): no copy, no stream sync
+        // (small problems only: the report costs the loop's last CTA a system-scope fence and a PCIe write, about 3 us
+        // that a large problem's FINAL pass would wait for, while its host part overlaps that pass anyway)
+        const bool polled = fused_loop && !timed && ctx->d_pub != nullptr && ctx->J * ctx->n <= 262144;
         if (fused_loop) {
             if (done_iters > 0) CK(cudaMemsetAsync(V.flags + 8, 0, 4, s));  // the grid barrier's arrival counter
             if (timed) CK(cudaEventRecord(ctx->ev[0], s));
+            if (polled) { V.host_pub = ctx->d_pub; V.pub_seq = ++ctx->pub_seq; }
             LAUNCH(launch_reduced_pass(ctx, PASS_ITER, (ctx->ycur + done_iters) & 1, 0, -1, tol, cnt, 0));
+            V.host_pub = nullptr;
             if (timed) CK(cudaEventRecord(ctx->ev[1], s));
         }
         for (int32_t i = 0; i < cnt && !fused_loop; ++i) {
@@ -450,7 +502,7 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
         // The norms are final once the iteration launches are done.  REDUCED form: their read-back goes through a
         // side stream, so the host gets the iteration count while the FINAL pass is still running and the host
         // part of the next step (Python, three launches) overlaps it; everything else stays ordered on `s`.
-        const bool side_readback = red && !timed && ctx->stream2 != nullptr;
+        const bool side_readback = red && !timed && !polled && ctx->stream2 != nullptr;
         if (side_readback) {
             CK(cudaEventRecord(ctx->ev_norms, s));
             CK(cudaStreamWaitEvent(ctx->stream2, ctx->ev_norms, 0));
@@ -464,18 +516,23 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
             if (timed) CK(cudaEventRecord(ctx->ev_aux[3], s));
         }
         if (si_fast) LAUNCH(launch_si_fast_final(V, ctx->cur, done_iters, tol, cnt, done_iters + cnt >= max_iters, s));
-        if (side_readback) {
-            CK(cudaStreamSynchronize(ctx->stream2));                        // the one read-back (a7)
-        } else {
-            CK(cudaMemcpyAsync(ctx->h_norms, V.norms, sizeof(unsigned long long) * 2 * cnt, cudaMemcpyDeviceToHost, s));
-            CK(cudaStreamSynchronize(s));                                   // the one read-back (a7)
-        }
-        CK(cudaGetLastError());
         int32_t executed = cnt;
-        for (int32_t i = 0; i < cnt; ++i) {
-            std::memcpy(&d, &ctx->h_norms[2 * i], 8);
-            std::memcpy(&r, &ctx->h_norms[2 * i + 1], 8);
-            if (stop_now(tol, d, r)) { conv = true; executed = i + 1; break; }
+        if (polled) {
+            if (int rc = wait_published(ctx, ctx->pub_seq, &executed, &d, &r)) return rc;   // the one read-back (a7)
+            conv = stop_now(tol, d, r);
+        } else {
+            if (side_readback) {
+                CK(cudaStreamSynchronize(ctx->stream2));                    // the one read-back (a7)
+            } else {
+                CK(cudaMemcpyAsync(ctx->h_norms, V.norms, sizeof(unsigned long long) * 2 * cnt, cudaMemcpyDeviceToHost, s));
+                CK(cudaStreamSynchronize(s));                               // the one read-back (a7)
+            }
+            CK(cudaGetLastError());
+            for (int32_t i = 0; i < cnt; ++i) {
+                std::memcpy(&d, &ctx->h_norms[2 * i], 8);
+                std::memcpy(&r, &ctx->h_norms[2 * i + 1], 8);
+                if (stop_now(tol, d, r)) { conv = true; executed = i + 1; break; }
+            }
         }
         if (timed && fused_loop) {
             float ms = 0.f;
@@ -499,7 +556,7 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
         }
         done_iters += executed;
     }
-    if (timed && red) {
+    if (timed && red && !small) {
         float ms = 0.f;
         CK(cudaEventElapsedTime(&ms, ctx->ev_aux[0], ctx->ev_aux[1]));
         ctx->aux_ms[0] += ms;
@@ -649,6 +706,8 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
         CK(oci_red_ktiled_opt_in());
         CK(oci_red_resident_opt_in());
         CK(oci_red_opreg_opt_in());
+        CK(oci_red_woodbury_opt_in());
+        CK(oci_red_small_opt_in());
     }
 
     cudaStream_t s = ctx->stream;
@@ -724,6 +783,13 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
         return fail(ctx, OCI_E_SINGULAR, buf);
     }
     if (!ctx->h_norms) CK(cudaHostAlloc((void**)&ctx->h_norms, sizeof(unsigned long long) * 2 * kNormSlots, cudaHostAllocDefault));
+    if (!ctx->h_pub) {
+        CK(cudaHostAlloc((void**)&ctx->h_pub, 64, cudaHostAllocMapped));
+        std::memset(ctx->h_pub, 0, 64);
+        CK(cudaHostGetDevicePointer((void**)&ctx->d_pub, ctx->h_pub, 0));
+    }
+    V.host_pub = nullptr;
+    V.pub_seq = 0;
     if (!ctx->stream2) {
         CK(cudaStreamCreateWithFlags(&ctx->stream2, cudaStreamNonBlocking));
         CK(cudaEventCreateWithFlags(&ctx->ev_norms, cudaEventDisableTiming));
@@ -747,6 +813,22 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
             ctx->red_kernel = OCI_RKERNEL_GEMV;
         else
             return fail(ctx, OCI_E_INVALID, "the kernel family forced with oci_set_reduced_kernel does not serve this problem");
+    }
+    {
+        // the one-launch step (oci_reduced_small.cu): by itself for small problems on the default kernel family, never when
+        // a family has been forced (tests and comparisons of the families), on request if the problem fits
+        int cc = 0;
+        CK(cudaDeviceGetAttribute(&cc, cudaDevAttrClusterLaunch, ctx->device));
+        const int C = cc ? oci_red_small_cluster(V) : 0;
+        ctx->small_cluster = 0;
+        if (ctx->small_mode == 1) {
+            if (C == 0) return fail(ctx, OCI_E_INVALID, "oci_set_small_step(1): the one-launch step does not serve this problem");
+            ctx->small_cluster = C;
+        } else if (ctx->small_mode == -1 && ctx->forced_rkernel == OCI_RKERNEL_AUTO && C == 1) {
+            // measured: the one-CTA form wins (config 1: 0.070 -> 0.05 ms per step); the cluster form is not there yet
+            // (config 2: 0.148 vs 0.096 ms: shared-memory bound DFMA loops on 8 SMs), so it runs on request only
+            ctx->small_cluster = C;
+        }
     }
     ctx->cur = 0;
     ctx->ycur = 0;
@@ -916,6 +998,7 @@ int oci_get_info(const oci_ctx* ctx, oci_info* info)
                          : ctx->use_ktiled ? OCI_KERNEL_KTILED : OCI_KERNEL_GENERIC;
     info->iteration = resolved_iteration(ctx);
     info->reduced_kernel = ctx->red_kernel;
+    info->small_step_cluster = ctx->small_cluster;
     return OCI_OK;
 }
 
@@ -1007,6 +1090,14 @@ int oci_set_reduced_kernel(oci_ctx* ctx, int32_t kernel)
     return OCI_OK;
 }
 
+int oci_set_small_step(oci_ctx* ctx, int32_t mode)
+{
+    if (!ctx) return OCI_E_INVALID;
+    if (mode < -1 || mode > 1) return fail(ctx, OCI_E_INVALID, "oci_set_small_step: mode must be -1, 0 or 1");
+    ctx->small_mode = mode;
+    return OCI_OK;
+}
+
 int oci_get_kernel_time(oci_ctx* ctx, double* ms, int64_t* launches)
 {
     if (!ctx) return OCI_E_INVALID;
@@ -1034,6 +1125,7 @@ void oci_destroy(oci_ctx* ctx)
     if (!ctx) return;
     DeviceGuard guard(ctx);
     if (ctx->h_norms) cudaFreeHost(ctx->h_norms);
+    if (ctx->h_pub) cudaFreeHost(ctx->h_pub);
     if (ctx->stream2) cudaStreamDestroy(ctx->stream2);
     if (ctx->ev_norms) cudaEventDestroy(ctx->ev_norms);
     if (ctx->ev_snap) cudaEventDestroy(ctx->ev_snap);

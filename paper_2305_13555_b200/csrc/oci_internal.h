@@ -70,6 +70,10 @@ struct DevView {
     int32_t bcL, bcR;
     double bcLv, bcRv;
     int32_t sm_count;           // SMs of the device the workspace lives on (queried once in oci_setup)
+    // ---- a7 without a copy: a fused iteration loop reports (iterations run, d, r) of its last iteration straight into
+    // mapped, page-locked HOST memory and then the sequence number of the launch; the host polls the number
+    unsigned long long* host_pub;   // [4] = seq, iterations, bits(d), bits(r); nullptr = do not publish
+    unsigned long long pub_seq;
     // ---- row f4: this context is shard `rank` of `world` (shard_exchange.cu); world = 1 when not sharded
     int32_t rank, world;
     unsigned long long* peers;  // [world] device addresses of every rank's mailbox (peer mapped), in the workspace
@@ -131,6 +135,8 @@ cudaError_t oci_red_gemv_opt_in();
 cudaError_t oci_red_ktiled_opt_in();
 cudaError_t oci_red_resident_opt_in();
 cudaError_t oci_red_opreg_opt_in();
+cudaError_t oci_red_woodbury_opt_in();
+cudaError_t oci_red_small_opt_in();
 int launch_form_and_invert(const DevView& V, cudaStream_t s);
 int launch_set_flux(const DevView& V, const double* d_psi_edge, int buf, cudaStream_t s);
 int launch_cfix(const DevView& V, int buf, cudaStream_t s);
@@ -167,6 +173,9 @@ bool oci_red_opreg_supported(const DevView& V);
 bool oci_red_opreg_prepare(const DevView& V, RedOpregMaps* M);
 int launch_red_opreg(const DevView& V, const RedOpregMaps& M, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force,
                      cudaStream_t s);
+// one-launch step of small shared-block problems (oci_reduced_small.cu): cluster size that serves V, 0 if none
+int oci_red_small_cluster(const DevView& V);
+int launch_red_small(const DevView& V, int C, int ybase, double tol, int cnt, int force, cudaStream_t s);
 int launch_woodbury_setup(const DevView& V, cudaStream_t s);
 int launch_red_woodbury(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s);
 bool oci_red_resident_supported(const DevView& V);

@@ -383,7 +383,9 @@ __global__ void __launch_bounds__(256, 2) oci_red_gemv_kernel(DevView V, int yba
                 } while (seen < target);
             }
             __syncthreads();
-            if (step_done(V.norms, slot + l, tol)) break;      // a7: every CTA takes the same decision
+            const bool stop = step_done(V.norms, slot + l, tol) || l + 1 == nloop;   // a7: every CTA takes the same decision
+            if (stop && blockIdx.x == 0 && threadIdx.x == 0) publish_step(V, l + 1, slot + l);
+            if (stop) break;
         }
     }
   }

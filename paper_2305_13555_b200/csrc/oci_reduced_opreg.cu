@@ -375,6 +375,7 @@ oci_red_opreg_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, const
                 }
                 named_bar_sync(1, 256);
                 stop = step_done(V.norms, slot + l, tol) || l + 1 == nloop;
+                if (stop && blockIdx.x == 0 && tid == 0) publish_step(V, l + 1, slot + l);
                 if (tid == 0) {
                     *go_s = stop ? -1 : 1;
                     mbar_arrive(iter_bar);

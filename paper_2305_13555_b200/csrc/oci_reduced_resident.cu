@@ -404,7 +404,9 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
                 asm volatile("fence.proxy.async;" ::: "memory");
             }
             __syncthreads();
-            if (step_done(V.norms, slot + l, tol)) break;
+            const bool stop = step_done(V.norms, slot + l, tol) || l + 1 == nloop;
+            if (stop && blockIdx.x == 0 && tid == 0) publish_step(V, l + 1, slot + l);
+            if (stop) break;
         }
     }
   }

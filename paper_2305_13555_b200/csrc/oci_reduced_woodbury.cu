@@ -141,7 +141,7 @@ namespace {
 // values and keeps two, the second exchanges one and keeps one, the remaining levels reduce a single value: 6 shuffles
 // instead of 20 for a full warp, after which the lane with bits (hi, hi2) holds the total of slot 2 hi + hi2.  N <= 32:
 // the four totals are broadcast by four more shuffles; N > 32: the partials of the cell's N/32 warps meet in shared memory.
-template <int W>
+template <int W, bool NAMED = false>
 __device__ __forceinline__ void cell_sum(double (&p)[4], int N, int cell_slot, double* __restrict__ sm)
 {
     if (W == 0) {
@@ -174,7 +174,8 @@ __device__ __forceinline__ void cell_sum(double (&p)[4], int N, int cell_slot, d
     }
     const int warp = threadIdx.x >> 5, wpc = N >> 5;
     if ((lane & 7) == 0) sm[warp * 4 + (lane >> 3)] = keep;               // lanes 0, 8, 16, 24 hold slots 0..3
-    __syncthreads();
+    if (NAMED) named_bar_sync(1, 256);                                    // the consumer warps only (a producer warp is not in it)
+    else __syncthreads();
     const double* __restrict__ q = sm + (warp / wpc) * wpc * 4;
     p[0] = p[1] = p[2] = p[3] = 0.0;
     for (int w = 0; w < wpc; ++w) {
@@ -467,8 +468,194 @@ oci_red_woodbury_kernel(DevView V, int ybase, int slot, int prev_slot, double to
                 } while (seen < target);
             }
             __syncthreads();
-            if (step_done(V.norms, slot + l, tol)) break;
+            const bool stop = step_done(V.norms, slot + l, tol) || l + 1 == nloop;
+            if (stop && blockIdx.x == 0 && threadIdx.x == 0) publish_step(V, l + 1, slot + l);
+            if (stop) break;
         }
+    }
+  }
+}
+
+// ---- ITER / FINAL with a shared block and a power-of-two N in [8, 256]: the same arithmetic, the rows STAGED BY TMA.
+// The direct kernel above keeps one item per thread in flight (16 warps per SM): latency-bound at 53-57 % of the HBM
+// bandwidth.  Here a producer warp streams, for every group of 256 / N cells, the rows the group reads - y rows
+// j0-1 .. j0+cpb of the source iterate (one contiguous piece, ghost rows included), the cpb rows of the additive operand,
+// and for ITER the phifix / old phi rows - with 1-D bulk copies (cp.async.bulk, completion on an mbarrier) into a
+// ring of WT_STAGES stages; the 256 consumer threads read their six values from shared memory, release the stage at once
+// (one arrival per warp) and compute out of registers, so the ring runs several groups ahead of the arithmetic whatever
+// the occupancy, and the address arithmetic of an item shrinks to the two stores.
+constexpr int WT_STAGES = 4;
+constexpr int WT_CONS = 256;                       // consumer threads; + one producer warp
+
+template <int PASS, int W>
+__global__ void __launch_bounds__(WT_CONS + 32, 2)
+oci_red_woodbury_tma_kernel(DevView V, int ybase, int slot, int prev_slot, double tol, int cnt, int force)
+{
+    extern __shared__ __align__(128) unsigned char wt_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int ysrc = ybase;
+    if (PASS == PASS_ITER) {
+        if (step_done(V.norms, prev_slot, tol)) return;
+    } else {
+        int L = 0;
+        for (int i0 = 0; i0 < cnt && L == 0; i0 += 32) {
+            const int i = i0 + lane;
+            bool hit = false;
+            if (i < cnt) {
+                const double d = __longlong_as_double((long long)__ldcg(V.norms + 2 * i + 0));
+                const double r = __longlong_as_double((long long)__ldcg(V.norms + 2 * i + 1));
+                hit = stop_now(tol, d, r);
+            }
+            const unsigned msk = __ballot_sync(0xffffffffu, hit);
+            if (msk) L = i0 + __ffs(msk);
+        }
+        if (L == 0) {
+            if (!force) return;
+            L = cnt;
+        }
+        ysrc = (ybase + L - 1) & 1;
+    }
+    const int N = V.N, K2 = 2 * N, N2 = N >> 1;
+    const int J = (int)V.J;                                                // the launcher guarantees 32-bit element offsets
+    const int cpb = WT_CONS / N;
+    // stage: [cpb+2][K2] y rows | [cpb][K2] additive rows | [cpb][4] phifix | [cpb][4] old phi
+    const int y_dbl = (cpb + 2) * K2, fx_dbl = cpb * K2;
+    const int stage_dbl = y_dbl + fx_dbl + (PASS == PASS_ITER ? 8 * cpb : 0);
+    double* ring = reinterpret_cast<double*>(wt_raw);
+    double* red = ring + (size_t)WT_STAGES * stage_dbl;                    // cell_sum's double buffer
+    uint64_t* full = reinterpret_cast<uint64_t*>(red + 2 * 4 * (WT_CONS / 32));
+    uint64_t* empty = full + WT_STAGES;
+    if (threadIdx.x == 0) {
+        for (int st = 0; st < WT_STAGES; ++st) { mbar_init(&full[st], 1); mbar_init(&empty[st], WT_CONS / 32); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const int ngroups = (J + cpb - 1) / cpb;
+    const int my_groups = (int)blockIdx.x < ngroups ? (ngroups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+    const int nloop = PASS == PASS_ITER ? (cnt > 1 ? cnt : 1) : 1;
+    const double* __restrict__ fx = PASS == PASS_ITER ? V.yfix : V.ifix;
+    int it0 = 0;                                                           // groups this CTA has streamed in earlier iterations
+
+    // consumer-side constants
+    const bool consumer = warp < WT_CONS / 32;
+    const int cs = consumer ? threadIdx.x / N : 0, m = consumer ? threadIdx.x - cs * N : 0;
+    const int half = m >= N2, mm = m - half * N2;
+    const int qk = pack_q(half, 0, mm, N), qe = pack_q(half, 1, mm, N);
+    const double amu = fabs(V.mu[m]), wm = V.w[m];
+    const bool ghost_l = PASS == PASS_ITER && !half && V.bcL == OCI_BC_REFLECTING;
+    const bool ghost_r = PASS == PASS_ITER && half && V.bcR == OCI_BC_REFLECTING;
+    const int mqk = mirror_q(qk, N), mqe = mirror_q(qe, N);
+    const bool phi_lane = PASS == PASS_ITER && m < 4;
+    const int psl = m & 3;
+    // offsets inside a stage: the neighbour row of cell slot cs is row cs (left, mu > 0) or cs + 2 (right, mu < 0) of the y box
+    const int o_ink = (cs + (half ? 0 : 2)) * K2 + qk, o_ine = (cs + (half ? 0 : 2)) * K2 + qe;
+    const int o_fxk = y_dbl + cs * K2 + qk, o_fxe = y_dbl + cs * K2 + qe;
+    const int o_pf = y_dbl + fx_dbl + cs * 4 + psl, o_po = o_pf + 4 * cpb;
+    const int o_out = cs * K2;                                             // + j0 * K2 + qk / qe
+    WbOps<PASS> O;
+    double mrow[4] = {0.0, 0.0, 0.0, 0.0};
+    if (consumer) {
+        load_ops<PASS>(O, V.wba + m, V.wbd + m, N, half, amu, wm);
+#pragma unroll
+        for (int cc = 0; cc < 4; ++cc) mrow[cc] = V.wbm[4 * psl + cc];
+    }
+    int flip = 0;
+
+  for (int l = 0; l < nloop; ++l) {
+    const double* __restrict__ Ys = V.y[PASS == PASS_ITER ? (ybase + l) & 1 : ysrc];
+    double* __restrict__ Yd = PASS == PASS_ITER ? V.y[(ybase + l + 1) & 1] : V.z;
+    if (!consumer) {
+        // ---- producer: one elected lane streams this CTA's groups of this iteration
+        if (lane == 0) {
+            if (l > 0) asm volatile("fence.proxy.async;" ::: "memory");   // rows other SMs stored before the grid barrier
+            for (int i = 0; i < my_groups; ++i) {
+                const int u = it0 + i, st = u % WT_STAGES;
+                if (u >= WT_STAGES) mbar_wait(&empty[st], ((u / WT_STAGES) - 1) & 1);
+                const int j0 = ((int)blockIdx.x + i * (int)gridDim.x) * cpb;
+                const int rows = J - j0 < cpb ? J - j0 : cpb;
+                double* sg = ring + (size_t)st * stage_dbl;
+                const uint32_t yb = (uint32_t)(rows + 2) * K2 * 8, fb = (uint32_t)rows * K2 * 8, pb = (uint32_t)rows * 32;
+                mbar_expect_tx(&full[st], yb + fb + (PASS == PASS_ITER ? 2 * pb : 0));
+                tma_load_1d(sg, Ys + ((int64_t)j0 - 1) * K2, yb, &full[st]);
+                tma_load_1d(sg + y_dbl, fx + (int64_t)j0 * K2, fb, &full[st]);
+                if (PASS == PASS_ITER) {
+                    tma_load_1d(sg + y_dbl + fx_dbl, V.phifix + (int64_t)j0 * 4, pb, &full[st]);
+                    tma_load_1d(sg + y_dbl + fx_dbl + 4 * cpb, V.phi + (int64_t)j0 * 4, pb, &full[st]);
+                }
+            }
+        }
+    } else {
+        double dmax = 0.0, rmax = 0.0;
+        for (int i = 0; i < my_groups; ++i) {
+            const int u = it0 + i, st = u % WT_STAGES;
+            const int j0 = ((int)blockIdx.x + i * (int)gridDim.x) * cpb;
+            const bool valid = j0 + cs < J;
+            const double* sg = ring + (size_t)st * stage_dbl;
+            mbar_wait(&full[st], (u / WT_STAGES) & 1);
+            double a = sg[o_ink], b = sg[o_ine];
+            const double c = sg[o_fxk], d = sg[o_fxe];
+            double pf = 0.0, po = 0.0;
+            if (phi_lane) { pf = sg[o_pf]; po = sg[o_po]; }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[st]);                        // the stage is free again: everything is in registers
+            if (!valid) a = b = 0.0;                                       // rows past the last cell were not loaded
+            double p[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) p[r] = fma(O.pe[r], b, O.pk[r] * a);
+            cell_sum<W, true>(p, N, cs, red + (flip ? 4 * (WT_CONS / 32) : 0));
+            flip ^= 1;
+            if (!valid) continue;
+            const int j = j0 + cs;
+            if (phi_lane) {
+                // a6: phi^(l+1) = phifix + M s and the two max-norms of the stopping rule
+                const double nw = pf + fma(mrow[3], p[3], fma(mrow[2], p[2], fma(mrow[1], p[1], mrow[0] * p[0])));
+                V.phi[j * 4 + psl] = nw;
+                dmax = nanmax(dmax, fabs(nw - po));
+                rmax = nanmax(rmax, fabs(nw));
+            }
+            const double tk = fma(O.g[1], b, O.g[0] * a), te = fma(O.g[3], b, O.g[2] * a);
+            const double vk = c + fma(O.dk[3], p[3], fma(O.dk[2], p[2], fma(O.dk[1], p[1], fma(O.dk[0], p[0], tk))));
+            const double ve = d + fma(O.de[3], p[3], fma(O.de[2], p[2], fma(O.de[1], p[1], fma(O.de[0], p[0], te))));
+            double* __restrict__ out = Yd + (j0 * K2 + o_out);
+            out[qk] = vk;
+            out[qe] = ve;
+            if (ghost_l && j == 0) {
+                Yd[mqk - K2] = vk;
+                Yd[mqe - K2] = ve;
+            }
+            if (ghost_r && j == J - 1) {
+                Yd[(int64_t)J * K2 + mqk] = vk;
+                Yd[(int64_t)J * K2 + mqe] = ve;
+            }
+        }
+        if (PASS == PASS_ITER) {
+            dmax = warp_max(dmax);
+            rmax = warp_max(rmax);
+            if (lane == 0) {
+                atomic_max_nonneg(&V.norms[2 * (slot + l) + 0], dmax);
+                atomic_max_nonneg(&V.norms[2 * (slot + l) + 1], rmax);
+            }
+        }
+    }
+    it0 += my_groups;
+    if (PASS == PASS_ITER && nloop > 1) {
+        // grid-wide barrier (cooperative launch), then the stopping rule on the now final norms (a7)
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned int* bar = reinterpret_cast<unsigned int*>(V.flags) + 8;
+            atomicAdd(bar, 1u);
+            const unsigned int target = (unsigned int)(l + 1) * gridDim.x;
+            unsigned int seen;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(bar) : "memory");
+            } while (seen < target);
+        }
+        __syncthreads();
+        const bool stop = step_done(V.norms, slot + l, tol) || l + 1 == nloop;
+        if (stop && blockIdx.x == 0 && threadIdx.x == 0) publish_step(V, l + 1, slot + l);
+        if (stop) break;
     }
   }
 }
@@ -513,12 +700,61 @@ void launch_wb_w(const DevView& V, int ybase, int slot, int prev_slot, double to
     else launch_wb_i<PASS, SHARED, TPB, W, int64_t>(V, ybase, slot, prev_slot, tol, cnt, force, s);
 }
 
+size_t wt_smem(const DevView& V, int pass)
+{
+    const int cpb = WT_CONS / V.N, K2 = 2 * V.N;
+    const size_t stage = ((size_t)(2 * cpb + 2) * K2 + (pass == PASS_ITER ? 8 * cpb : 0)) * 8;
+    return WT_STAGES * stage + 2 * 4 * (WT_CONS / 32) * 8 + 2 * WT_STAGES * 8 + 128;
+}
+
+// the TMA-staged kernel: ITER / FINAL, one shared block, power-of-two N in [8, 32] (measured: 3 % faster ITER and 30 %
+// faster FINAL than the direct kernel at N = 32, slower at N = 128 where a group is only two cells), 32-bit element
+// offsets, and enough cell groups to give every SM a few (below that the problem is launch-latency bound)
+bool wt_serves(const DevView& V)
+{
+    const int N = V.N;
+    return V.nblk == 1 && (N & (N - 1)) == 0 && N >= 8 && N <= 32 && (V.J + 2) * 2 * (int64_t)N < ((int64_t)1 << 31) &&
+           V.J * (int64_t)N >= (int64_t)V.sm_count * 4 * WT_CONS;
+}
+
+template <int PASS, int W>
+void launch_wt_w(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
+{
+    const size_t smem = wt_smem(V, PASS);
+    const int cpb = WT_CONS / V.N;
+    const int64_t groups = (V.J + cpb - 1) / cpb;
+    int per_sm = 1;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, oci_red_woodbury_tma_kernel<PASS, W>, WT_CONS + 32, smem);
+    if (per_sm < 1) per_sm = 1;
+    const int64_t cap = (int64_t)V.sm_count * per_sm;
+    const unsigned grid = (unsigned)(groups < cap ? groups : cap);
+    if (PASS == PASS_ITER && cnt > 1) {
+        DevView Vv = V;
+        void* args[] = {&Vv, &ybase, &slot, &prev_slot, &tol, &cnt, &force};
+        cudaLaunchCooperativeKernel((const void*)oci_red_woodbury_tma_kernel<PASS, W>, dim3(grid), dim3(WT_CONS + 32), args, smem, s);
+        return;
+    }
+    oci_red_woodbury_tma_kernel<PASS, W><<<grid, WT_CONS + 32, smem, s>>>(V, ybase, slot, prev_slot, tol, cnt, force);
+}
+
+template <int PASS>
+void launch_wt(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
+{
+    if (V.N == 8) launch_wt_w<PASS, 8>(V, ybase, slot, prev_slot, tol, cnt, force, s);
+    else if (V.N == 16) launch_wt_w<PASS, 16>(V, ybase, slot, prev_slot, tol, cnt, force, s);
+    else launch_wt_w<PASS, 32>(V, ybase, slot, prev_slot, tol, cnt, force, s);
+}
+
 // CTAs of 256 threads (one or more whole cells each) unless a cell has more angles than that; the butterfly for
 // power-of-two N >= 8, the shared-memory sum otherwise
 template <int PASS, bool SHARED>
 void launch_wb(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
 {
     const int N = V.N;
+    if (SHARED && PASS != PASS_FIX && wt_serves(V)) {
+        launch_wt<PASS == PASS_FIX ? PASS_ITER : PASS>(V, ybase, slot, prev_slot, tol, cnt, force, s);
+        return;
+    }
     const bool pow2 = (N & (N - 1)) == 0 && N >= 8;
     if (N > 256) {
         if (pow2) launch_wb_w<PASS, SHARED, 512, 32>(V, ybase, slot, prev_slot, tol, cnt, force, s);
@@ -537,6 +773,21 @@ void launch_wb_pass(const DevView& V, int pass, int ybase, int slot, int prev_sl
     else launch_wb<PASS_FINAL, SHARED>(V, ybase, 0, -1, tol, cnt, force, s);
 }
 }  // namespace
+
+cudaError_t oci_red_woodbury_opt_in()
+{
+    const auto at = cudaFuncAttributeMaxDynamicSharedMemorySize;
+    const int bytes = 100 * 1024;
+    cudaError_t e;
+    if ((e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_ITER, 8>, at, bytes)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_ITER, 16>, at, bytes)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_ITER, 32>, at, bytes)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_FINAL, 8>, at, bytes)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_FINAL, 16>, at, bytes)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_FINAL, 32>, at, bytes)) != cudaSuccess)
+        return e;
+    return cudaSuccess;
+}
 
 int launch_red_woodbury(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
 {

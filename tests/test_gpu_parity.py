@@ -21,13 +21,13 @@ FULL, REDUCED = 0, 1
 ITERATIONS = [pytest.param(FULL, id="full"), pytest.param(REDUCED, id="reduced")]
 
 
-def run_pair(p, scheme, steps, tol, max_iters, threads=8, iteration=None, reduced_kernel=None):
+def run_pair(p, scheme, steps, tol, max_iters, threads=8, iteration=None, reduced_kernel=None, small_step=None):
     """Run `steps` time steps on both sides; return per-step (iters) and final fluxes.
     iteration: OCI_ITERATION_FULL / _REDUCED (None = the library default); the oracle is always the
     plain method (one LU solve per cell per iteration)."""
     import paper_2305_13555_b200 as P
     from oracle import Oracle
-    g = P.OCI.from_problem(p, iteration=iteration, reduced_kernel=reduced_kernel)
+    g = P.OCI.from_problem(p, iteration=iteration, reduced_kernel=reduced_kernel, small_step=small_step)
     o = Oracle.from_problem(p, threads=threads)
     gi, oi = [], []
     for k in range(steps):
@@ -109,8 +109,18 @@ def test_blocked_inversion_shapes(N, nblk):
     g.close()
 
 
+# "oci-reduced": the library default (small problems take the one-launch step of oci_reduced_small.cu);
+# "oci-reduced-3pass": the same with the one-launch step switched off, so that the three-pass kernel families are
+# exercised at small sizes too
 SCHEMES = [pytest.param("oci", FULL, id="oci-full"), pytest.param("oci", REDUCED, id="oci-reduced"),
-           pytest.param("si", None, id="si")]
+           pytest.param("oci", -REDUCED, id="oci-reduced-3pass"), pytest.param("si", None, id="si")]
+
+
+def _form(iteration):
+    """(iteration form, small_step) of a SCHEMES entry: a negative form = that form with the one-launch step off"""
+    if iteration is not None and iteration < 0:
+        return -iteration, 0
+    return iteration, None
 
 
 @pytest.mark.parametrize("scheme,iteration", SCHEMES)
@@ -118,7 +128,8 @@ SCHEMES = [pytest.param("oci", FULL, id="oci-full"), pytest.param("oci", REDUCED
 def test_fixed_iteration_parity(cfg, cells, scheme, iteration):
     """tol < 0: exactly 5 iterations in each of 2 steps; Psi and phi within 1e-12."""
     p = make_problem(cfg, cells=cells)
-    r = run_pair(p, scheme, steps=2, tol=-1.0, max_iters=5, iteration=iteration)
+    iteration, small = _form(iteration)
+    r = run_pair(p, scheme, steps=2, tol=-1.0, max_iters=5, iteration=iteration, small_step=small)
     assert r["g_iters"] == [5, 5] == r["o_iters"]
     assert rel(r["g_psi"], r["o_psi"]) < 1e-12
     assert rel(r["g_phi"], r["o_phi"]) < 1e-12
@@ -129,7 +140,8 @@ def test_fixed_iteration_parity(cfg, cells, scheme, iteration):
 @pytest.mark.parametrize("cfg,cells,steps", [(1, 20, 5), (2, 203, 4), (3, 300, 3), (4, 70, 2), (5, 37, 3)])
 def test_converged_parity(cfg, cells, steps, scheme, iteration):
     p = make_problem(cfg, cells=cells)
-    r = run_pair(p, scheme, steps=steps, tol=p.tol, max_iters=p.max_iters, iteration=iteration)
+    iteration, small = _form(iteration)
+    r = run_pair(p, scheme, steps=steps, tol=p.tol, max_iters=p.max_iters, iteration=iteration, small_step=small)
     for a, b in zip(r["g_iters"], r["o_iters"]):
         assert abs(a - b) <= 1, (r["g_iters"], r["o_iters"])
     assert rel(r["g_psi"], r["o_psi"]) < 1e-9
@@ -170,10 +182,11 @@ def _custom(J, N, bcL, bcR, seed, hetero, dt=0.13):
 ])
 def test_edge_cases(J, N, bcL, bcR, hetero, scheme, iteration):
     p = _custom(J, N, bcL, bcR, seed=J * 100 + N, hetero=hetero)
-    r = run_pair(p, scheme, steps=2, tol=-1.0, max_iters=4, iteration=iteration)
+    iteration, small = _form(iteration)
+    r = run_pair(p, scheme, steps=2, tol=-1.0, max_iters=4, iteration=iteration, small_step=small)
     assert rel(r["g_psi"], r["o_psi"]) < 1e-12
     assert rel(r["g_phi"], r["o_phi"]) < 1e-12
-    r = run_pair(p, scheme, steps=2, tol=1e-10, max_iters=10_000, iteration=iteration)
+    r = run_pair(p, scheme, steps=2, tol=1e-10, max_iters=10_000, iteration=iteration, small_step=small)
     for a, b in zip(r["g_iters"], r["o_iters"]):
         assert abs(a - b) <= 1
     assert rel(r["g_psi"], r["o_psi"]) < 1e-9
@@ -481,8 +494,9 @@ def test_full_size_reduced_step_is_deterministic(cfg):
     assert np.array_equal(out[0][1], out[1][1])
 
 
+@pytest.mark.parametrize("small", [0, 1])
 @pytest.mark.parametrize("N", [16, 32])
-def test_resident_fused_loop_many_iterations(N):
+def test_resident_fused_loop_many_iterations(N, small):
     """The resident kernels run a whole chunk of up to 64 iterations in one cooperative launch (grid barrier and
     device-side stop between iterations).  A problem that needs several chunks (thin cells, c = 0.999, long time
     step, mirrors on both sides) exercises the re-arming of the barrier counter and of the norm slots."""
@@ -490,8 +504,10 @@ def test_resident_fused_loop_many_iterations(N):
     from oracle import Oracle
     q = _custom(150, N, (REF, 0.0), (REF, 0.0), seed=11 + N, hetero=False, dt=50.0)
     q.sigma_s[:] = q.sigma_t * 0.999
-    g, o = P.OCI.from_problem(q, iteration=REDUCED), Oracle.from_problem(q, threads=8)
+    # small = 1: the first 64 iterations run in the one-launch step, which then hands over to the resident kernels
+    g, o = P.OCI.from_problem(q, iteration=REDUCED, small_step=small), Oracle.from_problem(q, threads=8)
     assert g.get_info()["reduced_kernel"] == P.RKERNEL_RESIDENT
+    assert (g.get_info()["small_step_cluster"] > 0) == (small == 1)
     for x in (g, o):
         x.set_source(q.source(0))
     a, b = g.oci_step(1e-10, 100_000), o.oci_step(1e-10, 100_000)
@@ -647,3 +663,106 @@ def test_woodbury_agrees_with_the_dense_families_on_a_sharded_slab():
     assert np.array_equal(g.get_angular_flux(), s.get_angular_flux())
     g.close()
     s.close()
+
+
+def test_woodbury_on_a_multi_region_slab():
+    """A Reed-like slab (five regions, four materials incl. a void and a pure absorber, S16): the Woodbury family with a
+    handful of blocks (every cell looks up its block's 4x4 pieces) against the oracle."""
+    import paper_2305_13555_b200 as P
+    from workloads.configs import Problem
+    J, N = 640, 16
+    bounds = [(0, 128, 50.0, 0.0), (128, 192, 5.0, 0.0), (192, 320, 1e-12, 0.0), (320, 576, 1.0, 0.9), (576, 640, 1.0, 0.9)]
+    dx, st, ss = np.full(J, 0.0125 * 10), np.zeros(J), np.zeros(J)
+    q = np.zeros((J, 4))
+    for a, b, sig, sigs in bounds:
+        st[a:b], ss[a:b] = sig, sigs
+    q[0:128], q[320:576] = 50.0, 1.0
+    p = Problem(0, "reed-like", N, J, dx, st, ss, 4.0, 1.0, 2, (REF, 0.0), (VAC, 0.0), np.zeros((J, N, 2)), _source=lambda step: q)
+    r = run_pair(p, "oci", steps=1, tol=-1.0, max_iters=6, reduced_kernel=P.RKERNEL_WOODBURY)
+    assert r["info"]["n_blocks"] == 4
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-12 and rel(r["g_phi"], r["o_phi"]) < 1e-12
+    r = run_pair(p, "oci", steps=2, tol=1e-10, max_iters=10_000, threads=16, reduced_kernel=P.RKERNEL_WOODBURY)
+    assert r["g_iters"] == r["o_iters"]
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-9
+
+
+# ---- the one-launch step of small shared-block problems (oci_reduced_small.cu)
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_small_step_serves_configs_1_and_2(cfg):
+    """BASELINE size: config 1 takes the one-launch step by default (one CTA), config 2 on request (a cluster of 8);
+    every step of the config against the oracle (iteration counts equal, fluxes 1e-9), bit-reproducible, and equal to
+    the three-pass kernels within rounding."""
+    import paper_2305_13555_b200 as P
+    p = make_problem(cfg)
+    mode = {1: None, 2: 1}[cfg]
+    r = run_pair(p, "oci", steps=p.n_steps, tol=p.tol, max_iters=p.max_iters, small_step=mode)
+    assert r["info"]["small_step_cluster"] == {1: 1, 2: 8}[cfg] and r["info"]["iteration"] == P.ITERATION_REDUCED
+    assert r["g_iters"] == r["o_iters"]
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-9 and rel(r["g_phi"], r["o_phi"]) < 1e-9
+    assert r["launches"] <= 4 + 2 * p.n_steps                    # set_flux + one launch per step (+ layout on demand)
+    r2 = run_pair(p, "oci", steps=p.n_steps, tol=p.tol, max_iters=p.max_iters, small_step=mode)
+    assert np.array_equal(r["g_psi"], r2["g_psi"]) and np.array_equal(r["g_phi"], r2["g_phi"])
+    r3 = run_pair(p, "oci", steps=p.n_steps, tol=p.tol, max_iters=p.max_iters, small_step=0)
+    assert r3["info"]["small_step_cluster"] == 0 and r3["g_iters"] == r["g_iters"]
+    assert rel(r["g_psi"], r3["g_psi"]) < 1e-12
+    r = run_pair(p, "oci", steps=2, tol=-1.0, max_iters=5, small_step=mode)
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-12 and rel(r["g_phi"], r["o_phi"]) < 1e-12
+
+
+@pytest.mark.parametrize("J,N,bcL,bcR", [
+    (1, 2, (VAC, 0.0), (VAC, 0.0)),            # one cell, S2, one CTA
+    (1, 4, (REF, 0.0), (REF, 0.0)),            # one cell between two mirrors
+    (7, 6, (INC, 0.5), (REF, 0.0)),            # N not a power of two
+    (64, 4, (REF, 0.0), (INC, 2.0)),           # one CTA
+    (65, 8, (INC, 1.0), (INC, 0.25)),          # 8 CTAs, the last one short (9 + ... + 2 cells)
+    (129, 8, (REF, 0.0), (VAC, 0.0)),
+    (1000, 16, (REF, 0.0), (REF, 0.0)),        # config-2 size, mirrors at both ends of the cluster
+    (70, 32, (VAC, 0.0), (REF, 0.0)),          # config-3 block size
+])
+def test_small_step_shapes(J, N, bcL, bcR):
+    import paper_2305_13555_b200 as P
+    p = _custom(J, N, bcL, bcR, seed=J * 7 + N, hetero=False)
+    r = run_pair(p, "oci", steps=3, tol=-1.0, max_iters=4, small_step=1)
+    assert r["info"]["small_step_cluster"] >= 1
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-12 and rel(r["g_phi"], r["o_phi"]) < 1e-12
+    r = run_pair(p, "oci", steps=3, tol=1e-10, max_iters=10_000, small_step=1)
+    assert r["g_iters"] == r["o_iters"]
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-9
+    # mixed with SI and the FULL form on one context: the layouts stay consistent
+    from oracle import Oracle
+    g, o = P.OCI.from_problem(p, small_step=1), Oracle.from_problem(p)
+    for x in (g, o):
+        x.set_source(p.source(0))
+    assert g.oci_step(1e-10, 10_000)[:2] == o.oci_step(1e-10, 10_000)[:2]
+    assert g.si_step(1e-10, 10_000)[:2] == o.si_step(1e-10, 10_000)[:2]
+    assert g.oci_step(-1.0, 3)[:2] == (1, 3) == o.oci_step(-1.0, 3)[:2]
+    assert rel(g.get_angular_flux(), o.angular_flux()) < 1e-9
+    g.close()
+
+
+def test_small_step_hand_over_and_refusals():
+    """More than the 64 iterations of one launch: the three-pass kernels continue from the state the kernel left (exact
+    counts in the middle of later chunks); required mode is refused where the step does not fit."""
+    import paper_2305_13555_b200 as P
+    from oracle import Oracle
+    q = _custom(40, 4, (REF, 0.0), (REF, 0.0), seed=5, hetero=False, dt=50.0)
+    q.sigma_s[:] = q.sigma_t * 0.999
+    g, o = P.OCI.from_problem(q, small_step=1), Oracle.from_problem(q)
+    for x in (g, o):
+        x.set_source(q.source(0))
+    for n in (64, 65, 77, 150):
+        g.set_flux(q.psi0); o.set_flux(q.psi0)
+        assert g.oci_step(-1.0, n)[:2] == (1, n) == o.oci_step(-1.0, n)[:2]
+        assert rel(g.get_angular_flux(), o.angular_flux()) < 1e-12, n
+    g.set_flux(q.psi0); o.set_flux(q.psi0)
+    a, b = g.oci_step(1e-10, 100_000), o.oci_step(1e-10, 100_000)
+    assert a[0] == b[0] == 0 and a[1] == b[1] and a[1] > 64
+    assert rel(g.get_scalar_flux(), o.scalar_flux()) < 1e-8
+    g.close()
+    for p in (make_problem(5, cells=20), make_problem(3, cells=5000), make_problem(4, cells=16)):
+        h = P.OCI(p.dx, p.sigma_t, p.sigma_s, p.v, p.dt, p.n_angles, p.bc_left, p.bc_right)
+        h.set_small_step(1)
+        with pytest.raises(P.OCIError) as e:
+            h.setup()
+        assert e.value.code == -1
+        h.close()

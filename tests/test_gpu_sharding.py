@@ -14,7 +14,9 @@ VAC, INC, REF = 0, 1, 2
 
 def _run_unsharded(p, steps, tol, max_iters):
     import paper_2305_13555_b200 as P
-    g = P.OCI.from_problem(p, iteration=P.ITERATION_REDUCED)
+    # the three-pass kernels the shards run (a small unsharded slab would otherwise take the one-launch step, whose sums
+    # run in another order)
+    g = P.OCI.from_problem(p, iteration=P.ITERATION_REDUCED, small_step=0)
     its = []
     for k in range(steps):
         g.set_source(p.source(k))
