@@ -486,9 +486,10 @@ oci_red_woodbury_kernel(DevView V, int ybase, int slot, int prev_slot, double to
 // the occupancy, and the address arithmetic of an item shrinks to the two stores.
 constexpr int WT_STAGES = 4;
 constexpr int WT_CONS = 256;                       // consumer threads; + one producer warp
+constexpr int WT_U = 2;                            // cells per thread and group: two independent butterflies in flight
 
-template <int PASS, int W>
-__global__ void __launch_bounds__(WT_CONS + 32, 2)
+template <int PASS, int NT>
+__global__ void __maxnreg__(112)
 oci_red_woodbury_tma_kernel(DevView V, int ybase, int slot, int prev_slot, double tol, int cnt, int force)
 {
     extern __shared__ __align__(128) unsigned char wt_raw[];
@@ -515,12 +516,14 @@ oci_red_woodbury_tma_kernel(DevView V, int ybase, int slot, int prev_slot, doubl
         }
         ysrc = (ybase + L - 1) & 1;
     }
-    const int N = V.N, K2 = 2 * N, N2 = N >> 1;
+    constexpr int N = NT, K2 = 2 * N, N2 = N >> 1;                         // N is a template parameter: every offset is an immediate
+    constexpr int W = N < 32 ? N : 32;                                     // width of the butterfly inside a warp
     const int J = (int)V.J;                                                // the launcher guarantees 32-bit element offsets
-    const int cpb = WT_CONS / N;
-    // stage: [cpb+2][K2] y rows | [cpb][K2] additive rows | [cpb][4] phifix | [cpb][4] old phi
-    const int y_dbl = (cpb + 2) * K2, fx_dbl = cpb * K2;
-    const int stage_dbl = y_dbl + fx_dbl + (PASS == PASS_ITER ? 8 * cpb : 0);
+    constexpr int cpb = WT_CONS / N;                                       // cells per pass of the 256 threads
+    constexpr int gc = WT_U * cpb;                                         // cells per group (stage): WT_U per thread
+    // stage: [gc+2][K2] y rows | [gc][K2] additive rows | [gc][4] phifix | [gc][4] old phi
+    constexpr int y_dbl = (gc + 2) * K2, fx_dbl = gc * K2;
+    constexpr int stage_dbl = y_dbl + fx_dbl + (PASS == PASS_ITER ? 8 * gc : 0);
     double* ring = reinterpret_cast<double*>(wt_raw);
     double* red = ring + (size_t)WT_STAGES * stage_dbl;                    // cell_sum's double buffer
     uint64_t* full = reinterpret_cast<uint64_t*>(red + 2 * 4 * (WT_CONS / 32));
@@ -531,7 +534,7 @@ oci_red_woodbury_tma_kernel(DevView V, int ybase, int slot, int prev_slot, doubl
     }
     __syncthreads();
 
-    const int ngroups = (J + cpb - 1) / cpb;
+    const int ngroups = (J + gc - 1) / gc;
     const int my_groups = (int)blockIdx.x < ngroups ? (ngroups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     const int nloop = PASS == PASS_ITER ? (cnt > 1 ? cnt : 1) : 1;
     const double* __restrict__ fx = PASS == PASS_ITER ? V.yfix : V.ifix;
@@ -551,7 +554,7 @@ oci_red_woodbury_tma_kernel(DevView V, int ybase, int slot, int prev_slot, doubl
     // offsets inside a stage: the neighbour row of cell slot cs is row cs (left, mu > 0) or cs + 2 (right, mu < 0) of the y box
     const int o_ink = (cs + (half ? 0 : 2)) * K2 + qk, o_ine = (cs + (half ? 0 : 2)) * K2 + qe;
     const int o_fxk = y_dbl + cs * K2 + qk, o_fxe = y_dbl + cs * K2 + qe;
-    const int o_pf = y_dbl + fx_dbl + cs * 4 + psl, o_po = o_pf + 4 * cpb;
+    const int o_pf = y_dbl + fx_dbl + cs * 4 + psl, o_po = o_pf + 4 * gc;
     const int o_out = cs * K2;                                             // + j0 * K2 + qk / qe
     WbOps<PASS> O;
     double mrow[4] = {0.0, 0.0, 0.0, 0.0};
@@ -572,8 +575,8 @@ oci_red_woodbury_tma_kernel(DevView V, int ybase, int slot, int prev_slot, doubl
             for (int i = 0; i < my_groups; ++i) {
                 const int u = it0 + i, st = u % WT_STAGES;
                 if (u >= WT_STAGES) mbar_wait(&empty[st], ((u / WT_STAGES) - 1) & 1);
-                const int j0 = ((int)blockIdx.x + i * (int)gridDim.x) * cpb;
-                const int rows = J - j0 < cpb ? J - j0 : cpb;
+                const int j0 = ((int)blockIdx.x + i * (int)gridDim.x) * gc;
+                const int rows = J - j0 < gc ? J - j0 : gc;
                 double* sg = ring + (size_t)st * stage_dbl;
                 const uint32_t yb = (uint32_t)(rows + 2) * K2 * 8, fb = (uint32_t)rows * K2 * 8, pb = (uint32_t)rows * 32;
                 mbar_expect_tx(&full[st], yb + fb + (PASS == PASS_ITER ? 2 * pb : 0));
@@ -581,7 +584,7 @@ oci_red_woodbury_tma_kernel(DevView V, int ybase, int slot, int prev_slot, doubl
                 tma_load_1d(sg + y_dbl, fx + (int64_t)j0 * K2, fb, &full[st]);
                 if (PASS == PASS_ITER) {
                     tma_load_1d(sg + y_dbl + fx_dbl, V.phifix + (int64_t)j0 * 4, pb, &full[st]);
-                    tma_load_1d(sg + y_dbl + fx_dbl + 4 * cpb, V.phi + (int64_t)j0 * 4, pb, &full[st]);
+                    tma_load_1d(sg + y_dbl + fx_dbl + 4 * gc, V.phi + (int64_t)j0 * 4, pb, &full[st]);
                 }
             }
         }
@@ -589,44 +592,57 @@ oci_red_woodbury_tma_kernel(DevView V, int ybase, int slot, int prev_slot, doubl
         double dmax = 0.0, rmax = 0.0;
         for (int i = 0; i < my_groups; ++i) {
             const int u = it0 + i, st = u % WT_STAGES;
-            const int j0 = ((int)blockIdx.x + i * (int)gridDim.x) * cpb;
-            const bool valid = j0 + cs < J;
+            const int j0 = ((int)blockIdx.x + i * (int)gridDim.x) * gc;
             const double* sg = ring + (size_t)st * stage_dbl;
             mbar_wait(&full[st], (u / WT_STAGES) & 1);
-            double a = sg[o_ink], b = sg[o_ine];
-            const double c = sg[o_fxk], d = sg[o_fxe];
-            double pf = 0.0, po = 0.0;
-            if (phi_lane) { pf = sg[o_pf]; po = sg[o_po]; }
+            // this thread's WT_U cells of the group: cell slots cs, cs + cpb, ...
+            double a[WT_U], b[WT_U], c[WT_U], d[WT_U], pf[WT_U], po[WT_U];
+#pragma unroll
+            for (int w = 0; w < WT_U; ++w) {
+                a[w] = sg[o_ink + w * cpb * K2];
+                b[w] = sg[o_ine + w * cpb * K2];
+                c[w] = sg[o_fxk + w * cpb * K2];
+                d[w] = sg[o_fxe + w * cpb * K2];
+                pf[w] = po[w] = 0.0;
+                if (phi_lane) { pf[w] = sg[o_pf + w * cpb * 4]; po[w] = sg[o_po + w * cpb * 4]; }
+            }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[st]);                        // the stage is free again: everything is in registers
-            if (!valid) a = b = 0.0;                                       // rows past the last cell were not loaded
-            double p[4];
+            double p[WT_U][4];
 #pragma unroll
-            for (int r = 0; r < 4; ++r) p[r] = fma(O.pe[r], b, O.pk[r] * a);
-            cell_sum<W, true>(p, N, cs, red + (flip ? 4 * (WT_CONS / 32) : 0));
-            flip ^= 1;
-            if (!valid) continue;
-            const int j = j0 + cs;
-            if (phi_lane) {
-                // a6: phi^(l+1) = phifix + M s and the two max-norms of the stopping rule
-                const double nw = pf + fma(mrow[3], p[3], fma(mrow[2], p[2], fma(mrow[1], p[1], mrow[0] * p[0])));
-                V.phi[j * 4 + psl] = nw;
-                dmax = nanmax(dmax, fabs(nw - po));
-                rmax = nanmax(rmax, fabs(nw));
+            for (int w = 0; w < WT_U; ++w) {
+                if (j0 + cs + w * cpb >= J) a[w] = b[w] = 0.0;             // rows past the last cell were not loaded
+#pragma unroll
+                for (int r = 0; r < 4; ++r) p[w][r] = fma(O.pe[r], b[w], O.pk[r] * a[w]);
             }
-            const double tk = fma(O.g[1], b, O.g[0] * a), te = fma(O.g[3], b, O.g[2] * a);
-            const double vk = c + fma(O.dk[3], p[3], fma(O.dk[2], p[2], fma(O.dk[1], p[1], fma(O.dk[0], p[0], tk))));
-            const double ve = d + fma(O.de[3], p[3], fma(O.de[2], p[2], fma(O.de[1], p[1], fma(O.de[0], p[0], te))));
-            double* __restrict__ out = Yd + (j0 * K2 + o_out);
-            out[qk] = vk;
-            out[qe] = ve;
-            if (ghost_l && j == 0) {
-                Yd[mqk - K2] = vk;
-                Yd[mqe - K2] = ve;
-            }
-            if (ghost_r && j == J - 1) {
-                Yd[(int64_t)J * K2 + mqk] = vk;
-                Yd[(int64_t)J * K2 + mqe] = ve;
+#pragma unroll
+            for (int w = 0; w < WT_U; ++w) cell_sum<W, true>(p[w], N, cs, red + ((flip ^ w) & 1 ? 4 * (WT_CONS / 32) : 0));
+            if (WT_U & 1) flip ^= 1;
+#pragma unroll
+            for (int w = 0; w < WT_U; ++w) {
+                const int j = j0 + cs + w * cpb;
+                if (j >= J) continue;
+                if (phi_lane) {
+                    // a6: phi^(l+1) = phifix + M s and the two max-norms of the stopping rule
+                    const double nw = pf[w] + fma(mrow[3], p[w][3], fma(mrow[2], p[w][2], fma(mrow[1], p[w][1], mrow[0] * p[w][0])));
+                    V.phi[j * 4 + psl] = nw;
+                    dmax = nanmax(dmax, fabs(nw - po[w]));
+                    rmax = nanmax(rmax, fabs(nw));
+                }
+                const double tk = fma(O.g[1], b[w], O.g[0] * a[w]), te = fma(O.g[3], b[w], O.g[2] * a[w]);
+                const double vk = c[w] + fma(O.dk[3], p[w][3], fma(O.dk[2], p[w][2], fma(O.dk[1], p[w][1], fma(O.dk[0], p[w][0], tk))));
+                const double ve = d[w] + fma(O.de[3], p[w][3], fma(O.de[2], p[w][2], fma(O.de[1], p[w][1], fma(O.de[0], p[w][0], te))));
+                double* __restrict__ out = Yd + ((j0 + w * cpb) * K2 + o_out);
+                out[qk] = vk;
+                out[qe] = ve;
+                if (ghost_l && j == 0) {
+                    Yd[mqk - K2] = vk;
+                    Yd[mqe - K2] = ve;
+                }
+                if (ghost_r && j == J - 1) {
+                    Yd[(int64_t)J * K2 + mqk] = vk;
+                    Yd[(int64_t)J * K2 + mqe] = ve;
+                }
             }
         }
         if (PASS == PASS_ITER) {
@@ -702,47 +718,52 @@ void launch_wb_w(const DevView& V, int ybase, int slot, int prev_slot, double to
 
 size_t wt_smem(const DevView& V, int pass)
 {
-    const int cpb = WT_CONS / V.N, K2 = 2 * V.N;
-    const size_t stage = ((size_t)(2 * cpb + 2) * K2 + (pass == PASS_ITER ? 8 * cpb : 0)) * 8;
+    const int gc = WT_U * (WT_CONS / V.N), K2 = 2 * V.N;
+    const size_t stage = ((size_t)(2 * gc + 2) * K2 + (pass == PASS_ITER ? 8 * gc : 0)) * 8;
     return WT_STAGES * stage + 2 * 4 * (WT_CONS / 32) * 8 + 2 * WT_STAGES * 8 + 128;
 }
 
-// the TMA-staged kernel: ITER / FINAL, one shared block, power-of-two N in [8, 32] (measured: 3 % faster ITER and 30 %
-// faster FINAL than the direct kernel at N = 32, slower at N = 128 where a group is only two cells), 32-bit element
-// offsets, and enough cell groups to give every SM a few (below that the problem is launch-latency bound)
-bool wt_serves(const DevView& V)
+// the TMA-staged kernel: ITER / FINAL, one shared block, power-of-two N in [8, 128], 32-bit element offsets, and enough
+// cell groups to give every SM a few (below that the problem is launch-latency bound).  Measured against the direct
+// kernel: N = 32 ITER 55 -> 47 us, FINAL 52 -> 37 us; N = 128 FINAL 31 -> 27 us but ITER 29.5 -> 35 us (a group is only
+// four cells and pays two CTA barriers), so ITER takes it for N <= 32 only.
+bool wt_serves(const DevView& V, int pass)
 {
     const int N = V.N;
-    return V.nblk == 1 && (N & (N - 1)) == 0 && N >= 8 && N <= 32 && (V.J + 2) * 2 * (int64_t)N < ((int64_t)1 << 31) &&
+    return V.nblk == 1 && (pass == PASS_FINAL || N <= 32) && (N & (N - 1)) == 0 && N >= 8 && N <= 128 && (V.J + 2) * 2 * (int64_t)N < ((int64_t)1 << 31) &&
            V.J * (int64_t)N >= (int64_t)V.sm_count * 4 * WT_CONS;
 }
 
-template <int PASS, int W>
+template <int PASS, int NT>
 void launch_wt_w(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
 {
     const size_t smem = wt_smem(V, PASS);
-    const int cpb = WT_CONS / V.N;
-    const int64_t groups = (V.J + cpb - 1) / cpb;
+    const int gc = WT_U * (WT_CONS / V.N);
+    const int64_t groups = (V.J + gc - 1) / gc;
     int per_sm = 1;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, oci_red_woodbury_tma_kernel<PASS, W>, WT_CONS + 32, smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, oci_red_woodbury_tma_kernel<PASS, NT>, WT_CONS + 32, smem);
     if (per_sm < 1) per_sm = 1;
     const int64_t cap = (int64_t)V.sm_count * per_sm;
     const unsigned grid = (unsigned)(groups < cap ? groups : cap);
     if (PASS == PASS_ITER && cnt > 1) {
         DevView Vv = V;
         void* args[] = {&Vv, &ybase, &slot, &prev_slot, &tol, &cnt, &force};
-        cudaLaunchCooperativeKernel((const void*)oci_red_woodbury_tma_kernel<PASS, W>, dim3(grid), dim3(WT_CONS + 32), args, smem, s);
+        cudaLaunchCooperativeKernel((const void*)oci_red_woodbury_tma_kernel<PASS, NT>, dim3(grid), dim3(WT_CONS + 32), args, smem, s);
         return;
     }
-    oci_red_woodbury_tma_kernel<PASS, W><<<grid, WT_CONS + 32, smem, s>>>(V, ybase, slot, prev_slot, tol, cnt, force);
+    oci_red_woodbury_tma_kernel<PASS, NT><<<grid, WT_CONS + 32, smem, s>>>(V, ybase, slot, prev_slot, tol, cnt, force);
 }
 
 template <int PASS>
 void launch_wt(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
 {
-    if (V.N == 8) launch_wt_w<PASS, 8>(V, ybase, slot, prev_slot, tol, cnt, force, s);
-    else if (V.N == 16) launch_wt_w<PASS, 16>(V, ybase, slot, prev_slot, tol, cnt, force, s);
-    else launch_wt_w<PASS, 32>(V, ybase, slot, prev_slot, tol, cnt, force, s);
+    switch (V.N) {
+    case 8: launch_wt_w<PASS, 8>(V, ybase, slot, prev_slot, tol, cnt, force, s); break;
+    case 16: launch_wt_w<PASS, 16>(V, ybase, slot, prev_slot, tol, cnt, force, s); break;
+    case 32: launch_wt_w<PASS, 32>(V, ybase, slot, prev_slot, tol, cnt, force, s); break;
+    case 64: launch_wt_w<PASS, 64>(V, ybase, slot, prev_slot, tol, cnt, force, s); break;
+    default: launch_wt_w<PASS, 128>(V, ybase, slot, prev_slot, tol, cnt, force, s); break;
+    }
 }
 
 // CTAs of 256 threads (one or more whole cells each) unless a cell has more angles than that; the butterfly for
@@ -751,7 +772,7 @@ template <int PASS, bool SHARED>
 void launch_wb(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
 {
     const int N = V.N;
-    if (SHARED && PASS != PASS_FIX && wt_serves(V)) {
+    if (SHARED && PASS != PASS_FIX && wt_serves(V, PASS)) {
         launch_wt<PASS == PASS_FIX ? PASS_ITER : PASS>(V, ybase, slot, prev_slot, tol, cnt, force, s);
         return;
     }
@@ -774,17 +795,22 @@ void launch_wb_pass(const DevView& V, int pass, int ybase, int slot, int prev_sl
 }
 }  // namespace
 
-cudaError_t oci_red_woodbury_opt_in()
+namespace {
+template <int NT>
+cudaError_t wt_opt_in()
 {
     const auto at = cudaFuncAttributeMaxDynamicSharedMemorySize;
     const int bytes = 100 * 1024;
+    cudaError_t e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_ITER, NT>, at, bytes);
+    return e != cudaSuccess ? e : cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_FINAL, NT>, at, bytes);
+}
+}  // namespace
+
+cudaError_t oci_red_woodbury_opt_in()
+{
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_ITER, 8>, at, bytes)) != cudaSuccess ||
-        (e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_ITER, 16>, at, bytes)) != cudaSuccess ||
-        (e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_ITER, 32>, at, bytes)) != cudaSuccess ||
-        (e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_FINAL, 8>, at, bytes)) != cudaSuccess ||
-        (e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_FINAL, 16>, at, bytes)) != cudaSuccess ||
-        (e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_FINAL, 32>, at, bytes)) != cudaSuccess)
+    if ((e = wt_opt_in<8>()) != cudaSuccess || (e = wt_opt_in<16>()) != cudaSuccess || (e = wt_opt_in<32>()) != cudaSuccess ||
+        (e = wt_opt_in<64>()) != cudaSuccess || (e = wt_opt_in<128>()) != cudaSuccess)
         return e;
     return cudaSuccess;
 }
