@@ -196,13 +196,13 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
             const double* __restrict__ xr = src + (c + 1) * P;            // q < N: the right neighbour's outgoing flux
             const double* __restrict__ xl = src + (c - 1) * P;            // q >= N: the left neighbour's
             const double* __restrict__ op = opr + r0;
-#pragma unroll 8
+#pragma unroll 4
             for (int k = 0; k < N; ++k) {
                 const double x = xr[k];
                 const double4 w = *reinterpret_cast<const double4*>(op + k * MR);
                 a0 = fma(w.x, x, a0); a1 = fma(w.y, x, a1); a2 = fma(w.z, x, a2); a3 = fma(w.w, x, a3);
             }
-#pragma unroll 8
+#pragma unroll 4
             for (int k = N; k < K2; ++k) {
                 const double x = xl[k];
                 const double4 w = *reinterpret_cast<const double4*>(op + k * MR);
@@ -261,13 +261,13 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
             const double* __restrict__ xr = src + (c + 1) * P;
             const double* __restrict__ xl = src + (c - 1) * P;
             const double* __restrict__ op = opf + r0;
-#pragma unroll 8
+#pragma unroll 4
             for (int k = 0; k < N; ++k) {
                 const double x = xr[k];
                 const double4 w = *reinterpret_cast<const double4*>(op + k * K2);
                 a0 = fma(w.x, x, a0); a1 = fma(w.y, x, a1); a2 = fma(w.z, x, a2); a3 = fma(w.w, x, a3);
             }
-#pragma unroll 8
+#pragma unroll 4
             for (int k = N; k < K2; ++k) {
                 const double x = xl[k];
                 const double4 w = *reinterpret_cast<const double4*>(op + k * K2);
@@ -336,9 +336,12 @@ int launch_red_small(const DevView& V, int C, int ybase, double tol, int cnt, in
     const int Jc = (int)((V.J + C - 1) / C);
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)C);
-    // thread items of one iteration in the busiest CTA: a tiny problem gets a small CTA (cheaper barriers)
+    // thread items of one iteration in the busiest CTA: as many threads as there are items (a warp at least, 1024 at
+    // most), since for a tiny problem every barrier and every serial reduction over the warps is pure latency
     const int64_t items = (int64_t)Jc * ((2 * V.N + 4) / SM_R);
-    cfg.blockDim = dim3(items > 512 ? SM_MAX_THREADS : 256);
+    int threads = (int)((items + 31) / 32) * 32;
+    threads = threads < 32 ? 32 : threads > SM_MAX_THREADS ? SM_MAX_THREADS : threads;
+    cfg.blockDim = dim3((unsigned)threads);
     cfg.dynamicSmemBytes = (size_t)small_layout(V.N, Jc).total * 8;
     cfg.stream = s;
     cudaLaunchAttribute at[1];

@@ -19,6 +19,8 @@
 // Thread = (cell, angle); the 4-vector s is summed over the angles of a cell by warp shuffles (N a power of two)
 // and, across the warps of a cell or for other N, through shared memory in a fixed order (deterministic).
 // HBM-bound: per cell and iteration 6N doubles of state (+ 16N + 17 of operator when every cell has its own block).
+#include <cuda.h>
+
 #include "device_utils.cuh"
 
 namespace oci {
@@ -476,21 +478,30 @@ oci_red_woodbury_kernel(DevView V, int ybase, int slot, int prev_slot, double to
   }
 }
 
-// ---- ITER / FINAL with a shared block and a power-of-two N in [8, 256]: the same arithmetic, the rows STAGED BY TMA.
-// The direct kernel above keeps one item per thread in flight (16 warps per SM): latency-bound at 53-57 % of the HBM
-// bandwidth.  Here a producer warp streams, for every group of 256 / N cells, the rows the group reads - y rows
-// j0-1 .. j0+cpb of the source iterate (one contiguous piece, ghost rows included), the cpb rows of the additive operand,
-// and for ITER the phifix / old phi rows - with 1-D bulk copies (cp.async.bulk, completion on an mbarrier) into a
-// ring of WT_STAGES stages; the 256 consumer threads read their six values from shared memory, release the stage at once
-// (one arrival per warp) and compute out of registers, so the ring runs several groups ahead of the arithmetic whatever
-// the occupancy, and the address arithmetic of an item shrinks to the two stores.
-constexpr int WT_STAGES = 4;
+// ---- ITER / FINAL with a shared block and N in {16, 32, 64, 128}: the rows STAGED BY TMA, the sum over the angles ON
+// THE TENSOR PIPE.  The direct kernel above keeps one item per thread in flight and pays a 48-instruction shuffle
+// butterfly per cell for s = sum_m w_m t_m: latency- and issue-bound at 53-57 % of the HBM bandwidth.  But
+//     s[cell] = P inc[cell],   P = [w |mu| A_m^{-1}[:, I]]  (4 x 2N)
+// is a contraction of the gathered rows with a tiny operator - the scalar-flux block of the dense kernels with A^{-1}
+// in place of B^{-1} - so it runs as DMMA.8x8x4 straight from the staged rows:
+//   * a producer warp streams, per group of gc = 1024 / N cells, the two half rows every cell gathers (two tensor-map
+//     boxes of gc rows x (N + 4) columns: columns [0, N) of rows j0+1 .. j0+gc and columns [N, 2N) of rows j0-1 ..
+//     j0+gc-2; the 4 extra columns give the bank-conflict-free pitch, as in oci_reduced_resident.cu), the gc rows of the
+//     additive operand and, for ITER, the phifix / old-phi rows (1-D bulk copies) into a 2-stage ring (two CTAs per SM);
+//   * phase A: warp w takes k-steps [w KS/8, (w+1) KS/8) of the KS = N/2 k-steps for all gc/8 blocks of 8 cells
+//     (A fragments from the boxes, its slice of P as B fragments in registers) and leaves partial sums in shared memory;
+//     256 threads add the eight partials of (cell, slot) in warp order: s, deterministic;
+//   * phase B: thread = (cell, angle), four cells per thread: Psi_m = t_m + D_m s from registers and shared memory.
+// About 45 instructions per (cell, 32 angles) instead of 175.
+constexpr int WT_STAGES = 2;                       // two CTAs per SM: four stages in flight per SM
 constexpr int WT_CONS = 256;                       // consumer threads; + one producer warp
-constexpr int WT_U = 2;                            // cells per thread and group: two independent butterflies in flight
+constexpr int WT_WARPS = WT_CONS / 32;
 
+// (two CTAs of nine warps per SM put five warps on one SM partition: 16 K registers / 5 warps = 96 per thread)
 template <int PASS, int NT>
-__global__ void __maxnreg__(112)
-oci_red_woodbury_tma_kernel(DevView V, int ybase, int slot, int prev_slot, double tol, int cnt, int force)
+__global__ void __launch_bounds__(WT_CONS + 32, 2)
+oci_red_woodbury_tma_kernel(DevView V, const __grid_constant__ CUtensorMap map_y0, const __grid_constant__ CUtensorMap map_y1, int ybase,
+                            int slot, int prev_slot, double tol, int cnt, int force)
 {
     extern __shared__ __align__(128) unsigned char wt_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -517,19 +528,24 @@ oci_red_woodbury_tma_kernel(DevView V, int ybase, int slot, int prev_slot, doubl
         ysrc = (ybase + L - 1) & 1;
     }
     constexpr int N = NT, K2 = 2 * N, N2 = N >> 1;                         // N is a template parameter: every offset is an immediate
-    constexpr int W = N < 32 ? N : 32;                                     // width of the butterfly inside a warp
     const int J = (int)V.J;                                                // the launcher guarantees 32-bit element offsets
-    constexpr int cpb = WT_CONS / N;                                       // cells per pass of the 256 threads
-    constexpr int gc = WT_U * cpb;                                         // cells per group (stage): WT_U per thread
-    // stage: [gc+2][K2] y rows | [gc][K2] additive rows | [gc][4] phifix | [gc][4] old phi
-    constexpr int y_dbl = (gc + 2) * K2, fx_dbl = gc * K2;
-    constexpr int stage_dbl = y_dbl + fx_dbl + (PASS == PASS_ITER ? 8 * gc : 0);
+    constexpr int gc = 1024 / N;                                           // cells per group (stage)
+    constexpr int U = 4;                                                   // cells per thread and group: gc N / 256
+    constexpr int LDH = N + 4;                                             // pitch of a half-row box: 4 (mod 16) doubles
+    constexpr int KS = K2 / 4, KSW = KS / WT_WARPS;                        // k-steps of P inc, per warp
+    constexpr int NB = gc / 8;                                             // blocks of 8 cells
+    static_assert(KSW >= 1 && NB >= 1 && gc * N == U * WT_CONS, "shape");
+    // stage: lo box [gc][LDH] | hi box [gc][LDH] | additive rows [gc][K2] | phifix [gc][4] | old phi [gc][4]
+    constexpr int box_dbl = gc * LDH, fx_dbl = gc * K2;
+    constexpr int stage_dbl = 2 * box_dbl + fx_dbl + (PASS == PASS_ITER ? 8 * gc : 0);
+    static_assert((box_dbl * 8) % 128 == 0 && (stage_dbl * 8) % 128 == 0, "TMA destinations stay 128-byte aligned");
     double* ring = reinterpret_cast<double*>(wt_raw);
-    double* red = ring + (size_t)WT_STAGES * stage_dbl;                    // cell_sum's double buffer
-    uint64_t* full = reinterpret_cast<uint64_t*>(red + 2 * 4 * (WT_CONS / 32));
+    double* part = ring + (size_t)WT_STAGES * stage_dbl;                   // [8 warps][gc][4] partial sums of phase A
+    double* s_sm = part + WT_WARPS * gc * 4;                               // [gc][4]
+    uint64_t* full = reinterpret_cast<uint64_t*>(s_sm + gc * 4);
     uint64_t* empty = full + WT_STAGES;
     if (threadIdx.x == 0) {
-        for (int st = 0; st < WT_STAGES; ++st) { mbar_init(&full[st], 1); mbar_init(&empty[st], WT_CONS / 32); }
+        for (int st = 0; st < WT_STAGES; ++st) { mbar_init(&full[st], 1); mbar_init(&empty[st], WT_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -541,8 +557,10 @@ oci_red_woodbury_tma_kernel(DevView V, int ybase, int slot, int prev_slot, doubl
     int it0 = 0;                                                           // groups this CTA has streamed in earlier iterations
 
     // consumer-side constants
-    const bool consumer = warp < WT_CONS / 32;
-    const int cs = consumer ? threadIdx.x / N : 0, m = consumer ? threadIdx.x - cs * N : 0;
+    const bool consumer = warp < WT_WARPS;
+    const int tid = consumer ? threadIdx.x : 0;
+    const int m = tid % N, c0 = tid / N;                                   // angle; first cell slot (then c0 + 256/N, ...)
+    constexpr int cstep = WT_CONS / N;
     const int half = m >= N2, mm = m - half * N2;
     const int qk = pack_q(half, 0, mm, N), qe = pack_q(half, 1, mm, N);
     const double amu = fabs(V.mu[m]), wm = V.w[m];
@@ -551,23 +569,36 @@ oci_red_woodbury_tma_kernel(DevView V, int ybase, int slot, int prev_slot, doubl
     const int mqk = mirror_q(qk, N), mqe = mirror_q(qe, N);
     const bool phi_lane = PASS == PASS_ITER && m < 4;
     const int psl = m & 3;
-    // offsets inside a stage: the neighbour row of cell slot cs is row cs (left, mu > 0) or cs + 2 (right, mu < 0) of the y box
-    const int o_ink = (cs + (half ? 0 : 2)) * K2 + qk, o_ine = (cs + (half ? 0 : 2)) * K2 + qe;
-    const int o_fxk = y_dbl + cs * K2 + qk, o_fxe = y_dbl + cs * K2 + qe;
-    const int o_pf = y_dbl + fx_dbl + cs * 4 + psl, o_po = o_pf + 4 * gc;
-    const int o_out = cs * K2;                                             // + j0 * K2 + qk / qe
+    // phase B offsets inside a stage: mu < 0 (half 0) gathers from the lo box (the right neighbours' columns [0, N)),
+    // mu > 0 from the hi box (the left neighbours' columns [N, 2N))
+    const int o_a = (half ? box_dbl : 0) + c0 * LDH + (qk - half * N), o_b = (half ? box_dbl : 0) + c0 * LDH + (qe - half * N);
+    const int o_c = 2 * box_dbl + c0 * K2 + qk, o_d = 2 * box_dbl + c0 * K2 + qe;
+    const int o_pf = 2 * box_dbl + fx_dbl + c0 * 4 + psl, o_po = o_pf + 4 * gc;
     WbOps<PASS> O;
     double mrow[4] = {0.0, 0.0, 0.0, 0.0};
+    double bfr[KSW];                                                       // phase A: this warp's slice of P as DMMA B fragments
+    const int g4 = lane >> 2, t4 = lane & 3;
     if (consumer) {
         load_ops<PASS>(O, V.wba + m, V.wbd + m, N, half, amu, wm);
 #pragma unroll
         for (int cc = 0; cc < 4; ++cc) mrow[cc] = V.wbm[4 * psl + cc];
+        // B[k][n] = P[slot n][k], n = g4 < 4 (columns 4..7 of the n8 block are zero), k = 4 ks + t4 a packed entry q:
+        // P[slot][q] = w |mu| A_m^{-1}[slot][incident row of q]
+#pragma unroll
+        for (int i = 0; i < KSW; ++i) {
+            const int q = 4 * (warp * KSW + i) + t4;
+            int hq, hh, mq;
+            unpack_q(q, N, hq, hh, mq);
+            const int ma = hq * N2 + mq;                                   // angle of packed entry q
+            const int col = (hq ? 0 : 1) + 2 * hh;                         // its incident row: (m,1),(m,3) for mu < 0, (m,0),(m,2) for mu > 0
+            bfr[i] = g4 < 4 ? V.w[ma] * fabs(V.mu[ma]) * V.wba[(size_t)(4 * g4 + col) * N + ma] : 0.0;
+        }
     }
-    int flip = 0;
 
   for (int l = 0; l < nloop; ++l) {
-    const double* __restrict__ Ys = V.y[PASS == PASS_ITER ? (ybase + l) & 1 : ysrc];
-    double* __restrict__ Yd = PASS == PASS_ITER ? V.y[(ybase + l + 1) & 1] : V.z;
+    const int ys = PASS == PASS_ITER ? (ybase + l) & 1 : ysrc;
+    const CUtensorMap* my = ys ? &map_y1 : &map_y0;
+    double* __restrict__ Yd = PASS == PASS_ITER ? V.y[ys ^ 1] : V.z;
     if (!consumer) {
         // ---- producer: one elected lane streams this CTA's groups of this iteration
         if (lane == 0) {
@@ -578,13 +609,14 @@ oci_red_woodbury_tma_kernel(DevView V, int ybase, int slot, int prev_slot, doubl
                 const int j0 = ((int)blockIdx.x + i * (int)gridDim.x) * gc;
                 const int rows = J - j0 < gc ? J - j0 : gc;
                 double* sg = ring + (size_t)st * stage_dbl;
-                const uint32_t yb = (uint32_t)(rows + 2) * K2 * 8, fb = (uint32_t)rows * K2 * 8, pb = (uint32_t)rows * 32;
-                mbar_expect_tx(&full[st], yb + fb + (PASS == PASS_ITER ? 2 * pb : 0));
-                tma_load_1d(sg, Ys + ((int64_t)j0 - 1) * K2, yb, &full[st]);
-                tma_load_1d(sg + y_dbl, fx + (int64_t)j0 * K2, fb, &full[st]);
+                const uint32_t fb = (uint32_t)rows * K2 * 8, pb = (uint32_t)rows * 32;
+                mbar_expect_tx(&full[st], 2 * box_dbl * 8 + fb + (PASS == PASS_ITER ? 2 * pb : 0));
+                tma_load_2d(sg, my, 0, j0 + 2, &full[st]);                 // map row = cell + 1: the right neighbours j0+1 ..
+                tma_load_2d(sg + box_dbl, my, N, j0, &full[st]);           // the left neighbours j0-1 ..
+                tma_load_1d(sg + 2 * box_dbl, fx + (int64_t)j0 * K2, fb, &full[st]);
                 if (PASS == PASS_ITER) {
-                    tma_load_1d(sg + y_dbl + fx_dbl, V.phifix + (int64_t)j0 * 4, pb, &full[st]);
-                    tma_load_1d(sg + y_dbl + fx_dbl + 4 * gc, V.phi + (int64_t)j0 * 4, pb, &full[st]);
+                    tma_load_1d(sg + 2 * box_dbl + fx_dbl, V.phifix + (int64_t)j0 * 4, pb, &full[st]);
+                    tma_load_1d(sg + 2 * box_dbl + fx_dbl + 4 * gc, V.phi + (int64_t)j0 * 4, pb, &full[st]);
                 }
             }
         }
@@ -595,53 +627,78 @@ oci_red_woodbury_tma_kernel(DevView V, int ybase, int slot, int prev_slot, doubl
             const int j0 = ((int)blockIdx.x + i * (int)gridDim.x) * gc;
             const double* sg = ring + (size_t)st * stage_dbl;
             mbar_wait(&full[st], (u / WT_STAGES) & 1);
-            // this thread's WT_U cells of the group: cell slots cs, cs + cpb, ...
-            double a[WT_U], b[WT_U], c[WT_U], d[WT_U], pf[WT_U], po[WT_U];
+            // ---- phase A: partial s = P inc over this warp's k-steps, all blocks of 8 cells
+            {
+                double acc[NB][2];
 #pragma unroll
-            for (int w = 0; w < WT_U; ++w) {
-                a[w] = sg[o_ink + w * cpb * K2];
-                b[w] = sg[o_ine + w * cpb * K2];
-                c[w] = sg[o_fxk + w * cpb * K2];
-                d[w] = sg[o_fxe + w * cpb * K2];
-                pf[w] = po[w] = 0.0;
-                if (phi_lane) { pf[w] = sg[o_pf + w * cpb * 4]; po[w] = sg[o_po + w * cpb * 4]; }
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[st]);                        // the stage is free again: everything is in registers
-            double p[WT_U][4];
+                for (int bq = 0; bq < NB; ++bq) acc[bq][0] = acc[bq][1] = 0.0;
 #pragma unroll
-            for (int w = 0; w < WT_U; ++w) {
-                if (j0 + cs + w * cpb >= J) a[w] = b[w] = 0.0;             // rows past the last cell were not loaded
+                for (int ii = 0; ii < KSW; ++ii) {
+                    const int ks = warp * KSW + ii;                        // 4 ks < N: lo box, else hi box
+                    const double* ap = sg + (4 * ks < N ? 4 * ks : box_dbl + 4 * ks - N) + g4 * LDH + t4;
 #pragma unroll
-                for (int r = 0; r < 4; ++r) p[w][r] = fma(O.pe[r], b[w], O.pk[r] * a[w]);
-            }
-#pragma unroll
-            for (int w = 0; w < WT_U; ++w) cell_sum<W, true>(p[w], N, cs, red + ((flip ^ w) & 1 ? 4 * (WT_CONS / 32) : 0));
-            if (WT_U & 1) flip ^= 1;
-#pragma unroll
-            for (int w = 0; w < WT_U; ++w) {
-                const int j = j0 + cs + w * cpb;
-                if (j >= J) continue;
-                if (phi_lane) {
-                    // a6: phi^(l+1) = phifix + M s and the two max-norms of the stopping rule
-                    const double nw = pf[w] + fma(mrow[3], p[w][3], fma(mrow[2], p[w][2], fma(mrow[1], p[w][1], mrow[0] * p[w][0])));
-                    V.phi[j * 4 + psl] = nw;
-                    dmax = nanmax(dmax, fabs(nw - po[w]));
-                    rmax = nanmax(rmax, fabs(nw));
+                    for (int bq = 0; bq < NB; ++bq) dmma(acc[bq][0], acc[bq][1], ap[bq * 8 * LDH], bfr[ii]);
                 }
-                const double tk = fma(O.g[1], b[w], O.g[0] * a[w]), te = fma(O.g[3], b[w], O.g[2] * a[w]);
-                const double vk = c[w] + fma(O.dk[3], p[w][3], fma(O.dk[2], p[w][2], fma(O.dk[1], p[w][1], fma(O.dk[0], p[w][0], tk))));
-                const double ve = d[w] + fma(O.de[3], p[w][3], fma(O.de[2], p[w][2], fma(O.de[1], p[w][1], fma(O.de[0], p[w][0], te))));
-                double* __restrict__ out = Yd + ((j0 + w * cpb) * K2 + o_out);
-                out[qk] = vk;
-                out[qe] = ve;
-                if (ghost_l && j == 0) {
-                    Yd[mqk - K2] = vk;
-                    Yd[mqe - K2] = ve;
+                if (t4 < 2) {
+#pragma unroll
+                    for (int bq = 0; bq < NB; ++bq)
+                        *reinterpret_cast<double2*>(part + ((size_t)warp * gc + bq * 8 + g4) * 4 + 2 * t4) = make_double2(acc[bq][0], acc[bq][1]);
                 }
-                if (ghost_r && j == J - 1) {
-                    Yd[(int64_t)J * K2 + mqk] = vk;
-                    Yd[(int64_t)J * K2 + mqe] = ve;
+            }
+            named_bar_sync(1, WT_CONS);
+            if (tid < gc * 4) {
+                double sum = part[tid];
+#pragma unroll
+                for (int w = 1; w < WT_WARPS; ++w) sum += part[w * gc * 4 + tid];
+                s_sm[tid] = sum;
+            }
+            named_bar_sync(1, WT_CONS);
+            // ---- phase B: thread = (cell, angle), U cells per thread, two at a time
+#pragma unroll
+            for (int h2 = 0; h2 < U; h2 += 2) {
+                double a[2], b[2], c[2], d[2], pf[2], po[2];
+                double4 sv[2];
+#pragma unroll
+                for (int w = 0; w < 2; ++w) {
+                    const int cs = (h2 + w) * cstep;                       // + c0: this item's cell slot
+                    a[w] = sg[o_a + cs * LDH];
+                    b[w] = sg[o_b + cs * LDH];
+                    c[w] = sg[o_c + cs * K2];
+                    d[w] = sg[o_d + cs * K2];
+                    pf[w] = po[w] = 0.0;
+                    if (phi_lane) { pf[w] = sg[o_pf + cs * 4]; po[w] = sg[o_po + cs * 4]; }
+                    sv[w] = *reinterpret_cast<const double4*>(s_sm + (c0 + cs) * 4);
+                }
+                if (h2 + 2 == U) {
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&empty[st]);                // the stage is free again: everything is in registers
+                }
+#pragma unroll
+                for (int w = 0; w < 2; ++w) {
+                    const int j = j0 + c0 + (h2 + w) * cstep;
+                    if (j >= J) continue;
+                    const double p0 = sv[w].x, p1 = sv[w].y, p2 = sv[w].z, p3 = sv[w].w;
+                    if (phi_lane) {
+                        // a6: phi^(l+1) = phifix + M s and the two max-norms of the stopping rule
+                        const double nw = pf[w] + fma(mrow[3], p3, fma(mrow[2], p2, fma(mrow[1], p1, mrow[0] * p0)));
+                        V.phi[j * 4 + psl] = nw;
+                        dmax = nanmax(dmax, fabs(nw - po[w]));
+                        rmax = nanmax(rmax, fabs(nw));
+                    }
+                    const double tk = fma(O.g[1], b[w], O.g[0] * a[w]), te = fma(O.g[3], b[w], O.g[2] * a[w]);
+                    const double vk = c[w] + fma(O.dk[3], p3, fma(O.dk[2], p2, fma(O.dk[1], p1, fma(O.dk[0], p0, tk))));
+                    const double ve = d[w] + fma(O.de[3], p3, fma(O.de[2], p2, fma(O.de[1], p1, fma(O.de[0], p0, te))));
+                    double* __restrict__ out = Yd + j * K2;
+                    out[qk] = vk;
+                    out[qe] = ve;
+                    if (ghost_l && j == 0) {
+                        Yd[mqk - K2] = vk;
+                        Yd[mqe - K2] = ve;
+                    }
+                    if (ghost_r && j == J - 1) {
+                        Yd[(int64_t)J * K2 + mqk] = vk;
+                        Yd[(int64_t)J * K2 + mqe] = ve;
+                    }
                 }
             }
         }
@@ -718,27 +775,34 @@ void launch_wb_w(const DevView& V, int ybase, int slot, int prev_slot, double to
 
 size_t wt_smem(const DevView& V, int pass)
 {
-    const int gc = WT_U * (WT_CONS / V.N), K2 = 2 * V.N;
-    const size_t stage = ((size_t)(2 * gc + 2) * K2 + (pass == PASS_ITER ? 8 * gc : 0)) * 8;
-    return WT_STAGES * stage + 2 * 4 * (WT_CONS / 32) * 8 + 2 * WT_STAGES * 8 + 128;
+    const int N = V.N, gc = 1024 / N;
+    const size_t stage = ((size_t)2 * gc * (N + 4) + (size_t)gc * 2 * N + (pass == PASS_ITER ? 8 * gc : 0)) * 8;
+    return WT_STAGES * stage + (size_t)(WT_WARPS + 1) * gc * 4 * 8 + 2 * WT_STAGES * 8 + 128;
 }
 
-// the TMA-staged kernel: ITER / FINAL, one shared block, power-of-two N in [8, 128], 32-bit element offsets, and enough
-// cell groups to give every SM a few (below that the problem is launch-latency bound).  Measured against the direct
-// kernel: N = 32 ITER 55 -> 47 us, FINAL 52 -> 37 us; N = 128 FINAL 31 -> 27 us but ITER 29.5 -> 35 us (a group is only
-// four cells and pays two CTA barriers), so ITER takes it for N <= 32 only.
+// the TMA / tensor-pipe kernel: ITER / FINAL, one shared block, N in {16, 32, 64, 128}, 32-bit element offsets, and enough
+// cell groups to give every SM a few (below that the problem is launch-latency bound and the direct kernel serves it)
 bool wt_serves(const DevView& V, int pass)
 {
     const int N = V.N;
-    return V.nblk == 1 && (pass == PASS_FINAL || N <= 32) && (N & (N - 1)) == 0 && N >= 8 && N <= 128 && (V.J + 2) * 2 * (int64_t)N < ((int64_t)1 << 31) &&
+    (void)pass;
+    return V.nblk == 1 && (N == 16 || N == 32 || N == 64 || N == 128) && (V.J + 2) * 2 * (int64_t)N < ((int64_t)1 << 31) &&
            V.J * (int64_t)N >= (int64_t)V.sm_count * 4 * WT_CONS;
 }
 
+// tensor maps of the two y buffers (rows -1 .. J, boxes of 1024/N rows x N+4 columns), encoded per launch: a handful
+// of host instructions, and no state to keep in the context
 template <int PASS, int NT>
 void launch_wt_w(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
 {
     const size_t smem = wt_smem(V, PASS);
-    const int gc = WT_U * (WT_CONS / V.N);
+    const int gc = 1024 / NT, K2 = 2 * NT;
+    CUtensorMap m0, m1;
+    if (!oci_encode_2d(&m0, V.y[0] - K2, (uint64_t)V.J + 2, K2, gc, NT + 4, false) ||
+        !oci_encode_2d(&m1, V.y[1] - K2, (uint64_t)V.J + 2, K2, gc, NT + 4, false)) {
+        cudaMemsetAsync(nullptr, 0, 1, s);                                  // leaves an error for launched() to pick up
+        return;
+    }
     const int64_t groups = (V.J + gc - 1) / gc;
     int per_sm = 1;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, oci_red_woodbury_tma_kernel<PASS, NT>, WT_CONS + 32, smem);
@@ -747,18 +811,17 @@ void launch_wt_w(const DevView& V, int ybase, int slot, int prev_slot, double to
     const unsigned grid = (unsigned)(groups < cap ? groups : cap);
     if (PASS == PASS_ITER && cnt > 1) {
         DevView Vv = V;
-        void* args[] = {&Vv, &ybase, &slot, &prev_slot, &tol, &cnt, &force};
+        void* args[] = {&Vv, &m0, &m1, &ybase, &slot, &prev_slot, &tol, &cnt, &force};
         cudaLaunchCooperativeKernel((const void*)oci_red_woodbury_tma_kernel<PASS, NT>, dim3(grid), dim3(WT_CONS + 32), args, smem, s);
         return;
     }
-    oci_red_woodbury_tma_kernel<PASS, NT><<<grid, WT_CONS + 32, smem, s>>>(V, ybase, slot, prev_slot, tol, cnt, force);
+    oci_red_woodbury_tma_kernel<PASS, NT><<<grid, WT_CONS + 32, smem, s>>>(V, m0, m1, ybase, slot, prev_slot, tol, cnt, force);
 }
 
 template <int PASS>
 void launch_wt(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
 {
     switch (V.N) {
-    case 8: launch_wt_w<PASS, 8>(V, ybase, slot, prev_slot, tol, cnt, force, s); break;
     case 16: launch_wt_w<PASS, 16>(V, ybase, slot, prev_slot, tol, cnt, force, s); break;
     case 32: launch_wt_w<PASS, 32>(V, ybase, slot, prev_slot, tol, cnt, force, s); break;
     case 64: launch_wt_w<PASS, 64>(V, ybase, slot, prev_slot, tol, cnt, force, s); break;
@@ -800,7 +863,7 @@ template <int NT>
 cudaError_t wt_opt_in()
 {
     const auto at = cudaFuncAttributeMaxDynamicSharedMemorySize;
-    const int bytes = 100 * 1024;
+    const int bytes = 160 * 1024;
     cudaError_t e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_ITER, NT>, at, bytes);
     return e != cudaSuccess ? e : cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_FINAL, NT>, at, bytes);
 }
@@ -809,8 +872,8 @@ cudaError_t wt_opt_in()
 cudaError_t oci_red_woodbury_opt_in()
 {
     cudaError_t e;
-    if ((e = wt_opt_in<8>()) != cudaSuccess || (e = wt_opt_in<16>()) != cudaSuccess || (e = wt_opt_in<32>()) != cudaSuccess ||
-        (e = wt_opt_in<64>()) != cudaSuccess || (e = wt_opt_in<128>()) != cudaSuccess)
+    if ((e = wt_opt_in<16>()) != cudaSuccess || (e = wt_opt_in<32>()) != cudaSuccess || (e = wt_opt_in<64>()) != cudaSuccess ||
+        (e = wt_opt_in<128>()) != cudaSuccess)
         return e;
     return cudaSuccess;
 }
