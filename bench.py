@@ -34,7 +34,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from workloads import make_problem  # noqa: E402
+from workloads import make_problem, make_multi_region  # noqa: E402
 
 METRIC = "oci_unknown_updates_per_s"
 UNIT = "unknown-updates/s"
@@ -494,7 +494,32 @@ def per_config_table(torch, P, peaks=None, peak_src=None, peak_live=None):
         g.close()
         del g
         torch.cuda.empty_cache()
+    out["multi_region"] = multi_region_row(torch, P)
     return out
+
+
+def multi_region_row(torch, P):
+    """Context beside the five configs: a multi-region slab of the kind the paper times (Reed-type, S64, v = 4,
+    dt = 1, 5 steps; synthetic layout, workloads.make_multi_region): a handful of materials on the K-tiled tensor-core
+    kernels (row f2), the same through the Woodbury family, and the GPU SI scan.  Time per step and iterations only.
+    Thin cells and a void are the one-cell inversion's worst case (rho_OCI -> 1 as Sigma dx -> 0; information
+    crosses the void one cell per iteration), so OCI needs hundreds to thousands of iterations here where SI needs tens:
+    the paper's own Table 1 has OCI losing on this kind of problem on the CPU."""
+    p = make_multi_region(cells=1024)
+    row = {"workload": p.name, "S_N": p.n_angles, "cells": p.cells}
+    for name, kw, scheme in (("oci", {}, "oci"), ("oci_woodbury", {"reduced_kernel": P.RKERNEL_WOODBURY}, "oci"), ("si", {}, "si")):
+        g = P.OCI.from_problem(p, **kw)
+        if name == "oci":
+            row["n_blocks"] = g.get_info()["n_blocks"]
+            row["reduced_kernel"] = g.get_info()["reduced_kernel"]
+        for k in range(2):
+            g.set_source(p.source(k))
+            (g.oci_step if scheme == "oci" else g.si_step)(p.tol, p.max_iters)
+        ms, iters, each = time_gpu_steps(torch, g, p, p.n_steps, scheme)
+        row[f"{name}_ms_per_step"] = ms / p.n_steps
+        row[f"{name}_iters"] = iters
+        g.close()
+    return row
 
 
 def woodbury_row(torch, P, p, peaks):

@@ -6,4 +6,4 @@ numbers, lays out the arrays and names the boundary conditions.  It holds none
 of the method's arithmetic (no quadrature, no matrices, no iteration) and
 imports neither side.
 """
-from .configs import Problem, make_problem, CONFIG_NAMES, BC_VACUUM, BC_INCIDENT_ISOTROPIC, BC_REFLECTING  # noqa: F401
+from .configs import Problem, make_problem, make_multi_region, CONFIG_NAMES, BC_VACUUM, BC_INCIDENT_ISOTROPIC, BC_REFLECTING  # noqa: F401

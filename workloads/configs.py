@@ -119,3 +119,23 @@ def make_problem(cfg: int, cells: Optional[int] = None, n_steps: Optional[int] =
                        1.0, 0.05, n_steps or steps, (BC_VACUUM, 0.0), (BC_VACUUM, 0.0),
                        np.zeros((J, N, 2)), _source=lambda step: q)
     raise ValueError(f"unknown config {cfg}")
+
+
+def make_multi_region(cells: int = 4096, n_angles: int = 64, n_steps: int = 5) -> Problem:
+    """A multi-region slab of the kind the paper times (a Reed-type problem, S64, v = 4, dt = 1, 5 steps; its
+    region layout is in a figure that is not available, so the layout here is synthetic): five regions, four
+    materials - a strong absorber with a strong source, a weaker absorber, a void, and two scattering regions (c = 0.9),
+    one of them with a source; reflecting left, vacuum right, zero initial flux.  Region widths in units of cells/64:
+    16, 8, 16, 8, 16.  A context sees 4 distinct (dx, Sigma, Sigma_s) blocks."""
+    J = int(cells)
+    u = J / 64.0
+    edges = [0, int(16 * u), int(24 * u), int(40 * u), int(48 * u), J]
+    mats = [(50.0, 0.0, 50.0), (5.0, 0.0, 0.0), (1e-12, 0.0, 0.0), (1.0, 0.9, 1.0), (1.0, 0.9, 0.0)]
+    dx = _const(J, 8.0 / J)
+    st, ss = np.zeros(J), np.zeros(J)
+    q = np.zeros((J, 4))
+    for (a, b), (sig, sigs, src) in zip(zip(edges[:-1], edges[1:]), mats):
+        st[a:b], ss[a:b], q[a:b] = sig, sigs, src
+    return Problem(0, f"multi_region_S{n_angles}_J{J}_reed_like", n_angles, J, dx, st, ss, 4.0, 1.0, n_steps,
+                   (2, 0.0), (0, 0.0), np.zeros((J, n_angles, 2)), _source=lambda step: q)
+
