@@ -39,7 +39,7 @@ from workloads import make_problem, make_multi_region  # noqa: E402
 METRIC = "oci_unknown_updates_per_s"
 UNIT = "unknown-updates/s"
 
-def load_traffic(cfg, reduced):
+def load_traffic(cfg, reduced, suffix=""):
     """DRAM bytes per iteration of the dominant kernel from the committed `ncu --set full` capture: profiles/traffic.json,
     written by `python -m paper_2305_13555_b200.ncu_traffic` from the .ncu-rep together with the commit the capture was
     taken at, so that a stale capture is visible next to the number."""
@@ -48,7 +48,7 @@ def load_traffic(cfg, reduced):
         return None, None
     with open(path) as f:
         t = json.load(f)
-    e = t.get("entries", {}).get(f"cfg{cfg}_{'reduced' if reduced else 'full'}")
+    e = t.get("entries", {}).get(f"cfg{cfg}_{'reduced' if reduced else 'full'}{suffix}")
     if not e:
         return None, None
     return e["dram_bytes_per_iteration"], {"file": "profiles/traffic.json", "capture": e.get("capture"), "kernel": e.get("kernel"),
@@ -436,7 +436,20 @@ def iteration_roofline(P, p, info, cfg, kms, klaunch, aux, steps, peaks, peak_sr
                  "fix_pass_ms_per_step": fix_ms / max(fix_n, 1) if reduced else None,
                  "final_pass_ms_per_step": fin_ms / max(fin_n, 1) if reduced else None,
                  "operator_rows_x_cols": [M_op, K_op], "form": "reduced" if reduced else "full"}
-    if shared:
+    if info["reduced_kernel"] == P.RKERNEL_WOODBURY and reduced:
+        # O(N) apply: HBM-bound; algorithmic bytes = the state only, J (6N doubles of y in / yfix in /
+        # y out + 96 B of scalar flux), plus 16N doubles of 4x4 pieces, a row of M and the block index with per-cell blocks
+        N = n // 4
+        bytes_ = p.cells * (48.0 * N + 96.0 + (0.0 if shared else 128.0 * N + 132.0))
+        achieved = bytes_ / (k_avg_ms * 1e-3) * 1e-9
+        traffic, traffic_src = load_traffic(cfg, reduced, "_woodbury")
+        breakdown["operator_rows_x_cols"] = None
+        breakdown["form"] = "reduced, rank-4 (Woodbury) apply"
+        roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "traffic_source": traffic_src,
+                    "kernel": "oci iteration through the rank-4 scattering matrix (eq. 22)", "algorithmic_bytes_per_launch": bytes_,
+                    "avg_launch_ms": k_avg_ms, "launches_timed": klaunch, "peak_source": f"MEASURED_PEAKS hbm_gbs ({peak_src})"}
+    elif shared:
         flops = 2.0 * M_op * K_op * p.cells
         nominal_ratio = 45.0 / 2250.0        # guide: B200 fp64 tensor 45 TF vs bf16 2250 TF nominal
         peak_scaled = peaks["bf16_tflops"] * nominal_ratio
@@ -593,7 +606,7 @@ def run_ours(args):
             g.step(p.tol, p.max_iters)
     else:
         p = make_problem(args.config)
-        g = ctx = P.OCI.from_problem(p, device=f"cuda:{local}")
+        g = ctx = P.OCI.from_problem(p, device=f"cuda:{local}", reduced_kernel=P.RKERNEL_WOODBURY if args.family == "woodbury" else None)
 
         def warm_step(k):
             g.set_source(p.source(k))
@@ -624,7 +637,7 @@ def run_ours(args):
     kms, klaunch = ctx.get_kernel_time()
     aux = ctx.get_aux_kernel_time()
     ctx.enable_kernel_timing(False)
-    peak_live = P.probe_fp64_tensor_tflops(f"cuda:{local}") if shared else None
+    peak_live = P.probe_fp64_tensor_tflops(f"cuda:{local}") if shared and args.family != "woodbury" else None
     roofline = iteration_roofline(P, p_local, info, args.config, kms, klaunch, aux, args.steps, peaks, peak_src, peak_live)
     reduced = info["iteration"] == P.ITERATION_REDUCED
 
@@ -672,6 +685,7 @@ def run_ours(args):
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": p.name, "S_N": p.n_angles, "cells": p.cells, "unknowns": p.unknowns, "tol": p.tol,
                        "path": "shared" if shared else "per_cell",
+                       "kernel_family": "dense (the library default)" if args.family == "default" else "woodbury (rank-4 apply, on request)",
                        "parallelism": (f"one slab sharded over {world} GPUs by cell ranges ({p_local.cells} cells each), halo + norm exchange "
                                        "by peer-memory stores per iteration" if world > 1 else "1 gpu"),
                        "l2": l2_note},
@@ -697,6 +711,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-table", action="store_true", help="skip the per-config OCI/SI table")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--family", default="default", choices=["default", "woodbury"],
+                    help="kernel family of the timed arm: the library default (dense inverse, the headline) or the O(N) rank-4 apply")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
