@@ -7,15 +7,15 @@
 // Here a cluster of C <= 8 CTAs splits the cells into contiguous ranges; each CTA keeps, in its shared memory, the three
 // operators (X, [G; H], F, transposed), both buffers of its part of the iterate y with one ghost row on either side,
 // yfix, ifix, phifix and phi.  Per iteration:
-//   compute (thread = (cell, 4 operator rows), lanes = cells: the input row comes from shared memory conflict free
-//   (odd pitch), the operator as broadcast 32-byte loads) -> publish this CTA's two max-norms into every CTA's shared
-//   memory (DSMEM stores) -> ONE hardware cluster barrier -> ghost rows of the new iterate from the neighbour CTAs'
-//   edge rows (DSMEM loads) or the boundary condition, and the stopping decision from the C published pairs, taken
-//   identically by every thread of the cluster.
+//   compute (a warp takes tiles of 16 cells x up to 40 operator rows: DMMA.8x8x4 with both operands as fragments
+//   straight from shared memory, rows pitched 4 (mod 16) doubles) -> publish this CTA's two max-norms into every CTA's
+//   shared memory (DSMEM stores) -> ONE hardware cluster barrier -> ghost rows of the new iterate from the neighbour
+//   CTAs' edge rows (DSMEM loads) or the boundary condition, and the stopping decision from the C published pairs,
+//   taken identically by every thread of the cluster.
 // No global-memory traffic inside the loop except the (d, r) pair of every iteration for the host (row a7: it still
 // reads the norm slots once per step to learn the iteration count).  Sums run in a fixed order and the norms are exact
 // maxima, so a step is reproducible bit for bit.  The arithmetic is the dense method's: the same operators as the other
-// families of the reduced form, applied with DFMA (at these sizes a step is latency, not throughput).
+// families of the reduced form, on the same fp64 tensor pipe (at these sizes a step is latency, not throughput).
 //
 // Not served: per-cell blocks, OCI_BC_HALO faces (sharded slabs), problems whose state does not fit a cluster's shared
 // memory or that are large enough for the three-pass kernels to win; oci_step falls back to those by itself.  If a step
@@ -31,12 +31,16 @@ namespace oci {
 
 namespace {
 
-constexpr int SM_MAX_THREADS = 1024;                       // CTA size is chosen at launch: 256 (tiny problems) or 1024
-constexpr int SM_R = 4;                                    // operator rows per thread item
+constexpr int SM_MAX_THREADS = 256;                        // CTA size is chosen at launch: one warp per work item, 8 at most
+constexpr int SM_NBG = 5;                                  // n8 blocks of operator rows per work item (40 rows)
+
+// smallest pitch >= k that is 4 (mod 16) doubles: fragment loads of 8 rows x 4 columns hit 32 distinct banks
+__host__ __device__ inline int sm_pitch(int k) { return k + ((4 - k) % 16 + 16) % 16; }
 
 struct SmallLayout {                                       // offsets in doubles inside a CTA's dynamic shared memory
-    int Jc, P, K2;
-    int opx, opr, opf, y0, y1, yfix, ifix, zin, qin, phifix, phi, red, pub, total;
+    int Jc, P, K2, PX, PR;                                 // P: pitch of y / yfix / ifix rows; PX, PR: of the operator rows
+    int mx, mr, mf;                                        // operator rows, padded to whole n8 blocks
+    int opx, opr, opf, y0, y1, yfix, ifix, phifix, phi, red, pub, total;
 };
 
 __host__ __device__ inline SmallLayout small_layout(int N, int Jc)
@@ -45,24 +49,69 @@ __host__ __device__ inline SmallLayout small_layout(int N, int Jc)
     const int K2 = 2 * N;
     L.Jc = Jc;
     L.K2 = K2;
-    L.P = K2 + 1;                                          // odd pitch: lanes = cells read a column without bank conflicts
+    L.P = sm_pitch(K2 + 4);                                // a row of y, or the FIX input vector [K2 + 4] (which borrows buffer 1)
+    L.PX = sm_pitch(K2 + 4);
+    L.PR = sm_pitch(K2);
+    L.mx = (2 * K2 + 4 + 7) / 8 * 8;
+    L.mr = (K2 + 4 + 7) / 8 * 8;
+    L.mf = (K2 + 7) / 8 * 8;
     int o = 0;
     auto take = [&](int n) { const int at = o; o += (n + 3) & ~3; return at; };   // 32-byte aligned pieces
-    L.opx = take((K2 + 4) * (2 * K2 + 4));                 // X^T  [K2+4 inputs][2K2+4 rows]
-    L.opr = take(K2 * (K2 + 4));                           // [G; H]^T  [K2][K2+4]
-    L.opf = take(K2 * K2);                                 // F^T  [K2][K2]
+    L.opx = take(L.mx * L.PX);                             // X      [2K2+4 rows][K2+4]
+    L.opr = take(L.mr * L.PR);                             // [G; H] [K2+4 rows][K2]
+    L.opf = take(L.mf * L.PR);                             // F      [K2 rows][K2]
     L.y0 = take((Jc + 2) * L.P);                           // iterate, buffer 0, rows -1 .. Jc
-    L.y1 = take((Jc + 2) * L.P);
+    L.y1 = take((Jc + 2) * L.P);                           // buffer 1; during FIX: the input vectors [psi_{k-1/2}; Q]
     L.yfix = take(Jc * L.P);                               // also the staging area of z (FINAL)
     L.ifix = take(Jc * L.P);
-    L.zin = take(Jc * (N + 1));                            // the k+1/2 run of z (FIX input)
-    L.qin = take(Jc * 4);
     L.phifix = take(Jc * 4);
     L.phi = take(Jc * 4);
     L.red = take(2 * (SM_MAX_THREADS / 32));
     L.pub = take(2 * 8 * 2);                               // [parity][rank][d, r] published by every CTA of the cluster
     L.total = o;
     return L;
+}
+
+// One work item of a "gathered GEMM" pass: out[cell][row] = sum_k Op[row][k] in(cell, k) for the 16 cells c0 .. c0+15 and
+// the n8 blocks t0 .. t0+nb-1 of operator rows, as DMMA.8x8x4 (cells = the M dimension).  `in` returns the address of
+// element (cell, k) of the input; `out` receives (cell, row, v[row], v[row+1]) in accumulator layout.
+template <typename In, typename Out>
+__device__ __forceinline__ void small_item(const double* __restrict__ op, int opp, int K, int c0, int t0, int nb, In in, Out out)
+{
+    const int lane = threadIdx.x & 31, g4 = lane >> 2, t4 = lane & 3;
+    double acc[2][SM_NBG][2];
+#pragma unroll
+    for (int g = 0; g < 2; ++g)
+#pragma unroll
+        for (int t = 0; t < SM_NBG; ++t) acc[g][t][0] = acc[g][t][1] = 0.0;
+    const double* __restrict__ bp = op + (size_t)(8 * t0 + g4) * opp + t4;
+    // the fragments of k-step k + 4 are requested before the DMMAs of k-step k are issued
+    double a0 = *in(c0 + g4, t4), a1 = *in(c0 + 8 + g4, t4), b[SM_NBG];
+#pragma unroll
+    for (int t = 0; t < SM_NBG; ++t) b[t] = t < nb ? bp[(size_t)(8 * t) * opp] : 0.0;
+    for (int k = 0; k < K; k += 4) {
+        const int kn = k + 4 < K ? k + 4 : k;
+        const double na0 = *in(c0 + g4, kn + t4), na1 = *in(c0 + 8 + g4, kn + t4);
+        double nb_[SM_NBG];
+#pragma unroll
+        for (int t = 0; t < SM_NBG; ++t) nb_[t] = t < nb ? bp[(size_t)(8 * t) * opp + kn] : 0.0;
+#pragma unroll
+        for (int t = 0; t < SM_NBG; ++t) {
+            if (t < nb) {
+                dmma(acc[0][t][0], acc[0][t][1], a0, b[t]);
+                dmma(acc[1][t][0], acc[1][t][1], a1, b[t]);
+            }
+        }
+        a0 = na0;
+        a1 = na1;
+#pragma unroll
+        for (int t = 0; t < SM_NBG; ++t) b[t] = nb_[t];
+    }
+#pragma unroll
+    for (int g = 0; g < 2; ++g)
+#pragma unroll
+        for (int t = 0; t < SM_NBG; ++t)
+            if (t < nb) out(c0 + 8 * g + g4, 8 * (t0 + t) + 2 * t4, acc[g][t][0], acc[g][t][1]);
 }
 
 }  // namespace
@@ -85,73 +134,69 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
     double* opr = ssm + L.opr;
     double* opf = ssm + L.opf;
     double* ybuf[2] = {ssm + L.y0 + P, ssm + L.y1 + P};                   // row 0 of either buffer (ghost rows at -1, nc)
+    double* xin = ybuf[1];                                                // FIX input vectors [psi_{k-1/2}; Q], pitch P
     double* yfix = ssm + L.yfix;
     double* ifix = ssm + L.ifix;
-    double* zin = ssm + L.zin;
-    double* qin = ssm + L.qin;
     double* phifix = ssm + L.phifix;
     double* phi = ssm + L.phi;
     double* red = ssm + L.red;
     double* pub = ssm + L.pub;
-    const int MX = 2 * K2 + 4, KX = K2 + 4, MR = K2 + 4;
+    const int PX = L.PX, PR = L.PR;
+    const int nwarps = SM_THREADS >> 5;
+    const int ntile = (nc + 15) / 16;                                     // tiles of 16 cells
 
-    // ---- load: operators (transposed), my cells of the committed state, Q, the old scalar flux
+    // ---- load: operators (rows pitched for conflict-free fragment loads, padding rows zero), my cells of the committed
+    // state, the FIX input vectors [y(k+1/2 run) | z(k+1/2 run) | Q], the old scalar flux
     if (rank == 0) {
         for (int i = tid; i < 2 * kNormSlots; i += SM_THREADS) V.norms[i] = 0ull;
         if (tid == 0) V.flags[8] = 0;
     }
-    for (int e = tid; e < MX * KX; e += SM_THREADS) {
-        const int r = e / KX, u = e - r * KX;
-        opx[u * MX + r] = V.xop[(size_t)r * (K2 + 16) + u];
+    for (int e = tid; e < L.mx * (K2 + 4); e += SM_THREADS) {
+        const int r = e / (K2 + 4), u = e - r * (K2 + 4);
+        opx[r * PX + u] = r < 2 * K2 + 4 ? V.xop[(size_t)r * (K2 + 16) + u] : 0.0;
     }
-    for (int e = tid; e < MR * K2; e += SM_THREADS) {
+    for (int e = tid; e < L.mr * K2; e += SM_THREADS) {
         const int r = e / K2, k = e - r * K2;
-        opr[k * MR + r] = V.rop[(size_t)r * K2 + k];
+        opr[r * PR + k] = r < K2 + 4 ? V.rop[(size_t)r * K2 + k] : 0.0;
     }
-    for (int e = tid; e < K2 * K2; e += SM_THREADS) {
+    for (int e = tid; e < L.mf * K2; e += SM_THREADS) {
         const int r = e / K2, k = e - r * K2;
-        opf[k * K2 + r] = V.fop[(size_t)r * K2 + k];
+        opf[r * PR + k] = r < K2 ? V.fop[(size_t)r * K2 + k] : 0.0;
     }
     {
         const double* __restrict__ Yg = V.y[ybase];
         for (int e = tid; e < (nc + 2) * K2; e += SM_THREADS) {           // rows j0-1 .. j0+nc: the global ghost rows ride along
             const int r = e / K2, q = e - r * K2;
-            ybuf[0][(r - 1) * P + q] = Yg[((int64_t)j0 + r - 1) * K2 + q];
+            const double v = Yg[((int64_t)j0 + r - 1) * K2 + q];
+            ybuf[0][(r - 1) * P + q] = v;
+            if (r >= 1 && r <= nc && q >= N2 && q < N2 + N) xin[(r - 1) * P + (q - N2)] = v;
         }
         for (int e = tid; e < nc * N; e += SM_THREADS) {
             const int c = e / N, u = e - c * N;
-            zin[c * (N + 1) + u] = V.z[((int64_t)j0 + c) * K2 + N2 + u];
+            xin[c * P + N + u] = V.z[((int64_t)j0 + c) * K2 + N2 + u];
         }
         for (int e = tid; e < nc * 4; e += SM_THREADS) {
-            qin[e] = V.Q[(int64_t)j0 * 4 + e];
+            xin[(e >> 2) * P + K2 + (e & 3)] = V.Q[(int64_t)j0 * 4 + e];
             phi[e] = V.phi[(int64_t)j0 * 4 + e];
         }
     }
-    __syncthreads();
+    if (C > 1) cluster.sync();                     // every CTA of the cluster is running before anybody touches its shared memory
+    else __syncthreads();
 
     // ---- FIX: [yfix | ifix | phifix][c] = X [psi_{k-1/2}[c]; Q[c]]   (psi_{k-1/2} = the k+1/2 runs of y and z)
     {
-        const int groups = MX / SM_R;
-        for (int t = tid; t < groups * nc; t += SM_THREADS) {
-            const int g = t / nc, c = t - g * nc, r0 = g * SM_R;
-            double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-            const double* __restrict__ yr = ybuf[0] + c * P + N2;
-            const double* __restrict__ zr = zin + c * (N + 1);
-            const double* __restrict__ op = opx + r0;
-#pragma unroll 4
-            for (int u = 0; u < KX; ++u) {
-                const double x = u < N ? yr[u] : u < K2 ? zr[u - N] : qin[c * 4 + (u - K2)];
-                const double4 w = *reinterpret_cast<const double4*>(op + u * MX);
-                a0 = fma(w.x, x, a0); a1 = fma(w.y, x, a1); a2 = fma(w.z, x, a2); a3 = fma(w.w, x, a3);
-            }
-            const double a[4] = {a0, a1, a2, a3};
-#pragma unroll
-            for (int i = 0; i < SM_R; ++i) {
-                const int r = r0 + i;
-                if (r < K2) yfix[c * P + r] = a[i];
-                else if (r < 2 * K2) ifix[c * P + (r - K2)] = a[i];
-                else phifix[c * 4 + (r - 2 * K2)] = a[i];
-            }
+        const int nbt = L.mx / 8, ngr = (nbt + SM_NBG - 1) / SM_NBG;
+        for (int it = warp; it < ntile * ngr; it += nwarps) {
+            const int tile = it / ngr, gr = it - tile * ngr;
+            const int t0 = gr * SM_NBG, nb = nbt - t0 < SM_NBG ? nbt - t0 : SM_NBG;
+            small_item(opx, PX, K2 + 4, 16 * tile, t0, nb,
+                       [&](int c, int k) { return xin + (c < nc ? c : nc - 1) * P + k; },   // (a ragged tile's missing cells: dropped)
+                       [&](int c, int r, double v0, double v1) {
+                           if (c >= nc) return;
+                           if (r < K2) { yfix[c * P + r] = v0; yfix[c * P + r + 1] = v1; }
+                           else if (r < 2 * K2) { ifix[c * P + r - K2] = v0; ifix[c * P + r - K2 + 1] = v1; }
+                           else if (r < 2 * K2 + 4) { phifix[c * 4 + r - 2 * K2] = v0; phifix[c * 4 + r - 2 * K2 + 1] = v1; }
+                       });
         }
     }
     __syncthreads();
@@ -189,37 +234,30 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
         const double* __restrict__ src = ybuf[l & 1];
         double* __restrict__ dst = ybuf[(l + 1) & 1];
         double dmax = 0.0, rmax = 0.0;
-        const int groups = MR / SM_R;
-        for (int t = tid; t < groups * nc; t += SM_THREADS) {
-            const int g = t / nc, c = t - g * nc, r0 = g * SM_R;
-            double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-            const double* __restrict__ xr = src + (c + 1) * P;            // q < N: the right neighbour's outgoing flux
-            const double* __restrict__ xl = src + (c - 1) * P;            // q >= N: the left neighbour's
-            const double* __restrict__ op = opr + r0;
-#pragma unroll 4
-            for (int k = 0; k < N; ++k) {
-                const double x = xr[k];
-                const double4 w = *reinterpret_cast<const double4*>(op + k * MR);
-                a0 = fma(w.x, x, a0); a1 = fma(w.y, x, a1); a2 = fma(w.z, x, a2); a3 = fma(w.w, x, a3);
-            }
-#pragma unroll 4
-            for (int k = N; k < K2; ++k) {
-                const double x = xl[k];
-                const double4 w = *reinterpret_cast<const double4*>(op + k * MR);
-                a0 = fma(w.x, x, a0); a1 = fma(w.y, x, a1); a2 = fma(w.z, x, a2); a3 = fma(w.w, x, a3);
-            }
-            const double a[4] = {a0, a1, a2, a3};
-            if (r0 < K2) {
-#pragma unroll
-                for (int i = 0; i < SM_R; ++i) dst[c * P + r0 + i] = yfix[c * P + r0 + i] + a[i];
-            } else {
-#pragma unroll
-                for (int i = 0; i < SM_R; ++i) {
-                    const double nw = phifix[c * 4 + i] + a[i], old = phi[c * 4 + i];
-                    phi[c * 4 + i] = nw;
-                    dmax = nanmax(dmax, fabs(nw - old));
-                    rmax = nanmax(rmax, fabs(nw));
-                }
+        {
+            const int nbt = L.mr / 8, ngr = (nbt + SM_NBG - 1) / SM_NBG;
+            for (int it = warp; it < ntile * ngr; it += nwarps) {
+                const int tile = it / ngr, gr = it - tile * ngr;
+                const int t0 = gr * SM_NBG, nb = nbt - t0 < SM_NBG ? nbt - t0 : SM_NBG;
+                small_item(opr, PR, K2, 16 * tile, t0, nb,
+                           // q < N: the right neighbour's outgoing flux, q >= N: the left neighbour's (rows past the
+                           // CTA's last cell are stale but finite: their results are dropped)
+                           [&](int c, int k) { return src + ((c < nc ? c : nc - 1) + (k < N ? 1 : -1)) * P + k; },
+                           [&](int c, int r, double v0, double v1) {
+                               if (c >= nc) return;
+                               if (r < K2) {
+                                   dst[c * P + r] = yfix[c * P + r] + v0;
+                                   dst[c * P + r + 1] = yfix[c * P + r + 1] + v1;
+                               } else if (r < K2 + 4) {
+                                   const int i = r - K2;
+                                   const double n0 = phifix[c * 4 + i] + v0, n1 = phifix[c * 4 + i + 1] + v1;
+                                   const double o0 = phi[c * 4 + i], o1 = phi[c * 4 + i + 1];
+                                   phi[c * 4 + i] = n0;
+                                   phi[c * 4 + i + 1] = n1;
+                                   dmax = nanmax(dmax, nanmax(fabs(n0 - o0), fabs(n1 - o1)));
+                                   rmax = nanmax(rmax, nanmax(fabs(n0), fabs(n1)));
+                               }
+                           });
             }
         }
         dmax = warp_max(dmax);
@@ -254,28 +292,17 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
     // ---- FINAL: z = ifix + F inc^(L-1), staged in shared memory (yfix is dead) for a coalesced store
     if (finalize) {
         const double* __restrict__ src = ybuf[(Lit + 1) & 1];             // y^(L-1) with the ghost rows iteration L-1 read
-        const int groups = K2 / SM_R;
-        for (int t = tid; t < groups * nc; t += SM_THREADS) {
-            const int g = t / nc, c = t - g * nc, r0 = g * SM_R;
-            double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-            const double* __restrict__ xr = src + (c + 1) * P;
-            const double* __restrict__ xl = src + (c - 1) * P;
-            const double* __restrict__ op = opf + r0;
-#pragma unroll 4
-            for (int k = 0; k < N; ++k) {
-                const double x = xr[k];
-                const double4 w = *reinterpret_cast<const double4*>(op + k * K2);
-                a0 = fma(w.x, x, a0); a1 = fma(w.y, x, a1); a2 = fma(w.z, x, a2); a3 = fma(w.w, x, a3);
-            }
-#pragma unroll 4
-            for (int k = N; k < K2; ++k) {
-                const double x = xl[k];
-                const double4 w = *reinterpret_cast<const double4*>(op + k * K2);
-                a0 = fma(w.x, x, a0); a1 = fma(w.y, x, a1); a2 = fma(w.z, x, a2); a3 = fma(w.w, x, a3);
-            }
-            const double a[4] = {a0, a1, a2, a3};
-#pragma unroll
-            for (int i = 0; i < SM_R; ++i) yfix[c * P + r0 + i] = ifix[c * P + r0 + i] + a[i];   // z, in place of yfix
+        const int nbt = L.mf / 8, ngr = (nbt + SM_NBG - 1) / SM_NBG;
+        for (int it = warp; it < ntile * ngr; it += nwarps) {
+            const int tile = it / ngr, gr = it - tile * ngr;
+            const int t0 = gr * SM_NBG, nb = nbt - t0 < SM_NBG ? nbt - t0 : SM_NBG;
+            small_item(opf, PR, K2, 16 * tile, t0, nb,
+                       [&](int c, int k) { return src + ((c < nc ? c : nc - 1) + (k < N ? 1 : -1)) * P + k; },
+                       [&](int c, int r, double v0, double v1) {
+                           if (c >= nc || r >= K2) return;
+                           yfix[c * P + r] = ifix[c * P + r] + v0;          // z, in place of yfix
+                           yfix[c * P + r + 1] = ifix[c * P + r + 1] + v1;
+                       });
         }
         __syncthreads();
         for (int e = tid; e < nc * K2; e += SM_THREADS) {
@@ -336,10 +363,10 @@ int launch_red_small(const DevView& V, int C, int ybase, double tol, int cnt, in
     const int Jc = (int)((V.J + C - 1) / C);
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)C);
-    // thread items of one iteration in the busiest CTA: as many threads as there are items (a warp at least, 1024 at
-    // most), since for a tiny problem every barrier and every serial reduction over the warps is pure latency
-    const int64_t items = (int64_t)Jc * ((2 * V.N + 4) / SM_R);
-    int threads = (int)((items + 31) / 32) * 32;
+    // one warp per work item of an iteration (tile of 16 cells x up to 40 operator rows) in the busiest CTA, 8 at most:
+    // for a tiny problem every barrier and every serial reduction over the warps is pure latency
+    const int64_t items = (int64_t)((Jc + 15) / 16) * (((2 * V.N + 4 + 7) / 8 + SM_NBG - 1) / SM_NBG);
+    int threads = (int)(items * 32);
     threads = threads < 32 ? 32 : threads > SM_MAX_THREADS ? SM_MAX_THREADS : threads;
     cfg.blockDim = dim3((unsigned)threads);
     cfg.dynamicSmemBytes = (size_t)small_layout(V.N, Jc).total * 8;
