@@ -16,8 +16,10 @@
 //   FIX  :  c = c_fix (eqs. 27,28 without the (l) terms)            -> yfix, ifix, phifix
 //   ITER :  c = |mu| inc^(l) on the two incident rows of each angle -> y^(l+1) = yfix + Psi[O], phi^(l+1) = phifix + phi
 //   FINAL:  the same from inc^(L-1)                                 -> z = ifix + Psi[I]
-// Thread = (cell, angle); the 4-vector s is summed over the angles of a cell by warp shuffles (N a power of two)
-// and, across the warps of a cell or for other N, through shared memory in a fixed order (deterministic).
+// Two kernels.  The direct one (any N, per-cell blocks, FIX, small problems): thread = (cell, angle), the 4-vector s
+// summed over the angles of a cell by warp shuffles (N a power of two) and, across the warps of a cell or for other N,
+// through shared memory in a fixed order.  The TMA-staged one (ITER / FINAL, one shared block, N in {16, 32, 64, 128}):
+// s = P inc as DMMA straight from the staged rows.  Both deterministic.
 // HBM-bound: per cell and iteration 6N doubles of state (+ 16N + 17 of operator when every cell has its own block).
 #include <cuda.h>
 
@@ -143,7 +145,7 @@ namespace {
 // values and keeps two, the second exchanges one and keeps one, the remaining levels reduce a single value: 6 shuffles
 // instead of 20 for a full warp, after which the lane with bits (hi, hi2) holds the total of slot 2 hi + hi2.  N <= 32:
 // the four totals are broadcast by four more shuffles; N > 32: the partials of the cell's N/32 warps meet in shared memory.
-template <int W, bool NAMED = false>
+template <int W>
 __device__ __forceinline__ void cell_sum(double (&p)[4], int N, int cell_slot, double* __restrict__ sm)
 {
     if (W == 0) {
@@ -176,8 +178,7 @@ __device__ __forceinline__ void cell_sum(double (&p)[4], int N, int cell_slot, d
     }
     const int warp = threadIdx.x >> 5, wpc = N >> 5;
     if ((lane & 7) == 0) sm[warp * 4 + (lane >> 3)] = keep;               // lanes 0, 8, 16, 24 hold slots 0..3
-    if (NAMED) named_bar_sync(1, 256);                                    // the consumer warps only (a producer warp is not in it)
-    else __syncthreads();
+    __syncthreads();
     const double* __restrict__ q = sm + (warp / wpc) * wpc * 4;
     p[0] = p[1] = p[2] = p[3] = 0.0;
     for (int w = 0; w < wpc; ++w) {
