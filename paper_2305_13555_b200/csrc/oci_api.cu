@@ -472,13 +472,14 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
         int32_t cnt = guess - done_iters;
         if (cnt < 4) cnt = 4;
         if (cnt > kNormSlots) cnt = kNormSlots;
-        if (red && ctx->red_kernel != OCI_RKERNEL_KTILED && ctx->coop) cnt = kNormSlots;   // the fused loop stops itself
+        const bool loop_kernel = red && ctx->coop && (ctx->red_kernel != OCI_RKERNEL_KTILED || oci_red_ktiled_fuses_loop(V));
+        if (loop_kernel) cnt = kNormSlots;                                  // the fused loop stops itself
         if (cnt > max_iters - done_iters) cnt = max_iters - done_iters;
         // (the FIX pass has already cleared the norm slots and the barrier counter for the first chunk)
         if (!(red && done_iters == 0)) CK(cudaMemsetAsync(V.norms, 0, sizeof(unsigned long long) * 2 * cnt, s));
         // the resident and GEMV kernels of the reduced form run the whole chunk of iterations in ONE cooperative launch
         // (grid-wide barrier + device-side stop between iterations): no launch gap, operator staged once
-        const bool fused_loop = red && ctx->red_kernel != OCI_RKERNEL_KTILED && ctx->coop && cnt > 1;
+        const bool fused_loop = loop_kernel && cnt > 1;
         // ... and reports its iteration count straight into mapped host memory (publish_step): no copy, no stream sync
         // (small problems only: the report costs the loop's last CTA a system-scope fence and a PCIe write, about 3 us
         // that a large problem's FINAL pass would wait for, while its host part overlaps that pass anyway)

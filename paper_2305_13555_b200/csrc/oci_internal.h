@@ -165,6 +165,7 @@ bool oci_encode_2d(CUtensorMap* m, const double* base, uint64_t rows, uint64_t c
                    bool swizzle128);
 bool oci_red_ktiled_supported(const DevView& V);
 bool oci_red_ktiled_prepare(const DevView& V, RedKtiledMaps* M);
+bool oci_red_ktiled_fuses_loop(const DevView& V);
 int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int ybase, int slot, int prev_slot, double tol,
                       int cnt, int force, cudaStream_t s);
 int launch_shard_push(const DevView& V, int ybuf, int slot, int prev_slot, double tol, unsigned long long tag, cudaStream_t s);

@@ -44,7 +44,7 @@ constexpr int RK_B_BYTES = RK_N * RK_K * 8;   // 16 KB
 constexpr int RK_P_BYTES = 8 * RK_K * 8;      // 1 KB: the scalar-flux rows (4 used)
 constexpr int RK_STAGE_BYTES = RK_A_BYTES + RK_B_BYTES + RK_P_BYTES + 1024;   // keeps every stage 2 KB-aligned
 constexpr size_t RK_SMEM = 1024 /*alignment slack*/ + (size_t)RK_STAGES * RK_STAGE_BYTES + 2 * 4 * RK_M * 4 * 8 /*phi_s, 2 buffers*/ +
-                           2 * RK_STAGES * 8 + 64;
+                           2 * RK_STAGES * 8 + 16 /*iter_bar, go*/ + 64;
 
 }  // namespace
 
@@ -67,7 +67,9 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
         }
         ysrc = (ybase + L - 1) & 1;
     }
-    const CUtensorMap* my = (ysrc == ybase) ? &map_y : &map_y_alt;
+    // ITER: `cnt` > 1 iterations run inside this one (cooperative) launch, separated by a grid-wide barrier; iteration l
+    // reads y[(ybase + l) & 1], reports its norms in slot `slot + l`, and the loop ends at the first converged one
+    const int nloop = PASS == PASS_ITER ? (cnt > 1 ? cnt : 1) : 1;
     if (PASS == PASS_FIX) clear_step_state(V);
 
     extern __shared__ unsigned char smem_raw[];
@@ -77,6 +79,8 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
     double* phi_s2 = reinterpret_cast<double*>(base + (size_t)RK_STAGES * RK_STAGE_BYTES);  // [2][4 wn][64][4]
     uint64_t* full = reinterpret_cast<uint64_t*>(phi_s2 + 2 * 4 * RK_M * 4);
     uint64_t* empty = full + RK_STAGES;
+    uint64_t* iter_bar = empty + RK_STAGES;   // MMA warps -> producer: "the grid barrier after iteration l has been passed"
+    volatile int* go_s = reinterpret_cast<volatile int*>(iter_bar + 1);   // ... and whether another iteration follows
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int N = V.N, K2 = V.n >> 1, N2 = N >> 1;
@@ -108,6 +112,7 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
             mbar_init(&full[s], 1);
             mbar_init(&empty[s], 8);
         }
+        mbar_init(iter_bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -116,7 +121,8 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
         // =========================== TMA producer (one thread of the auxiliary warpgroup) ===========================
         asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
         if (warp == 8 && lane == 0) {
-            asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(my)) : "memory");
+            asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&map_y)) : "memory");
+            asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&map_y_alt)) : "memory");
             asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&map_op)) : "memory");
             if (PASS != PASS_FINAL) asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&map_op8)) : "memory");
             if (PASS == PASS_FIX) {
@@ -124,6 +130,16 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
                 asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&map_q)) : "memory");
             }
             int q = 0;
+          for (int l = 0; l < nloop; ++l) {
+            const int ysrc_l = PASS == PASS_ITER ? (ybase + l) & 1 : ysrc;
+            const CUtensorMap* my = (ysrc_l == ybase) ? &map_y : &map_y_alt;
+            if (PASS == PASS_ITER && l > 0) {
+                // the rows other CTAs stored in iteration l-1 are visible once the grid barrier has been passed (thread 0
+                // says so through iter_bar); they are read next through the async proxy (TMA)
+                mbar_wait(iter_bar, (l - 1) & 1);
+                if (*go_s < 0) break;                                 // the step has converged: no more iterations
+                asm volatile("fence.proxy.async;" ::: "memory");
+            }
             for (int it = 0; it < my_items; ++it) {
                 const int64_t item = (int64_t)blockIdx.x + (int64_t)it * gridDim.x;
                 int64_t ct;
@@ -155,6 +171,7 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
                     if (with_phi) tma_load_2d(st + RK_A_BYTES + RK_B_BYTES, &map_op8, k0, blk * rpb + prow, &full[s]);
                 }
             }
+          }
         }
         return;
     }
@@ -174,12 +191,13 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
     // whole foff array into local memory and put a local load in front of every fragment load)
     const int p_off = g4 * 128 + (((wn + 4 * (t4 >> 1)) ^ g4) << 4) + ((t4 & 1) << 3);
 
-    double* __restrict__ Yd = V.y[ysrc ^ 1];
-    double dmax = 0.0, rmax = 0.0;
     const bool refl_l = V.bcL == OCI_BC_REFLECTING, refl_r = V.bcR == OCI_BC_REFLECTING;
 
-    int q = 0;
-    for (int it = 0; it < my_items; ++it) {
+    int q = 0, itc = 0;
+  for (int l = 0; l < nloop; ++l) {
+    double* __restrict__ Yd = V.y[(PASS == PASS_ITER ? (ybase + l) & 1 : ysrc) ^ 1];
+    double dmax = 0.0, rmax = 0.0;
+    for (int it = 0; it < my_items; ++it, ++itc) {
         const int64_t item = (int64_t)blockIdx.x + (int64_t)it * gridDim.x;
         int64_t ct;
         int nt, blk;
@@ -215,7 +233,7 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
             pfix = V.phifix[j * 4 + (tid & 3)];
             pold = V.phi[j * 4 + (tid & 3)];
         }
-        double* phi_s = phi_s2 + (it & 1) * (4 * RK_M * 4);    // alternating buffers: one barrier per item
+        double* phi_s = phi_s2 + (itc & 1) * (4 * RK_M * 4);   // alternating buffers: one barrier per item
 
         double acc[4][4][2], accp[4][2];
 #pragma unroll
@@ -309,10 +327,34 @@ oci_red_ktiled_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, cons
         dmax = warp_max(dmax);
         rmax = warp_max(rmax);
         if (lane == 0) {
-            atomic_max_nonneg(&V.norms[2 * slot + 0], dmax);
-            atomic_max_nonneg(&V.norms[2 * slot + 1], rmax);
+            atomic_max_nonneg(&V.norms[2 * (slot + l) + 0], dmax);
+            atomic_max_nonneg(&V.norms[2 * (slot + l) + 1], rmax);
+        }
+        if (nloop > 1) {
+            // ---- grid-wide barrier over the MMA warps of all CTAs (cooperative launch: all resident), then the stopping
+            // rule (a7) on the now final norms; the producer thread follows through iter_bar / go_s
+            __threadfence();
+            named_bar_sync(1, 256);
+            if (tid == 0) {
+                unsigned int* bar = reinterpret_cast<unsigned int*>(V.flags) + 8;
+                atomicAdd(bar, 1u);
+                const unsigned int target = (unsigned int)(l + 1) * gridDim.x;
+                unsigned int seen;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(bar) : "memory");
+                } while (seen < target);
+            }
+            named_bar_sync(1, 256);
+            const bool stop = step_done(V.norms, slot + l, tol) || l + 1 == nloop;
+            if (stop && blockIdx.x == 0 && tid == 0) publish_step(V, l + 1, slot + l);
+            if (tid == 0) {
+                *go_s = stop ? -1 : 1;
+                mbar_arrive(iter_bar);
+            }
+            if (stop) break;
         }
     }
+  }
 }
 
 // ---- ping-pong variant of the same kernel, used when every CTA has at least one item per math group.
@@ -627,6 +669,16 @@ bool oci_red_ktiled_prepare(const DevView& V, RedKtiledMaps* M)
            oci_encode_2d(&M->fop, V.fop, nb * K2, K2, RK_N, RK_K, true);
 }
 
+// the eight-warp kernel runs all iterations of a chunk in one cooperative launch; the ping-pong kernel (two producer
+// threads, two staggered math groups) keeps one launch per iteration
+bool oci_red_ktiled_fuses_loop(const DevView& V)
+{
+    const int K2 = V.n / 2;
+    const int64_t nitems = (V.gitems ? V.ngroups : (V.J + RK_M - 1) / RK_M) * ((K2 + RK_N - 1) / RK_N);
+    const int64_t grid = nitems < V.sm_count ? nitems : V.sm_count;
+    return nitems < 2 * grid;
+}
+
 int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int ybase, int slot, int prev_slot, double tol, int cnt,
                       int force, cudaStream_t s)
 {
@@ -649,7 +701,14 @@ int launch_red_ktiled(const DevView& V, const RedKtiledMaps& M, int pass, int yb
     }
     if (pass == PASS_FIX)
         oci_red_ktiled_kernel<PASS_FIX><<<grid, 384, RK_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.xop, M.xop8, ybase, 0, -1, tol, 0, 0);
-    else if (pass == PASS_ITER)
+    else if (pass == PASS_ITER && cnt > 1) {
+        // `cnt` iterations in one launch with a grid-wide barrier between them: every CTA is resident (grid <= SMs)
+        DevView Vv = V;
+        CUtensorMap a0 = ya, a1 = yb, a2 = M.z, a3 = M.q16, a4 = M.rop, a5 = M.rop8;
+        int zero = 0;
+        void* args[] = {&Vv, &a0, &a1, &a2, &a3, &a4, &a5, &ybase, &slot, &prev_slot, &tol, &cnt, &zero};
+        cudaLaunchCooperativeKernel((const void*)oci_red_ktiled_kernel<PASS_ITER>, dim3(grid), dim3(384), args, RK_SMEM, s);
+    } else if (pass == PASS_ITER)
         oci_red_ktiled_kernel<PASS_ITER><<<grid, 384, RK_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.rop, M.rop8, ybase, slot, prev_slot, tol, 0, 0);
     else
         oci_red_ktiled_kernel<PASS_FINAL><<<grid, 384, RK_SMEM, s>>>(V, ya, yb, M.z, M.q16, M.fop, M.fop, ybase, 0, -1, tol, cnt, force);

@@ -766,3 +766,27 @@ def test_small_step_hand_over_and_refusals():
             h.setup()
         assert e.value.code == -1
         h.close()
+
+
+def test_ktiled_fused_loop_many_iterations():
+    """The eight-warp K-tiled kernel runs a chunk of up to 64 iterations in one cooperative launch (the producer thread
+    follows the MMA warps through the grid barrier).  More than one chunk, an exact count that ends inside a later chunk,
+    and a handful of materials (masked tiles)."""
+    import paper_2305_13555_b200 as P
+    from oracle import Oracle
+    q = _custom(150, 48, (REF, 0.0), (REF, 0.0), seed=77, hetero=False, dt=50.0)
+    q.sigma_s[:] = q.sigma_t * 0.999
+    q.sigma_t[40:90] *= 1.5                                  # a second material: interfaces inside the 64-cell tiles
+    q.sigma_s[40:90] *= 1.5
+    g, o = P.OCI.from_problem(q, reduced_kernel=P.RKERNEL_KTILED), Oracle.from_problem(q, threads=8)
+    info = g.get_info()
+    assert info["reduced_kernel"] == P.RKERNEL_KTILED and info["n_blocks"] == 2 and info["small_step_cluster"] == 0
+    for x in (g, o):
+        x.set_source(q.source(0))
+    a, b = g.oci_step(1e-10, 100_000), o.oci_step(1e-10, 100_000)
+    assert a[0] == b[0] == 0 and abs(a[1] - b[1]) <= 1 and a[1] > 128, (a, b)
+    assert rel(g.get_scalar_flux(), o.scalar_flux()) < 1e-8
+    g.set_flux(q.psi0); o.set_flux(q.psi0)
+    assert g.oci_step(-1.0, 77)[:2] == (1, 77) == o.oci_step(-1.0, 77)[:2]
+    assert rel(g.get_angular_flux(), o.angular_flux()) < 1e-12
+    g.close()
