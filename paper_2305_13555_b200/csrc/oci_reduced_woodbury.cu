@@ -734,6 +734,159 @@ oci_red_woodbury_tma_kernel(DevView V, const __grid_constant__ CUtensorMap map_y
   }
 }
 
+// ---- FIX with a shared block and N in {16, 32, 64, 128}, the same way: s = P_fix [psi_{k-1/2}; Q] on the tensor pipe.
+// c_fix (eqs. 27,28 without the (l) terms) has 2N entries that carry psi_{k-1/2} (rows (m,0), (m,1), factor alpha) and
+// an isotropic Q, so s = sum_m w_m A_m^{-1} c_fix,m = P_fix x with x = [y(k+1/2 run) | z(k+1/2 run) | Q] (the input
+// vector of the dense FIX operator) and P_fix 4 x (2N + 4).  Column m of either k+1/2 run belongs to angle m, so the two
+// boxes (gc rows x N + 4 columns at column N/2 of y and z) serve phase A as A fragments and phase B as per-angle reads.
+// One CTA per SM (phase B holds all of A_m^{-1} and D_m: 32 doubles), three stages.
+constexpr int WF_STAGES = 3;
+
+template <int NT>
+__global__ void __launch_bounds__(WT_CONS + 32, 1)
+oci_red_woodbury_fix_kernel(DevView V, const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_z, int ybase)
+{
+    extern __shared__ __align__(128) unsigned char wt_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    clear_step_state(V);
+    constexpr int N = NT, K2 = 2 * N, N2 = N >> 1;
+    const int J = (int)V.J;
+    constexpr int gc = 1024 / N, U = 4, LDH = N + 4, KS = K2 / 4, KSW = KS / WT_WARPS, NB = gc / 8;
+    constexpr int box_dbl = gc * LDH;
+    constexpr int stage_dbl = 2 * box_dbl + 4 * gc;                        // y box | z box | Q rows
+    static_assert((box_dbl * 8) % 128 == 0 && (stage_dbl * 8) % 128 == 0, "TMA destinations stay 128-byte aligned");
+    double* ring = reinterpret_cast<double*>(wt_raw);
+    double* part = ring + (size_t)WF_STAGES * stage_dbl;                   // [8 warps][gc][4]
+    double* s_sm = part + WT_WARPS * gc * 4;                               // [gc][4]
+    uint64_t* full = reinterpret_cast<uint64_t*>(s_sm + gc * 4);
+    uint64_t* empty = full + WF_STAGES;
+    if (threadIdx.x == 0) {
+        for (int st = 0; st < WF_STAGES; ++st) { mbar_init(&full[st], 1); mbar_init(&empty[st], WT_WARPS); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const int ngroups = (J + gc - 1) / gc;
+    const int my_groups = (int)blockIdx.x < ngroups ? (ngroups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+
+    if (warp >= WT_WARPS) {
+        // ---- producer
+        if (lane == 0) {
+            for (int i = 0; i < my_groups; ++i) {
+                const int st = i % WF_STAGES;
+                if (i >= WF_STAGES) mbar_wait(&empty[st], ((i / WF_STAGES) - 1) & 1);
+                const int j0 = ((int)blockIdx.x + i * (int)gridDim.x) * gc;
+                const int rows = J - j0 < gc ? J - j0 : gc;
+                double* sg = ring + (size_t)st * stage_dbl;
+                mbar_expect_tx(&full[st], 2 * box_dbl * 8 + (uint32_t)rows * 32);
+                tma_load_2d(sg, &map_y, N2, j0 + 1, &full[st]);            // y map row = cell + 1
+                tma_load_2d(sg + box_dbl, &map_z, N2, j0, &full[st]);
+                tma_load_1d(sg + 2 * box_dbl, V.Q + (int64_t)j0 * 4, (uint32_t)rows * 32, &full[st]);
+            }
+        }
+        return;
+    }
+    // ---- consumers
+    const int tid = threadIdx.x;
+    const int m = tid % N, c0 = tid / N;                                   // angle; first cell slot (then c0 + 256/N, ...)
+    constexpr int cstep = WT_CONS / N;
+    const int half = m >= N2, mm = m - half * N2;
+    const int qk = pack_q(half, 0, mm, N), qe = pack_q(half, 1, mm, N);
+    const double wm = V.w[m];
+    const bool phi_lane = m < 4;
+    const int psl = m & 3;
+    const double h = V.dx[V.rep[0]];
+    const double alpha = h / (2.0 * V.v * V.dt), q4 = 0.25 * h;
+    WbOps<PASS_FIX> O;                                                     // all of A_m^{-1} (columns 0..3) and D_m (rows 0..3)
+    load_ops<PASS_FIX>(O, V.wba + m, V.wbd + m, N, half, 0.0, wm);
+    double mrow[4];
+#pragma unroll
+    for (int cc = 0; cc < 4; ++cc) mrow[cc] = V.wbm[4 * psl + cc];
+    // phase A: this warp's slice of P_fix as DMMA B fragments.  B[k][n] = P_fix[slot n][k], n = g4 < 4.  Input column u < N
+    // is angle u's entry of the y run: psi_{k-1/2,L} (row (m,0)) for mu < 0, psi_{k-1/2,R} (row (m,1)) for mu > 0; column
+    // N + u its entry of the z run: the other corner.  The last k-step is Q: P_fix[slot][2N + s'] = (h/4) sum_m w_m A_m^{-1}[slot][s'].
+    const int g4 = lane >> 2, t4 = lane & 3;
+    double bfr[KSW], bq = 0.0;
+#pragma unroll
+    for (int i = 0; i < KSW; ++i) {
+        const int u = 4 * (warp * KSW + i) + t4;
+        const int ma = u < N ? u : u - N;
+        const int col = (u < N) == (ma < N2) ? 0 : 1;
+        bfr[i] = g4 < 4 ? V.w[ma] * alpha * V.wba[(size_t)(4 * g4 + col) * N + ma] : 0.0;
+    }
+    if (warp == 0 && g4 < 4) {
+        for (int ma = 0; ma < N; ++ma) bq = fma(V.w[ma], V.wba[(size_t)(4 * g4 + t4) * N + ma], bq);
+        bq *= q4;
+    }
+
+    for (int i = 0; i < my_groups; ++i) {
+        const int st = i % WF_STAGES;
+        const int j0 = ((int)blockIdx.x + i * (int)gridDim.x) * gc;
+        const double* sg = ring + (size_t)st * stage_dbl;
+        mbar_wait(&full[st], (i / WF_STAGES) & 1);
+        // ---- phase A: partial s over this warp's k-steps (warp 0: + the Q k-step), all blocks of 8 cells
+        {
+            double acc[NB][2];
+#pragma unroll
+            for (int bb = 0; bb < NB; ++bb) acc[bb][0] = acc[bb][1] = 0.0;
+#pragma unroll
+            for (int ii = 0; ii < KSW; ++ii) {
+                const int ks = warp * KSW + ii;                            // 4 ks < N: the y run, else the z run
+                const double* ap = sg + (4 * ks < N ? 4 * ks : box_dbl + 4 * ks - N) + g4 * LDH + t4;
+#pragma unroll
+                for (int bb = 0; bb < NB; ++bb) dmma(acc[bb][0], acc[bb][1], ap[bb * 8 * LDH], bfr[ii]);
+            }
+            if (warp == 0) {
+                const double* ap = sg + 2 * box_dbl + g4 * 4 + t4;
+#pragma unroll
+                for (int bb = 0; bb < NB; ++bb) dmma(acc[bb][0], acc[bb][1], ap[bb * 32], bq);
+            }
+            if (t4 < 2) {
+#pragma unroll
+                for (int bb = 0; bb < NB; ++bb)
+                    *reinterpret_cast<double2*>(part + ((size_t)warp * gc + bb * 8 + g4) * 4 + 2 * t4) = make_double2(acc[bb][0], acc[bb][1]);
+            }
+        }
+        named_bar_sync(1, WT_CONS);
+        if (tid < gc * 4) {
+            double sum = part[tid];
+#pragma unroll
+            for (int w = 1; w < WT_WARPS; ++w) sum += part[w * gc * 4 + tid];
+            s_sm[tid] = sum;
+        }
+        named_bar_sync(1, WT_CONS);
+        // ---- phase B: thread = (cell, angle): c = c_fix,m, t = A_m^{-1} c, Psi_fix,m = t + D_m s
+#pragma unroll
+        for (int u4 = 0; u4 < U; ++u4) {
+            const int cs = c0 + u4 * cstep;
+            const double a = sg[cs * LDH + m], b = sg[box_dbl + cs * LDH + m];
+            const double4 Q = *reinterpret_cast<const double4*>(sg + 2 * box_dbl + cs * 4);
+            const double4 sv = *reinterpret_cast<const double4*>(s_sm + cs * 4);
+            if (u4 + 1 == U) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[st]);                    // the stage is free again
+            }
+            const int j = j0 + cs;
+            if (j >= J) continue;
+            const double pL = half ? b : a, pR = half ? a : b;             // slots (k+1/2,L), (k+1/2,R) of the committed state (a8)
+            const double c0v = fma(alpha, pL, q4 * Q.x), c1v = fma(alpha, pR, q4 * Q.y), c2v = q4 * Q.z, c3v = q4 * Q.w;
+            double psi[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) psi[r] = fma(O.pe2[r], c3v, fma(O.pk2[r], c2v, fma(O.pe[r], c1v, O.pk[r] * c0v)));
+            psi[0] = fma(O.dk[3], sv.w, fma(O.dk[2], sv.z, fma(O.dk[1], sv.y, fma(O.dk[0], sv.x, psi[0]))));
+            psi[1] = fma(O.de[3], sv.w, fma(O.de[2], sv.z, fma(O.de[1], sv.y, fma(O.de[0], sv.x, psi[1]))));
+            psi[2] = fma(O.dk2[3], sv.w, fma(O.dk2[2], sv.z, fma(O.dk2[1], sv.y, fma(O.dk2[0], sv.x, psi[2]))));
+            psi[3] = fma(O.de2[3], sv.w, fma(O.de2[2], sv.z, fma(O.de2[1], sv.y, fma(O.de2[0], sv.x, psi[3]))));
+            double* __restrict__ yf = V.yfix + j * K2;
+            double* __restrict__ jf = V.ifix + j * K2;
+            yf[qk] = half ? psi[1] : psi[0];                               // O rows (a neighbour reads them)
+            yf[qe] = half ? psi[3] : psi[2];
+            jf[qk] = half ? psi[0] : psi[1];                               // I rows
+            jf[qe] = half ? psi[2] : psi[3];
+            if (phi_lane) V.phifix[j * 4 + psl] = fma(mrow[3], sv.w, fma(mrow[2], sv.z, fma(mrow[1], sv.y, mrow[0] * sv.x)));
+        }
+    }
+}
+
 namespace {
 struct WbLaunch { unsigned grid; size_t smem; };
 
@@ -819,6 +972,37 @@ void launch_wt_w(const DevView& V, int ybase, int slot, int prev_slot, double to
     oci_red_woodbury_tma_kernel<PASS, NT><<<grid, WT_CONS + 32, smem, s>>>(V, m0, m1, ybase, slot, prev_slot, tol, cnt, force);
 }
 
+size_t wf_smem(int N)
+{
+    const int gc = 1024 / N;
+    return WF_STAGES * ((size_t)2 * gc * (N + 4) + 4 * gc) * 8 + (size_t)(WT_WARPS + 1) * gc * 4 * 8 + 2 * WF_STAGES * 8 + 128;
+}
+
+template <int NT>
+void launch_wf_w(const DevView& V, int ybase, cudaStream_t s)
+{
+    const int gc = 1024 / NT, K2 = 2 * NT;
+    CUtensorMap my, mz;
+    if (!oci_encode_2d(&my, V.y[ybase & 1] - K2, (uint64_t)V.J + 2, K2, gc, NT + 4, false) ||
+        !oci_encode_2d(&mz, V.z, (uint64_t)V.J, K2, gc, NT + 4, false)) {
+        cudaMemsetAsync(nullptr, 0, 1, s);                                  // leaves an error for launched() to pick up
+        return;
+    }
+    const int64_t groups = (V.J + gc - 1) / gc;
+    const unsigned grid = (unsigned)(groups < V.sm_count ? groups : V.sm_count);   // (two CTAs per SM: 96 registers, spills, 82 vs 49 us)
+    oci_red_woodbury_fix_kernel<NT><<<grid, WT_CONS + 32, wf_smem(NT), s>>>(V, my, mz, ybase);
+}
+
+void launch_wf(const DevView& V, int ybase, cudaStream_t s)
+{
+    switch (V.N) {
+    case 16: launch_wf_w<16>(V, ybase, s); break;
+    case 32: launch_wf_w<32>(V, ybase, s); break;
+    case 64: launch_wf_w<64>(V, ybase, s); break;
+    default: launch_wf_w<128>(V, ybase, s); break;
+    }
+}
+
 template <int PASS>
 void launch_wt(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
 {
@@ -836,8 +1020,9 @@ template <int PASS, bool SHARED>
 void launch_wb(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
 {
     const int N = V.N;
-    if (SHARED && PASS != PASS_FIX && wt_serves(V, PASS)) {
-        launch_wt<PASS == PASS_FIX ? PASS_ITER : PASS>(V, ybase, slot, prev_slot, tol, cnt, force, s);
+    if (SHARED && wt_serves(V, PASS)) {
+        if (PASS == PASS_FIX) launch_wf(V, ybase, s);
+        else launch_wt<PASS == PASS_FIX ? PASS_ITER : PASS>(V, ybase, slot, prev_slot, tol, cnt, force, s);
         return;
     }
     const bool pow2 = (N & (N - 1)) == 0 && N >= 8;
@@ -866,7 +1051,8 @@ cudaError_t wt_opt_in()
     const auto at = cudaFuncAttributeMaxDynamicSharedMemorySize;
     const int bytes = 160 * 1024;
     cudaError_t e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_ITER, NT>, at, bytes);
-    return e != cudaSuccess ? e : cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_FINAL, NT>, at, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_FINAL, NT>, at, bytes);
+    return e != cudaSuccess ? e : cudaFuncSetAttribute(oci_red_woodbury_fix_kernel<NT>, at, bytes);
 }
 }  // namespace
 
