@@ -73,45 +73,57 @@ __host__ __device__ inline SmallLayout small_layout(int N, int Jc)
 }
 
 // One work item of a "gathered GEMM" pass: out[cell][row] = sum_k Op[row][k] in(cell, k) for the 16 cells c0 .. c0+15 and
-// the n8 blocks t0 .. t0+nb-1 of operator rows, as DMMA.8x8x4 (cells = the M dimension).  `in` returns the address of
-// element (cell, k) of the input; `out` receives (cell, row, v[row], v[row+1]) in accumulator layout.
-template <typename In, typename Out>
-__device__ __forceinline__ void small_item(const double* __restrict__ op, int opp, int K, int c0, int t0, int nb, In in, Out out)
+// NB n8 blocks of operator rows from block t0 on, as DMMA.8x8x4 (cells = the M dimension).  The input of the lane's two
+// cells (c0 + g4, c0 + 8 + g4) is row lo[g] for k < split and row hi[g] from there on (ITER / FINAL: the right / left
+// neighbour's row; FIX: one row); `out` receives (cell, row, v[row], v[row+1]) in accumulator layout.
+template <int NB, typename Out>
+__device__ __forceinline__ void small_item_nb(const double* __restrict__ op, int opp, int K, int split, const double* const (&lo)[2],
+                                              const double* const (&hi)[2], int c0, int t0, Out out)
 {
     const int lane = threadIdx.x & 31, g4 = lane >> 2, t4 = lane & 3;
-    double acc[2][SM_NBG][2];
+    double acc[2][NB][2];
 #pragma unroll
     for (int g = 0; g < 2; ++g)
 #pragma unroll
-        for (int t = 0; t < SM_NBG; ++t) acc[g][t][0] = acc[g][t][1] = 0.0;
+        for (int t = 0; t < NB; ++t) acc[g][t][0] = acc[g][t][1] = 0.0;
     const double* __restrict__ bp = op + (size_t)(8 * t0 + g4) * opp + t4;
     // the fragments of k-step k + 4 are requested before the DMMAs of k-step k are issued
-    double a0 = *in(c0 + g4, t4), a1 = *in(c0 + 8 + g4, t4), b[SM_NBG];
+    double a0 = (t4 < split ? lo[0] : hi[0])[t4], a1 = (t4 < split ? lo[1] : hi[1])[t4], b[NB];
 #pragma unroll
-    for (int t = 0; t < SM_NBG; ++t) b[t] = t < nb ? bp[(size_t)(8 * t) * opp] : 0.0;
+    for (int t = 0; t < NB; ++t) b[t] = bp[(size_t)(8 * t) * opp];
     for (int k = 0; k < K; k += 4) {
-        const int kn = k + 4 < K ? k + 4 : k;
-        const double na0 = *in(c0 + g4, kn + t4), na1 = *in(c0 + 8 + g4, kn + t4);
-        double nb_[SM_NBG];
+        const int kn = (k + 4 < K ? k + 4 : k) + t4;
+        const double na0 = (kn < split ? lo[0] : hi[0])[kn], na1 = (kn < split ? lo[1] : hi[1])[kn];
+        double nb_[NB];
 #pragma unroll
-        for (int t = 0; t < SM_NBG; ++t) nb_[t] = t < nb ? bp[(size_t)(8 * t) * opp + kn] : 0.0;
+        for (int t = 0; t < NB; ++t) nb_[t] = bp[(size_t)(8 * t) * opp + kn - t4];
 #pragma unroll
-        for (int t = 0; t < SM_NBG; ++t) {
-            if (t < nb) {
-                dmma(acc[0][t][0], acc[0][t][1], a0, b[t]);
-                dmma(acc[1][t][0], acc[1][t][1], a1, b[t]);
-            }
+        for (int t = 0; t < NB; ++t) {
+            dmma(acc[0][t][0], acc[0][t][1], a0, b[t]);
+            dmma(acc[1][t][0], acc[1][t][1], a1, b[t]);
         }
         a0 = na0;
         a1 = na1;
 #pragma unroll
-        for (int t = 0; t < SM_NBG; ++t) b[t] = nb_[t];
+        for (int t = 0; t < NB; ++t) b[t] = nb_[t];
     }
 #pragma unroll
     for (int g = 0; g < 2; ++g)
 #pragma unroll
-        for (int t = 0; t < SM_NBG; ++t)
-            if (t < nb) out(c0 + 8 * g + g4, 8 * (t0 + t) + 2 * t4, acc[g][t][0], acc[g][t][1]);
+        for (int t = 0; t < NB; ++t) out(c0 + 8 * g + g4, 8 * (t0 + t) + 2 * t4, acc[g][t][0], acc[g][t][1]);
+}
+
+template <typename Out>
+__device__ __forceinline__ void small_item(const double* __restrict__ op, int opp, int K, int split, const double* const (&lo)[2],
+                                           const double* const (&hi)[2], int c0, int t0, int nb, Out out)
+{
+    switch (nb) {                                          // the block count as a template argument: no predicated DMMA
+    case 5: small_item_nb<5>(op, opp, K, split, lo, hi, c0, t0, out); break;
+    case 4: small_item_nb<4>(op, opp, K, split, lo, hi, c0, t0, out); break;
+    case 3: small_item_nb<3>(op, opp, K, split, lo, hi, c0, t0, out); break;
+    case 2: small_item_nb<2>(op, opp, K, split, lo, hi, c0, t0, out); break;
+    default: small_item_nb<1>(op, opp, K, split, lo, hi, c0, t0, out); break;
+    }
 }
 
 }  // namespace
@@ -189,8 +201,10 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
         for (int it = warp; it < ntile * ngr; it += nwarps) {
             const int tile = it / ngr, gr = it - tile * ngr;
             const int t0 = gr * SM_NBG, nb = nbt - t0 < SM_NBG ? nbt - t0 : SM_NBG;
-            small_item(opx, PX, K2 + 4, 16 * tile, t0, nb,
-                       [&](int c, int k) { return xin + (c < nc ? c : nc - 1) * P + k; },   // (a ragged tile's missing cells: dropped)
+            const int g4 = lane >> 2;
+            const int ca = 16 * tile + g4 < nc ? 16 * tile + g4 : nc - 1, cb = 16 * tile + 8 + g4 < nc ? 16 * tile + 8 + g4 : nc - 1;
+            const double* const rows[2] = {xin + ca * P, xin + cb * P};    // (a ragged tile's missing cells: clamped, dropped)
+            small_item(opx, PX, K2 + 4, K2 + 4, rows, rows, 16 * tile, t0, nb,
                        [&](int c, int r, double v0, double v1) {
                            if (c >= nc) return;
                            if (r < K2) { yfix[c * P + r] = v0; yfix[c * P + r + 1] = v1; }
@@ -239,10 +253,13 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
             for (int it = warp; it < ntile * ngr; it += nwarps) {
                 const int tile = it / ngr, gr = it - tile * ngr;
                 const int t0 = gr * SM_NBG, nb = nbt - t0 < SM_NBG ? nbt - t0 : SM_NBG;
-                small_item(opr, PR, K2, 16 * tile, t0, nb,
-                           // q < N: the right neighbour's outgoing flux, q >= N: the left neighbour's (rows past the
-                           // CTA's last cell are stale but finite: their results are dropped)
-                           [&](int c, int k) { return src + ((c < nc ? c : nc - 1) + (k < N ? 1 : -1)) * P + k; },
+                // q < N: the right neighbour's outgoing flux, q >= N: the left neighbour's (a ragged tile's missing
+                // cells: clamped, their results dropped)
+                const int g4 = lane >> 2;
+                const int ca = 16 * tile + g4 < nc ? 16 * tile + g4 : nc - 1, cb = 16 * tile + 8 + g4 < nc ? 16 * tile + 8 + g4 : nc - 1;
+                const double* const rr[2] = {src + (ca + 1) * P, src + (cb + 1) * P};
+                const double* const rl[2] = {src + (ca - 1) * P, src + (cb - 1) * P};
+                small_item(opr, PR, K2, N, rr, rl, 16 * tile, t0, nb,
                            [&](int c, int r, double v0, double v1) {
                                if (c >= nc) return;
                                if (r < K2) {
@@ -296,8 +313,11 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
         for (int it = warp; it < ntile * ngr; it += nwarps) {
             const int tile = it / ngr, gr = it - tile * ngr;
             const int t0 = gr * SM_NBG, nb = nbt - t0 < SM_NBG ? nbt - t0 : SM_NBG;
-            small_item(opf, PR, K2, 16 * tile, t0, nb,
-                       [&](int c, int k) { return src + ((c < nc ? c : nc - 1) + (k < N ? 1 : -1)) * P + k; },
+            const int g4 = lane >> 2;
+            const int ca = 16 * tile + g4 < nc ? 16 * tile + g4 : nc - 1, cb = 16 * tile + 8 + g4 < nc ? 16 * tile + 8 + g4 : nc - 1;
+            const double* const rr[2] = {src + (ca + 1) * P, src + (cb + 1) * P};
+            const double* const rl[2] = {src + (ca - 1) * P, src + (cb - 1) * P};
+            small_item(opf, PR, K2, N, rr, rl, 16 * tile, t0, nb,
                        [&](int c, int r, double v0, double v1) {
                            if (c >= nc || r >= K2) return;
                            yfix[c * P + r] = ifix[c * P + r] + v0;          // z, in place of yfix
