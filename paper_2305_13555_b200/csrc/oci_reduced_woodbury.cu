@@ -499,8 +499,8 @@ constexpr int WT_CONS = 256;                       // consumer threads; + one pr
 constexpr int WT_WARPS = WT_CONS / 32;
 
 // (two CTAs of nine warps per SM put five warps on one SM partition: 16 K registers / 5 warps = 96 per thread)
-template <int PASS, int NT>
-__global__ void __launch_bounds__(WT_CONS + 32, 2)
+template <int PASS, int NT, int CONS>
+__global__ void __launch_bounds__(CONS + 32, CONS == 256 ? 2 : 4)
 oci_red_woodbury_tma_kernel(DevView V, const __grid_constant__ CUtensorMap map_y0, const __grid_constant__ CUtensorMap map_y1, int ybase,
                             int slot, int prev_slot, double tol, int cnt, int force)
 {
@@ -530,23 +530,24 @@ oci_red_woodbury_tma_kernel(DevView V, const __grid_constant__ CUtensorMap map_y
     }
     constexpr int N = NT, K2 = 2 * N, N2 = N >> 1;                         // N is a template parameter: every offset is an immediate
     const int J = (int)V.J;                                                // the launcher guarantees 32-bit element offsets
-    constexpr int gc = 1024 / N;                                           // cells per group (stage)
+    constexpr int WARPS = CONS / 32;                                       // consumer warps; + one producer warp
+    constexpr int gc = 4 * CONS / N;                                       // cells per group (stage)
     constexpr int U = 4;                                                   // cells per thread and group: gc N / 256
     constexpr int LDH = N + 4;                                             // pitch of a half-row box: 4 (mod 16) doubles
-    constexpr int KS = K2 / 4, KSW = KS / WT_WARPS;                        // k-steps of P inc, per warp
+    constexpr int KS = K2 / 4, KSW = KS / WARPS;                        // k-steps of P inc, per warp
     constexpr int NB = gc / 8;                                             // blocks of 8 cells
-    static_assert(KSW >= 1 && NB >= 1 && gc * N == U * WT_CONS, "shape");
+    static_assert(KSW >= 1 && NB >= 1 && gc * N == U * CONS && KSW * WARPS == KS, "shape");
     // stage: lo box [gc][LDH] | hi box [gc][LDH] | additive rows [gc][K2] | phifix [gc][4] | old phi [gc][4]
     constexpr int box_dbl = gc * LDH, fx_dbl = gc * K2;
     constexpr int stage_dbl = 2 * box_dbl + fx_dbl + (PASS == PASS_ITER ? 8 * gc : 0);
     static_assert((box_dbl * 8) % 128 == 0 && (stage_dbl * 8) % 128 == 0, "TMA destinations stay 128-byte aligned");
     double* ring = reinterpret_cast<double*>(wt_raw);
     double* part = ring + (size_t)WT_STAGES * stage_dbl;                   // [8 warps][gc][4] partial sums of phase A
-    double* s_sm = part + WT_WARPS * gc * 4;                               // [gc][4]
+    double* s_sm = part + WARPS * gc * 4;                               // [gc][4]
     uint64_t* full = reinterpret_cast<uint64_t*>(s_sm + gc * 4);
     uint64_t* empty = full + WT_STAGES;
     if (threadIdx.x == 0) {
-        for (int st = 0; st < WT_STAGES; ++st) { mbar_init(&full[st], 1); mbar_init(&empty[st], WT_WARPS); }
+        for (int st = 0; st < WT_STAGES; ++st) { mbar_init(&full[st], 1); mbar_init(&empty[st], WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -558,10 +559,10 @@ oci_red_woodbury_tma_kernel(DevView V, const __grid_constant__ CUtensorMap map_y
     int it0 = 0;                                                           // groups this CTA has streamed in earlier iterations
 
     // consumer-side constants
-    const bool consumer = warp < WT_WARPS;
+    const bool consumer = warp < WARPS;
     const int tid = consumer ? threadIdx.x : 0;
     const int m = tid % N, c0 = tid / N;                                   // angle; first cell slot (then c0 + 256/N, ...)
-    constexpr int cstep = WT_CONS / N;
+    constexpr int cstep = CONS / N;
     const int half = m >= N2, mm = m - half * N2;
     const int qk = pack_q(half, 0, mm, N), qe = pack_q(half, 1, mm, N);
     const double amu = fabs(V.mu[m]), wm = V.w[m];
@@ -646,14 +647,14 @@ oci_red_woodbury_tma_kernel(DevView V, const __grid_constant__ CUtensorMap map_y
                         *reinterpret_cast<double2*>(part + ((size_t)warp * gc + bq * 8 + g4) * 4 + 2 * t4) = make_double2(acc[bq][0], acc[bq][1]);
                 }
             }
-            named_bar_sync(1, WT_CONS);
+            named_bar_sync(1, CONS);
             if (tid < gc * 4) {
                 double sum = part[tid];
 #pragma unroll
-                for (int w = 1; w < WT_WARPS; ++w) sum += part[w * gc * 4 + tid];
+                for (int w = 1; w < WARPS; ++w) sum += part[w * gc * 4 + tid];
                 s_sm[tid] = sum;
             }
-            named_bar_sync(1, WT_CONS);
+            named_bar_sync(1, CONS);
             // ---- phase B: thread = (cell, angle), U cells per thread, two at a time
 #pragma unroll
             for (int h2 = 0; h2 < U; h2 += 2) {
@@ -927,11 +928,15 @@ void launch_wb_w(const DevView& V, int ybase, int slot, int prev_slot, double to
     else launch_wb_i<PASS, SHARED, TPB, W, int64_t>(V, ybase, slot, prev_slot, tol, cnt, force, s);
 }
 
+// consumer threads of a CTA: 128 (four CTAs per SM: the CTA barriers of one group overlap another CTA's work) where a
+// group of 4 * 128 / N cells still has a whole block of 8 cells, else 256
+int wt_cons(int N) { return N <= 64 ? 128 : 256; }
+
 size_t wt_smem(const DevView& V, int pass)
 {
-    const int N = V.N, gc = 1024 / N;
+    const int N = V.N, cons = wt_cons(N), gc = 4 * cons / N;
     const size_t stage = ((size_t)2 * gc * (N + 4) + (size_t)gc * 2 * N + (pass == PASS_ITER ? 8 * gc : 0)) * 8;
-    return WT_STAGES * stage + (size_t)(WT_WARPS + 1) * gc * 4 * 8 + 2 * WT_STAGES * 8 + 128;
+    return WT_STAGES * stage + (size_t)(cons / 32 + 1) * gc * 4 * 8 + 2 * WT_STAGES * 8 + 128;
 }
 
 // the TMA / tensor-pipe kernel: ITER / FINAL, one shared block, N in {16, 32, 64, 128}, 32-bit element offsets, and enough
@@ -949,8 +954,9 @@ bool wt_serves(const DevView& V, int pass)
 template <int PASS, int NT>
 void launch_wt_w(const DevView& V, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
 {
+    constexpr int CONS = NT <= 64 ? 128 : 256;
     const size_t smem = wt_smem(V, PASS);
-    const int gc = 1024 / NT, K2 = 2 * NT;
+    const int gc = 4 * CONS / NT, K2 = 2 * NT;
     CUtensorMap m0, m1;
     if (!oci_encode_2d(&m0, V.y[0] - K2, (uint64_t)V.J + 2, K2, gc, NT + 4, false) ||
         !oci_encode_2d(&m1, V.y[1] - K2, (uint64_t)V.J + 2, K2, gc, NT + 4, false)) {
@@ -959,17 +965,17 @@ void launch_wt_w(const DevView& V, int ybase, int slot, int prev_slot, double to
     }
     const int64_t groups = (V.J + gc - 1) / gc;
     int per_sm = 1;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, oci_red_woodbury_tma_kernel<PASS, NT>, WT_CONS + 32, smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, oci_red_woodbury_tma_kernel<PASS, NT, CONS>, CONS + 32, smem);
     if (per_sm < 1) per_sm = 1;
     const int64_t cap = (int64_t)V.sm_count * per_sm;
     const unsigned grid = (unsigned)(groups < cap ? groups : cap);
     if (PASS == PASS_ITER && cnt > 1) {
         DevView Vv = V;
         void* args[] = {&Vv, &m0, &m1, &ybase, &slot, &prev_slot, &tol, &cnt, &force};
-        cudaLaunchCooperativeKernel((const void*)oci_red_woodbury_tma_kernel<PASS, NT>, dim3(grid), dim3(WT_CONS + 32), args, smem, s);
+        cudaLaunchCooperativeKernel((const void*)oci_red_woodbury_tma_kernel<PASS, NT, CONS>, dim3(grid), dim3(CONS + 32), args, smem, s);
         return;
     }
-    oci_red_woodbury_tma_kernel<PASS, NT><<<grid, WT_CONS + 32, smem, s>>>(V, m0, m1, ybase, slot, prev_slot, tol, cnt, force);
+    oci_red_woodbury_tma_kernel<PASS, NT, CONS><<<grid, CONS + 32, smem, s>>>(V, m0, m1, ybase, slot, prev_slot, tol, cnt, force);
 }
 
 size_t wf_smem(int N)
@@ -1050,8 +1056,9 @@ cudaError_t wt_opt_in()
 {
     const auto at = cudaFuncAttributeMaxDynamicSharedMemorySize;
     const int bytes = 160 * 1024;
-    cudaError_t e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_ITER, NT>, at, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_FINAL, NT>, at, bytes);
+    constexpr int CONS = NT <= 64 ? 128 : 256;
+    cudaError_t e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_ITER, NT, CONS>, at, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(oci_red_woodbury_tma_kernel<PASS_FINAL, NT, CONS>, at, bytes);
     return e != cudaSuccess ? e : cudaFuncSetAttribute(oci_red_woodbury_fix_kernel<NT>, at, bytes);
 }
 }  // namespace
