@@ -21,7 +21,10 @@ __device__ __forceinline__ void clear_step_state(const DevView& V)
 {
     if (blockIdx.x == 0) {
         for (int i = threadIdx.x; i < 2 * kNormSlots; i += blockDim.x) V.norms[i] = 0ull;
-        if (threadIdx.x == 0) V.flags[8] = 0;          // arrival counter of the grid-wide barrier
+        if (threadIdx.x == 0) {
+            V.flags[8] = 0;                            // arrival counter of the grid-wide barrier
+            V.flags[12] = 0;                           // ticket counter of the fused loops that hand out work dynamically
+        }
     }
 }
 

@@ -485,7 +485,7 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
         // that a large problem's FINAL pass would wait for, while its host part overlaps that pass anyway)
         const bool polled = fused_loop && !timed && ctx->d_pub != nullptr && ctx->J * ctx->n <= 262144;
         if (fused_loop) {
-            if (done_iters > 0) CK(cudaMemsetAsync(V.flags + 8, 0, 4, s));  // the grid barrier's arrival counter
+            if (done_iters > 0) CK(cudaMemsetAsync(V.flags + 8, 0, 20, s));  // the grid barrier's arrival counter, the work tickets
             if (timed) CK(cudaEventRecord(ctx->ev[0], s));
             if (polled) { V.host_pub = ctx->d_pub; V.pub_seq = ++ctx->pub_seq; }
             LAUNCH(launch_reduced_pass(ctx, PASS_ITER, (ctx->ycur + done_iters) & 1, 0, -1, tol, cnt, 0));

@@ -46,7 +46,7 @@ struct DevView {
     double* phi_part;           // [ceil(n/128)][J][4]  per-item scalar-flux partials (K-tiled kernel)
     int32_t* tickets;           // [ceil(J/64)]  arrival counters of the K-tiled kernel's cell tiles (0 between launches)
     unsigned long long* norms;  // [kNormSlots][2]  bit patterns of (d, r), atomicMax targets
-    int32_t* flags;             // [0] = 1 + index of a singular block, 0 if none; [8] grid-barrier counter of the fused loops
+    int32_t* flags;             // [0] = 1 + index of a singular block, 0 if none; [8] grid-barrier counter of the fused loops; [12] their work-ticket counter
     int32_t* perm;              // [nblk][n]  pivot rows of the blocked inversion (setup)
     int32_t* team_bar;          // [min(nblk, SMs)]  team-barrier counters of the blocked inversion (setup)
     // ---- interface-reduced step (oci_reduced.cu), K2 = 2N

@@ -161,7 +161,7 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
     // state, the FIX input vectors [y(k+1/2 run) | z(k+1/2 run) | Q], the old scalar flux
     if (rank == 0) {
         for (int i = tid; i < 2 * kNormSlots; i += SM_THREADS) V.norms[i] = 0ull;
-        if (tid == 0) V.flags[8] = 0;
+        if (tid == 0) { V.flags[8] = 0; V.flags[12] = 0; }
     }
     for (int e = tid; e < L.mx * (K2 + 4); e += SM_THREADS) {
         const int r = e / (K2 + 4), u = e - r * (K2 + 4);

@@ -546,6 +546,7 @@ oci_red_woodbury_tma_kernel(DevView V, const __grid_constant__ CUtensorMap map_y
     double* s_sm = part + WARPS * gc * 4;                               // [gc][4]
     uint64_t* full = reinterpret_cast<uint64_t*>(s_sm + gc * 4);
     uint64_t* empty = full + WT_STAGES;
+    volatile int* grp_s = reinterpret_cast<volatile int*>(empty + WT_STAGES);   // first cell of the group in a stage, -1: no more
     if (threadIdx.x == 0) {
         for (int st = 0; st < WT_STAGES; ++st) { mbar_init(&full[st], 1); mbar_init(&empty[st], WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -553,7 +554,13 @@ oci_red_woodbury_tma_kernel(DevView V, const __grid_constant__ CUtensorMap map_y
     __syncthreads();
 
     const int ngroups = (J + gc - 1) / gc;
-    const int my_groups = (int)blockIdx.x < ngroups ? (ngroups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+    // Which groups a CTA takes.  Inside the fused loop (grid-wide barrier per iteration) they are handed out by a global
+    // ticket counter, so that a CTA that runs ahead takes more and all reach the barrier together; iteration l owns the
+    // tickets [l (ngroups + grid), +ngroups), and every CTA draws exactly one ticket past the end per iteration.  A
+    // single pass (FINAL, one iteration per launch) takes them strided.  The producer announces the group of a stage
+    // in shared memory (-1: no more) before it arms the stage.
+    const bool dynamic = PASS == PASS_ITER && cnt > 1;
+    int* ticket = V.flags + 12;
     const int nloop = PASS == PASS_ITER ? (cnt > 1 ? cnt : 1) : 1;
     const double* __restrict__ fx = PASS == PASS_ITER ? V.yfix : V.ifix;
     int it0 = 0;                                                           // groups this CTA has streamed in earlier iterations
@@ -605,10 +612,19 @@ oci_red_woodbury_tma_kernel(DevView V, const __grid_constant__ CUtensorMap map_y
         // ---- producer: one elected lane streams this CTA's groups of this iteration
         if (lane == 0) {
             if (l > 0) asm volatile("fence.proxy.async;" ::: "memory");   // rows other SMs stored before the grid barrier
-            for (int i = 0; i < my_groups; ++i) {
+            for (int i = 0;; ++i) {
                 const int u = it0 + i, st = u % WT_STAGES;
+                int g = (int)blockIdx.x + i * (int)gridDim.x;
+                if (dynamic) g = atomicAdd(ticket, 1) - l * (ngroups + (int)gridDim.x);
                 if (u >= WT_STAGES) mbar_wait(&empty[st], ((u / WT_STAGES) - 1) & 1);
-                const int j0 = ((int)blockIdx.x + i * (int)gridDim.x) * gc;
+                if (g >= ngroups) {                                        // no more groups in this iteration
+                    grp_s[st] = -1;
+                    mbar_arrive(&full[st]);
+                    it0 = u + 1;
+                    break;
+                }
+                const int j0 = g * gc;
+                grp_s[st] = j0;
                 const int rows = J - j0 < gc ? J - j0 : gc;
                 double* sg = ring + (size_t)st * stage_dbl;
                 const uint32_t fb = (uint32_t)rows * K2 * 8, pb = (uint32_t)rows * 32;
@@ -624,11 +640,17 @@ oci_red_woodbury_tma_kernel(DevView V, const __grid_constant__ CUtensorMap map_y
         }
     } else {
         double dmax = 0.0, rmax = 0.0;
-        for (int i = 0; i < my_groups; ++i) {
+        for (int i = 0;; ++i) {
             const int u = it0 + i, st = u % WT_STAGES;
-            const int j0 = ((int)blockIdx.x + i * (int)gridDim.x) * gc;
             const double* sg = ring + (size_t)st * stage_dbl;
             mbar_wait(&full[st], (u / WT_STAGES) & 1);
+            const int j0 = grp_s[st];
+            if (j0 < 0) {                                                  // (uniform over the CTA) the iteration's last stage
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[st]);
+                it0 = u + 1;
+                break;
+            }
             // ---- phase A: partial s = P inc over this warp's k-steps, all blocks of 8 cells
             {
                 double acc[NB][2];
@@ -713,7 +735,6 @@ oci_red_woodbury_tma_kernel(DevView V, const __grid_constant__ CUtensorMap map_y
             }
         }
     }
-    it0 += my_groups;
     if (PASS == PASS_ITER && nloop > 1) {
         // grid-wide barrier (cooperative launch), then the stopping rule on the now final norms (a7)
         __threadfence();
@@ -936,7 +957,7 @@ size_t wt_smem(const DevView& V, int pass)
 {
     const int N = V.N, cons = wt_cons(N), gc = 4 * cons / N;
     const size_t stage = ((size_t)2 * gc * (N + 4) + (size_t)gc * 2 * N + (pass == PASS_ITER ? 8 * gc : 0)) * 8;
-    return WT_STAGES * stage + (size_t)(cons / 32 + 1) * gc * 4 * 8 + 2 * WT_STAGES * 8 + 128;
+    return WT_STAGES * stage + (size_t)(cons / 32 + 1) * gc * 4 * 8 + 2 * WT_STAGES * 8 + WT_STAGES * 4 + 128;
 }
 
 // the TMA / tensor-pipe kernel: ITER / FINAL, one shared block, N in {16, 32, 64, 128}, 32-bit element offsets, and enough
