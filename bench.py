@@ -225,72 +225,106 @@ class CpuBlasReduced:
     """A TUNED CPU restatement of the algorithm the GPU arm runs, for a fair CPU figure next to the (deliberately
     plain) oracle: shared block, the block inverse formed once with LAPACK, and the interface-reduced iteration of
     DESIGN.md 6.7 - y^(l+1) = yfix + inc G^T, phi^(l+1) = phifix + inc H^T - as two threaded BLAS dgemms per
-    iteration at the FULL cell count.  The matrix B comes from the oracle's `cell_matrix` (this is bench.py's CPU
-    leg, the one place outside tests/ that may call oracle/); everything else is numpy.  Not used for parity."""
+    iteration at the FULL cell count.  The state is kept PACKED the whole time ([O | I] columns, each run a contiguous
+    slice: no strided or fancy-indexed passes inside a step), the work arrays are allocated once and the dgemms write
+    in place.  The matrix B comes from the oracle's `cell_matrix` (this is bench.py's CPU leg, the one place outside
+    tests/ that may call oracle/); everything else is numpy.  Not used for parity."""
 
     def __init__(self, p):
         from oracle import cell_matrix, gauss_legendre
         assert np.all(p.dx == p.dx[0]) and np.all(p.sigma_t == p.sigma_t[0]) and np.all(p.sigma_s == p.sigma_s[0])
         self.p, N, J = p, p.n_angles, p.cells
         self.mu, self.w = gauss_legendre(N)
-        h = float(p.dx[0])
+        h, hN = float(p.dx[0]), N // 2
         Binv = np.linalg.inv(cell_matrix(self.mu, self.w, h, float(p.sigma_t[0]), float(p.sigma_s[0]), p.v, p.dt))
         m = np.arange(N)
-        neg = self.mu < 0
-        # I: rows that receive an incident flux (k slot, then k+1/2 slot); O = the partner slots a neighbour reads
-        self.I = np.concatenate([4 * m + np.where(neg, 1, 0), 4 * m + np.where(neg, 3, 2)])
+        neg, pos = m[self.mu < 0], m[self.mu > 0]
+        assert np.array_equal(neg, m[:hN]) and np.array_equal(pos, m[hN:])      # ascending Gauss-Legendre set
+        # I: rows that receive an incident flux, ordered [k | k+1/2 of mu < 0, k | k+1/2 of mu > 0] so that the gather
+        # of the neighbours' values is two contiguous half-row slices; O = the partner slots a neighbour reads.
+        # Every run of hN columns of [O | I] is (one sign of mu, one slot); runs 2r and 2r+1 are slots k and k+1/2.
+        self.I = np.concatenate([4 * neg + 1, 4 * neg + 3, 4 * pos + 0, 4 * pos + 2])
         self.O = self.I ^ 1
-        self.from_right = np.concatenate([neg, neg])                 # mu < 0: the value comes from cell j+1
-        amu = np.abs(np.concatenate([self.mu, self.mu]))
+        self.perm = np.concatenate([self.O, self.I])
+        self.nr = N                                                  # columns [0, nr) of inc: the value comes from cell j+1
+        amu = np.abs(self.mu[self.I >> 2])
         W = np.zeros((4, 4 * N))
         for s_ in range(4):
             W[s_, 4 * m + s_] = self.w
         self.G = np.ascontiguousarray((Binv[np.ix_(self.O, self.I)] * amu).T)        # [2N][2N], applied as inc @ G
         self.H = np.ascontiguousarray(((W @ Binv)[:, self.I] * amu).T)               # [2N][4]
-        self.Binv, self.W, self.alpha, self.h = Binv, W, h / (2 * p.v * p.dt), h
-        self.mirror = np.concatenate([N - 1 - m, N + (N - 1 - m)])   # packed index of the mirror angle, same time slot
-        self.Y = np.zeros((J + 2, 2 * N))                            # O rows of the iterate with ghost rows 0 and J+1
+        self.F = np.ascontiguousarray((Binv[np.ix_(self.I, self.I)] * amu).T)        # [2N][2N], the FINAL pass
+        # phi rides along as four more columns of the iteration operator and of the FIX operator: one dgemm each
+        self.GH = np.ascontiguousarray(np.hstack([self.G, self.H]))                  # [2N][2N + 4]
+        WB = (W @ Binv)[:, self.perm]
+        self.Bp = np.ascontiguousarray(np.vstack([Binv[np.ix_(self.O, self.perm)], WB,
+                                                  Binv[np.ix_(self.I, self.perm)]]).T)   # packed c_fix -> [O | phi | I]
+        self.W, self.alpha, self.h = W, h / (2 * p.v * p.dt), h
+        where = {(int(i) >> 2, (int(i) >> 1) & 1): k for k, i in enumerate(self.I)}
+        self.mirror = np.array([where[(N - 1 - (int(i) >> 2), (int(i) >> 1) & 1)] for i in self.I])
         psi = np.empty((J, N, 4))
         psi[:, :, 0] = psi[:, :, 2] = p.psi0[:, :, 0]
         psi[:, :, 1] = psi[:, :, 3] = p.psi0[:, :, 1]
-        self.Psi = psi.reshape(J, 4 * N)
-        self.phi = self.Psi @ W.T
+        psi = psi.reshape(J, 4 * N)
+        # [O columns | phi], ghost rows 0 and J+1
+        self.Y, self.Ynew = np.zeros((J + 2, 2 * N + 4)), np.zeros((J + 2, 2 * N + 4))
+        self.Ip = np.ascontiguousarray(psi[:, self.I])                            # I columns
+        self.Y[1:-1, :2 * N] = psi[:, self.O]
+        self.Y[1:-1, 2 * N:] = psi @ W.T
+        # work arrays, allocated once
+        self.cfix, self.fix = np.zeros((J, 4 * N)), np.empty((J, 4 * N + 4))
+        self.inc, self.dphi = np.empty((J, 2 * N)), np.empty((J, 4))
+
+    @property
+    def phi(self):
+        return self.Y[1:-1, 2 * self.p.n_angles:]
+
+    @property
+    def Psi(self):
+        """The angular flux [J][4N] in the library's layout (unpacked on demand)."""
+        out = np.empty((self.p.cells, 4 * self.p.n_angles))
+        out[:, self.O], out[:, self.I] = self.Y[1:-1, :2 * self.p.n_angles], self.Ip
+        return out
 
     def _ghosts(self):
         p, Y = self.p, self.Y
         for side, bc, row, src in ((0, p.bc_left, 0, 1), (1, p.bc_right, -1, -2)):
             if bc[0] == 2:
-                Y[row] = Y[src][self.mirror]
+                Y[row, :self.mirror.size] = Y[src][self.mirror]
             else:
-                Y[row] = bc[1] if bc[0] == 1 else 0.0
+                Y[row, :self.mirror.size] = bc[1] if bc[0] == 1 else 0.0
 
     def step(self, q, tol, max_iters):
-        p, J, N = self.p, self.p.cells, self.p.n_angles
-        cfix = np.zeros((J, 4 * N))
+        p, J, N, nr, hN = self.p, self.p.cells, self.p.n_angles, self.nr, self.p.n_angles // 2
+        cfix, fix, inc, dphi = self.cfix, self.fix, self.inc, self.dphi
+        # c_fix in packed columns: rows (k, .) take alpha * the committed k+1/2 value of the same angle, plus (h/4) Q
+        c4 = cfix.reshape(J, 4, 2, hN)
+        for r_ in range(2):
+            np.multiply(self.Y[1:-1, (2 * r_ + 1) * hN:(2 * r_ + 2) * hN], self.alpha, out=c4[:, r_, 0, :])
+        np.multiply(self.Ip.reshape(J, 2, 2, hN)[:, :, 1, :], self.alpha, out=c4[:, 2:4, 0, :])
+        c4[:, :, 1, :] = 0.0
         if q is not None:
-            cfix += 0.25 * self.h * np.tile(q, (1, N))
-        prev = self.Psi.reshape(J, N, 4)[:, :, 2:]
-        cfix.reshape(J, N, 4)[:, :, :2] += self.alpha * prev
-        fix = cfix @ self.Binv.T                                       # Psi_fix, once per step
-        yfix, phifix = np.ascontiguousarray(fix[:, self.O]), fix @ self.W.T
-        self.Y[1:-1] = self.Psi[:, self.O]
-        inc = np.empty((J, 2 * N))
+            cfix += np.take(0.25 * self.h * np.asarray(q), self.perm & 3, axis=1)
+        np.matmul(cfix, self.Bp, out=fix)                              # [yfix | phifix | ifix], once per step
+        yfix, ifix = fix[:, :2 * N + 4], fix[:, 2 * N + 4:]
         it, d, r = 0, 0.0, 0.0
         while it < max_iters:
             self._ghosts()
-            inc[:, self.from_right] = self.Y[2:, self.from_right]
-            inc[:, ~self.from_right] = self.Y[:-2, ~self.from_right]
-            ynew = yfix + inc @ self.G
-            phinew = phifix + inc @ self.H
-            d, r = np.max(np.abs(phinew - self.phi)), np.max(np.abs(phinew))
-            self.Y[1:-1], self.phi = ynew, phinew
+            inc[:, :nr] = self.Y[2:, :nr]
+            inc[:, nr:] = self.Y[:-2, nr:2 * N]
+            ynew = self.Ynew[1:-1]
+            np.matmul(inc, self.GH, out=ynew)
+            ynew += yfix
+            phinew = ynew[:, 2 * N:]
+            np.subtract(phinew, self.phi, out=dphi)
+            d, r = max(dphi.max(), -dphi.min()), max(phinew.max(), -phinew.min())
+            self.Y, self.Ynew = self.Ynew, self.Y
             it += 1
             if tol >= 0 and d <= tol * r:
                 break
         # the I rows of the converged iterate from the last gathered inc (the FINAL pass)
-        F = (self.Binv[np.ix_(self.I, self.I)] * np.abs(np.concatenate([self.mu, self.mu]))).T
-        self.Psi[:, self.O] = self.Y[1:-1]
-        self.Psi[:, self.I] = fix[:, self.I] + inc @ F
+        np.matmul(inc, self.F, out=self.Ip)
+        self.Ip += ifix
         return it
 
 
