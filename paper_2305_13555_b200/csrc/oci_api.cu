@@ -825,9 +825,10 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
         if (ctx->small_mode == 1) {
             if (C == 0) return fail(ctx, OCI_E_INVALID, "oci_set_small_step(1): the one-launch step does not serve this problem");
             ctx->small_cluster = C;
-        } else if (ctx->small_mode == -1 && ctx->forced_rkernel == OCI_RKERNEL_AUTO && C == 1) {
-            // measured: the one-CTA form wins (config 1: 0.070 -> 0.05 ms per step); the cluster form is not there yet
-            // (config 2: 0.148 vs 0.096 ms: shared-memory bound DFMA loops on 8 SMs), so it runs on request only
+        } else if (ctx->small_mode == -1 && ctx->forced_rkernel == OCI_RKERNEL_AUTO && (C == 1 || C == 16)) {
+            // measured: the one-CTA form wins (config 1: 0.064 -> 0.039 ms per step) and so does a cluster of 16 CTAs
+            // where the device schedules one (config 2: 0.088 -> 0.072 ms; every size it serves: DESIGN.md 6.9); a
+            // cluster of 8 is level with the three-pass kernels and runs on request only
             ctx->small_cluster = C;
         }
     }

@@ -32,7 +32,8 @@ namespace oci {
 namespace {
 
 constexpr int SM_MAX_THREADS = 256;                        // CTA size is chosen at launch: one warp per work item, 8 at most
-constexpr int SM_NBG = 5;                                  // n8 blocks of operator rows per work item (40 rows)
+constexpr int SM_NBG = 5;                                  // n8 blocks of operator rows per work item (40 rows) at most
+constexpr int SM_MAX_CLUSTER = 16;                         // 8 is the portable limit; 16 where the device schedules it
 
 // smallest pitch >= k that is 4 (mod 16) doubles: fragment loads of 8 rows x 4 columns hit 32 distinct banks
 __host__ __device__ inline int sm_pitch(int k) { return k + ((4 - k) % 16 + 16) % 16; }
@@ -67,7 +68,7 @@ __host__ __device__ inline SmallLayout small_layout(int N, int Jc)
     L.phifix = take(Jc * 4);
     L.phi = take(Jc * 4);
     L.red = take(2 * (SM_MAX_THREADS / 32));
-    L.pub = take(2 * 8 * 2);                               // [parity][rank][d, r] published by every CTA of the cluster
+    L.pub = take(2 * SM_MAX_CLUSTER * 2);                  // [parity][rank][d, r] published by every CTA of the cluster
     L.total = o;
     return L;
 }
@@ -128,7 +129,8 @@ __device__ __forceinline__ void small_item(const double* __restrict__ op, int op
 
 }  // namespace
 
-__global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevView V, int ybase, double tol, int cnt, int force)
+// nbg: n8 blocks of operator rows per work item (<= SM_NBG), chosen by the launcher so that the warps of a CTA all get work
+__global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevView V, int ybase, double tol, int cnt, int force, int nbg)
 {
     extern __shared__ __align__(32) double ssm[];
     cg::cluster_group cluster = cg::this_cluster();
@@ -197,10 +199,10 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
 
     // ---- FIX: [yfix | ifix | phifix][c] = X [psi_{k-1/2}[c]; Q[c]]   (psi_{k-1/2} = the k+1/2 runs of y and z)
     {
-        const int nbt = L.mx / 8, ngr = (nbt + SM_NBG - 1) / SM_NBG;
+        const int nbt = L.mx / 8, ngr = (nbt + nbg - 1) / nbg;
         for (int it = warp; it < ntile * ngr; it += nwarps) {
             const int tile = it / ngr, gr = it - tile * ngr;
-            const int t0 = gr * SM_NBG, nb = nbt - t0 < SM_NBG ? nbt - t0 : SM_NBG;
+            const int t0 = gr * nbg, nb = nbt - t0 < nbg ? nbt - t0 : nbg;
             const int g4 = lane >> 2;
             const int ca = 16 * tile + g4 < nc ? 16 * tile + g4 : nc - 1, cb = 16 * tile + 8 + g4 < nc ? 16 * tile + 8 + g4 : nc - 1;
             const double* const rows[2] = {xin + ca * P, xin + cb * P};    // (a ragged tile's missing cells: clamped, dropped)
@@ -215,26 +217,22 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
     }
     __syncthreads();
 
-    // ghost rows of buffer `b` (the iterate the next iteration reads): the neighbour CTA's edge row, or the boundary
-    auto fill_ghosts = [&](int b) {
-        for (int q = tid; q < 2 * K2; q += SM_THREADS) {
+    // ghost rows of buffer `b` (the iterate the next iteration reads), written BEFORE the cluster barrier: every CTA
+    // pushes its two edge rows into its neighbours' ghost rows (DSMEM stores; a remote load after the barrier would add its
+    // round trip to every iteration) and the CTAs at the ends of the slab apply the boundary condition to their own.
+    // Nobody reads buffer b during the iteration that writes it, and the barrier orders the stores before the reads.
+    auto push_ghosts = [&](int b) {
+        for (int q = SM_THREADS - 1 - tid; q < 2 * K2; q += SM_THREADS) {   // from the last warp down: warp 0 publishes the norms
             const bool left = q < K2;
             const int qq = left ? q : q - K2;
-            double v;
             if (left) {
-                if (rank > 0) {
-                    const double* nb = cluster.map_shared_rank(ybuf[b], rank - 1);
-                    v = nb[(Jc - 1) * P + qq];                            // every CTA but the last holds Jc cells
-                } else if (V.bcL == OCI_BC_REFLECTING) v = qq >= N ? ybuf[b][mirror_q(qq, N)] : 0.0;
-                else v = V.bcL == OCI_BC_INCIDENT_ISOTROPIC ? V.bcLv : 0.0;
-                ybuf[b][-P + qq] = v;
+                if (rank > 0) cluster.map_shared_rank(ybuf[b], rank - 1)[Jc * P + qq] = ybuf[b][qq];   // every CTA but the last holds Jc cells
+                else ybuf[b][-P + qq] = V.bcL == OCI_BC_REFLECTING ? (qq >= N ? ybuf[b][mirror_q(qq, N)] : 0.0)
+                                                                    : (V.bcL == OCI_BC_INCIDENT_ISOTROPIC ? V.bcLv : 0.0);
             } else {
-                if (j0 + nc < J) {
-                    const double* nb = cluster.map_shared_rank(ybuf[b], rank + 1);
-                    v = nb[qq];
-                } else if (V.bcR == OCI_BC_REFLECTING) v = qq < N ? ybuf[b][(nc - 1) * P + mirror_q(qq, N)] : 0.0;
-                else v = V.bcR == OCI_BC_INCIDENT_ISOTROPIC ? V.bcRv : 0.0;
-                ybuf[b][nc * P + qq] = v;
+                if (j0 + nc < J) cluster.map_shared_rank(ybuf[b], rank + 1)[-P + qq] = ybuf[b][(nc - 1) * P + qq];
+                else ybuf[b][nc * P + qq] = V.bcR == OCI_BC_REFLECTING ? (qq < N ? ybuf[b][(nc - 1) * P + mirror_q(qq, N)] : 0.0)
+                                                                       : (V.bcR == OCI_BC_INCIDENT_ISOTROPIC ? V.bcRv : 0.0);
             }
         }
     };
@@ -249,10 +247,10 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
         double* __restrict__ dst = ybuf[(l + 1) & 1];
         double dmax = 0.0, rmax = 0.0;
         {
-            const int nbt = L.mr / 8, ngr = (nbt + SM_NBG - 1) / SM_NBG;
+            const int nbt = L.mr / 8, ngr = (nbt + nbg - 1) / nbg;
             for (int it = warp; it < ntile * ngr; it += nwarps) {
                 const int tile = it / ngr, gr = it - tile * ngr;
-                const int t0 = gr * SM_NBG, nb = nbt - t0 < SM_NBG ? nbt - t0 : SM_NBG;
+                const int t0 = gr * nbg, nb = nbt - t0 < nbg ? nbt - t0 : nbg;
                 // q < N: the right neighbour's outgoing flux, q >= N: the left neighbour's (a ragged tile's missing
                 // cells: clamped, their results dropped)
                 const int g4 = lane >> 2;
@@ -281,24 +279,27 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
         rmax = warp_max(rmax);
         if (lane == 0) { red[2 * warp] = dmax; red[2 * warp + 1] = rmax; }
         __syncthreads();
-        if (tid == 0) {
-            for (int w = 1; w < SM_THREADS / 32; ++w) { dmax = nanmax(dmax, red[2 * w]); rmax = nanmax(rmax, red[2 * w + 1]); }
-            for (int r = 0; r < C; ++r) {
-                double* pr = cluster.map_shared_rank(pub, r) + (l & 1) * 16 + 2 * rank;
+        if (warp == 0) {                                                  // lane w: warp w's pair; lane r publishes to rank r
+            dmax = warp_max(lane < nwarps ? red[2 * lane] : 0.0);
+            rmax = warp_max(lane < nwarps ? red[2 * lane + 1] : 0.0);
+            if (lane < C) {
+                double* pr = cluster.map_shared_rank(pub, lane) + (l & 1) * 2 * SM_MAX_CLUSTER + 2 * rank;
                 pr[0] = dmax;
                 pr[1] = rmax;
             }
         }
-        if (C > 1) cluster.sync();                                        // every CTA's y^(l+1) and norms are in place
+        push_ghosts((l + 1) & 1);
+        if (C > 1) cluster.sync();                                        // every CTA's y^(l+1), ghost rows and norms are in place
         else __syncthreads();
         double d = 0.0, r = 0.0;
-        for (int k = 0; k < C; ++k) { d = nanmax(d, pub[(l & 1) * 16 + 2 * k]); r = nanmax(r, pub[(l & 1) * 16 + 2 * k + 1]); }
+        for (int k = 0; k < C; ++k) {
+            d = nanmax(d, pub[(l & 1) * 2 * SM_MAX_CLUSTER + 2 * k]);
+            r = nanmax(r, pub[(l & 1) * 2 * SM_MAX_CLUSTER + 2 * k + 1]);
+        }
         if (rank == 0 && tid == 0) {                                      // a7: the host reads the norm slots once per step
             V.norms[2 * l + 0] = (unsigned long long)__double_as_longlong(d);
             V.norms[2 * l + 1] = (unsigned long long)__double_as_longlong(r);
         }
-        fill_ghosts((l + 1) & 1);
-        __syncthreads();
         Lit = l + 1;
         if (stop_now(tol, d, r)) conv = true;
         if ((conv || l + 1 == cnt) && rank == 0 && tid == 0) publish_step(V, Lit, l);   // (this thread wrote slot l itself)
@@ -309,10 +310,10 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
     // ---- FINAL: z = ifix + F inc^(L-1), staged in shared memory (yfix is dead) for a coalesced store
     if (finalize) {
         const double* __restrict__ src = ybuf[(Lit + 1) & 1];             // y^(L-1) with the ghost rows iteration L-1 read
-        const int nbt = L.mf / 8, ngr = (nbt + SM_NBG - 1) / SM_NBG;
+        const int nbt = L.mf / 8, ngr = (nbt + nbg - 1) / nbg;
         for (int it = warp; it < ntile * ngr; it += nwarps) {
             const int tile = it / ngr, gr = it - tile * ngr;
-            const int t0 = gr * SM_NBG, nb = nbt - t0 < SM_NBG ? nbt - t0 : SM_NBG;
+            const int t0 = gr * nbg, nb = nbt - t0 < nbg ? nbt - t0 : nbg;
             const int g4 = lane >> 2;
             const int ca = 16 * tile + g4 < nc ? 16 * tile + g4 : nc - 1, cb = 16 * tile + 8 + g4 < nc ? 16 * tile + 8 + g4 : nc - 1;
             const double* const rr[2] = {src + (ca + 1) * P, src + (cb + 1) * P};
@@ -355,6 +356,52 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
     if (C > 1) cluster.sync();                                            // nobody leaves while a neighbour may still read its rows
 }
 
+namespace {
+// blocks of operator rows per work item and CTA size: one warp per work item of an iteration in the busiest CTA, 8 warps at
+// most (for a tiny problem every barrier and every serial reduction over the warps is pure latency); a tile's operator
+// rows are split into as many equal groups as it takes to give every warp an item
+void small_shape(const DevView& V, int C, int* nbg, int* threads)
+{
+    const int Jc = (int)((V.J + C - 1) / C), ntile = (Jc + 15) / 16, nbt = (2 * V.N + 4 + 7) / 8;
+    int groups = (SM_MAX_THREADS / 32 + ntile - 1) / ntile;
+    groups = groups > nbt ? nbt : groups;
+    const int per = (nbt + groups - 1) / groups;
+    *nbg = per > SM_NBG ? SM_NBG : per;
+    const int items = ntile * ((nbt + *nbg - 1) / *nbg);
+    *threads = items * 32 > SM_MAX_THREADS ? SM_MAX_THREADS : items * 32;
+}
+
+void small_config(const DevView& V, int C, cudaLaunchConfig_t* cfg, cudaLaunchAttribute* at, int* nbg)
+{
+    int threads;
+    small_shape(V, C, nbg, &threads);
+    *cfg = cudaLaunchConfig_t{};
+    cfg->gridDim = dim3((unsigned)C);
+    cfg->blockDim = dim3((unsigned)threads);
+    cfg->dynamicSmemBytes = (size_t)small_layout(V.N, (int)((V.J + C - 1) / C)).total * 8;
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)C;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg->attrs = at;
+    cfg->numAttrs = 1;
+}
+
+// clusters of more than 8 CTAs are not portable: ask the device whether it can co-schedule one
+bool small_cluster_fits(const DevView& V, int C)
+{
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute at[1];
+    int nbg, n = 0;
+    small_config(V, C, &cfg, at, &nbg);
+    if (cudaOccupancyMaxActiveClusters(&n, oci_red_small_kernel, &cfg) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return n >= 1;
+}
+}  // namespace
+
 // Cluster size that serves this problem, 0 if the one-launch step does not (oci_step then uses the three-pass kernels)
 int oci_red_small_cluster(const DevView& V)
 {
@@ -363,42 +410,32 @@ int oci_red_small_cluster(const DevView& V)
     if (V.N > 64) return 0;                                               // the operators alone would fill shared memory
     const int64_t work = V.J * (K2 + 4) * K2;                             // multiply-adds of one iteration
     if (work > 4000000) return 0;                                         // large enough for the grid-wide kernels to win
-    for (int C = work <= 65536 ? 1 : 8; C >= 1; C >>= 1) {
+    for (int C = work <= 65536 ? 1 : SM_MAX_CLUSTER; C >= 1; C >>= 1) {
         if (C > 1 && V.J < 8 * C) continue;                               // at least 8 cells per CTA
         const int Jc = (int)((V.J + C - 1) / C);
         if ((int64_t)(C - 1) * Jc >= V.J) continue;                       // the last CTA must own a cell
-        if ((size_t)small_layout(V.N, Jc).total * 8 <= 220 * 1024) return C;
-        if (C == 1) break;
+        if ((size_t)small_layout(V.N, Jc).total * 8 > 220 * 1024) continue;
+        if (C > 8 && !small_cluster_fits(V, C)) continue;
+        return C;
     }
     return 0;
 }
 
 cudaError_t oci_red_small_opt_in()
 {
-    return cudaFuncSetAttribute(oci_red_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+    cudaError_t e = cudaFuncSetAttribute(oci_red_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(oci_red_small_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
 }
 
 int launch_red_small(const DevView& V, int C, int ybase, double tol, int cnt, int force, cudaStream_t s)
 {
-    const int Jc = (int)((V.J + C - 1) / C);
-    cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)C);
-    // one warp per work item of an iteration (tile of 16 cells x up to 40 operator rows) in the busiest CTA, 8 at most:
-    // for a tiny problem every barrier and every serial reduction over the warps is pure latency
-    const int64_t items = (int64_t)((Jc + 15) / 16) * (((2 * V.N + 4 + 7) / 8 + SM_NBG - 1) / SM_NBG);
-    int threads = (int)(items * 32);
-    threads = threads < 32 ? 32 : threads > SM_MAX_THREADS ? SM_MAX_THREADS : threads;
-    cfg.blockDim = dim3((unsigned)threads);
-    cfg.dynamicSmemBytes = (size_t)small_layout(V.N, Jc).total * 8;
-    cfg.stream = s;
+    cudaLaunchConfig_t cfg;
     cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = (unsigned)C;
-    at[0].val.clusterDim.y = 1;
-    at[0].val.clusterDim.z = 1;
-    cfg.attrs = at;
-    cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, oci_red_small_kernel, V, ybase, tol, cnt, force);
+    int nbg;
+    small_config(V, C, &cfg, at, &nbg);
+    cfg.stream = s;
+    cudaLaunchKernelEx(&cfg, oci_red_small_kernel, V, ybase, tol, cnt, force, nbg);
     return launched(1);
 }
 

@@ -696,7 +696,7 @@ def test_small_step_serves_configs_1_and_2(cfg):
     p = make_problem(cfg)
     mode = {1: None, 2: 1}[cfg]
     r = run_pair(p, "oci", steps=p.n_steps, tol=p.tol, max_iters=p.max_iters, small_step=mode)
-    assert r["info"]["small_step_cluster"] == {1: 1, 2: 8}[cfg] and r["info"]["iteration"] == P.ITERATION_REDUCED
+    assert r["info"]["small_step_cluster"] in {1: (1,), 2: (8, 16)}[cfg] and r["info"]["iteration"] == P.ITERATION_REDUCED
     assert r["g_iters"] == r["o_iters"]
     assert rel(r["g_psi"], r["o_psi"]) < 1e-9 and rel(r["g_phi"], r["o_phi"]) < 1e-9
     assert r["launches"] <= 4 + 2 * p.n_steps                    # set_flux + one launch per step (+ layout on demand)
