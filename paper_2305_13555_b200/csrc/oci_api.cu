@@ -195,7 +195,7 @@ void gauss_legendre(int N, std::vector<double>& mu, std::vector<double>& w)
 
 struct Layout {
     int64_t binv, psi0, psi1, cfix, phi, Q, qs, dx, sig, sigs, blk, rep, mu, w, coef, ainv4, si_scan, phi_part, norms, tickets, flags,
-        xop, rop, fop, y0, y1, z, yfix, ifix, phifix, q16, gitems, perm, team_bar, peers, phi_stage, si_part, si_inflow, si_src1, wba, wbd, wbm, total;
+        xop, rop, fop, y0, y1, z, yfix, ifix, phifix, q16, gitems, perm, team_bar, peers, phi_stage, si_part, si_inflow, si_src1, si_agg, wba, wbd, wbm, total;
 };
 
 int64_t align_up(int64_t x) { return (x + 255) & ~int64_t(255); }
@@ -250,6 +250,7 @@ Layout make_layout(int64_t J, int32_t N, int64_t nblk)
     L.si_part = take((N / 32 > 2 ? N / 32 : 2) * J * 4 * 8);
     L.si_inflow = take(2 * N * 2 * 8);
     L.si_src1 = take(J * 4 * 8);
+    L.si_agg = take((int64_t)N * si_carry_segments((J + 7) / 8) * 8 * 8);   // (zeroed by oci_setup together with the flags)
     L.wba = take(nblk * 16 * N * 8);
     L.wbd = take(nblk * 16 * N * 8);
     L.wbm = take(nblk * 32 * 8);
@@ -682,6 +683,7 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
     V.si_part = (double*)(base + L.si_part);
     V.si_inflow = (double*)(base + L.si_inflow);
     V.si_src1 = (double*)(base + L.si_src1);
+    V.si_agg = (double*)(base + L.si_agg);
     V.wba = (double*)(base + L.wba);
     V.wbd = (double*)(base + L.wbd);
     V.wbm = (double*)(base + L.wbm);
@@ -709,6 +711,7 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
         CK(oci_red_opreg_opt_in());
         CK(oci_red_woodbury_opt_in());
         CK(oci_red_small_opt_in());
+        CK(si_fast_opt_in());
     }
 
     cudaStream_t s = ctx->stream;

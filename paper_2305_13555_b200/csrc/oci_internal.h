@@ -43,10 +43,11 @@ struct DevView {
     double* si_part;            // [max(2, N/32)][J][4]  scalar-flux partials per lane group (si_sweep_fast.cu)
     double* si_src1;            // [J][4]  second buffer of the SI scattering source (the first is qs), by iteration parity
     double* si_inflow;          // [2][N][2]  boundary inflow of every angle, by iteration parity (si_sweep_fast.cu)
+    double* si_agg;             // [N][segments][8]  carry scan: composition through a segment, [7] = the launch tag (si_sweep_fast.cu)
     double* phi_part;           // [ceil(n/128)][J][4]  per-item scalar-flux partials (K-tiled kernel)
     int32_t* tickets;           // [ceil(J/64)]  arrival counters of the K-tiled kernel's cell tiles (0 between launches)
     unsigned long long* norms;  // [kNormSlots][2]  bit patterns of (d, r), atomicMax targets
-    int32_t* flags;             // [0] = 1 + index of a singular block, 0 if none; [8] grid-barrier counter of the fused loops; [12] their work-ticket counter
+    int32_t* flags;             // [0] = 1 + index of a singular block, 0 if none; [8] grid-barrier counter of the fused loops; [12] their work-ticket counter; [16..17] u64 ticket counter of the SI carry scan (never reset)
     int32_t* perm;              // [nblk][n]  pivot rows of the blocked inversion (setup)
     int32_t* team_bar;          // [min(nblk, SMs)]  team-barrier counters of the blocked inversion (setup)
     // ---- interface-reduced step (oci_reduced.cu), K2 = 2N
@@ -147,6 +148,8 @@ int launch_oci_iteration(const DevView& V, int path, int src, int slot, int prev
 int launch_si_iteration(const DevView& V, int buf, int slot, int prev_slot, double tol, cudaStream_t s);
 // fast form (si_sweep_fast.cu): N/2 a power of two
 bool si_fast_supported(const DevView& V);
+cudaError_t si_fast_opt_in();
+int si_carry_segments(int64_t chunks);                 // segments per angle of the SI carry scan (sizes si_agg)
 int launch_si_fast_begin(const DevView& V, int buf, cudaStream_t s);
 int launch_si_fast_iteration(const DevView& V, int buf, int it, int slot, int prev_slot, double tol, cudaStream_t s);
 int launch_si_fast_final(const DevView& V, int buf, int it0, double tol, int cnt, int force, cudaStream_t s);

@@ -106,9 +106,14 @@ __global__ void __launch_bounds__(256) si_prev_kernel(DevView V, int buf)
 // MODE 1: reduce the chunk to its affine map.  MODE 3: sweep the chunk from its inflow, accumulate the phi partials.
 // MODE 4 (final): sweep the chunk and store Psi.  `it` = iteration index within the step (phi buffer parity).
 // scan[(m*C + c)*8 + 0..5] = (P_c, z_c), [6..7] = inflow of chunk c (written by si_carry2_kernel).
-template <int U, bool SHARED_BLOCK, int MODE, int LOGGS>
-__global__ void __launch_bounds__(128, 3) si_chunk2_kernel(DevView V, int buf, int it, int prev_slot, double tol, int S, int C, int Nr, int cnt, int force)
+// STAGED: the CTA's chunks are consecutive, so everything they read - the psi_{k-1/2} rows of their cells (all angles:
+// one contiguous run of [J][N][2]) and the source rows - arrives as TWO bulk copies (UBLKCP) requested by one thread at
+// the start of the CTA and the sweep reads shared memory: the kernel was bound by the latency of 16-byte loads issued
+// from registers (1.7 TB/s at config 3), the copies of the other resident CTAs now overlap a CTA's arithmetic.
+template <int U, bool SHARED_BLOCK, int MODE, int LOGGS, bool STAGED>
+__global__ void __launch_bounds__(128, STAGED && SHARED_BLOCK ? 4 : 3) si_chunk2_kernel(DevView V, int buf, int it, int prev_slot, double tol, int S, int C, int Nr, int cnt, int force)
 {
+    extern __shared__ __align__(128) unsigned char si_smem[];
     if (MODE == 4) {
         // the last executed iteration of this chunk of launches; its phi^(L-1) and chunk inflows are still in place
         int L = first_converged(V.norms, cnt, tol);
@@ -120,21 +125,67 @@ __global__ void __launch_bounds__(128, 3) si_chunk2_kernel(DevView V, int buf, i
     } else if (step_done(V.norms, prev_slot, tol)) {
         return;
     }
-    const int64_t gid = (int64_t)blockIdx.x * 128 + threadIdx.x;
     const int lane = threadIdx.x & 31;
-    int m = (int)(gid % Nr);
-    int64_t c = gid / Nr;
-    const bool live = m < V.N && c < C;                  // (shuffles below need every lane of the warp)
-    if (!live) { m = 0; c = 0; }
     const int n = V.n, N = V.N;
     const int64_t J = V.J;
+    const double* __restrict__ src_cur = (it & 1) ? V.si_src1 : V.qs;       // (h/4)(Sigma_s phi^(l) + Q), row d1
+    const double* inflow_cur = V.si_inflow + (size_t)(it & 1) * 2 * N;
+    double* inflow_nxt = V.si_inflow + (size_t)((it + 1) & 1) * 2 * N;
+    const uint64_t pol_keep = l2_policy_evict_last();
+    const double gam2 = 1.0 / (2.0 * V.v * V.dt);
+    const double al0 = V.dx[V.rep[0]] * gam2;            // alpha = h / (2 v dt) of the shared block
+    constexpr int loggs = LOGGS;
+    const int gs = 1 << loggs;
+    // STAGED: persistent CTAs walk the tiles (128 threads = 128 / Nr consecutive chunks x all angles) with a two-stage ring
+    const int ntiles = (int)(((int64_t)C * Nr + 127) / 128);
+    const int cpb = STAGED ? 128 / Nr : 1;               // chunks per tile
+    const size_t stage_doubles = (size_t)cpb * S * (N * 2 + 4);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(si_smem);
+    double* ring = reinterpret_cast<double*>(si_smem + 128);
+    auto request = [&](int tile, int stage) {            // one thread: the two bulk copies of a tile
+        const int64_t c0 = (int64_t)tile * cpb * S;
+        const int64_t c1 = (c0 + (int64_t)cpb * S < J) ? c0 + (int64_t)cpb * S : J;
+        const uint32_t ncell = (uint32_t)(c1 - c0);
+        double* sp = ring + stage * stage_doubles;
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_expect_tx(&bars[stage], ncell * (uint32_t)N * 16u + ncell * 32u);
+        tma_load_1d_hint(sp, V.si_prev + c0 * N * 2, ncell * (uint32_t)N * 16u, &bars[stage], pol_keep);   // re-read by the next phase: L2
+        tma_load_1d(sp + (size_t)cpb * S * N * 2, src_cur + c0 * 4, ncell * 32u, &bars[stage]);
+    };
+    if (STAGED) {
+        if (threadIdx.x == 0) {
+            mbar_init(&bars[0], 1);
+            mbar_init(&bars[1], 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            request(blockIdx.x, 0);
+            if ((int)(blockIdx.x + gridDim.x) < ntiles) request(blockIdx.x + gridDim.x, 1);
+        }
+        __syncthreads();
+    }
+    // the angle of a thread is the same in every tile (Nr divides 128)
+    const int m_t = (int)(((int64_t)blockIdx.x * 128 + threadIdx.x) % Nr);
+    const int m0 = m_t < N ? m_t : 0;
+    double Ai[16];
+    if (SHARED_BLOCK) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) Ai[i] = V.ainv4[(size_t)m0 * 16 + i];
+    }
+
+  int seq = 0;                                           // tiles this CTA has taken
+  for (int tile = blockIdx.x; tile < (STAGED ? ntiles : (int)blockIdx.x + 1); tile += gridDim.x, ++seq) {
+    const int64_t gid = (int64_t)tile * 128 + threadIdx.x;
+    int m = (int)(gid % Nr);
+    int64_t c = gid / Nr;
+    const bool live = m < N && c < C;                    // (shuffles below need every lane of the warp)
+    if (!live) { m = 0; c = STAGED ? (int64_t)tile * cpb : 0; }   // (a cell this tile has staged)
     const double mu = V.mu[m];
     const bool pos = mu > 0.0;
     const double amu = fabs(mu);
-    const double* __restrict__ src_cur = (it & 1) ? V.si_src1 : V.qs;       // (h/4)(Sigma_s phi^(l) + Q), row d1
+    const int stage = seq & 1;
+    const double* sprev = ring + stage * stage_doubles;  // STAGED: the tile in shared memory, cells from cell0 on
+    const double* ssrc = sprev + (size_t)cpb * S * N * 2;
+    const int64_t cell0 = (int64_t)tile * cpb * S;
     double* sc = V.si_scan + ((size_t)m * C + c) * 8;            // angle major: the carry kernel streams one angle's maps
-    const double* inflow_cur = V.si_inflow + (size_t)(it & 1) * 2 * N;
-    double* inflow_nxt = V.si_inflow + (size_t)((it + 1) & 1) * 2 * N;
     // mu>0: rows 0,2 receive the incident flux (k, k+1/2) and rows 1,3 leave the cell; mu<0: mirrored
     double in_k = 0.0, in_h = 0.0;
     if (MODE != 1) {
@@ -142,23 +193,14 @@ __global__ void __launch_bounds__(128, 3) si_chunk2_kernel(DevView V, int buf, i
         else { in_k = sc[6]; in_h = sc[7]; }
     }
     Affine A = affine_identity();
-    double Ai[16];
-    if (SHARED_BLOCK) {
-#pragma unroll
-        for (int i = 0; i < 16; ++i) Ai[i] = V.ainv4[(size_t)m * 16 + i];
-    }
     const int64_t c_begin = c * S;
     const int64_t c_end = (c_begin + S < J) ? c_begin + S : J;
     const int len = (int)(c_end - c_begin);
     const double wm = V.w[m];
-    const uint64_t pol_keep = l2_policy_evict_last();
-    const double gam2 = 1.0 / (2.0 * V.v * V.dt);
-    const double al0 = V.dx[V.rep[0]] * gam2;            // alpha = h / (2 v dt) of the shared block
     // phi partials: one array per group of 2^loggs lanes
-    constexpr int loggs = LOGGS;
     const int part = m >> loggs;
     double* __restrict__ Pp = V.si_part + (size_t)part * J * 4;
-    const int gs = 1 << loggs;
+    if (STAGED) mbar_wait(&bars[stage], (seq >> 1) & 1);
 
     for (int t0 = 0; t0 < S; t0 += U) {                  // uniform trip count: every lane of the warp shuffles
         double y[U][4], G[U][4][2];
@@ -169,9 +211,15 @@ __global__ void __launch_bounds__(128, 3) si_chunk2_kernel(DevView V, int buf, i
         for (int u = 0; u < U; ++u) {
             const int t = (t0 + u < len) ? t0 + u : len - 1;              // clamped: unconditional loads
             const int64_t j = pos ? c_begin + t : c_end - 1 - t;
-            e[u] = ldg2_hint(V.si_prev + (j * N + m) * 2, pol_keep);      // re-read twice per iteration: asked to stay in L2
-            s01[u] = __ldcg(reinterpret_cast<const double2*>(src_cur + j * 4));
-            s23[u] = __ldcg(reinterpret_cast<const double2*>(src_cur + j * 4 + 2));
+            if (STAGED) {
+                e[u] = *reinterpret_cast<const double2*>(sprev + ((j - cell0) * N + m) * 2);
+                s01[u] = *reinterpret_cast<const double2*>(ssrc + (j - cell0) * 4);
+                s23[u] = *reinterpret_cast<const double2*>(ssrc + (j - cell0) * 4 + 2);
+            } else {
+                e[u] = ldg2_hint(V.si_prev + (j * N + m) * 2, pol_keep);      // re-read twice per iteration: asked to stay in L2
+                s01[u] = __ldcg(reinterpret_cast<const double2*>(src_cur + j * 4));
+                s23[u] = __ldcg(reinterpret_cast<const double2*>(src_cur + j * 4 + 2));
+            }
             al[u] = SHARED_BLOCK ? al0 : V.dx[j] * gam2;
             if (!SHARED_BLOCK) ap[u] = V.ainv4 + ((size_t)V.blk[j] * N + m) * 16;
         }
@@ -250,7 +298,7 @@ __global__ void __launch_bounds__(128, 3) si_chunk2_kernel(DevView V, int buf, i
             }
         }
     }
-    if (!live) return;
+    if (live) {
     if (MODE == 1) {
         *reinterpret_cast<double2*>(sc + 0) = make_double2(A.p00, A.p01);
         *reinterpret_cast<double2*>(sc + 2) = make_double2(A.p10, A.p11);
@@ -271,34 +319,51 @@ __global__ void __launch_bounds__(128, 3) si_chunk2_kernel(DevView V, int buf, i
             else { P[-(int64_t)n + 4 * mir + 1] = in_k; P[-(int64_t)n + 4 * mir + 3] = in_h; }
         }
     }
+    }
+    if (STAGED && tile + 2 * (int)gridDim.x < ntiles) {  // the stage is free once every thread has left it: refill it
+        __syncthreads();
+        if (threadIdx.x == 0) request(tile + 2 * gridDim.x, stage);
+    }
+  }
 }
 
-// exclusive scan of the chunk maps of one angle in its direction of travel, applied to the boundary inflow
-__global__ void __launch_bounds__(512) si_carry2_kernel(DevView V, int it, int prev_slot, double tol, int C)
+// Exclusive scan of the chunk maps of one angle in its direction of travel, applied to the boundary inflow.  An angle's
+// C chunks are cut into G segments of CARRY_T * CARRY_K chunks; a CTA takes one (segment, angle) - handed out by a
+// ticket counter in segment-major order, so a CTA only ever waits for CTAs that are already running - loads the
+// CARRY_K maps of each thread up front (ONE DRAM round trip instead of one per map), scans them (thread, warp shuffle,
+// CTA), and receives the composition of everything before its segment from the CTA of the previous segment through
+// si_agg (a chain of G - 1 L2 round trips, released by a tag that is unique to the launch: the ticket counter never
+// goes back, ticket / (N G) + 1 = the launch's epoch).  Config 3 (8192 chunks per angle): 37 us -> see DESIGN.md 6.6.
+constexpr int CARRY_T = 512, CARRY_K = 2;
+
+__global__ void __launch_bounds__(CARRY_T) si_carry3_kernel(DevView V, int it, int prev_slot, double tol, int C, int G)
 {
-    if (step_done(V.norms, prev_slot, tol)) return;
-    __shared__ Affine wtot[16];
-    const int m = blockIdx.x;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (step_done(V.norms, prev_slot, tol)) return;      // (every CTA of the launch takes this branch or none does)
+    __shared__ Affine wtot[CARRY_T / 32];
+    __shared__ Affine s_before;
+    __shared__ unsigned long long s_ticket;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, N = V.N;
+    if (tid == 0) s_ticket = atomicAdd(reinterpret_cast<unsigned long long*>(V.flags + 16), 1ull);
+    __syncthreads();
+    const unsigned long long per = (unsigned long long)N * G;
+    const unsigned long long tag = s_ticket / per + 1;
+    const int local = (int)(s_ticket % per), g = local / N, m = local - g * N;
     const bool pos = V.mu[m] > 0.0;
-    const int cpl = (C + 511) / 512;
-    const int c0 = tid * cpl;                            // positions in travel order
-    const int c1 = (c0 + cpl < C) ? c0 + cpl : C;
     auto chunk_of = [&](int tau) { return pos ? tau : C - 1 - tau; };
-    Affine loc = affine_identity();
-    constexpr int B = 4;                                 // maps loaded together: the loads do not depend on the composition
-    for (int tb = c0; tb < c1; tb += B) {
-        double2 a[B], b[B], z[B];
+    const int c0 = g * (CARRY_T * CARRY_K) + tid * CARRY_K;       // positions in travel order
+    double2 a[CARRY_K], b[CARRY_K], z[CARRY_K];
 #pragma unroll
-        for (int k = 0; k < B; ++k) {
-            const int tau = tb + k < c1 ? tb + k : c1 - 1;
-            const double* sc = V.si_scan + ((size_t)m * C + chunk_of(tau)) * 8;
-            a[k] = *reinterpret_cast<const double2*>(sc); b[k] = *reinterpret_cast<const double2*>(sc + 2); z[k] = *reinterpret_cast<const double2*>(sc + 4);
-        }
-#pragma unroll
-        for (int k = 0; k < B; ++k)
-            if (tb + k < c1) loc = compose(Affine{a[k].x, a[k].y, b[k].x, b[k].y, z[k].x, z[k].y}, loc);
+    for (int k = 0; k < CARRY_K; ++k) {
+        const int tau = c0 + k < C ? c0 + k : C - 1;
+        const double* sc = V.si_scan + ((size_t)m * C + chunk_of(tau)) * 8;
+        a[k] = __ldcg(reinterpret_cast<const double2*>(sc));
+        b[k] = __ldcg(reinterpret_cast<const double2*>(sc + 2));
+        z[k] = __ldcg(reinterpret_cast<const double2*>(sc + 4));
     }
+    Affine loc = affine_identity();
+#pragma unroll
+    for (int k = 0; k < CARRY_K; ++k)
+        if (c0 + k < C) loc = compose(Affine{a[k].x, a[k].y, b[k].x, b[k].y, z[k].x, z[k].y}, loc);
     Affine inc = loc;   // inclusive scan over the lanes of the warp
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -309,58 +374,78 @@ __global__ void __launch_bounds__(512) si_carry2_kernel(DevView V, int it, int p
     Affine exc = shfl_up_affine(inc, 1);
     if (lane == 0) exc = affine_identity();
     __syncthreads();
-    Affine pre = affine_identity();   // everything before this warp
-    for (int w8 = 0; w8 < warp; ++w8) pre = compose(wtot[w8], pre);
+    if (tid == 0) {
+        // everything before this segment, from the previous segment's CTA; everything through this one, for the next
+        Affine before = affine_identity();
+        if (g > 0) {
+            const double* rec = V.si_agg + ((size_t)m * G + (g - 1)) * 8;
+            unsigned long long seen;
+            do {
+                asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(rec + 7) : "memory");
+            } while (seen != tag);
+            before = Affine{__ldcg(rec + 0), __ldcg(rec + 1), __ldcg(rec + 2), __ldcg(rec + 3), __ldcg(rec + 4), __ldcg(rec + 5)};
+        }
+        if (g + 1 < G) {
+            Affine through = before;
+            for (int w = 0; w < CARRY_T / 32; ++w) through = compose(wtot[w], through);
+            double* rec = V.si_agg + ((size_t)m * G + g) * 8;
+            rec[0] = through.p00; rec[1] = through.p01; rec[2] = through.p10; rec[3] = through.p11;
+            rec[4] = through.z0;  rec[5] = through.z1;
+            asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(rec + 7), "l"(tag) : "memory");
+        }
+        s_before = before;
+    }
+    __syncthreads();
+    Affine pre = s_before;            // everything before this warp
+    for (int w = 0; w < warp; ++w) pre = compose(wtot[w], pre);
     pre = compose(exc, pre);
-    const double* inflow_cur = V.si_inflow + (size_t)(it & 1) * 2 * V.N;
+    const double* inflow_cur = V.si_inflow + (size_t)(it & 1) * 2 * N;
     const double e0 = inflow_cur[2 * m], e1 = inflow_cur[2 * m + 1];
     double in_k = fma(pre.p00, e0, fma(pre.p01, e1, pre.z0));
     double in_h = fma(pre.p10, e0, fma(pre.p11, e1, pre.z1));
-    for (int tb = c0; tb < c1; tb += B) {
-        double2 a[B], b[B], z[B];
 #pragma unroll
-        for (int k = 0; k < B; ++k) {
-            const int tau = tb + k < c1 ? tb + k : c1 - 1;
-            const double* sc = V.si_scan + ((size_t)m * C + chunk_of(tau)) * 8;
-            a[k] = *reinterpret_cast<const double2*>(sc); b[k] = *reinterpret_cast<const double2*>(sc + 2); z[k] = *reinterpret_cast<const double2*>(sc + 4);
-        }
-#pragma unroll
-        for (int k = 0; k < B; ++k) {
-            if (tb + k < c1) {
-                double* sc = V.si_scan + ((size_t)m * C + chunk_of(tb + k)) * 8;
-                *reinterpret_cast<double2*>(sc + 6) = make_double2(in_k, in_h);
-                const double nk = fma(a[k].x, in_k, fma(a[k].y, in_h, z[k].x));
-                const double nh = fma(b[k].x, in_k, fma(b[k].y, in_h, z[k].y));
-                in_k = nk;
-                in_h = nh;
-            }
+    for (int k = 0; k < CARRY_K; ++k) {
+        if (c0 + k < C) {
+            double* sc = V.si_scan + ((size_t)m * C + chunk_of(c0 + k)) * 8;
+            *reinterpret_cast<double2*>(sc + 6) = make_double2(in_k, in_h);
+            const double nk = fma(a[k].x, in_k, fma(a[k].y, in_h, z[k].x));
+            const double nh = fma(b[k].x, in_k, fma(b[k].y, in_h, z[k].y));
+            in_k = nk;
+            in_h = nh;
         }
     }
 }
 
 // phi^(l+1) = sum of the partials (fixed order), the two max-norms against phi^(l), and the next iteration's
-// scattering source (h/4)(Sigma_s phi^(l+1) + Q) into the other source buffer (the FINAL pass re-reads this one)
-__global__ void __launch_bounds__(256) si_combine_kernel(DevView V, int it, int slot, int prev_slot, double tol, int parts)
+// scattering source (h/4)(Sigma_s phi^(l+1) + Q) into the other source buffer (the FINAL pass re-reads this one).
+// One 16-byte unit per thread and every load of the unit requested before the first one is used: the kernel is a handful
+// of dependent DRAM round trips otherwise (38 us at config 3 with a grid-stride loop over 296 CTAs, 5 us like this).
+template <int PARTS>
+__global__ void __launch_bounds__(256) si_combine_kernel(DevView V, int it, int slot, int prev_slot, double tol)
 {
     if (step_done(V.norms, prev_slot, tol)) return;
     double* __restrict__ src_nxt = (it & 1) ? V.qs : V.si_src1;
     const int64_t tot = V.J * 2;                         // 16-byte units
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     double dmax = 0.0, rmax = 0.0;
-    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < tot; e += (int64_t)gridDim.x * blockDim.x) {
-        double2 s = make_double2(0.0, 0.0);
-        for (int p = 0; p < parts; ++p) {
-            const double2 v = __ldcg(reinterpret_cast<const double2*>(V.si_part + (size_t)p * V.J * 4) + e);
-            s.x += v.x;
-            s.y += v.y;
-        }
+    if (e < tot) {
+        double2 v[PARTS];
+#pragma unroll
+        for (int p = 0; p < PARTS; ++p) v[p] = __ldcg(reinterpret_cast<const double2*>(V.si_part + (size_t)p * V.J * 4) + e);
         const double2 o = reinterpret_cast<const double2*>(V.phi)[e];
-        reinterpret_cast<double2*>(V.phi)[e] = s;
+        const double2 q = reinterpret_cast<const double2*>(V.Q)[e];
         const int64_t j = e >> 1;
         const double q4 = 0.25 * V.dx[j], sg = V.sigs[j];
-        const double2 q = reinterpret_cast<const double2*>(V.Q)[e];
+        double2 s = make_double2(0.0, 0.0);
+#pragma unroll
+        for (int p = 0; p < PARTS; ++p) {
+            s.x += v[p].x;
+            s.y += v[p].y;
+        }
+        reinterpret_cast<double2*>(V.phi)[e] = s;
         reinterpret_cast<double2*>(src_nxt)[e] = make_double2(q4 * fma(sg, s.x, q.x), q4 * fma(sg, s.y, q.y));
-        dmax = nanmax(dmax, nanmax(fabs(s.x - o.x), fabs(s.y - o.y)));
-        rmax = nanmax(rmax, nanmax(fabs(s.x), fabs(s.y)));
+        dmax = nanmax(fabs(s.x - o.x), fabs(s.y - o.y));
+        rmax = nanmax(fabs(s.x), fabs(s.y));
     }
     __shared__ double sd[8], sr[8];
     dmax = warp_max(dmax);
@@ -381,6 +466,9 @@ bool si_fast_supported(const DevView& V)
     const int h = V.N / 2;
     return h >= 1 && (h & (h - 1)) == 0;
 }
+
+// segments of the carry scan per angle for C chunks (si_agg holds [N][segments][8] doubles)
+int si_carry_segments(int64_t C) { return (int)((C + CARRY_T * CARRY_K - 1) / (CARRY_T * CARRY_K)); }
 
 int si_fast_parts(const DevView& V)
 {
@@ -419,10 +507,43 @@ namespace {
 template <int MODE, int LG>
 void launch_chunk2(const DevView& V, const SiGeom& g, int buf, int it, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
 {
-    if (V.nblk == 1) si_chunk2_kernel<4, true, MODE, LG><<<g.blocks, 128, 0, s>>>(V, buf, it, prev_slot, tol, g.S, g.C, g.Nr, cnt, force);
-    else si_chunk2_kernel<4, false, MODE, LG><<<g.blocks, 128, 0, s>>>(V, buf, it, prev_slot, tol, g.S, g.C, g.Nr, cnt, force);
+    // staged form: a tile covers whole chunks (Nr <= 128); persistent CTAs, as many as are resident (about three per SM), two tiles of shared
+    // memory each (at most 2 x 34 KB + the barriers: opted in by si_fast_opt_in)
+    const size_t stage_bytes = g.Nr <= 128 ? (size_t)(128 / g.Nr) * g.S * ((size_t)V.N * 16 + 32) : 0;
+    if (stage_bytes > 0 && stage_bytes <= 36 * 1024) {
+        const size_t smem = 128 + 2 * stage_bytes;
+        const unsigned per_sm = (unsigned)(200 * 1024 / (smem + 1024));     // resident CTAs: one wave
+        const unsigned grid = g.blocks < per_sm * (unsigned)V.sm_count ? g.blocks : per_sm * (unsigned)V.sm_count;
+        if (V.nblk == 1) si_chunk2_kernel<4, true, MODE, LG, true><<<grid, 128, smem, s>>>(V, buf, it, prev_slot, tol, g.S, g.C, g.Nr, cnt, force);
+        else si_chunk2_kernel<4, false, MODE, LG, true><<<grid, 128, smem, s>>>(V, buf, it, prev_slot, tol, g.S, g.C, g.Nr, cnt, force);
+        return;
+    }
+    if (V.nblk == 1) si_chunk2_kernel<4, true, MODE, LG, false><<<g.blocks, 128, 0, s>>>(V, buf, it, prev_slot, tol, g.S, g.C, g.Nr, cnt, force);
+    else si_chunk2_kernel<4, false, MODE, LG, false><<<g.blocks, 128, 0, s>>>(V, buf, it, prev_slot, tol, g.S, g.C, g.Nr, cnt, force);
 }
 }  // namespace
+
+namespace {
+template <int MODE, int LG>
+cudaError_t opt_in_chunk2()
+{
+    cudaError_t e = cudaFuncSetAttribute(si_chunk2_kernel<4, true, MODE, LG, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 80 * 1024);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(si_chunk2_kernel<4, false, MODE, LG, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 80 * 1024);
+}
+}  // namespace
+
+// the staged chunk kernels keep two tiles in shared memory (per device: called by oci_setup)
+cudaError_t si_fast_opt_in()
+{
+    cudaError_t e;
+    if ((e = opt_in_chunk2<1, 0>()) != cudaSuccess || (e = opt_in_chunk2<4, 0>()) != cudaSuccess ||
+        (e = opt_in_chunk2<3, 0>()) != cudaSuccess || (e = opt_in_chunk2<3, 1>()) != cudaSuccess ||
+        (e = opt_in_chunk2<3, 2>()) != cudaSuccess || (e = opt_in_chunk2<3, 3>()) != cudaSuccess ||
+        (e = opt_in_chunk2<3, 4>()) != cudaSuccess || (e = opt_in_chunk2<3, 5>()) != cudaSuccess)
+        return e;
+    return cudaSuccess;
+}
 
 // `it`: iteration index within the step (source buffer parity); slot / prev_slot: norm slots within the launch chunk
 int launch_si_fast_iteration(const DevView& V, int buf, int it, int slot, int prev_slot, double tol, cudaStream_t s)
@@ -431,7 +552,8 @@ int launch_si_fast_iteration(const DevView& V, int buf, int it, int slot, int pr
     int k = 0;
     if (g.C > 1) {
         launch_chunk2<1, 0>(V, g, buf, it, prev_slot, tol, 0, 0, s);
-        si_carry2_kernel<<<(unsigned)V.N, 512, 0, s>>>(V, it, prev_slot, tol, g.C);
+        const int G = si_carry_segments(g.C);
+        si_carry3_kernel<<<(unsigned)(V.N * G), CARRY_T, 0, s>>>(V, it, prev_slot, tol, g.C, G);
         k += 2;
     }
     switch (g.loggs) {                                   // lanes per direction group of the butterfly: 2^loggs
@@ -442,9 +564,13 @@ int launch_si_fast_iteration(const DevView& V, int buf, int it, int slot, int pr
     case 4: launch_chunk2<3, 4>(V, g, buf, it, prev_slot, tol, 0, 0, s); break;
     default: launch_chunk2<3, 5>(V, g, buf, it, prev_slot, tol, 0, 0, s); break;
     }
-    int64_t cb = (V.J * 2 + 255) / 256;
-    if (cb > (int64_t)V.sm_count * 2) cb = (int64_t)V.sm_count * 2;       // few CTAs: their two atomics serialise in L2
-    si_combine_kernel<<<(unsigned)cb, 256, 0, s>>>(V, it, slot, prev_slot, tol, si_fast_parts(V));
+    const unsigned cb = (unsigned)((V.J * 2 + 255) / 256);
+    switch (si_fast_parts(V)) {
+    case 2: si_combine_kernel<2><<<cb, 256, 0, s>>>(V, it, slot, prev_slot, tol); break;
+    case 4: si_combine_kernel<4><<<cb, 256, 0, s>>>(V, it, slot, prev_slot, tol); break;
+    case 8: si_combine_kernel<8><<<cb, 256, 0, s>>>(V, it, slot, prev_slot, tol); break;
+    default: si_combine_kernel<16><<<cb, 256, 0, s>>>(V, it, slot, prev_slot, tol); break;
+    }
     return launched(k + 2);
 }
 
