@@ -331,10 +331,10 @@ __global__ void __launch_bounds__(128, STAGED && SHARED_BLOCK ? 4 : 3) si_chunk2
 // C chunks are cut into G segments of CARRY_T * CARRY_K chunks; a CTA takes one (segment, angle) - handed out by a
 // ticket counter in segment-major order, so a CTA only ever waits for CTAs that are already running - loads the
 // CARRY_K maps of each thread up front (ONE DRAM round trip instead of one per map), scans them (thread, warp shuffle,
-// CTA), and receives the composition of everything before its segment from the CTA of the previous segment through
-// si_agg (a chain of G - 1 L2 round trips, released by a tag that is unique to the launch: the ticket counter never
-// goes back, ticket / (N G) + 1 = the launch's epoch).  Config 3 (8192 chunks per angle): 37 us -> see DESIGN.md 6.6.
-constexpr int CARRY_T = 512, CARRY_K = 2;
+// CTA), publishes the composition of its segment in si_agg and composes the segments before its own from there (they
+// are all published at about the same time: one L2 round trip; released by a tag that is unique to the launch: the
+// ticket counter never goes back, ticket / (N G) + 1 = the launch's epoch).  Config 3 (8192 chunks per angle): 37 us -> see DESIGN.md 6.6.
+constexpr int CARRY_T = 512, CARRY_K = 4;
 
 __global__ void __launch_bounds__(CARRY_T) si_carry3_kernel(DevView V, int it, int prev_slot, double tol, int C, int G)
 {
@@ -374,26 +374,40 @@ __global__ void __launch_bounds__(CARRY_T) si_carry3_kernel(DevView V, int it, i
     Affine exc = shfl_up_affine(inc, 1);
     if (lane == 0) exc = affine_identity();
     __syncthreads();
-    if (tid == 0) {
-        // everything before this segment, from the previous segment's CTA; everything through this one, for the next
-        Affine before = affine_identity();
-        if (g > 0) {
-            const double* rec = V.si_agg + ((size_t)m * G + (g - 1)) * 8;
-            unsigned long long seen;
-            do {
-                asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(rec + 7) : "memory");
-            } while (seen != tag);
-            before = Affine{__ldcg(rec + 0), __ldcg(rec + 1), __ldcg(rec + 2), __ldcg(rec + 3), __ldcg(rec + 4), __ldcg(rec + 5)};
-        }
-        if (g + 1 < G) {
-            Affine through = before;
-            for (int w = 0; w < CARRY_T / 32; ++w) through = compose(wtot[w], through);
+    if (warp == 0) {
+        // every CTA publishes the composition of ITS segment as soon as it has it (nobody waits to publish), then lane q
+        // of warp 0 fetches segment q's and the lanes compose them in order: one L2 round trip, not a chain of G - 1
+        if (lane == 0 && g + 1 < G) {
+            Affine own = affine_identity();
+            for (int w = 0; w < CARRY_T / 32; ++w) own = compose(wtot[w], own);
             double* rec = V.si_agg + ((size_t)m * G + g) * 8;
-            rec[0] = through.p00; rec[1] = through.p01; rec[2] = through.p10; rec[3] = through.p11;
-            rec[4] = through.z0;  rec[5] = through.z1;
+            rec[0] = own.p00; rec[1] = own.p01; rec[2] = own.p10; rec[3] = own.p11;
+            rec[4] = own.z0;  rec[5] = own.z1;
             asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(rec + 7), "l"(tag) : "memory");
         }
-        s_before = before;
+        Affine before = affine_identity();
+        for (int q0 = 0; q0 < g; q0 += 32) {             // (G <= 32 for every slab up to 2^21 cells: one pass)
+            Affine mine = affine_identity();
+            if (q0 + lane < g) {
+                const double* rec = V.si_agg + ((size_t)m * G + q0 + lane) * 8;
+                unsigned long long seen;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(rec + 7) : "memory");
+                } while (seen != tag);
+                mine = Affine{__ldcg(rec + 0), __ldcg(rec + 1), __ldcg(rec + 2), __ldcg(rec + 3), __ldcg(rec + 4), __ldcg(rec + 5)};
+            }
+            // inclusive scan over the lanes (identity beyond g), the last lane holds the composition of this pass
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const Affine up = shfl_up_affine(mine, o);
+                if (lane >= o) mine = compose(mine, up);
+            }
+            const Affine all = Affine{__shfl_sync(0xffffffffu, mine.p00, 31), __shfl_sync(0xffffffffu, mine.p01, 31),
+                                      __shfl_sync(0xffffffffu, mine.p10, 31), __shfl_sync(0xffffffffu, mine.p11, 31),
+                                      __shfl_sync(0xffffffffu, mine.z0, 31),  __shfl_sync(0xffffffffu, mine.z1, 31)};
+            before = compose(all, before);
+        }
+        if (lane == 0) s_before = before;
     }
     __syncthreads();
     Affine pre = s_before;            // everything before this warp
