@@ -418,6 +418,27 @@ def test_full_size_si_fixed_iterations_cfg3():
     assert rel(r["g_phi"], r["o_phi"]) < 1e-12
 
 
+@pytest.mark.parametrize("J,N,bcL,bcR,hetero", [
+    (70001, 2, (REF, 0.0), (INC, 1.0), False),    # 8751 chunks of 8: five carry segments, a one-cell last chunk, staged tiles of 64 chunks
+    (40007, 32, (REF, 0.0), (REF, 0.0), False),   # 2501 chunks of 16: two carry segments, ragged last chunk and tile, mirrors at both ends
+    (300, 256, (VAC, 0.0), (REF, 0.0), False),    # a chunk's angles span two CTAs: the unstaged kernel
+    (1500, 8, (INC, 0.5), (VAC, 0.0), True),      # per-cell blocks through the staged kernel
+    (40, 64, (INC, 2.0), (VAC, 0.0), False),      # three chunks, two per tile
+])
+def test_si_scan_shapes(J, N, bcL, bcR, hetero):
+    """The SI scan's fast form (si_sweep_fast.cu) at the shapes its pieces branch on: staged / unstaged chunk kernels,
+    ragged last chunks and tiles, one and several segments of the carry scan, shared and per-cell blocks."""
+    from oracle import threads_available
+    p = _custom(J, N, bcL, bcR, seed=J + N, hetero=hetero)
+    r = run_pair(p, "si", steps=2, tol=-1.0, max_iters=3, threads=threads_available())
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-12 and rel(r["g_phi"], r["o_phi"]) < 1e-12
+    r = run_pair(p, "si", steps=2, tol=1e-10, max_iters=10_000, threads=threads_available())
+    assert r["g_iters"] == r["o_iters"]
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-9 and rel(r["g_phi"], r["o_phi"]) < 1e-9
+    r2 = run_pair(p, "si", steps=2, tol=1e-10, max_iters=10_000, threads=threads_available())
+    assert np.array_equal(r["g_psi"], r2["g_psi"])              # the ticketed carry scan composes in a fixed order
+
+
 @pytest.mark.parametrize("scheme", ["oci", "si"])
 @pytest.mark.parametrize("cfg,steps", [(2, 3), (3, 1), (4, 2), (5, 1)])
 def test_full_size_converged_parity(cfg, steps, scheme):
