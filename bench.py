@@ -627,6 +627,23 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
         barrier = dist.barrier
 
+    if args.si_only:
+        # the comparator alone (rows d1-d3): the SI steps of one config, nothing else - for launch lists and profiles
+        p = make_problem(args.config)
+        g = P.OCI.from_problem(p, device=f"cuda:{local}")
+        for k in range(args.warmup):
+            g.set_source(p.source(k))
+            g.si_step(p.tol, p.max_iters)
+        l0 = g.launch_count()
+        ms, iters, each = time_gpu_steps(torch, g, p, args.steps, "si")
+        print(json.dumps({"metric": "si_time_to_converge_ms_per_step", "value": ms / args.steps, "unit": "ms", "higher_is_better": False,
+                          "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step_median": float(np.median(each)),
+                          "iters_per_step": iters, "si_unknown_updates_per_s": p.unknowns * sum(iters) / (ms * 1e-3),
+                          "gpu_launches": int(g.launch_count() - l0), "dtype": "f64", "data": "synthetic",
+                          "config": {"workload": p.name, "S_N": p.n_angles, "cells": p.cells, "tol": p.tol, "scheme": "source iteration"}}))
+        g.close()
+        return 0
+
     peaks, peak_src = load_peaks()
     if world > 1:
         # row f4: ONE slab of world x (config's cells), sharded by contiguous cell ranges (weak scaling)
@@ -745,6 +762,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-table", action="store_true", help="skip the per-config OCI/SI table")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--si-only", action="store_true", help="time only the GPU SI comparator on --config (one small JSON line; for profiles)")
     ap.add_argument("--family", default="default", choices=["default", "woodbury"],
                     help="kernel family of the timed arm: the library default (dense inverse, the headline) or the O(N) rank-4 apply")
     args = ap.parse_args()
