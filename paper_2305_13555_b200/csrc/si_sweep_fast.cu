@@ -142,6 +142,14 @@ __global__ void __launch_bounds__(128, STAGED && SHARED_BLOCK ? 4 : 3) si_chunk2
     const size_t stage_doubles = (size_t)cpb * S * (N * 2 + 4);
     uint64_t* bars = reinterpret_cast<uint64_t*>(si_smem);
     double* ring = reinterpret_cast<double*>(si_smem + 128);
+    // MODE 3, staged: the scalar-flux partials of a tile stay in shared memory ([tile parity][lane group][cell][4]) and the
+    // tile's threads finish phi, the norms and the next scattering source themselves (the combine kernel's work, in its order)
+    constexpr bool FUSED = STAGED && MODE == 3;
+    const int nparts = N / 2 >= 32 ? N / 32 : 2;
+    const int tile_cells = cpb * S;
+    double* sphi = ring + 2 * stage_doubles;
+    double dmax = 0.0, rmax = 0.0;
+    const int slot = cnt;                                // MODE 3: the norm slot of this iteration rides in `cnt`
     auto request = [&](int tile, int stage) {            // one thread: the two bulk copies of a tile
         const int64_t c0 = (int64_t)tile * cpb * S;
         const int64_t c1 = (c0 + (int64_t)cpb * S < J) ? c0 + (int64_t)cpb * S : J;
@@ -291,7 +299,8 @@ __global__ void __launch_bounds__(128, STAGED && SHARED_BLOCK ? 4 : 3) si_chunk2
                         const int idx = (lg >> sh) * R + i, u = idx >> 2, r = idx & 3;
                         if (t0 + u < len && live) {
                             const int64_t j = pos ? c_begin + t0 + u : c_end - 1 - (t0 + u);
-                            Pp[j * 4 + r] = v[i];
+                            if (FUSED) sphi[(((size_t)(seq & 1) * nparts + part) * tile_cells + (j - cell0)) * 4 + r] = v[i];
+                            else Pp[j * 4 + r] = v[i];
                         }
                     }
                 }
@@ -320,10 +329,44 @@ __global__ void __launch_bounds__(128, STAGED && SHARED_BLOCK ? 4 : 3) si_chunk2
         }
     }
     }
-    if (STAGED && tile + 2 * (int)gridDim.x < ntiles) {  // the stage is free once every thread has left it: refill it
+    if (FUSED || (STAGED && tile + 2 * (int)gridDim.x < ntiles)) {   // the stage is free once every thread has left it: refill it
         __syncthreads();
-        if (threadIdx.x == 0) request(tile + 2 * gridDim.x, stage);
+        if (threadIdx.x == 0 && tile + 2 * (int)gridDim.x < ntiles) request(tile + 2 * gridDim.x, stage);
     }
+    if (FUSED) {
+        double* __restrict__ src_nxt = (it & 1) ? V.qs : V.si_src1;
+        const int64_t cell1 = (cell0 + tile_cells < J) ? cell0 + tile_cells : J;
+        const int units = (int)(cell1 - cell0) * 2;          // 16-byte units of phi
+        for (int e = threadIdx.x; e < units; e += 128) {
+            const int64_t ge = cell0 * 2 + e;
+            const double2 o = reinterpret_cast<const double2*>(V.phi)[ge];
+            const double2 q = reinterpret_cast<const double2*>(V.Q)[ge];
+            const int64_t j = ge >> 1;
+            const double q4 = 0.25 * V.dx[j], sg = V.sigs[j];
+            double2 sum = make_double2(0.0, 0.0);
+            for (int pp = 0; pp < nparts; ++pp) {
+                const double2 v2 = *reinterpret_cast<const double2*>(sphi + (((size_t)(seq & 1) * nparts + pp) * tile_cells) * 4 + 2 * e);
+                sum.x += v2.x;
+                sum.y += v2.y;
+            }
+            reinterpret_cast<double2*>(V.phi)[ge] = sum;
+            reinterpret_cast<double2*>(src_nxt)[ge] = make_double2(q4 * fma(sg, sum.x, q.x), q4 * fma(sg, sum.y, q.y));
+            dmax = nanmax(dmax, nanmax(fabs(sum.x - o.x), fabs(sum.y - o.y)));
+            rmax = nanmax(rmax, nanmax(fabs(sum.x), fabs(sum.y)));
+        }
+    }
+  }
+  if (FUSED) {
+      __shared__ double sd[4], sr[4];
+      dmax = warp_max(dmax);
+      rmax = warp_max(rmax);
+      if (lane == 0) { sd[threadIdx.x >> 5] = dmax; sr[threadIdx.x >> 5] = rmax; }
+      __syncthreads();
+      if (threadIdx.x == 0) {
+          for (int q = 1; q < 4; ++q) { dmax = nanmax(dmax, sd[q]); rmax = nanmax(rmax, sr[q]); }
+          atomic_max_nonneg(&V.norms[2 * slot + 0], dmax);
+          atomic_max_nonneg(&V.norms[2 * slot + 1], rmax);
+      }
   }
 }
 
@@ -518,22 +561,24 @@ int launch_si_fast_begin(const DevView& V, int buf, cudaStream_t s)
 }
 
 namespace {
+// returns true when the staged form ran (MODE 3: it has then done the combine kernel's work as well)
 template <int MODE, int LG>
-void launch_chunk2(const DevView& V, const SiGeom& g, int buf, int it, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
+bool launch_chunk2(const DevView& V, const SiGeom& g, int buf, int it, int prev_slot, double tol, int cnt, int force, cudaStream_t s)
 {
     // staged form: a tile covers whole chunks (Nr <= 128); persistent CTAs, as many as are resident (about three per SM), two tiles of shared
     // memory each (at most 2 x 34 KB + the barriers: opted in by si_fast_opt_in)
     const size_t stage_bytes = g.Nr <= 128 ? (size_t)(128 / g.Nr) * g.S * ((size_t)V.N * 16 + 32) : 0;
-    if (stage_bytes > 0 && stage_bytes <= 36 * 1024) {
-        const size_t smem = 128 + 2 * stage_bytes;
+    const size_t smem = stage_bytes == 0 ? 0 : 128 + 2 * stage_bytes + (MODE == 3 ? 2 * (size_t)si_fast_parts(V) * (128 / g.Nr) * g.S * 32 : 0);
+    if (stage_bytes > 0 && stage_bytes <= 36 * 1024 && smem <= 80 * 1024) {
         const unsigned per_sm = (unsigned)(200 * 1024 / (smem + 1024));     // resident CTAs: one wave
         const unsigned grid = g.blocks < per_sm * (unsigned)V.sm_count ? g.blocks : per_sm * (unsigned)V.sm_count;
         if (V.nblk == 1) si_chunk2_kernel<4, true, MODE, LG, true><<<grid, 128, smem, s>>>(V, buf, it, prev_slot, tol, g.S, g.C, g.Nr, cnt, force);
         else si_chunk2_kernel<4, false, MODE, LG, true><<<grid, 128, smem, s>>>(V, buf, it, prev_slot, tol, g.S, g.C, g.Nr, cnt, force);
-        return;
+        return true;
     }
     if (V.nblk == 1) si_chunk2_kernel<4, true, MODE, LG, false><<<g.blocks, 128, 0, s>>>(V, buf, it, prev_slot, tol, g.S, g.C, g.Nr, cnt, force);
     else si_chunk2_kernel<4, false, MODE, LG, false><<<g.blocks, 128, 0, s>>>(V, buf, it, prev_slot, tol, g.S, g.C, g.Nr, cnt, force);
+    return false;
 }
 }  // namespace
 
@@ -570,14 +615,16 @@ int launch_si_fast_iteration(const DevView& V, int buf, int it, int slot, int pr
         si_carry3_kernel<<<(unsigned)(V.N * G), CARRY_T, 0, s>>>(V, it, prev_slot, tol, g.C, G);
         k += 2;
     }
+    bool fused = false;                                  // (MODE 3 takes the norm slot in place of `cnt`)
     switch (g.loggs) {                                   // lanes per direction group of the butterfly: 2^loggs
-    case 0: launch_chunk2<3, 0>(V, g, buf, it, prev_slot, tol, 0, 0, s); break;
-    case 1: launch_chunk2<3, 1>(V, g, buf, it, prev_slot, tol, 0, 0, s); break;
-    case 2: launch_chunk2<3, 2>(V, g, buf, it, prev_slot, tol, 0, 0, s); break;
-    case 3: launch_chunk2<3, 3>(V, g, buf, it, prev_slot, tol, 0, 0, s); break;
-    case 4: launch_chunk2<3, 4>(V, g, buf, it, prev_slot, tol, 0, 0, s); break;
-    default: launch_chunk2<3, 5>(V, g, buf, it, prev_slot, tol, 0, 0, s); break;
+    case 0: fused = launch_chunk2<3, 0>(V, g, buf, it, prev_slot, tol, slot, 0, s); break;
+    case 1: fused = launch_chunk2<3, 1>(V, g, buf, it, prev_slot, tol, slot, 0, s); break;
+    case 2: fused = launch_chunk2<3, 2>(V, g, buf, it, prev_slot, tol, slot, 0, s); break;
+    case 3: fused = launch_chunk2<3, 3>(V, g, buf, it, prev_slot, tol, slot, 0, s); break;
+    case 4: fused = launch_chunk2<3, 4>(V, g, buf, it, prev_slot, tol, slot, 0, s); break;
+    default: fused = launch_chunk2<3, 5>(V, g, buf, it, prev_slot, tol, slot, 0, s); break;
     }
+    if (fused) return launched(k + 1);
     const unsigned cb = (unsigned)((V.J * 2 + 255) / 256);
     switch (si_fast_parts(V)) {
     case 2: si_combine_kernel<2><<<cb, 256, 0, s>>>(V, it, slot, prev_slot, tol); break;
