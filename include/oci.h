@@ -123,6 +123,7 @@ typedef struct {
     int32_t iteration;    /* OCI_ITERATION_* */
     int32_t reduced_kernel; /* OCI_RKERNEL_* */
     int32_t small_step_cluster; /* CTAs of the one-launch step's cluster, 0 = the three-pass kernels (oci_set_small_step) */
+    int32_t si_small_step_cluster; /* the same for si_step: CTAs of its one-launch step, 0 = three kernels per iteration */
 } oci_info;
 
 /* Problem statement (per-cell dx_j, Sigma_j, Sigma_s,j P:74-82).
@@ -220,7 +221,9 @@ int oci_set_reduced_kernel(oci_ctx* ctx, int32_t kernel);
  * family has been forced; 0: never; 1: required (oci_setup returns -1 if the problem does not fit: per-cell blocks, HALO
  * faces, N > 32, or a state larger than a cluster's shared memory).  Call BEFORE oci_setup.  oci_get_info reports the
  * cluster size in use.  A step that does not converge within the 64 iterations of one launch continues on the three-pass
- * kernels.  Errors: -1. */
+ * kernels.  The same switch governs si_step, whose comparator gets the same treatment at the same sizes (every SI
+ * iteration and the final sweep in one launch; modes -1 and 1 take it where it fits, and mode 1 never fails because of
+ * si_step: where it does not fit, si_step runs its three kernels per iteration).  Errors: -1. */
 int oci_set_small_step(oci_ctx* ctx, int32_t mode);
 
 /* Results of the current state.  phi: [cells][4] (eq. 18);

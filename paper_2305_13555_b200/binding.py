@@ -36,7 +36,8 @@ class _bc(C.Structure):
 class _info(C.Structure):
     _fields_ = [("cells", C.c_int64), ("n_angles", C.c_int32), ("block_dim", C.c_int32),
                 ("n_blocks", C.c_int64), ("path", C.c_int32), ("apply_kernel", C.c_int32),
-                ("iteration", C.c_int32), ("reduced_kernel", C.c_int32), ("small_step_cluster", C.c_int32)]
+                ("iteration", C.c_int32), ("reduced_kernel", C.c_int32), ("small_step_cluster", C.c_int32),
+                ("si_small_step_cluster", C.c_int32)]
 
 
 _dp = C.POINTER(C.c_double)
@@ -283,7 +284,8 @@ class OCI:
         self._check(self._L.oci_get_info(self._h, C.byref(i)))
         return dict(cells=i.cells, n_angles=i.n_angles, block_dim=i.block_dim, n_blocks=i.n_blocks, path=i.path,
                     apply_kernel=i.apply_kernel, iteration=i.iteration, reduced_kernel=i.reduced_kernel,
-                    small_step_cluster=i.small_step_cluster)
+                    small_step_cluster=i.small_step_cluster,
+                    si_small_step_cluster=i.si_small_step_cluster)
 
     def get_block_inverse(self, blk=0):
         n = 4 * self.n_angles

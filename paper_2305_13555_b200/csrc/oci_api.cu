@@ -46,6 +46,7 @@ struct oci_ctx {
     int32_t forced_rkernel = OCI_RKERNEL_AUTO;   // oci_set_reduced_kernel
     int32_t small_mode = -1;                     // oci_set_small_step: -1 auto, 0 off, 1 required
     int32_t small_cluster = 0;                   // cluster size of the one-launch step, 0 = not used (resolved in oci_setup)
+    int32_t si_small_cluster = 0;                // the same for the SI comparator's one-launch step (si_small.cu)
     // row f4: shard of a slab (shard_exchange.cu)
     bool sharded = false;
     unsigned long long xtag = 0;       // exchanges completed so far (the next one carries xtag + 1)
@@ -465,8 +466,23 @@ int run_step(oci_ctx* ctx, bool si, double tol, int32_t max_iters, int32_t* iter
     } else {
         LAUNCH(ensure_psi(ctx));
         ctx->yz_valid = false;
-        if (si_fast) LAUNCH(launch_si_fast_begin(V, ctx->cur, s));          // psi_{k-1/2}, compact (+ a8 of the previous step)
+        const bool si_small = si_fast && ctx->si_small_cluster > 0 && ctx->d_pub != nullptr;
+        if (si_small) {}                                                    // (the one-launch step commits psi_{k-1/2} itself)
+        else if (si_fast) LAUNCH(launch_si_fast_begin(V, ctx->cur, s));     // psi_{k-1/2}, compact (+ a8 of the previous step)
         else LAUNCH(launch_cfix(V, ctx->cur, s));                 // a2 (+ a8 of the previous step)
+        if (si_small) {
+            // small shared-block problems: every iteration and the final sweep in ONE launch on one cluster (si_small.cu)
+            const int32_t cnt = max_iters < kNormSlots ? max_iters : kNormSlots;
+            V.host_pub = ctx->d_pub;
+            V.pub_seq = ++ctx->pub_seq;
+            LAUNCH(launch_si_small(V, ctx->si_small_cluster, ctx->cur, tol, cnt, cnt >= max_iters, s));
+            V.host_pub = nullptr;
+            int32_t executed = 0;
+            if (int rc = wait_published(ctx, ctx->pub_seq, &executed, &d, &r)) return rc;   // the one read-back (a7), no copy
+            conv = stop_now(tol, d, r);
+            done_iters = executed;
+            // (not converged and max_iters not reached: the three-kernel iterations go on from the state the kernel left)
+        }
     }
     int32_t guess = ctx->predicted[si ? 1 : 0] > 0 ? ctx->predicted[si ? 1 : 0] + 1 : 8;
     while (done_iters < max_iters && !conv) {
@@ -712,6 +728,7 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
         CK(oci_red_woodbury_opt_in());
         CK(oci_red_small_opt_in());
         CK(si_fast_opt_in());
+        CK(si_small_opt_in());
     }
 
     cudaStream_t s = ctx->stream;
@@ -834,6 +851,9 @@ int oci_setup(oci_ctx* ctx, void* d_workspace, int64_t bytes, void* cuda_stream)
             // cluster of 8 is level with the three-pass kernels and runs on request only
             ctx->small_cluster = C;
         }
+        // the comparator gets the same treatment at the same sizes (same switch: oci_set_small_step)
+        const int Cs = cc && ctx->small_mode != 0 ? si_small_cluster(V) : 0;
+        ctx->si_small_cluster = (Cs == 1 || Cs == 16 || (ctx->small_mode == 1 && Cs > 0)) ? Cs : 0;
     }
     ctx->cur = 0;
     ctx->ycur = 0;
@@ -1004,6 +1024,7 @@ int oci_get_info(const oci_ctx* ctx, oci_info* info)
     info->iteration = resolved_iteration(ctx);
     info->reduced_kernel = ctx->red_kernel;
     info->small_step_cluster = ctx->small_cluster;
+    info->si_small_step_cluster = ctx->si_small_cluster;
     return OCI_OK;
 }
 

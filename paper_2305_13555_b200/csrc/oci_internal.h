@@ -180,6 +180,10 @@ int launch_red_opreg(const DevView& V, const RedOpregMaps& M, int pass, int ybas
 // one-launch step of small shared-block problems (oci_reduced_small.cu): cluster size that serves V, 0 if none
 int oci_red_small_cluster(const DevView& V);
 int launch_red_small(const DevView& V, int C, int ybase, double tol, int cnt, int force, cudaStream_t s);
+// one-launch SI step of small shared-block problems (si_small.cu; runs after launch_si_fast_begin): cluster size, 0 if none
+int si_small_cluster(const DevView& V);
+cudaError_t si_small_opt_in();
+int launch_si_small(const DevView& V, int C, int buf, double tol, int cnt, int force, cudaStream_t s);
 int launch_woodbury_setup(const DevView& V, cudaStream_t s);
 int launch_red_woodbury(const DevView& V, int pass, int ybase, int slot, int prev_slot, double tol, int cnt, int force, cudaStream_t s);
 bool oci_red_resident_supported(const DevView& V);

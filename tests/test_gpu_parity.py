@@ -789,6 +789,60 @@ def test_small_step_hand_over_and_refusals():
         h.close()
 
 
+@pytest.mark.parametrize("J,N,bcL,bcR", [
+    (1, 2, (VAC, 0.0), (VAC, 0.0)),            # one cell, S2: one CTA, one chunk
+    (1, 4, (REF, 0.0), (REF, 0.0)),            # one cell between two mirrors
+    (20, 4, (INC, 0.5), (REF, 0.0)),           # config-1 size
+    (129, 8, (REF, 0.0), (VAC, 0.0)),          # one CTA, eleven chunks, the last one short
+    (65, 32, (INC, 1.0), (INC, 0.25)),         # a cluster whose last CTA is short
+    (300, 8, (VAC, 0.0), (REF, 0.0)),          # cluster, 19 cells per CTA
+    (1000, 16, (REF, 0.0), (REF, 0.0)),        # config-2 size, mirrors at both ends of the cluster
+])
+def test_si_small_step_shapes(J, N, bcL, bcR):
+    """The comparator's one-launch step (si_small.cu): against the oracle at a fixed iteration count and converged,
+    bit-reproducible, and equal to the three-kernel iterations within rounding."""
+    p = _custom(J, N, bcL, bcR, seed=3 * J + N, hetero=False)
+    r = run_pair(p, "si", steps=3, tol=-1.0, max_iters=4, small_step=1)
+    assert r["info"]["si_small_step_cluster"] in ((1,) if J * N <= 2048 else (2, 4, 8, 16))
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-12 and rel(r["g_phi"], r["o_phi"]) < 1e-12
+    assert r["launches"] <= 6 + 2 * 3                            # set_flux, layout on demand + one launch per step
+    r = run_pair(p, "si", steps=3, tol=1e-10, max_iters=10_000, small_step=1)
+    assert r["g_iters"] == r["o_iters"]
+    assert rel(r["g_psi"], r["o_psi"]) < 1e-9 and rel(r["g_phi"], r["o_phi"]) < 1e-9
+    r2 = run_pair(p, "si", steps=3, tol=1e-10, max_iters=10_000, small_step=1)
+    assert np.array_equal(r["g_psi"], r2["g_psi"]) and np.array_equal(r["g_phi"], r2["g_phi"])
+    r3 = run_pair(p, "si", steps=3, tol=1e-10, max_iters=10_000, small_step=0)
+    assert r3["info"]["si_small_step_cluster"] == 0
+    assert r3["g_iters"] == r["g_iters"] and rel(r["g_psi"], r3["g_psi"]) < 1e-12
+    assert r3["launches"] > r["launches"]
+
+
+def test_si_small_step_hand_over():
+    """More than the 64 iterations of one launch: the three-kernel iterations continue from the state the kernel left
+    (exact counts in the middle of later chunks), and SI after OCI (and back) on one context commits the right state."""
+    import paper_2305_13555_b200 as P
+    from oracle import Oracle
+    q = _custom(40, 4, (REF, 0.0), (INC, 1.0), seed=9, hetero=False, dt=50.0)
+    q.sigma_s[:] = q.sigma_t * 0.99
+    g, o = P.OCI.from_problem(q, small_step=1), Oracle.from_problem(q)
+    for x in (g, o):
+        x.set_source(q.source(0))
+    for n in (64, 65, 77, 150):
+        g.set_flux(q.psi0); o.set_flux(q.psi0)
+        assert g.si_step(-1.0, n)[:2] == (1, n) == o.si_step(-1.0, n)[:2]
+        assert rel(g.get_angular_flux(), o.angular_flux()) < 1e-12, n
+    g.set_flux(q.psi0); o.set_flux(q.psi0)
+    a, b = g.si_step(1e-10, 100_000), o.si_step(1e-10, 100_000)
+    assert a[0] == b[0] == 0 and a[1] == b[1] and a[1] > 64
+    assert rel(g.get_scalar_flux(), o.scalar_flux()) < 1e-8
+    for scheme in ("oci", "si", "si", "oci", "si"):
+        a = (g.oci_step if scheme == "oci" else g.si_step)(1e-10, 100_000)
+        b = (o.oci_step if scheme == "oci" else o.si_step)(1e-10, 100_000)
+        assert a[0] == b[0] == 0 and abs(a[1] - b[1]) <= 1
+        assert rel(g.get_angular_flux(), o.angular_flux()) < 1e-8
+    g.close()
+
+
 def test_ktiled_fused_loop_many_iterations():
     """The eight-warp K-tiled kernel runs a chunk of up to 64 iterations in one cooperative launch (the producer thread
     follows the MMA warps through the grid barrier).  More than one chunk, an exact count that ends inside a later chunk,
