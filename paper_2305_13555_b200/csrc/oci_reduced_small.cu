@@ -4,7 +4,7 @@
 //
 // The three-pass path costs a small problem three launches and, per iteration, a grid-wide barrier through global
 // memory plus a round trip of the iterate through L2 (about 5 us per iteration at config 2 for 1.2 MFLOP of work).
-// Here a cluster of C <= 8 CTAs splits the cells into contiguous ranges; each CTA keeps, in its shared memory, the three
+// Here a cluster of C <= 16 CTAs (8 portable; 16 where the device co-schedules one) splits the cells into contiguous ranges; each CTA keeps, in its shared memory, the three
 // operators (X, [G; H], F, transposed), both buffers of its part of the iterate y with one ghost row on either side,
 // yfix, ifix, phifix and phi.  Per iteration:
 //   compute (a warp takes tiles of 16 cells x up to 40 operator rows: DMMA.8x8x4 with both operands as fragments

@@ -8,8 +8,9 @@
 //   * reads psi_{k-1/2} from a compact [J][N][2] copy made once per step (half the bytes of c_fix) and the
 //     angle-independent part of the right-hand side of eqs. (14),(17), (h/4)(Sigma_s phi^(l) + Q) (row d1), from a
 //     [J][4] array, two buffers by iteration parity;
-//   * a tiny combine kernel adds the partials in a fixed order (deterministic), overwrites phi, takes the two
-//     max-norms of the stopping rule and forms the next iteration's scattering source;
+//   * the partials are added in a fixed order (deterministic), phi overwritten, the two max-norms of the stopping rule
+//     taken and the next iteration's scattering source formed by the threads of the tile that produced them (staged
+//     chunk kernels: the partials never leave shared memory) or by a tiny combine kernel (the unstaged shapes);
 //   * the reflecting-boundary inflow (reading S4: lagged) travels through a per-angle inflow array instead of the
 //     ghost rows of Psi.
 // After the device-side stop a FINAL pass repeats the last sweep from phi^(L-1) and the stored chunk inflows and writes
@@ -105,7 +106,7 @@ __global__ void __launch_bounds__(256) si_prev_kernel(DevView V, int buf)
 
 // MODE 1: reduce the chunk to its affine map.  MODE 3: sweep the chunk from its inflow, accumulate the phi partials.
 // MODE 4 (final): sweep the chunk and store Psi.  `it` = iteration index within the step (phi buffer parity).
-// scan[(m*C + c)*8 + 0..5] = (P_c, z_c), [6..7] = inflow of chunk c (written by si_carry2_kernel).
+// scan[(m*C + c)*8 + 0..5] = (P_c, z_c), [6..7] = inflow of chunk c (written by si_carry3_kernel).
 // STAGED: the CTA's chunks are consecutive, so everything they read - the psi_{k-1/2} rows of their cells (all angles:
 // one contiguous run of [J][N][2]) and the source rows - arrives as TWO bulk copies (UBLKCP) requested by one thread at
 // the start of the CTA and the sweep reads shared memory: the kernel was bound by the latency of 16-byte loads issued
