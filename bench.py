@@ -171,8 +171,9 @@ def dist_env():
 
 # ------------------------------------------------------------------------------------------ oracle arm
 def oracle_sample_problem(cfg):
-    """A bounded sample of config `cfg` for the CPU oracle (about 10-30 s of CPU work per run)."""
-    sample = {1: None, 2: None, 3: 32768, 4: 2048, 5: 512}[cfg]
+    """A bounded sample of config `cfg` for the CPU oracle (about 10-30 s of CPU work per run on 16 cores): config 3
+    (the bench default) runs at FULL size, the O(N^2)-per-cell configs 4 and 5 on their first 2048 / 512 cells."""
+    sample = {1: None, 2: None, 3: None, 4: 2048, 5: 512}[cfg]
     p = make_problem(cfg, cells=sample)
     desc = (f"config {cfg} at full size" if sample is None else
             f"config {cfg} with the first {sample} of {FULL_CELLS[cfg]} cells (same materials, angles, dt, BCs)")
@@ -210,14 +211,14 @@ def time_oracle(cfg, steps, warmup, threads, scheme="oci", cells=None):
 def oracle_legs(cfg, threads):
     """SURVEY 8(d) "Oracle timing": the oracle as it stands, OCI and SI, on (i) one thread and (ii) all host cores
     (threads over cells for OCI, over angles for SI, as the paper's CPU runs).  The one-thread legs use a
-    quarter of the sample so that the whole baseline stays within tens of seconds."""
+    quarter of the sample and one step so that the whole baseline stays within tens of seconds."""
     p, _ = oracle_sample_problem(cfg)
     small = max(1, p.cells // 4) if cfg in (3, 4, 5) else None
-    steps = 1 if cfg in (3, 4, 5) else 5
+    steps = 3 if cfg == 3 else 2 if cfg in (4, 5) else 5
     legs = {}
     for scheme in ("oci", "si"):
         legs[f"{scheme}_all_cores"] = time_oracle(cfg, steps, 0, threads, scheme)
-        legs[f"{scheme}_1_thread"] = time_oracle(cfg, steps, 0, 1, scheme, cells=small)
+        legs[f"{scheme}_1_thread"] = time_oracle(cfg, 1 if cfg in (3, 4, 5) else steps, 0, 1, scheme, cells=small)
     return legs
 
 
@@ -350,16 +351,25 @@ def time_cpu_blas(cfg, steps):
 
 
 def run_reference(args):
+    """The base contract's reference arm = the oracle as it stands on the host cores: EXACTLY --steps timed steps after
+    --warmup untimed ones, each on a bounded sample of the config (oracle_sample_problem; one calibration step first, and
+    the sample shrinks if the whole run would not end within a few minutes)."""
     rank, world, _ = dist_env()
     if rank != 0:
         return 0
     from oracle import threads_available
     threads = threads_available()
-    steps = max(1, min(args.steps, 2)) if args.config in (3, 4, 5) else args.steps
-    r = time_oracle(args.config, steps, min(args.warmup, 1), threads)
+    steps, warmup = max(1, args.steps), max(0, args.warmup)
+    p, _ = oracle_sample_problem(args.config)
+    cells = p.cells
+    need = time_oracle(args.config, 1, 0, threads)["seconds"] * (steps + warmup)
+    budget = 150.0
+    if need > budget:
+        cells = max(16, int(cells * budget / need) // 16 * 16)
+    r = time_oracle(args.config, steps, warmup, threads, cells=cells)
     line = {
         "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
-        "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+        "steps": steps, "warmup": warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": make_problem(args.config, cells=1).name},
         "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": threads, "kind": "oracle", "sample": r["sample"]},
