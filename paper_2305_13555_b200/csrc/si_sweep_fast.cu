@@ -143,7 +143,7 @@ __global__ void __launch_bounds__(128, STAGED && SHARED_BLOCK ? 4 : 3) si_chunk2
     const size_t stage_doubles = (size_t)cpb * S * (N * 2 + 4);
     uint64_t* bars = reinterpret_cast<uint64_t*>(si_smem);
     double* ring = reinterpret_cast<double*>(si_smem + 128);
-    // MODE 3, staged: the scalar-flux partials of a tile stay in shared memory ([tile parity][lane group][cell][4]) and the
+    // MODE 3, staged: the scalar-flux partials of a tile stay in shared memory ([lane group][cell][4]) and the
     // tile's threads finish phi, the norms and the next scattering source themselves (the combine kernel's work, in its order)
     constexpr bool FUSED = STAGED && MODE == 3;
     const int nparts = N / 2 >= 32 ? N / 32 : 2;
@@ -300,7 +300,7 @@ __global__ void __launch_bounds__(128, STAGED && SHARED_BLOCK ? 4 : 3) si_chunk2
                         const int idx = (lg >> sh) * R + i, u = idx >> 2, r = idx & 3;
                         if (t0 + u < len && live) {
                             const int64_t j = pos ? c_begin + t0 + u : c_end - 1 - (t0 + u);
-                            if (FUSED) sphi[(((size_t)(seq & 1) * nparts + part) * tile_cells + (j - cell0)) * 4 + r] = v[i];
+                            if (FUSED) sphi[((size_t)part * tile_cells + (j - cell0)) * 4 + r] = v[i];
                             else Pp[j * 4 + r] = v[i];
                         }
                     }
@@ -346,7 +346,7 @@ __global__ void __launch_bounds__(128, STAGED && SHARED_BLOCK ? 4 : 3) si_chunk2
             const double q4 = 0.25 * V.dx[j], sg = V.sigs[j];
             double2 sum = make_double2(0.0, 0.0);
             for (int pp = 0; pp < nparts; ++pp) {
-                const double2 v2 = *reinterpret_cast<const double2*>(sphi + (((size_t)(seq & 1) * nparts + pp) * tile_cells) * 4 + 2 * e);
+                const double2 v2 = *reinterpret_cast<const double2*>(sphi + ((size_t)pp * tile_cells) * 4 + 2 * e);
                 sum.x += v2.x;
                 sum.y += v2.y;
             }
@@ -355,6 +355,7 @@ __global__ void __launch_bounds__(128, STAGED && SHARED_BLOCK ? 4 : 3) si_chunk2
             dmax = nanmax(dmax, nanmax(fabs(sum.x - o.x), fabs(sum.y - o.y)));
             rmax = nanmax(rmax, nanmax(fabs(sum.x), fabs(sum.y)));
         }
+        __syncthreads();                                     // the next tile's partials go to the same place
     }
   }
   if (FUSED) {
@@ -569,9 +570,9 @@ bool launch_chunk2(const DevView& V, const SiGeom& g, int buf, int it, int prev_
     // staged form: a tile covers whole chunks (Nr <= 128); persistent CTAs, as many as are resident (about three per SM), two tiles of shared
     // memory each (at most 2 x 34 KB + the barriers: opted in by si_fast_opt_in)
     const size_t stage_bytes = g.Nr <= 128 ? (size_t)(128 / g.Nr) * g.S * ((size_t)V.N * 16 + 32) : 0;
-    const size_t smem = stage_bytes == 0 ? 0 : 128 + 2 * stage_bytes + (MODE == 3 ? 2 * (size_t)si_fast_parts(V) * (128 / g.Nr) * g.S * 32 : 0);
+    const size_t smem = stage_bytes == 0 ? 0 : 128 + 2 * stage_bytes + (MODE == 3 ? (size_t)si_fast_parts(V) * (128 / g.Nr) * g.S * 32 : 0);
     if (stage_bytes > 0 && stage_bytes <= 36 * 1024 && smem <= 80 * 1024) {
-        const unsigned per_sm = (unsigned)(200 * 1024 / (smem + 1024));     // resident CTAs: one wave
+        const unsigned per_sm = (unsigned)(227 * 1024 / (smem + 1024));     // resident CTAs: one wave
         const unsigned grid = g.blocks < per_sm * (unsigned)V.sm_count ? g.blocks : per_sm * (unsigned)V.sm_count;
         if (V.nblk == 1) si_chunk2_kernel<4, true, MODE, LG, true><<<grid, 128, smem, s>>>(V, buf, it, prev_slot, tol, g.S, g.C, g.Nr, cnt, force);
         else si_chunk2_kernel<4, false, MODE, LG, true><<<grid, 128, smem, s>>>(V, buf, it, prev_slot, tol, g.S, g.C, g.Nr, cnt, force);
