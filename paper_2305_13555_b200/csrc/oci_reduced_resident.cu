@@ -208,14 +208,17 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
     const int64_t J = V.J;
 
     const int64_t ntiles = (J + RT_M - 1) / RT_M;
-    // warp-major numbering: warp 0 of every CTA first, so a small problem spreads over all SMs (one busy warp per SM
-    // partition has the DMMA pipe to itself) instead of filling the eight warps of a few CTAs
-    const int64_t wid = (int64_t)warp * gridDim.x + blockIdx.x, nw = (int64_t)gridDim.x * RT_WARPS;
-    const int my_tiles = wid < ntiles ? (int)((ntiles - wid + nw - 1) / nw) : 0;
+    // CTA b owns the tiles b, b + grid, b + 2 grid, ... (a small problem spreads over all SMs, and the grid sweeps the
+    // slab front to back); its warps CLAIM them one at a time from a counter in shared memory, one tile ahead of the one
+    // they compute: the time a tile takes varies by +-10 % between the warps of an SM (measured), and with a fixed
+    // seven tiles per warp an iteration lasts as long as its unluckiest warp
+    __shared__ int tile_ctr;
+    const int Mcta = (int64_t)blockIdx.x < ntiles ? (int)((ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;
     unsigned char* my_ring = ring + (size_t)warp * RT_STAGES * C::STAGE_BYTES;
     uint64_t* my_full = full + warp * RT_STAGES;
 
     if (tid == 0) {
+        tile_ctr = 0;
         for (int s = 0; s < RT_WARPS * RT_STAGES; ++s) mbar_init(&full[s], 1);
         mbar_init(op_bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -240,16 +243,21 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
     // that its most recently written part is still in L2 when iteration l+1 reads it - which is why odd iterations
     // walk the tiles in the opposite order (`rev`).  ifix is only read by the FINAL pass: written evict_first.
     const uint64_t pol_last = l2_policy_evict_last(), pol_first = l2_policy_evict_first();
-    bool rev = false;                    // this iteration walks the warp's tiles from the last one down
-    auto tile_at = [&](int it) -> int64_t { return wid + (int64_t)(rev ? my_tiles - 1 - it : it) * nw; };
+    bool rev = false;                    // this iteration walks the CTA's tiles from the last one down
+    auto tile_at = [&](int m) -> int64_t { return blockIdx.x + (int64_t)(rev ? Mcta - 1 - m : m) * gridDim.x; };
+    auto claim = [&]() -> int {
+        int m = 0;
+        if (lane == 0) m = atomicAdd(&tile_ctr, 1);
+        return __shfl_sync(0xffffffffu, m, 0);
+    };
 
     // one lane requests a tile: tensor-map boxes straight into the warp's private ring
     const CUtensorMap* my = nullptr;     // tensor map of this iteration's source y
-    int tc0 = 0;                         // tiles this warp has consumed in earlier iterations (ring position)
-    auto prefetch = [&](int it) {
+    int tc = 0;                          // tiles this warp has consumed so far (ring position)
+    auto prefetch = [&](int m, int tcm) {   // tile m of the CTA into the stage of the warp's tcm-th tile
         if (lane == 0) {
-            const int s = (tc0 + it) & 1;
-            const int j0 = (int)(tile_at(it) * RT_M);
+            const int s = tcm & 1;
+            const int j0 = (int)(tile_at(m) * RT_M);
             unsigned char* st = my_ring + (size_t)s * C::STAGE_BYTES;
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             mbar_expect_tx(&my_full[s], C::TX_BYTES);
@@ -304,22 +312,25 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
     Yd = V.y[ysrc_l ^ 1];
     if (PASS == PASS_ITER) E.out = Yd;
     rev = PASS == PASS_ITER && ((slot + l) & 1);
-    tc0 = l * my_tiles;
-    if (my_tiles > 0) prefetch(0);
+    int m_cur = claim();
+    if (m_cur < Mcta) prefetch(m_cur, tc);
     double dmax = 0.0, rmax = 0.0;
     double pend[2][NBP][2];
 #pragma unroll
     for (int g = 0; g < 2; ++g)
 #pragma unroll
         for (int t = 0; t < NBP; ++t) pend[g][t][0] = pend[g][t][1] = 0.0;
-    int64_t pj0 = my_tiles > 0 ? tile_at(0) * RT_M : 0;
+    int64_t pj0 = m_cur < Mcta ? tile_at(m_cur) * RT_M : 0;
     int prows = 0;                                                 // nothing pending yet: loads clamped, stores off
+    bool worked = false;
 
-    for (int it = 0; it < my_tiles; ++it) {
-        const int s = (tc0 + it) & 1;
-        const int64_t j0 = tile_at(it) * RT_M;
+    for (; m_cur < Mcta; ++tc) {
+        const int s = tc & 1;
+        const int64_t j0 = tile_at(m_cur) * RT_M;
         const int rows = (int)((J - j0 < RT_M) ? (J - j0) : RT_M);
-        if (it + 1 < my_tiles) prefetch(it + 1);
+        m_cur = claim();                                           // the NEXT tile, requested before this one is computed
+        if (m_cur < Mcta) prefetch(m_cur, tc + 1);
+        worked = true;
         // the additive operands of THIS tile's epilogue (drained during the next phase) -> L2, so that the loads
         // issued DIST k-steps ahead of their use see an L2 hit instead of a DRAM round trip
         if (PASS != PASS_FIX) {
@@ -339,7 +350,7 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
 #pragma unroll
             for (int t = 0; t < C::NB0; ++t) acc[g][t][0] = acc[g][t][1] = 0.0;
 
-        mbar_wait(&my_full[s], ((tc0 + it) >> 1) & 1);
+        mbar_wait(&my_full[s], (tc >> 1) & 1);
         const double* st = reinterpret_cast<const double*>(my_ring + (size_t)s * C::STAGE_BYTES);
         if (PASS == PASS_FIX) {
             const double* pa = st + g4 * C::LDH + t4;
@@ -383,7 +394,7 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
     if (PASS == PASS_ITER) {
         dmax = warp_max(dmax);
         rmax = warp_max(rmax);
-        if (lane == 0 && my_tiles > 0) {
+        if (lane == 0 && worked) {
             atomic_max_nonneg(&V.norms[2 * (slot + l) + 0], dmax);
             atomic_max_nonneg(&V.norms[2 * (slot + l) + 1], rmax);
         }
@@ -402,6 +413,7 @@ oci_red_resident_kernel(DevView V, const __grid_constant__ CUtensorMap map_a, co
                 } while (seen < target);
                 // the y rows other CTAs have just stored are read next through the async proxy (TMA)
                 asm volatile("fence.proxy.async;" ::: "memory");
+                tile_ctr = 0;                                      // every warp of the CTA has made its last claim
             }
             __syncthreads();
             const bool stop = step_done(V.norms, slot + l, tol) || l + 1 == nloop;
