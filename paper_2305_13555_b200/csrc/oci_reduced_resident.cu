@@ -11,7 +11,8 @@
 //
 //   * one persistent CTA per SM, 8 warps, and EVERY WARP IS AN INDEPENDENT WORKER on tiles of 16 cells:
 //     it owns all output rows of its cells, so there is no cross-warp reduction and no CTA barrier after
-//     start-up (the scalar-flux rows are just one more n8 block of the same warp);
+//     start-up (the scalar-flux rows are just one more n8 block of the same warp); the warps of a CTA claim its
+//     tiles from a counter in shared memory, so that a warp whose tiles run slow takes fewer of them;
 //   * the operator (39 KB for ITER, 74 KB for FIX at K2 = 64) lives in shared memory, rows padded to K2+4
 //     doubles so that the DMMA fragment loads are bank-conflict free; per k-step a warp loads 2 A fragments
 //     (cells) and NB B fragments (operator) for 2*NB DMMA.8x8x4;
