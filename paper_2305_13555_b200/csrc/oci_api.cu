@@ -871,6 +871,15 @@ static int set_flux_common(oci_ctx* ctx, const double* d_edge)
     ctx->yz_valid = false;
     ctx->psi_valid = true;
     LAUNCH(launch_phi_norm(ctx->V, 0, 0, -1, -1.0, false, ctx->stream));   // phi^(0), ghost rows
+    const bool halo = ctx->bcL.kind == OCI_BC_HALO || ctx->bcR.kind == OCI_BC_HALO;
+    if (resolved_iteration(ctx) == OCI_ITERATION_REDUCED && !ctx->sharded && !halo) {
+        // the packed layout the REDUCED steps work in belongs to setting the flux, not to the first step after it
+        // (both layouts are valid from here on; a step of either form invalidates the other one).  A shard packs in its
+        // first step instead, where the neighbours' edge values are exchanged as well.
+        LAUNCH(launch_pack_yz(ctx->V, ctx->cur, 0, ctx->stream));
+        ctx->ycur = 0;
+        ctx->yz_valid = true;
+    }
     CK(cudaStreamSynchronize(ctx->stream));
     CK(cudaGetLastError());
     ctx->have_flux = true;
