@@ -239,9 +239,14 @@ class OCI:
         self._check(self._L.oci_set_source_dev(self._h, C.c_void_p(t.data_ptr()) if t is not None else None))
 
     def _step(self, f, tol, max_iters):
-        it, res = C.c_int32(0), C.c_double(0.0)
-        rc = self._check(f(self._h, float(tol), int(max_iters), C.byref(it), C.byref(res)), allow_not_converged=True)
-        return rc, it.value, res.value
+        out = self.__dict__.get("_step_out")             # the two out-parameters, made once (a small step is ~40 us in all)
+        if out is None:
+            it, res = C.c_int32(0), C.c_double(0.0)
+            out = self.__dict__["_step_out"] = (it, res, C.byref(it), C.byref(res))
+        rc = f(self._h, tol, max_iters, out[2], out[3])
+        if rc < 0:
+            self._check(rc, allow_not_converged=True)
+        return rc, out[0].value, out[1].value
 
     def oci_step(self, tol=1e-10, max_iters=10_000):
         return self._step(self._L.oci_step, tol, max_iters)

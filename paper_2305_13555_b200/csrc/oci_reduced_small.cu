@@ -158,6 +158,15 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
     const int PX = L.PX, PR = L.PR;
     const int nwarps = SM_THREADS >> 5;
     const int ntile = (nc + 15) / 16;                                     // tiles of 16 cells
+    // A TINY problem (config 1: 20 cells x 12 rows) is a chain of latencies, not arithmetic: a DMMA work item is ~2000
+    // cycles of dependent tensor-pipe and shared-memory round trips for 8 k-steps of 4.  There thread = (cell, operator row)
+    // and a row is K2 (+4) dependent DFMAs on broadcast operands: a few hundred cycles per pass.
+    const bool tiny = C == 1 && nc * (2 * K2 + 4) <= 4 * SM_MAX_THREADS && K2 <= 16;
+    auto dot = [&](const double* __restrict__ orow, const double* __restrict__ lo, const double* __restrict__ hi, int K, int split) {
+        double a = 0.0;
+        for (int k = 0; k < K; ++k) a = fma(orow[k], (k < split ? lo : hi)[k], a);
+        return a;
+    };
 
     // ---- load: operators (rows pitched for conflict-free fragment loads, padding rows zero), my cells of the committed
     // state, the FIX input vectors [y(k+1/2 run) | z(k+1/2 run) | Q], the old scalar flux
@@ -198,7 +207,15 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
     else __syncthreads();
 
     // ---- FIX: [yfix | ifix | phifix][c] = X [psi_{k-1/2}[c]; Q[c]]   (psi_{k-1/2} = the k+1/2 runs of y and z)
-    {
+    if (tiny) {
+        for (int e = tid; e < nc * (2 * K2 + 4); e += SM_THREADS) {
+            const int c = e / (2 * K2 + 4), r = e - c * (2 * K2 + 4);
+            const double v = dot(opx + r * PX, xin + c * P, xin + c * P, K2 + 4, K2 + 4);
+            if (r < K2) yfix[c * P + r] = v;
+            else if (r < 2 * K2) ifix[c * P + r - K2] = v;
+            else phifix[c * 4 + r - 2 * K2] = v;
+        }
+    } else {
         const int nbt = L.mx / 8, ngr = (nbt + nbg - 1) / nbg;
         for (int it = warp; it < ntile * ngr; it += nwarps) {
             const int tile = it / ngr, gr = it - tile * ngr;
@@ -246,7 +263,21 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
         const double* __restrict__ src = ybuf[l & 1];
         double* __restrict__ dst = ybuf[(l + 1) & 1];
         double dmax = 0.0, rmax = 0.0;
-        {
+        if (tiny) {
+            for (int e = tid; e < nc * (K2 + 4); e += SM_THREADS) {
+                const int c = e / (K2 + 4), r = e - c * (K2 + 4);
+                const double v = dot(opr + r * PR, src + (c + 1) * P, src + (c - 1) * P, K2, N);
+                if (r < K2) {
+                    dst[c * P + r] = yfix[c * P + r] + v;
+                } else {
+                    const int i = r - K2;
+                    const double nv = phifix[c * 4 + i] + v, ov = phi[c * 4 + i];
+                    phi[c * 4 + i] = nv;
+                    dmax = nanmax(dmax, fabs(nv - ov));
+                    rmax = nanmax(rmax, fabs(nv));
+                }
+            }
+        } else {
             const int nbt = L.mr / 8, ngr = (nbt + nbg - 1) / nbg;
             for (int it = warp; it < ntile * ngr; it += nwarps) {
                 const int tile = it / ngr, gr = it - tile * ngr;
@@ -311,7 +342,13 @@ __global__ void __launch_bounds__(SM_MAX_THREADS, 1) oci_red_small_kernel(DevVie
     if (finalize) {
         const double* __restrict__ src = ybuf[(Lit + 1) & 1];             // y^(L-1) with the ghost rows iteration L-1 read
         const int nbt = L.mf / 8, ngr = (nbt + nbg - 1) / nbg;
-        for (int it = warp; it < ntile * ngr; it += nwarps) {
+        if (tiny) {
+            for (int e = tid; e < nc * K2; e += SM_THREADS) {
+                const int c = e / K2, r = e - c * K2;
+                yfix[c * P + r] = ifix[c * P + r] + dot(opf + r * PR, src + (c + 1) * P, src + (c - 1) * P, K2, N);
+            }
+        }
+        for (int it = tiny ? ntile * ngr : warp; it < ntile * ngr; it += nwarps) {
             const int tile = it / ngr, gr = it - tile * ngr;
             const int t0 = gr * nbg, nb = nbt - t0 < nbg ? nbt - t0 : nbg;
             const int g4 = lane >> 2;
@@ -369,6 +406,12 @@ void small_shape(const DevView& V, int C, int* nbg, int* threads)
     *nbg = per > SM_NBG ? SM_NBG : per;
     const int items = ntile * ((nbt + *nbg - 1) / *nbg);
     *threads = items * 32 > SM_MAX_THREADS ? SM_MAX_THREADS : items * 32;
+    // a tiny problem runs thread = (cell, operator row) (the kernel's `tiny` test): one thread per row of an ITER pass
+    const int K2 = 2 * V.N;
+    if (C == 1 && V.J * (2 * K2 + 4) <= 4 * SM_MAX_THREADS && K2 <= 16) {
+        int t = ((int)V.J * (K2 + 4) + 31) / 32 * 32;
+        *threads = t > SM_MAX_THREADS ? SM_MAX_THREADS : t < 32 ? 32 : t;
+    }
 }
 
 void small_config(const DevView& V, int C, cudaLaunchConfig_t* cfg, cudaLaunchAttribute* at, int* nbg)
